@@ -1,0 +1,562 @@
+// ===========================================================================
+// CPU ORACLE of the ALICE-HLT-style TPC sector tracker  --  TEST INFRASTRUCTURE
+// ===========================================================================
+// Plain, slow, single-threaded restatement of what the hot path computes:
+// Cellular-Automaton seeding + Kalman fit / track following, per TPC sector
+// ("Cellular Automaton principle to build track seeds: short
+// track candidate of around 5 to 10 hits. Afterwards, it uses the Kalman filter
+// for track fitting and track following"; L123 cluster-wise then track-wise;
+// L138 sectors processed individually; L182 159 pad rows; L213 clusters are
+// identified by index).  The paper prints no formula; every formula is a
+// reading, written out as numbered fp32 sequences in docs/ARITH_SPEC.md
+// (sections cited below as "SPEC n / tag").
+//
+// THIS FILE IS NOT PART OF THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may call it.  It shares
+// no code, header, table or constant with paper_1712_09434_b200/csrc: the
+// struct layouts and the defaults below are its own.
+//
+// Pins (tests/test_oracle_*.py, CPU only): exhaustive neighbour search on small
+// events (neighbours_bruteforce below) == grid search; transport vs closed-form
+// helix + finite-difference Jacobian; update vs matrix-form Kalman; noiseless
+// helices recovered to 1e-5 (fp64 instantiation); unit pulls; mirror / batch /
+// grid-size invariances; hand-built examples.
+// PARITY UNPINNED: the numeric defaults (windows, cuts, initial covariance,
+// gap, minimum lengths) - nothing in the paper fixes them.
+//
+// Build: g++ -O2 -ffp-contract=off -fno-fast-math -shared -fPIC  (oracle/build.py)
+// ===========================================================================
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct OGeometry {  // mirrors nothing: the oracle's own view of the detector
+  int32_t n_sectors;
+  int32_t n_rows;
+  const float* row_x;
+  float tan_half_angle;
+  float z_max;
+};
+
+struct OParams {  // SPEC 8
+  float sigma_y, sigma_z, nf_hy, nf_hz, nf_chi2_max, grid_bin_min, grid_bin_max, max_sinphi, c0_sinphi,
+      c0_dzds, c0_qpt, accept_k2, search_max, turn_cov_scale;
+  int32_t min_seed_hits, max_row_gap, min_track_hits;
+};
+
+enum Counter {
+  CN_CLUSTERS = 0, CN_BINS, CN_NF_PAIRS, CN_START_HITS, CN_TRACKLETS_BUILT, CN_TRACKLETS_KEPT, CN_CHAIN_HITS,
+  CN_SEARCH_UP, CN_SEARCH_DN, CN_CANDIDATES, CN_TRACKLET_HITS, CN_OUT_HITS, CN_OUT_TRACKS, CN_ROW_STEPS, CN_COUNT
+};
+
+template <class R> R rsqrt_(R v) { return std::sqrt(v); }
+template <class R> R rabs(R v) { return std::fabs(v); }
+template <class R> R rmin(R a, R b) { return std::fmin(a, b); }
+template <class R> R rmax(R a, R b) { return std::fmax(a, b); }
+
+// ---- SPEC 5: track model ---------------------------------------------------
+template <class R> struct State {
+  R x;
+  R p[5];   // y, z, sinphi, dz/dl, q/pT
+  R c[15];  // lower triangle: 00 10 11 20 21 22 30 31 32 33 40 41 42 43 44
+  R chi2;
+  int32_t ndf;
+};
+
+inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
+
+// SPEC 5.1 TRANSPORT (P1..P24). Returns false and leaves st untouched on failure.
+template <class R> bool transport(State<R>& st, R xnew, R a, R max_sinphi) {
+  const R y = st.p[0], z = st.p[1], s = st.p[2], t = st.p[3], q = st.p[4];
+  const R dx = xnew - st.x;                                  // P1
+  const R k = a * q;                                         // P2
+  const R s1 = s + k * dx;                                   // P3
+  if (!(rabs(s) <= max_sinphi && rabs(s1) <= max_sinphi)) return false;  // P4
+  const R c = rsqrt_(R(1) - s * s);                          // P5
+  const R c1 = rsqrt_(R(1) - s1 * s1);
+  const R cs = c + c1;                                       // P6
+  const R tt = (s + s1) / cs;                                // P7
+  const R dy = dx * tt;                                      // P8
+  const R dl = dx * rsqrt_(R(1) + tt * tt);                  // P9
+  const R u = (R(0.5) * k) * dl;                             // P10
+  const R u2 = u * u;
+  const R A1 = R(0.16666667f), A2 = R(0.075f), A3 = R(0.044642857f);
+  const R dS = dl * (R(1) + u2 * (A1 + u2 * (A2 + u2 * A3)));  // P11
+  const R g = s * dy + c * dx;                               // P13
+  const R cc = c * c1;                                       // P14
+  const R f02 = g / cc;                                      // P15
+  const R f04 = ((a * dx) * g) / (c1 * cs);                  // P16
+  const R f12 = (t * dy) / cc;                               // P17
+  const R f13 = dS;                                          // P18
+  const R f14 = ((t * a) * ((R(0.5) * dx) * dy)) / cc;       // P19
+  const R f24 = a * dx;                                      // P20
+  const R* C = st.c;
+  const R c00 = C[0], c10 = C[1], c11 = C[2], c20 = C[3], c21 = C[4], c22 = C[5], c30 = C[6], c31 = C[7],
+          c32 = C[8], c33 = C[9], c40 = C[10], c41 = C[11], c42 = C[12], c43 = C[13], c44 = C[14];
+  // P21 row 0 of M = F*C
+  const R m00 = c00 + f02 * c20 + f04 * c40;
+  const R m02 = c20 + f02 * c22 + f04 * c42;
+  const R m04 = c40 + f02 * c42 + f04 * c44;
+  // P22 row 1
+  const R m10 = c10 + f12 * c20 + f13 * c30 + f14 * c40;
+  const R m11 = c11 + f12 * c21 + f13 * c31 + f14 * c41;
+  const R m12 = c21 + f12 * c22 + f13 * c32 + f14 * c42;
+  const R m13 = c31 + f12 * c32 + f13 * c33 + f14 * c43;
+  const R m14 = c41 + f12 * c42 + f13 * c43 + f14 * c44;
+  // P23 row 2
+  const R m20 = c20 + f24 * c40;
+  const R m21 = c21 + f24 * c41;
+  const R m22 = c22 + f24 * c42;
+  const R m23 = c32 + f24 * c43;
+  const R m24 = c42 + f24 * c44;
+  // P24 C' = M*F^T
+  R n[15];
+  n[0] = m00 + f02 * m02 + f04 * m04;
+  n[1] = m10 + f02 * m12 + f04 * m14;
+  n[2] = m11 + f12 * m12 + f13 * m13 + f14 * m14;
+  n[3] = m20 + f02 * m22 + f04 * m24;
+  n[4] = m21 + f12 * m22 + f13 * m23 + f14 * m24;
+  n[5] = m22 + f24 * m24;
+  n[6] = c30 + f02 * c32 + f04 * c43;
+  n[7] = c31 + f12 * c32 + f13 * c33 + f14 * c43;
+  n[8] = c32 + f24 * c43;
+  n[9] = c33;
+  n[10] = c40 + f02 * c42 + f04 * c44;
+  n[11] = c41 + f12 * c42 + f13 * c43 + f14 * c44;
+  n[12] = c42 + f24 * c44;
+  n[13] = c43;
+  n[14] = c44;
+  st.x = xnew;
+  st.p[0] = y + dy;                                          // P12
+  st.p[1] = z + dS * t;
+  st.p[2] = s1;
+  for (int i = 0; i < 15; ++i) st.c[i] = n[i];
+  return true;
+}
+
+// SPEC 5.2 UPDATE(i, m, e) (U1..U7)
+template <class R> void update(State<R>& st, int i, R m, R e) {
+  const R w = R(1) / (st.c[tri(i, i)] + e);                  // U1
+  const R res = m - st.p[i];                                 // U2
+  R col[5], k[5];
+  for (int j = 0; j < 5; ++j) col[j] = st.c[tri(j, i)];      // U3
+  for (int j = 0; j < 5; ++j) k[j] = col[j] * w;             // U4
+  for (int j = 0; j < 5; ++j) st.p[j] = st.p[j] + k[j] * res;  // U5
+  for (int j = 0; j < 5; ++j)
+    for (int l = 0; l <= j; ++l) st.c[tri(j, l)] = st.c[tri(j, l)] - k[j] * col[l];  // U6
+  st.chi2 = st.chi2 + (res * res) * w;                       // U7
+  st.ndf += 1;
+}
+
+// ---- tables (SPEC 1) --------------------------------------------------------
+template <class R> struct Tables {
+  int n_sectors, n_rows;
+  std::vector<R> X, ymax, dx_up, dx_dn, ratio_up, ratio_dn;
+  R a, sy2, sz2, wy, wz, smax2, z_max;
+  OParams prm;
+  Tables(const OGeometry& g, float bz, const OParams& p) : n_sectors(g.n_sectors), n_rows(g.n_rows), prm(p) {
+    const int n = n_rows;
+    X.resize(n); ymax.resize(n); dx_up.assign(n, R(0)); dx_dn.assign(n, R(0));
+    ratio_up.assign(n, R(0)); ratio_dn.assign(n, R(0));
+    for (int r = 0; r < n; ++r) X[r] = R(g.row_x[r]);
+    for (int r = 0; r < n; ++r) ymax[r] = X[r] * R(g.tan_half_angle) + R(1);           // T1
+    for (int r = 0; r + 1 < n; ++r) { dx_up[r] = X[r + 1] - X[r]; ratio_up[r] = X[r + 1] / X[r]; }  // T2 T4
+    for (int r = 1; r < n; ++r) { dx_dn[r] = X[r] - X[r - 1]; ratio_dn[r] = X[r - 1] / X[r]; }      // T3 T5
+    a = R(-0.000299792458f) * R(bz);                                                     // T6
+    sy2 = R(p.sigma_y) * R(p.sigma_y); sz2 = R(p.sigma_z) * R(p.sigma_z);               // T7
+    wy = R(1) / sy2; wz = R(1) / sz2;
+    smax2 = R(p.search_max) * R(p.search_max);                                           // T8
+    z_max = R(g.z_max);
+  }
+  bool a_side(int task) const { return 2 * (task % n_sectors) < n_sectors; }
+};
+
+// ---- SPEC 2: the oracle's own grid (acceleration only) ----------------------
+template <class R> struct RowGrid {
+  int ny = 1, nz = 1;
+  R inv = 0, y0 = 0, z0 = 0;
+  std::vector<uint32_t> bin_start;  // [ny*nz+1], positions into `order`
+  std::vector<uint32_t> order;      // gids of the row sorted by bin
+  static int clampi(R f, int n) { return (int)rmin(rmax(f, R(0)), R(n - 1)); }
+  int by(R y) const { return clampi((y - y0) * inv, ny); }
+  int bz(R z) const { return clampi((z - z0) * inv, nz); }
+};
+const float GRID_MARGIN = 0.01f;
+
+template <class R> struct Oracle {
+  const Tables<R>& T;
+  const R* Y;
+  const R* Z;
+  const uint32_t* row_off;
+  uint32_t n_clusters, n_tasks;
+  std::vector<RowGrid<R>> grids;  // [n_tasks*n_rows]
+  uint64_t cnt[CN_COUNT];
+
+  Oracle(const Tables<R>& t, const R* y, const R* z, const uint32_t* ro, uint32_t n, uint32_t nt)
+      : T(t), Y(y), Z(z), row_off(ro), n_clusters(n), n_tasks(nt) {
+    std::memset(cnt, 0, sizeof(cnt));
+    cnt[CN_CLUSTERS] = n;
+  }
+
+  // SPEC 2
+  void build_grids() {
+    const int nr = T.n_rows;
+    grids.resize((size_t)n_tasks * nr);
+    for (uint32_t task = 0; task < n_tasks; ++task)
+      for (int r = 0; r < nr; ++r) {
+        RowGrid<R>& G = grids[(size_t)task * nr + r];
+        const uint32_t lo = row_off[(size_t)task * nr + r], hi = row_off[(size_t)task * nr + r + 1];
+        const uint32_t n = hi - lo;
+        const R W = R(2) * T.ymax[r], L = T.z_max + R(2);
+        R B = rsqrt_((W * L) / R(n > 0 ? n : 1));
+        B = rmin(rmax(B, R(T.prm.grid_bin_min)), R(T.prm.grid_bin_max));
+        G.inv = R(1) / B;
+        G.ny = (int)(W * G.inv) + 1;
+        G.nz = (int)(L * G.inv) + 1;
+        G.y0 = -T.ymax[r];
+        G.z0 = T.a_side(task) ? R(-1) : -(T.z_max + R(1));
+        const int nb = G.ny * G.nz;
+        cnt[CN_BINS] += nb;
+        G.bin_start.assign(nb + 1, 0);
+        std::vector<int> b(n);
+        for (uint32_t i = 0; i < n; ++i) {
+          b[i] = G.bz(Z[lo + i]) * G.ny + G.by(Y[lo + i]);
+          G.bin_start[b[i] + 1]++;
+        }
+        for (int i = 0; i < nb; ++i) G.bin_start[i + 1] += G.bin_start[i];
+        G.order.resize(n);
+        std::vector<uint32_t> fill(G.bin_start.begin(), G.bin_start.end() - 1);
+        for (uint32_t i = 0; i < n; ++i) G.order[fill[b[i]]++] = lo + i;
+      }
+  }
+
+  // visit every cluster of the grid whose bin overlaps [ylo,yhi]x[zlo,zhi]
+  template <class F> void for_window(const RowGrid<R>& G, R ylo, R yhi, R zlo, R zhi, F&& f) const {
+    const int iy0 = G.by(ylo), iy1 = G.by(yhi), iz0 = G.bz(zlo), iz1 = G.bz(zhi);
+    for (int iz = iz0; iz <= iz1; ++iz) {
+      const uint32_t b0 = G.bin_start[iz * G.ny + iy0], b1 = G.bin_start[iz * G.ny + iy1 + 1];
+      for (uint32_t i = b0; i < b1; ++i) f(G.order[i]);
+    }
+  }
+
+  // ---- SPEC 3: neighbour finder (N1..N5); use_grid=false is the plain definition ----
+  void neighbours(int32_t* up, int32_t* dn, bool use_grid) {
+    const int nr = T.n_rows;
+    for (uint32_t i = 0; i < n_clusters; ++i) up[i] = dn[i] = -1;
+    const R HY = R(T.prm.nf_hy), HZ = R(T.prm.nf_hz), CHI_MAX = R(T.prm.nf_chi2_max), M = R(GRID_MARGIN);
+    std::vector<uint32_t> cu, cd;
+    for (uint32_t task = 0; task < n_tasks; ++task)
+      for (int r = 1; r + 1 < nr; ++r) {
+        const size_t tr = (size_t)task * nr + r;
+        const uint32_t lo = row_off[tr], hi = row_off[tr + 1];
+        const uint32_t ulo = row_off[tr + 1], uhi = row_off[tr + 2], dlo = row_off[tr - 1], dhi = row_off[tr];
+        const R b = T.dx_dn[r], a_ = T.dx_up[r];
+        for (uint32_t h = lo; h < hi; ++h) {
+          const R y = Y[h], z = Z[h];
+          const R zu = z * T.ratio_up[r], zd = z * T.ratio_dn[r];                      // N1
+          cu.clear(); cd.clear();
+          auto test_u = [&](uint32_t u) { if (rabs(Y[u] - y) <= HY && rabs(Z[u] - zu) <= HZ) cu.push_back(u); };  // N2
+          auto test_d = [&](uint32_t d) { if (rabs(Y[d] - y) <= HY && rabs(Z[d] - zd) <= HZ) cd.push_back(d); };  // N3
+          if (use_grid) {
+            for_window(grids[tr + 1], (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, test_u);
+            for_window(grids[tr - 1], (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, test_d);
+          } else {
+            for (uint32_t u = ulo; u < uhi; ++u) test_u(u);
+            for (uint32_t d = dlo; d < dhi; ++d) test_d(d);
+          }
+          bool have = false;
+          R best = 0; uint32_t bu = 0, bd = 0;
+          for (uint32_t u : cu)
+            for (uint32_t d : cd) {                                                      // N4
+              const R dy = ((Y[u] - y) * b) - ((y - Y[d]) * a_);
+              const R dz = ((Z[u] - z) * b) - ((z - Z[d]) * a_);
+              const R chi = ((dy * dy) * T.wy) + ((dz * dz) * T.wz);
+              cnt[CN_NF_PAIRS]++;
+              if (!(chi < CHI_MAX)) continue;                                            // N5
+              if (!have || chi < best || (chi == best && (u < bu || (u == bu && d < bd)))) {
+                have = true; best = chi; bu = u; bd = d;
+              }
+            }
+          if (have) { up[h] = (int32_t)bu; dn[h] = (int32_t)bd; }
+        }
+      }
+  }
+
+  // ---- SPEC 4: cleaner (C1,C2) and start hits (S1) ----
+  void clean(const int32_t* up, const int32_t* dn, int32_t* cu, int32_t* cd) const {
+    for (uint32_t h = 0; h < n_clusters; ++h) {
+      cu[h] = (up[h] >= 0 && dn[up[h]] == (int32_t)h) ? up[h] : -1;
+      cd[h] = (dn[h] >= 0 && up[dn[h]] == (int32_t)h) ? dn[h] : -1;
+    }
+  }
+
+  // SPEC 5.3 SEARCH (H1..H6): gid of the best cluster of (task,row) or -1
+  int64_t search(const State<R>& st, uint32_t task, int row) {
+    const RowGrid<R>& G = grids[(size_t)task * T.n_rows + row];
+    const R y = st.p[0], z = st.p[1];
+    const R ey = st.c[0] + T.sy2, ez = st.c[2] + T.sz2;                                  // H1
+    const R hy2 = rmin(R(T.prm.accept_k2) * ey, T.smax2);                                // H2
+    const R hz2 = rmin(R(T.prm.accept_k2) * ez, T.smax2);
+    const R wy_ = rsqrt_(rmax(hy2, R(0))) + R(GRID_MARGIN), wz_ = rsqrt_(rmax(hz2, R(0))) + R(GRID_MARGIN);
+    bool have = false;
+    R best = 0; uint32_t bg = 0;
+    for_window(G, y - wy_, y + wy_, z - wz_, z + wz_, [&](uint32_t c) {
+      cnt[CN_CANDIDATES]++;
+      const R dy = Y[c] - y, dz = Z[c] - z;                                              // H3
+      const R dy2 = dy * dy, dz2 = dz * dz;
+      if (!(dy2 <= hy2 && dz2 <= hz2)) return;                                           // H4
+      const R d = (dy2 * ez) + (dz2 * ey);                                               // H5
+      if (!have || d < best || (d == best && c < bg)) { have = true; best = d; bg = c; }  // H6
+    });
+    return have ? (int64_t)bg : -1;
+  }
+
+  void apply_hit(State<R>& st, uint32_t h) {
+    update(st, 0, Y[h], T.sy2);
+    update(st, 1, Z[h], T.sz2);
+  }
+
+  struct Tracklet {
+    uint32_t h0;
+    uint32_t task;
+    int first_row, last_row, n_hits;
+    State<R> st;
+    std::vector<int64_t> map;  // [n_rows] gid or -1
+  };
+
+  // ---- SPEC 6: tracklet constructor (K1..K6). Returns false if chain too short (S3). ----
+  bool construct(uint32_t h0, uint32_t task, int r0, const int32_t* cu, Tracklet& tk) {
+    const int nr = T.n_rows;
+    // S2/S3 chain length
+    int len = 1;
+    for (int32_t h = cu[h0]; h >= 0; h = cu[h]) ++len;
+    if (len < T.prm.min_seed_hits) return false;
+    cnt[CN_TRACKLETS_BUILT]++;
+    cnt[CN_CHAIN_HITS] += len;
+    tk.h0 = h0; tk.task = task;
+    tk.map.assign(nr, -1);
+    State<R>& st = tk.st;
+    const uint32_t h1 = (uint32_t)cu[h0];
+    {  // K1
+      const R dx = T.X[r0 + 1] - T.X[r0], dy = Y[h1] - Y[h0], dz = Z[h1] - Z[h0];
+      const R ri = R(1) / rsqrt_(dx * dx + dy * dy);
+      st.x = T.X[r0 + 1];
+      st.p[0] = Y[h1]; st.p[1] = Z[h1]; st.p[2] = dy * ri; st.p[3] = dz * ri; st.p[4] = R(0);
+      for (int i = 0; i < 15; ++i) st.c[i] = R(0);
+      st.c[0] = T.sy2; st.c[2] = T.sz2; st.c[5] = R(T.prm.c0_sinphi); st.c[9] = R(T.prm.c0_dzds);
+      st.c[14] = R(T.prm.c0_qpt);
+      st.chi2 = R(0); st.ndf = -5;
+    }
+    tk.map[r0] = h0; tk.map[r0 + 1] = h1;
+    tk.first_row = r0; tk.last_row = r0 + 1; tk.n_hits = 2;
+    bool chain_ok = true;
+    {  // K2
+      int r = r0 + 2;
+      for (int32_t h = cu[h1]; h >= 0; h = cu[h], ++r) {
+        cnt[CN_ROW_STEPS]++;
+        if (!transport(st, T.X[r], T.a, R(T.prm.max_sinphi))) { chain_ok = false; break; }
+        apply_hit(st, (uint32_t)h);
+        tk.map[r] = h; tk.last_row = r; tk.n_hits++;
+      }
+    }
+    if (chain_ok) {  // K3
+      int gap = 0;
+      for (int r = tk.last_row + 1; r < nr; ++r) {
+        cnt[CN_ROW_STEPS]++;
+        if (!transport(st, T.X[r], T.a, R(T.prm.max_sinphi))) break;
+        cnt[CN_SEARCH_UP]++;
+        const int64_t h = search(st, task, r);
+        if (h >= 0) { apply_hit(st, (uint32_t)h); tk.map[r] = h; tk.last_row = r; tk.n_hits++; gap = 0; }
+        else if (++gap > T.prm.max_row_gap) break;
+      }
+    }
+    {  // K4
+      if (st.x != T.X[tk.last_row]) transport(st, T.X[tk.last_row], T.a, R(T.prm.max_sinphi));
+      for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);
+      st.chi2 = R(0); st.ndf = -5;
+    }
+    {  // K5
+      int gap = 0;
+      for (int r = tk.last_row - 1; r >= 0; --r) {
+        cnt[CN_ROW_STEPS]++;
+        if (!transport(st, T.X[r], T.a, R(T.prm.max_sinphi))) break;
+        if (tk.map[r] >= 0) { apply_hit(st, (uint32_t)tk.map[r]); continue; }
+        cnt[CN_SEARCH_DN]++;
+        const int64_t h = search(st, task, r);
+        if (h >= 0) {
+          apply_hit(st, (uint32_t)h); tk.map[r] = h; tk.n_hits++;
+          if (r < tk.first_row) { tk.first_row = r; gap = 0; }
+        } else if (r < tk.first_row) {
+          if (++gap > T.prm.max_row_gap) break;
+        }
+      }
+    }
+    if (st.x != T.X[tk.first_row]) transport(st, T.X[tk.first_row], T.a, R(T.prm.max_sinphi));  // K6
+    return true;
+  }
+};
+
+struct OTrackOut {  // caller-allocated outputs (any pointer may be NULL)
+  int32_t *link_up, *link_dn, *clean_up, *clean_dn;   // [n_clusters]
+  uint32_t* start_hits;                               // [n_clusters]
+  uint32_t track_capacity, hit_capacity;
+  uint32_t *track_task, *track_hit_begin, *track_nhits;
+  int32_t* track_ndf;
+  void *track_x, *track_par, *track_cov, *track_chi2;  // R* ; par [5][cap], cov [15][cap]
+  uint32_t* hit_cluster;
+  // optional tracklet dump (before selection), capacity = tracklet_capacity
+  uint32_t tracklet_capacity;
+  uint32_t *tracklet_start, *tracklet_nhits;
+  int32_t* tracklet_map;  // [cap][n_rows]
+  void* tracklet_par;     // [cap][5]
+  uint64_t* counters;     // [CN_COUNT]
+  uint32_t n_start_hits, n_tracklets, n_tracks, n_hits;  // results
+};
+
+template <class R>
+int run(const OGeometry* g, float bz, const OParams* p, uint32_t n, uint32_t nt, const R* y, const R* z,
+        const uint32_t* ro, OTrackOut* o, int use_grid_nf) {
+  Tables<R> T(*g, bz, *p);
+  Oracle<R> O(T, y, z, ro, n, nt);
+  const int nr = T.n_rows;
+  O.build_grids();
+  std::vector<int32_t> up(n), dn(n), cu(n), cd(n);
+  O.neighbours(up.data(), dn.data(), use_grid_nf != 0);
+  O.clean(up.data(), dn.data(), cu.data(), cd.data());
+  if (o->link_up) std::memcpy(o->link_up, up.data(), n * 4);
+  if (o->link_dn) std::memcpy(o->link_dn, dn.data(), n * 4);
+  if (o->clean_up) std::memcpy(o->clean_up, cu.data(), n * 4);
+  if (o->clean_dn) std::memcpy(o->clean_dn, cd.data(), n * 4);
+  // S1 start hits, ascending gid
+  std::vector<uint32_t> starts;
+  for (uint32_t h = 0; h < n; ++h)
+    if (cu[h] >= 0 && cd[h] < 0) starts.push_back(h);
+  O.cnt[CN_START_HITS] = starts.size();
+  o->n_start_hits = (uint32_t)starts.size();
+  if (o->start_hits) std::memcpy(o->start_hits, starts.data(), starts.size() * 4);
+  // task,row of a gid
+  std::vector<uint32_t> tr_of(n);
+  for (size_t tr = 0; tr < (size_t)nt * nr; ++tr)
+    for (uint32_t h = ro[tr]; h < ro[tr + 1]; ++h) tr_of[h] = (uint32_t)tr;
+  // K1..K7
+  std::vector<typename Oracle<R>::Tracklet> kept;
+  std::vector<uint64_t> owner(n, 0), keys;
+  uint32_t n_tracklets = 0;
+  for (uint32_t h0 : starts) {
+    typename Oracle<R>::Tracklet tk;
+    const uint32_t tr = tr_of[h0];
+    if (!O.construct(h0, tr / nr, (int)(tr % nr), cu.data(), tk)) continue;
+    if (n_tracklets < o->tracklet_capacity) {
+      const uint32_t i = n_tracklets;
+      if (o->tracklet_start) o->tracklet_start[i] = h0;
+      if (o->tracklet_nhits) o->tracklet_nhits[i] = tk.n_hits;
+      if (o->tracklet_map) for (int r = 0; r < nr; ++r) o->tracklet_map[(size_t)i * nr + r] = (int32_t)tk.map[r];
+      if (o->tracklet_par) for (int j = 0; j < 5; ++j) ((R*)o->tracklet_par)[(size_t)i * 5 + j] = tk.st.p[j];
+    }
+    ++n_tracklets;
+    if (tk.n_hits < p->min_track_hits) continue;                                         // K6
+    O.cnt[CN_TRACKLETS_KEPT]++;
+    O.cnt[CN_TRACKLET_HITS] += tk.n_hits;
+    const uint64_t key = ((uint64_t)tk.n_hits << 32) | (uint64_t)(0xFFFFFFFFu - h0);     // K7
+    for (int r = 0; r < nr; ++r)
+      if (tk.map[r] >= 0) owner[tk.map[r]] = std::max(owner[tk.map[r]], key);
+    keys.push_back(key);
+    kept.push_back(std::move(tk));
+  }
+  o->n_tracklets = n_tracklets;
+  // L1..L3
+  uint32_t n_tracks = 0, n_hits = 0;
+  int status = 0;
+  for (size_t i = 0; i < kept.size(); ++i) {
+    const auto& tk = kept[i];
+    std::vector<uint32_t> hits;
+    for (int r = 0; r < nr; ++r)
+      if (tk.map[r] >= 0 && owner[tk.map[r]] == keys[i]) hits.push_back((uint32_t)tk.map[r]);
+    if ((int)hits.size() < p->min_track_hits) continue;
+    if (n_tracks >= o->track_capacity || n_hits + hits.size() > o->hit_capacity) { status = 1; break; }
+    const uint32_t t = n_tracks++;
+    const uint32_t cap = o->track_capacity;
+    if (o->track_task) o->track_task[t] = tk.task;
+    if (o->track_hit_begin) o->track_hit_begin[t] = n_hits;
+    if (o->track_nhits) o->track_nhits[t] = (uint32_t)hits.size();
+    if (o->track_ndf) o->track_ndf[t] = tk.st.ndf;
+    if (o->track_x) ((R*)o->track_x)[t] = tk.st.x;
+    if (o->track_chi2) ((R*)o->track_chi2)[t] = tk.st.chi2;
+    if (o->track_par) for (int j = 0; j < 5; ++j) ((R*)o->track_par)[(size_t)j * cap + t] = tk.st.p[j];
+    if (o->track_cov) for (int j = 0; j < 15; ++j) ((R*)o->track_cov)[(size_t)j * cap + t] = tk.st.c[j];
+    if (o->hit_cluster) for (uint32_t h : hits) o->hit_cluster[n_hits++] = h; else n_hits += hits.size();
+  }
+  O.cnt[CN_OUT_TRACKS] = n_tracks;
+  O.cnt[CN_OUT_HITS] = n_hits;
+  o->n_tracks = n_tracks;
+  o->n_hits = n_hits;
+  if (o->counters) std::memcpy(o->counters, O.cnt, sizeof(O.cnt));
+  return status;
+}
+
+}  // namespace
+
+extern "C" {
+
+int oracle_n_counters() { return CN_COUNT; }
+size_t oracle_sizeof_out() { return sizeof(OTrackOut); }
+
+int oracle_track_f32(const OGeometry* g, float bz, const OParams* p, uint32_t n, uint32_t nt, const float* y,
+                     const float* z, const uint32_t* ro, OTrackOut* o, int use_grid_nf) {
+  return run<float>(g, bz, p, n, nt, y, z, ro, o, use_grid_nf);
+}
+int oracle_track_f64(const OGeometry* g, float bz, const OParams* p, uint32_t n, uint32_t nt, const double* y,
+                     const double* z, const uint32_t* ro, OTrackOut* o, int use_grid_nf) {
+  return run<double>(g, bz, p, n, nt, y, z, ro, o, use_grid_nf);
+}
+
+// --- unit entry points for the pins -----------------------------------------
+// state layout: x, p[5], c[15], chi2  (22 reals) ; ndf separately
+int oracle_transport_f64(double* s22, double xnew, double a, double max_sinphi) {
+  State<double> st; st.x = s22[0];
+  for (int i = 0; i < 5; ++i) st.p[i] = s22[1 + i];
+  for (int i = 0; i < 15; ++i) st.c[i] = s22[6 + i];
+  st.chi2 = s22[21]; st.ndf = 0;
+  const bool ok = transport(st, xnew, a, max_sinphi);
+  s22[0] = st.x;
+  for (int i = 0; i < 5; ++i) s22[1 + i] = st.p[i];
+  for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
+  return ok ? 1 : 0;
+}
+int oracle_transport_f32(float* s22, float xnew, float a, float max_sinphi) {
+  State<float> st; st.x = s22[0];
+  for (int i = 0; i < 5; ++i) st.p[i] = s22[1 + i];
+  for (int i = 0; i < 15; ++i) st.c[i] = s22[6 + i];
+  st.chi2 = s22[21]; st.ndf = 0;
+  const bool ok = transport(st, xnew, a, max_sinphi);
+  s22[0] = st.x;
+  for (int i = 0; i < 5; ++i) s22[1 + i] = st.p[i];
+  for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
+  return ok ? 1 : 0;
+}
+void oracle_update_f64(double* s22, int32_t* ndf, int i, double m, double e) {
+  State<double> st; st.x = s22[0];
+  for (int j = 0; j < 5; ++j) st.p[j] = s22[1 + j];
+  for (int j = 0; j < 15; ++j) st.c[j] = s22[6 + j];
+  st.chi2 = s22[21]; st.ndf = *ndf;
+  update(st, i, m, e);
+  for (int j = 0; j < 5; ++j) s22[1 + j] = st.p[j];
+  for (int j = 0; j < 15; ++j) s22[6 + j] = st.c[j];
+  s22[21] = st.chi2; *ndf = st.ndf;
+}
+void oracle_update_f32(float* s22, int32_t* ndf, int i, float m, float e) {
+  State<float> st; st.x = s22[0];
+  for (int j = 0; j < 5; ++j) st.p[j] = s22[1 + j];
+  for (int j = 0; j < 15; ++j) st.c[j] = s22[6 + j];
+  st.chi2 = s22[21]; st.ndf = *ndf;
+  update(st, i, m, e);
+  for (int j = 0; j < 5; ++j) s22[1 + j] = st.p[j];
+  for (int j = 0; j < 15; ++j) s22[6 + j] = st.c[j];
+  s22[21] = st.chi2; *ndf = st.ndf;
+}
+
+}  // extern "C"
