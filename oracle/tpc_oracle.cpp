@@ -378,6 +378,8 @@ template <class R> struct Oracle {
       if (st.x != T.X[tk.last_row]) transport(st, T.X[tk.last_row], T.a, R(T.prm.max_sinphi));
       for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);
       st.chi2 = R(0); st.ndf = -5;
+      // the hit of lastRow opens the down pass, so that the final fit uses every hit of the map
+      if (st.x == T.X[tk.last_row]) apply_hit(st, (uint32_t)tk.map[tk.last_row]);
     }
     {  // K5
       int gap = 0;

@@ -199,6 +199,37 @@ def _crossings(geom: Geometry, pt, charge, phi0, eta, z0):
     return {n: (np.concatenate(a) if a else np.zeros(0)) for n, a in out.items()}, n_trk
 
 
+def _crossings_straight(geom: Geometry, pt, charge, phi0, eta, z0):
+    """Bz = 0: straight lines from (0, 0, z0); same output as ``_crossings`` (leg 0 only)."""
+    X = geom.row_x.astype(np.float64)
+    tan_h = np.tan(np.deg2rad(10.0))
+    t = np.sinh(eta)
+    if not geom.two_sided:
+        t = np.abs(t)
+    out = {n: [] for n in ("trk", "sec", "row", "leg", "y", "z", "s", "sin", "t", "q")}
+    rows = np.arange(geom.n_rows)
+    for i in range(pt.shape[0]):
+        for k in range(geom.n_phi):
+            d = np.mod(phi0[i] - (k + 0.5) * SECTOR_PITCH + np.pi, 2.0 * np.pi) - np.pi
+            if abs(d) >= 0.5 * np.pi:
+                continue
+            yl = X * np.tan(d)
+            s_xy = X / np.cos(d)
+            zz = z0[i] + t[i] * s_xy
+            ok = (np.abs(yl) <= X * tan_h) & (np.abs(zz) <= geom.z_max) & (zz != 0.0) & (s_xy < R_OUT)
+            if not geom.two_sided:
+                ok &= zz > 0.0
+            ri_ = np.nonzero(ok)[0]
+            side = (zz[ri_] < 0.0).astype(np.int64) if geom.two_sided else 0
+            n = ri_.shape[0]
+            out["trk"].append(np.full(n, i)); out["sec"].append(k + side * geom.n_phi)
+            out["row"].append(rows[ri_]); out["leg"].append(np.zeros(n, np.int8))
+            out["y"].append(yl[ri_]); out["z"].append(zz[ri_]); out["s"].append(s_xy[ri_])
+            out["sin"].append(np.full(n, np.sin(d))); out["t"].append(np.full(n, t[i]))
+            out["q"].append(np.full(n, charge[i] / pt[i]))
+    return {n: (np.concatenate([np.atleast_1d(v) for v in a]) if a else np.zeros(0)) for n, a in out.items()}, pt.shape[0]
+
+
 def _moyal_charge(rng, n, mpv=50.0, width=10.0):
     """Moyal(mpv, width) stand-in for a Landau: x = mpv - width*ln(Z^2)."""
     zn = rng.standard_normal(n)
@@ -216,7 +247,10 @@ def generate_tracks_event(geom: Geometry, pt, charge, phi0, eta, z0,
     phi0 = np.asarray(phi0, np.float64)
     eta = np.asarray(eta, np.float64)
     z0 = np.asarray(z0, np.float64)
-    cr, _ = _crossings(geom, pt, charge, phi0, eta, z0)
+    if geom.bz_kgauss == 0.0:
+        cr, _ = _crossings_straight(geom, pt, charge, phi0, eta, z0)
+    else:
+        cr, _ = _crossings(geom, pt, charge, phi0, eta, z0)
     n_rows = geom.n_rows
     n_sr = geom.n_sectors * n_rows
     sr = cr["sec"].astype(np.int64) * n_rows + cr["row"].astype(np.int64)
