@@ -1,0 +1,191 @@
+/* ===========================================================================
+ * tpc_tracker.h  --  C ABI of the B200 (sm_100a) TPC sector tracker
+ * ===========================================================================
+ * The data-parallel hot path of the ALICE HLT TPC track finder of
+ * arXiv:1712.09434 section 3 ("Cellular Automaton principle to
+ * build track seeds ... Afterwards, it uses the Kalman filter for track fitting
+ * and track following"; L123: cluster-wise CA phase, track-wise following phase;
+ * L138: sectors processed individually and concurrently; L127: several events
+ * concurrently on one GPU; L182: 159 pad rows; L213: clusters are identified by
+ * their index).  The paper prints no formula: the arithmetic of every stage is
+ * the numbered fp32 sequence of docs/ARITH_SPEC.md (cited below as SPEC n).
+ *
+ * Stages run by tpc_track_batch, one launch each for the WHOLE batch
+ * (SURVEY.md section 8(a), rows a1..a8):
+ *   a1 grid build (SPEC 2)           a2 neighbour finder (SPEC 3)
+ *   a3 neighbour cleaner (SPEC 4)    a4 start-hit finder (SPEC 4, S1-S3)
+ *   a5 tracklet constructor (SPEC 5, 6)
+ *   a6 tracklet selector + a7 output compaction (SPEC 7)
+ *   a8 batching: task = event * n_sectors + sector, all tasks in one call.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  Every pointer says HOST or DEVICE.
+ *   - Ownership: every buffer passed in is caller-owned.  The library allocates
+ *     device memory only in tpc_tracker_create (geometry tables, < 8 KB) and
+ *     frees it in tpc_tracker_destroy.  Inputs are never written.
+ *   - tpc_track_batch only ENQUEUES work on `cuda_stream` (a cudaStream_t cast
+ *     to void*; NULL = the legacy default stream).  It never synchronises and
+ *     never allocates.  Results are valid once the caller has synchronised the
+ *     stream.  tpc_track_batch_host is the synchronous variant on host buffers.
+ *   - Errors: 0 = ok, TPC_ERR_* < 0 otherwise, text in tpc_last_error().
+ *     Data-dependent overflow (too many tracklets / tracks / hits for the
+ *     capacities given) never writes out of bounds: it sets bits in header[2]
+ *     and drops the items that do not fit, deterministically.
+ *   - There is no CPU fallback: without a CUDA device every compute entry
+ *     point fails with TPC_ERR_CUDA.
+ * ===========================================================================*/
+#ifndef TPC_TRACKER_H_
+#define TPC_TRACKER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPC_OK 0
+#define TPC_ERR_ARGUMENT (-1)  /* NULL / inconsistent argument                     */
+#define TPC_ERR_WORKSPACE (-2) /* workspace smaller than tpc_workspace_bytes says  */
+#define TPC_ERR_CUDA (-3)      /* CUDA runtime error (no device, launch failure)   */
+
+/* bits of header[2] (status), set on the device */
+#define TPC_STATUS_TRACKLET_OVERFLOW 1u /* more tracklets than max_tracklets: the surplus was not built */
+#define TPC_STATUS_TRACK_OVERFLOW 2u    /* more tracks than track_capacity: the surplus was not written */
+#define TPC_STATUS_HIT_OVERFLOW 4u      /* more hits than hit_capacity: tracks that do not fit dropped  */
+
+/* Detector geometry (SPEC 1).  HOST memory; copied by tpc_tracker_create. */
+typedef struct {
+  int32_t n_sectors;    /* sector s = task % n_sectors; A side (z >= 0) iff 2*s < n_sectors */
+  int32_t n_rows;       /* pad rows per sector (159), 3 <= n_rows <= 1024    */
+  const float* row_x;   /* HOST [n_rows]: local x of every row, strictly increasing, > 0    */
+  float tan_half_angle; /* row r spans |y| <= row_x[r]*tan_half_angle (+1 cm margin, T1)    */
+  float z_max;          /* drift length; row z extent is [-1, z_max+1] (A) or mirrored (C)  */
+} tpc_geometry;
+
+/* Parameters (SPEC 8).  HOST memory; NULL in tpc_tracker_create = the defaults of SPEC 8. */
+typedef struct {
+  float sigma_y, sigma_z;           /* cluster errors [cm] (T7)                                 */
+  float nf_hy, nf_hz, nf_chi2_max;  /* neighbour finder window and cut (N2, N3, N5)             */
+  float grid_bin_min, grid_bin_max; /* grid bin size clamp [cm]; acceleration only (SPEC 2)     */
+  float max_sinphi;                 /* transport fails beyond it (P4)                           */
+  float c0_sinphi, c0_dzds, c0_qpt; /* seed covariance diagonal (K1)                            */
+  float accept_k2, search_max;      /* pick-up window (H2)                                      */
+  float turn_cov_scale;             /* covariance inflation at the turn-around (K4)             */
+  int32_t min_seed_hits;            /* S3                                                       */
+  int32_t max_row_gap;              /* K3, K5                                                   */
+  int32_t min_track_hits;           /* K6, L2                                                   */
+} tpc_params;
+
+/* Input clusters.  Arrays are DEVICE memory for tpc_track_batch and HOST
+ * memory for tpc_track_batch_host.  Clusters are sorted by (task, row); the
+ * index of a cluster in these arrays is its identity (gid).
+ * x and charge are accepted and NOT read (the tracker uses
+ * row_x[row]; R23: nothing in the method uses the charge); they may be NULL. */
+typedef struct {
+  const float* x;              /* [n_clusters] or NULL                                         */
+  const float* y;              /* [n_clusters] local y [cm], finite                            */
+  const float* z;              /* [n_clusters] z [cm], finite                                  */
+  const uint16_t* charge;      /* [n_clusters] or NULL                                         */
+  const uint32_t* row_offsets; /* [n_tasks*n_rows + 1], non-decreasing, [0] = 0, last = n_clusters */
+  uint32_t n_clusters;         /* < 2^31                                                       */
+  uint32_t n_tasks;            /* task = event*n_sectors + sector                              */
+} tpc_clusters;
+
+/* Outputs.  Arrays are DEVICE memory for tpc_track_batch and HOST memory for
+ * tpc_track_batch_host.  Track t (0 <= t < header[0]) has its hits in
+ * hit_cluster[track_hit_begin[t] .. + track_nhits[t]) as cluster gids in
+ * ascending row order (L3).  Track order is deterministic run to run and
+ * otherwise unspecified (L4).  Parameters are the state (y, z, sinphi, dz/dl,
+ * q/pT) at x = track_x (the first row of the tracklet), covariance as 15
+ * lower-triangular entries c00 c10 c11 c20 ... c44 (SPEC 5).
+ * track_par is [5][track_capacity], track_cov is [15][track_capacity].
+ * Every dbg_* pointer may be NULL; non-NULL ones are filled by extra untimed
+ * kernels: links / cleaned links as gids indexed by gid (-1 = none), start
+ * hits (S1) as an UNORDERED gid list, tracklets (before selection, K1-K6) in
+ * tracklet order. */
+typedef struct {
+  uint32_t track_capacity, hit_capacity;
+  uint32_t* header; /* [4]: n_tracks, n_hits, status bits, n_tracklets built.  On overflow [0],[1] hold
+                       the totals that WOULD have been written; a track t < track_capacity is valid iff
+                       track_hit_begin[t] + track_nhits[t] <= hit_capacity.                            */
+  uint32_t* track_task;
+  uint32_t* track_hit_begin;
+  uint32_t* track_nhits;
+  int32_t* track_ndf;
+  float* track_x;
+  float* track_par;
+  float* track_cov;
+  float* track_chi2;
+  uint32_t* hit_cluster;
+  int32_t *dbg_link_up, *dbg_link_dn, *dbg_clean_up, *dbg_clean_dn; /* [n_clusters] each */
+  uint32_t* dbg_start_hits;   /* [n_clusters]                                             */
+  uint32_t* dbg_n_start_hits; /* [1]                                                      */
+  uint32_t dbg_tracklet_capacity;
+  uint32_t* dbg_tracklet_start; /* [cap] gid of the start hit                             */
+  uint32_t* dbg_tracklet_nhits; /* [cap]                                                  */
+  int32_t* dbg_tracklet_map;    /* [cap][n_rows] gid or -1                                */
+  float* dbg_tracklet_par;      /* [cap][5]                                               */
+} tpc_tracks;
+
+typedef struct tpc_tracker tpc_tracker;
+
+/* Builds the fp32 tables T1..T8 of SPEC 1 on the host in the order written
+ * there and uploads them.  geometry and params are HOST pointers (params may be
+ * NULL).  bz_kgauss: solenoid field in kG (0.5 T = 5).  *out receives the handle. */
+int tpc_tracker_create(const tpc_geometry* geometry, float bz_kgauss, const tpc_params* params,
+                       tpc_tracker** out);
+void tpc_tracker_destroy(tpc_tracker* tracker);
+
+/* The defaults of SPEC 8 (HOST pointer out). */
+void tpc_default_params(tpc_params* out);
+
+/* Bytes of DEVICE workspace tpc_track_batch needs for inputs of at most
+ * max_clusters clusters in max_tasks tasks.  max_tracklets bounds the number of
+ * tracklets built (a5); 0 = the worst case max_clusters / min_seed_hits (chains
+ * are vertex disjoint, S2).  The tracklet row maps dominate:
+ * 4 * n_rows * max_tracklets bytes. */
+size_t tpc_workspace_bytes(const tpc_tracker* tracker, uint32_t max_clusters, uint32_t max_tasks,
+                           uint32_t max_tracklets);
+
+/* Runs a1..a8 on DEVICE buffers, asynchronously on cuda_stream.  workspace is
+ * DEVICE memory of at least tpc_workspace_bytes(tracker, n_clusters, n_tasks,
+ * max_tracklets) bytes, 256-byte aligned, contents undefined before and after.
+ * The same tracker may be used from one stream at a time. */
+int tpc_track_batch(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_tracks* tracks, void* workspace,
+                    size_t workspace_bytes, uint32_t max_tracklets, void* cuda_stream);
+
+/* Same on HOST buffers (pinned memory recommended): copies y, z, row_offsets to
+ * the device, runs a1..a8, copies the header and the used part of every
+ * non-NULL output back, and synchronises.  workspace is DEVICE memory of at
+ * least tpc_host_workspace_bytes(...).  dbg_* pointers must be NULL.
+ * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied. */
+size_t tpc_host_workspace_bytes(const tpc_tracker* tracker, uint32_t max_clusters, uint32_t max_tasks,
+                                uint32_t max_tracklets, uint32_t track_capacity, uint32_t hit_capacity);
+int tpc_track_batch_host(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_tracks* tracks,
+                         void* workspace, size_t workspace_bytes, uint32_t max_tracklets, void* cuda_stream,
+                         uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
+/* Per-stage device counters of the LAST tpc_track_batch call on this tracker
+ * (HOST pointer out, [TPC_N_COUNTERS] uint64; synchronises the stream given).
+ * Only filled when the tracker was created with counters enabled through
+ * tpc_tracker_enable_counters(tracker, 1) - counting costs atomics, so timed
+ * runs leave it off. */
+#define TPC_N_COUNTERS 12
+/* 0 clusters, 1 grid bins, 2 start hits (S1), 3 tracklets built (S3), 4 tracklets kept (K6),
+ * 5 chain hits fitted (K1, K2), 6 row searches (K3, K5), 7 candidates examined (H3),
+ * 8 hits of kept tracklets, 9 row steps (transports of K2, K3, K5), 10 neighbour pairs (N4), 11 unused */
+void tpc_tracker_enable_counters(tpc_tracker* tracker, int on);
+int tpc_read_counters(tpc_tracker* tracker, void* cuda_stream, uint64_t* out);
+
+/* Number of kernels one tpc_track_batch call launches (debug kernels excluded). */
+int tpc_launches_per_batch(const tpc_tracker* tracker);
+
+/* Text of the last error on this tracker (never NULL). With tracker == NULL: the
+ * last error of tpc_tracker_create on this thread. */
+const char* tpc_last_error(const tpc_tracker* tracker);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_TRACKER_H_ */

@@ -1,0 +1,309 @@
+"""ctypes binding of ``libtpc_tracker.so`` (include/tpc_tracker.h) - argument marshalling only.
+
+PyTorch is used for device memory and streams; nothing here computes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+from dataclasses import dataclass, fields
+from typing import Dict, List, Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(HERE, "libtpc_tracker.so")
+_HEADER = os.path.join(os.path.dirname(HERE), "include", "tpc_tracker.h")
+
+STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_HIT_OVERFLOW = 1, 2, 4
+COUNTER_NAMES = ["clusters", "bins", "start_hits", "tracklets_built", "tracklets_kept", "chain_hits", "searches",
+                 "candidates", "tracklet_hits", "row_steps", "nf_pairs", "unused"]
+
+
+class TpcError(RuntimeError):
+    pass
+
+
+class _Geometry(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.POINTER(C.c_float)),
+                ("tan_half_angle", C.c_float), ("z_max", C.c_float)]
+
+
+_PARAM_FLOATS = ("sigma_y", "sigma_z", "nf_hy", "nf_hz", "nf_chi2_max", "grid_bin_min", "grid_bin_max", "max_sinphi",
+                 "c0_sinphi", "c0_dzds", "c0_qpt", "accept_k2", "search_max", "turn_cov_scale")
+_PARAM_INTS = ("min_seed_hits", "max_row_gap", "min_track_hits")
+
+
+class _Params(C.Structure):
+    _fields_ = [(n, C.c_float) for n in _PARAM_FLOATS] + [(n, C.c_int32) for n in _PARAM_INTS]
+
+
+class _Clusters(C.Structure):
+    _fields_ = [("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p), ("charge", C.c_void_p),
+                ("row_offsets", C.c_void_p), ("n_clusters", C.c_uint32), ("n_tasks", C.c_uint32)]
+
+
+class _Tracks(C.Structure):
+    _fields_ = [("track_capacity", C.c_uint32), ("hit_capacity", C.c_uint32), ("header", C.c_void_p),
+                ("track_task", C.c_void_p), ("track_hit_begin", C.c_void_p), ("track_nhits", C.c_void_p),
+                ("track_ndf", C.c_void_p), ("track_x", C.c_void_p), ("track_par", C.c_void_p),
+                ("track_cov", C.c_void_p), ("track_chi2", C.c_void_p), ("hit_cluster", C.c_void_p),
+                ("dbg_link_up", C.c_void_p), ("dbg_link_dn", C.c_void_p), ("dbg_clean_up", C.c_void_p),
+                ("dbg_clean_dn", C.c_void_p), ("dbg_start_hits", C.c_void_p), ("dbg_n_start_hits", C.c_void_p),
+                ("dbg_tracklet_capacity", C.c_uint32), ("dbg_tracklet_start", C.c_void_p),
+                ("dbg_tracklet_nhits", C.c_void_p), ("dbg_tracklet_map", C.c_void_p),
+                ("dbg_tracklet_par", C.c_void_p)]
+
+
+@dataclass
+class TrackerParams:
+    """tpc_params; the defaults come from the library (tpc_default_params), not from here."""
+    sigma_y: Optional[float] = None
+    sigma_z: Optional[float] = None
+    nf_hy: Optional[float] = None
+    nf_hz: Optional[float] = None
+    nf_chi2_max: Optional[float] = None
+    grid_bin_min: Optional[float] = None
+    grid_bin_max: Optional[float] = None
+    max_sinphi: Optional[float] = None
+    c0_sinphi: Optional[float] = None
+    c0_dzds: Optional[float] = None
+    c0_qpt: Optional[float] = None
+    accept_k2: Optional[float] = None
+    search_max: Optional[float] = None
+    turn_cov_scale: Optional[float] = None
+    min_seed_hits: Optional[int] = None
+    max_row_gap: Optional[int] = None
+    min_track_hits: Optional[int] = None
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def exported_symbols() -> List[str]:
+    """Function names declared in include/tpc_tracker.h (parsed from the header text)."""
+    text = open(_HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(tpc_[a-z_]+)\s*\(", text)))
+
+
+_lib = None
+
+
+def load_library():
+    """Loads the in-tree extension; raises (never falls back) when it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise TpcError(f"{_LIB_PATH} is missing: run `python -m paper_1712_09434_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = C.CDLL(_LIB_PATH)
+    vp, u32, u64p = C.c_void_p, C.c_uint32, C.POINTER(C.c_uint64)
+    lib.tpc_tracker_create.restype = C.c_int
+    lib.tpc_tracker_create.argtypes = [C.POINTER(_Geometry), C.c_float, C.POINTER(_Params), C.POINTER(vp)]
+    lib.tpc_tracker_destroy.restype = None
+    lib.tpc_tracker_destroy.argtypes = [vp]
+    lib.tpc_default_params.restype = None
+    lib.tpc_default_params.argtypes = [C.POINTER(_Params)]
+    lib.tpc_workspace_bytes.restype = C.c_size_t
+    lib.tpc_workspace_bytes.argtypes = [vp, u32, u32, u32]
+    lib.tpc_host_workspace_bytes.restype = C.c_size_t
+    lib.tpc_host_workspace_bytes.argtypes = [vp, u32, u32, u32, u32, u32]
+    lib.tpc_track_batch.restype = C.c_int
+    lib.tpc_track_batch.argtypes = [vp, C.POINTER(_Clusters), C.POINTER(_Tracks), vp, C.c_size_t, u32, vp]
+    lib.tpc_track_batch_host.restype = C.c_int
+    lib.tpc_track_batch_host.argtypes = [vp, C.POINTER(_Clusters), C.POINTER(_Tracks), vp, C.c_size_t, u32, vp,
+                                         u64p, u64p]
+    lib.tpc_tracker_enable_counters.restype = None
+    lib.tpc_tracker_enable_counters.argtypes = [vp, C.c_int]
+    lib.tpc_read_counters.restype = C.c_int
+    lib.tpc_read_counters.argtypes = [vp, vp, u64p]
+    lib.tpc_launches_per_batch.restype = C.c_int
+    lib.tpc_launches_per_batch.argtypes = [vp]
+    lib.tpc_last_error.restype = C.c_char_p
+    lib.tpc_last_error.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+@dataclass
+class TrackResult:
+    """Device (or pinned host) tensors of one tpc_track_batch call; sizes are capacities."""
+    header: "object"
+    track_task: "object"
+    track_hit_begin: "object"
+    track_nhits: "object"
+    track_ndf: "object"
+    track_x: "object"
+    track_par: "object"   # [5, track_capacity]
+    track_cov: "object"   # [15, track_capacity]
+    track_chi2: "object"
+    hit_cluster: "object"
+    debug: Dict[str, "object"]
+
+    def to_numpy(self) -> Dict[str, np.ndarray]:
+        """Copies to host and trims to header counts (synchronises)."""
+        h = self.header.cpu().numpy().astype(np.int64)
+        nt, nh = int(min(h[0], self.track_task.shape[0])), int(min(h[1], self.hit_cluster.shape[0]))
+        out = {"n_tracks": int(h[0]), "n_hits": int(h[1]), "status": int(h[2]), "n_tracklets": int(h[3])}
+        for f in ("track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_chi2"):
+            out[f] = getattr(self, f)[:nt].cpu().numpy()
+        out["track_par"] = self.track_par[:, :nt].cpu().numpy()
+        out["track_cov"] = self.track_cov[:, :nt].cpu().numpy()
+        out["hit_cluster"] = self.hit_cluster[:nh].cpu().numpy()
+        for k, v in self.debug.items():
+            out[k] = v.cpu().numpy()
+        return out
+
+
+class Tracker:
+    """Owns one ``tpc_tracker`` handle.  ``geometry``: object with n_sectors, n_rows, row_x (fp32),
+    tan_half_angle, z_max, bz_kgauss (e.g. tpc_workload.Geometry)."""
+
+    def __init__(self, geometry, params: Optional[TrackerParams] = None, bz_kgauss: Optional[float] = None):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        self.n_rows = int(geometry.n_rows)
+        self.n_sectors = int(geometry.n_sectors)
+        row_x = np.ascontiguousarray(geometry.row_x, dtype=np.float32)
+        g = _Geometry(self.n_sectors, self.n_rows, row_x.ctypes.data_as(C.POINTER(C.c_float)),
+                      float(geometry.tan_half_angle), float(geometry.z_max))
+        p = _Params()
+        self._lib.tpc_default_params(C.byref(p))
+        if params is not None:
+            for f in fields(params):
+                v = getattr(params, f.name)
+                if v is not None:
+                    setattr(p, f.name, v)
+        self.params = {n: getattr(p, n) for n, _ in _Params._fields_}
+        bz = float(geometry.bz_kgauss if bz_kgauss is None else bz_kgauss)
+        rc = self._lib.tpc_tracker_create(C.byref(g), bz, C.byref(p), C.byref(self._h))
+        if rc != 0:
+            raise TpcError(f"tpc_tracker_create failed ({rc}): {self._lib.tpc_last_error(None).decode()}")
+        self._ws = None
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.tpc_tracker_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise TpcError(f"{what} failed ({rc}): {self._lib.tpc_last_error(self._h).decode()}")
+
+    # ---- sizes ------------------------------------------------------------
+    def workspace_bytes(self, max_clusters: int, max_tasks: int, max_tracklets: int = 0) -> int:
+        return int(self._lib.tpc_workspace_bytes(self._h, max_clusters, max_tasks, max_tracklets))
+
+    def host_workspace_bytes(self, max_clusters, max_tasks, max_tracklets, track_capacity, hit_capacity) -> int:
+        return int(self._lib.tpc_host_workspace_bytes(self._h, max_clusters, max_tasks, max_tracklets,
+                                                      track_capacity, hit_capacity))
+
+    def launches_per_batch(self) -> int:
+        return int(self._lib.tpc_launches_per_batch(self._h))
+
+    def enable_counters(self, on: bool):
+        self._lib.tpc_tracker_enable_counters(self._h, 1 if on else 0)
+
+    def read_counters(self, stream=None) -> Dict[str, int]:
+        buf = (C.c_uint64 * len(COUNTER_NAMES))()
+        self._check(self._lib.tpc_read_counters(self._h, _stream_ptr(stream), buf), "tpc_read_counters")
+        return {n: int(v) for n, v in zip(COUNTER_NAMES, buf)}
+
+    # ---- allocation helpers (torch = device memory only) ---------------------
+    def alloc_outputs(self, n_clusters: int, device, track_capacity: Optional[int] = None,
+                      hit_capacity: Optional[int] = None, debug: bool = False, debug_tracklets: int = 0,
+                      pinned_host: bool = False) -> TrackResult:
+        import torch
+        tcap = int(track_capacity if track_capacity is not None else n_clusters // max(self.params["min_track_hits"], 1) + 1)
+        hcap = int(hit_capacity if hit_capacity is not None else n_clusters + 1)
+        kw = dict(device="cpu", pin_memory=True) if pinned_host else dict(device=device)
+        e = lambda shape, dt: torch.empty(shape, dtype=dt, **kw)  # noqa: E731
+        dbg = {}
+        if debug:
+            for k in ("dbg_link_up", "dbg_link_dn", "dbg_clean_up", "dbg_clean_dn"):
+                dbg[k] = e(max(n_clusters, 1), torch.int32)
+            dbg["dbg_start_hits"] = e(max(n_clusters, 1), torch.int32)
+            dbg["dbg_n_start_hits"] = e(1, torch.int32)
+        if debug_tracklets:
+            dbg["dbg_tracklet_start"] = e(debug_tracklets, torch.int32)
+            dbg["dbg_tracklet_nhits"] = e(debug_tracklets, torch.int32)
+            dbg["dbg_tracklet_map"] = e((debug_tracklets, self.n_rows), torch.int32)
+            dbg["dbg_tracklet_par"] = e((debug_tracklets, 5), torch.float32)
+        return TrackResult(
+            header=e(4, torch.int32), track_task=e(tcap, torch.int32), track_hit_begin=e(tcap, torch.int32),
+            track_nhits=e(tcap, torch.int32), track_ndf=e(tcap, torch.int32), track_x=e(tcap, torch.float32),
+            track_par=e((5, tcap), torch.float32), track_cov=e((15, tcap), torch.float32),
+            track_chi2=e(tcap, torch.float32), hit_cluster=e(hcap, torch.int32), debug=dbg)
+
+    def alloc_workspace(self, nbytes: int, device):
+        import torch
+        return torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+
+    @staticmethod
+    def _aligned(ws):
+        p = ws.data_ptr()
+        off = (-p) % 256
+        return p + off, ws.numel() - off
+
+    def _tracks_struct(self, out: TrackResult) -> _Tracks:
+        t = _Tracks()
+        t.track_capacity = int(out.track_task.shape[0])
+        t.hit_capacity = int(out.hit_cluster.shape[0])
+        for f in ("header", "track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_par",
+                  "track_cov", "track_chi2", "hit_cluster"):
+            setattr(t, f, getattr(out, f).data_ptr())
+        for k, v in out.debug.items():
+            setattr(t, k, v.data_ptr())
+        if "dbg_tracklet_start" in out.debug:
+            t.dbg_tracklet_capacity = int(out.debug["dbg_tracklet_start"].shape[0])
+        return t
+
+    # ---- the two compute entry points ---------------------------------------
+    def track_batch(self, y, z, row_offsets, n_tasks: int, out: TrackResult, workspace, max_tracklets: int = 0,
+                    stream=None, x=None, charge=None) -> TrackResult:
+        """tpc_track_batch on DEVICE tensors (y, z fp32; row_offsets int32/uint32 viewed as uint32).
+        Asynchronous on ``stream`` (a torch.cuda.Stream; default: the current stream)."""
+        import torch
+        if not (y.is_cuda and z.is_cuda and row_offsets.is_cuda):
+            raise TpcError("track_batch needs CUDA tensors; there is no CPU path")
+        assert y.dtype == torch.float32 and z.dtype == torch.float32 and row_offsets.dtype == torch.int32
+        assert y.is_contiguous() and z.is_contiguous() and row_offsets.is_contiguous()
+        assert row_offsets.numel() == n_tasks * self.n_rows + 1
+        cl = _Clusters(x.data_ptr() if x is not None else None, y.data_ptr(), z.data_ptr(),
+                       charge.data_ptr() if charge is not None else None, row_offsets.data_ptr(),
+                       int(y.numel()), int(n_tasks))
+        tr = self._tracks_struct(out)
+        wp, wn = self._aligned(workspace)
+        s = stream if stream is not None else torch.cuda.current_stream(y.device)
+        self._check(self._lib.tpc_track_batch(self._h, C.byref(cl), C.byref(tr), wp, wn, int(max_tracklets),
+                                              _stream_ptr(s)), "tpc_track_batch")
+        return out
+
+    def track_batch_host(self, y, z, row_offsets, n_tasks: int, out: TrackResult, workspace,
+                         max_tracklets: int = 0, stream=None):
+        """tpc_track_batch_host on HOST tensors (pinned recommended); synchronous.
+        Returns (h2d_bytes, d2h_bytes)."""
+        import torch
+        assert not y.is_cuda and not z.is_cuda and not row_offsets.is_cuda and workspace.is_cuda
+        assert y.dtype == torch.float32 and z.dtype == torch.float32 and row_offsets.dtype == torch.int32
+        cl = _Clusters(None, y.data_ptr(), z.data_ptr(), None, row_offsets.data_ptr(), int(y.numel()), int(n_tasks))
+        tr = self._tracks_struct(out)
+        wp, wn = self._aligned(workspace)
+        s = stream if stream is not None else torch.cuda.current_stream(workspace.device)
+        up, down = C.c_uint64(0), C.c_uint64(0)
+        self._check(self._lib.tpc_track_batch_host(self._h, C.byref(cl), C.byref(tr), wp, wn, int(max_tracklets),
+                                                   _stream_ptr(s), C.byref(up), C.byref(down)),
+                    "tpc_track_batch_host")
+        return int(up.value), int(down.value)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return C.c_void_p(int(stream.cuda_stream))

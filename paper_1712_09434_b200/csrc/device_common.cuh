@@ -1,0 +1,161 @@
+// Device-side context, grid (spatial index) helpers and the ordered block scan
+// shared by the stage kernels of the TPC sector tracker (include/tpc_tracker.h).
+//
+// Arithmetic rules (docs/ARITH_SPEC.md section 0): this translation unit is
+// compiled with -fmad=false -prec-div=true -prec-sqrt=true -ftz=false, so every
+// `a*b + c` below is a rounded multiply followed by a rounded add, and `/`,
+// sqrtf are IEEE correctly rounded.  No libdevice transcendental is used.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpc_tracker.h"
+
+namespace tpc {
+
+constexpr int kMaxRows = 1024;        // include/tpc_tracker.h: n_rows <= 1024
+constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at row_off[tr] + tr*kBinPad
+constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the grid build
+constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
+
+enum CounterId {
+  CN_CLUSTERS = 0, CN_BINS, CN_START_HITS, CN_TRACKLETS_BUILT, CN_TRACKLETS_KEPT, CN_CHAIN_HITS, CN_SEARCHES,
+  CN_CANDIDATES, CN_TRACKLET_HITS, CN_ROW_STEPS, CN_NF_PAIRS, CN_RESERVED, CN_COUNT
+};
+static_assert(CN_COUNT == TPC_N_COUNTERS, "counter list and header disagree");
+
+// Grid of one (task,row): bin = iz*ny + iy, iy = clamp((y - y0)*inv), iz likewise.
+// 16 bytes so that one vector load fetches it.
+struct __align__(16) RowGrid {
+  float inv;   // 1 / bin size
+  int32_t ny;  // bins across y
+  int32_t nz;  // bins along z
+  int32_t pad;
+};
+
+// Everything a kernel needs, passed by value (about 300 bytes of kernel parameters).
+struct Ctx {
+  // geometry and tables (SPEC 1), device pointers [n_rows]
+  int32_t n_sectors, n_rows;
+  const float *X, *ymax, *dx_up, *dx_dn, *ratio_up, *ratio_dn;
+  float z_max;
+  float a, sy2, sz2, wy, wz, smax2;  // T6..T8
+  tpc_params prm;
+  // input (device)
+  const float *y, *z;
+  const uint32_t* row_off;  // [n_tr + 1]
+  uint32_t n, n_tasks, n_tr;
+  // workspace (device); "idx" = position of a cluster in the bin-sorted order, the internal identity
+  float2* yz;              // [n]  (y,z) in bin-sorted order: rows keep their [row_off[tr], row_off[tr+1]) range
+  uint32_t* gid;           // [n]  idx -> gid (index in the input arrays)
+  uint32_t* bins;          // [n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
+  RowGrid* rowgrid;        // [n_tr]
+  int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
+  int32_t* clean_up;       // [n] cleaned up-link (C1)
+  unsigned long long* owner;  // [n] K7 ownership key
+  uint32_t* trk_start;     // [max_tracklets] idx of the start hit
+  uint32_t* trk_tr;        // [max_tracklets] task*n_rows + row of the start hit
+  int32_t* trk_map;        // [ceil(max_tracklets/32)][n_rows][32] idx or -1
+  int32_t* trk_rows;       // [3][max_tracklets] firstRow, lastRow, nHits
+  int32_t* trk_ndf;        // [max_tracklets]
+  float* trk_state;        // [22][max_tracklets] x, p[5], c[15], chi2
+  unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
+  unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
+  uint32_t* tickets;       // [4] dynamic tile counters: 0 seeds, 1 output, 2 finished output tiles
+  uint32_t* n_tracklets;   // [1] tracklets built (clamped to max_tracklets)
+  uint32_t max_tracklets;
+  unsigned long long* counters;  // [CN_COUNT] or nullptr
+  // outputs (device)
+  tpc_tracks out;
+};
+
+__device__ __forceinline__ uint32_t bins_base(const Ctx& c, uint32_t tr, uint32_t row_lo) {
+  return row_lo + tr * kBinPad;
+}
+
+// Monotone clamped bin coordinate; the float is clamped before the conversion (SPEC 0).
+__device__ __forceinline__ int bin_coord(float v, float v0, float inv, int n) {
+  return (int)fminf(fmaxf((v - v0) * inv, 0.0f), (float)(n - 1));
+}
+
+__device__ __forceinline__ float side_z0(const Ctx& c, uint32_t task) {
+  const bool a_side = 2 * (int)(task % (uint32_t)c.n_sectors) < c.n_sectors;
+  return a_side ? -1.0f : -(c.z_max + 1.0f);
+}
+
+// ---------------------------------------------------------------------------
+// Ordered compaction across blocks: single-pass chained scan with decoupled
+// look-back.  Tiles are numbered by a ticket taken when the block starts, so a
+// tile only ever waits for tiles that are already running or finished.
+// One 64-bit word per tile: bits 63..62 = 0 empty / 1 aggregate / 2 inclusive
+// prefix, bits 61..0 the value.  Called by the 32 lanes of warp 0.
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long* p) {
+  return *reinterpret_cast<const volatile unsigned long long*>(p);
+}
+__device__ __forceinline__ void st_volatile_u64(unsigned long long* p, unsigned long long v) {
+  *reinterpret_cast<volatile unsigned long long*>(p) = v;
+}
+
+__device__ __forceinline__ unsigned long long lookback_exclusive(unsigned long long* st, uint32_t tile,
+                                                                 unsigned long long agg) {
+  const unsigned long long kAgg = 1ull << 62, kPre = 2ull << 62, kMask = (1ull << 62) - 1;
+  const int lane = threadIdx.x & 31;
+  if (tile == 0) {
+    if (lane == 0) st_volatile_u64(&st[0], kPre | agg);
+    return 0ull;
+  }
+  if (lane == 0) st_volatile_u64(&st[tile], kAgg | agg);
+  unsigned long long excl = 0ull;
+  long long j = (long long)tile - 1;
+  while (true) {
+    const long long idx = j - lane;
+    const unsigned long long v = idx >= 0 ? ld_volatile_u64(&st[idx]) : kPre;
+    const unsigned flag = (unsigned)(v >> 62);
+    const unsigned ready = __ballot_sync(0xffffffffu, flag != 0u);
+    const unsigned is_pre = __ballot_sync(0xffffffffu, flag == 2u);
+    const int first_pre = is_pre ? (__ffs(is_pre) - 1) : 32;
+    const unsigned need = first_pre >= 31 ? 0xffffffffu : ((2u << first_pre) - 1u);
+    if ((ready & need) != need) continue;  // a predecessor has not published yet: read again
+    unsigned long long contrib = (lane <= first_pre) ? (v & kMask) : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
+    excl += contrib;
+    if (first_pre < 32) break;
+    j -= 32;
+  }
+  if (lane == 0) st_volatile_u64(&st[tile], kPre | (excl + agg));
+  return excl;
+}
+
+// Exclusive scan of one uint32 per thread over the block (blockDim.x <= 1024, multiple of 32).
+// Returns the exclusive prefix; *total receives the block sum.  s_warp: shared [33].
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s_warp, uint32_t* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+  uint32_t incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  if (warp == 0) {
+    uint32_t w = lane < n_warps ? s_warp[lane] : 0u;
+    uint32_t wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+      if (lane >= o) wi += t;
+    }
+    if (lane < n_warps) s_warp[lane] = wi - w;
+    if (lane == 31) s_warp[32] = wi;
+  }
+  __syncthreads();
+  const uint32_t r = s_warp[warp] + incl - v;
+  *total = s_warp[32];
+  __syncthreads();  // s_warp may be reused by the caller
+  return r;
+}
+
+}  // namespace tpc

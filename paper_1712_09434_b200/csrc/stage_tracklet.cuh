@@ -1,0 +1,317 @@
+// a5  tracklet constructor ("Kalman filter for track fitting and
+// track following"; L123: "in the track following phase, 1 GPU thread handles 1
+// track").  docs/ARITH_SPEC.md sections 5 (track model) and 6 (K1..K7).
+//
+// One thread per tracklet, the whole filter state (5 parameters, 15 covariance
+// entries, chi2) in registers.  The five passes of SPEC 6 (chain fit, up pass,
+// turn-around, down pass, finish) are ONE loop whose body is a single row step
+//     transport -> choose the hit (chain link / row map / search) -> update
+// with a per-thread phase, so that threads of a warp that are in different
+// passes still execute the same instructions.  Consecutive tracklets start in
+// the same (task,row) (start hits are compacted in idx order), so a warp walks
+// neighbouring rows and bins.
+#pragma once
+#include "device_common.cuh"
+
+namespace tpc {
+
+constexpr int kTrackletThreads = 128;
+
+struct TrackState {
+  float y, z, s, t, q;  // SPEC 5: y, z, sinphi, dz/dl, q/pT
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+  float chi2;
+  int32_t ndf;
+};
+
+// SPEC 5.1 P1..P24.  dx = X[target] - X[current].  Fails (state untouched) beyond max_sinphi.
+__device__ __forceinline__ bool transport(TrackState& S, float dx, float a, float max_sinphi) {
+  const float y = S.y, z = S.z, s = S.s, t = S.t, q = S.q;
+  const float k = a * q;                                   // P2
+  const float s1 = s + k * dx;                             // P3
+  if (!(fabsf(s) <= max_sinphi && fabsf(s1) <= max_sinphi)) return false;  // P4
+  const float c = sqrtf(1.0f - s * s);                     // P5
+  const float c1 = sqrtf(1.0f - s1 * s1);
+  const float cs = c + c1;                                 // P6
+  const float tt = (s + s1) / cs;                          // P7
+  const float dy = dx * tt;                                // P8
+  const float dl = dx * sqrtf(1.0f + tt * tt);             // P9
+  const float u = (0.5f * k) * dl;                         // P10
+  const float u2 = u * u;
+  const float A1 = 0.16666667f, A2 = 0.075f, A3 = 0.044642857f;
+  const float dS = dl * (1.0f + u2 * (A1 + u2 * (A2 + u2 * A3)));  // P11
+  const float g = s * dy + c * dx;                         // P13
+  const float cc = c * c1;                                 // P14
+  const float f02 = g / cc;                                // P15
+  const float f04 = ((a * dx) * g) / (c1 * cs);            // P16
+  const float f12 = (t * dy) / cc;                         // P17
+  const float f13 = dS;                                    // P18
+  const float f14 = ((t * a) * ((0.5f * dx) * dy)) / cc;   // P19
+  const float f24 = a * dx;                                // P20
+  const float c00 = S.c00, c10 = S.c10, c11 = S.c11, c20 = S.c20, c21 = S.c21, c22 = S.c22, c30 = S.c30,
+              c31 = S.c31, c32 = S.c32, c33 = S.c33, c40 = S.c40, c41 = S.c41, c42 = S.c42, c43 = S.c43,
+              c44 = S.c44;
+  // P21 row 0 of M = F*C
+  const float m00 = c00 + f02 * c20 + f04 * c40;
+  const float m02 = c20 + f02 * c22 + f04 * c42;
+  const float m04 = c40 + f02 * c42 + f04 * c44;
+  // P22 row 1
+  const float m10 = c10 + f12 * c20 + f13 * c30 + f14 * c40;
+  const float m11 = c11 + f12 * c21 + f13 * c31 + f14 * c41;
+  const float m12 = c21 + f12 * c22 + f13 * c32 + f14 * c42;
+  const float m13 = c31 + f12 * c32 + f13 * c33 + f14 * c43;
+  const float m14 = c41 + f12 * c42 + f13 * c43 + f14 * c44;
+  // P23 row 2
+  const float m20 = c20 + f24 * c40;
+  const float m21 = c21 + f24 * c41;
+  const float m22 = c22 + f24 * c42;
+  const float m23 = c32 + f24 * c43;
+  const float m24 = c42 + f24 * c44;
+  // P24 C' = M*F^T
+  S.c00 = m00 + f02 * m02 + f04 * m04;
+  S.c10 = m10 + f02 * m12 + f04 * m14;
+  S.c11 = m11 + f12 * m12 + f13 * m13 + f14 * m14;
+  S.c20 = m20 + f02 * m22 + f04 * m24;
+  S.c21 = m21 + f12 * m22 + f13 * m23 + f14 * m24;
+  S.c22 = m22 + f24 * m24;
+  S.c30 = c30 + f02 * c32 + f04 * c43;
+  S.c31 = c31 + f12 * c32 + f13 * c33 + f14 * c43;
+  S.c32 = c32 + f24 * c43;
+  S.c40 = c40 + f02 * c42 + f04 * c44;
+  S.c41 = c41 + f12 * c42 + f13 * c43 + f14 * c44;
+  S.c42 = c42 + f24 * c44;
+  S.y = y + dy;                                            // P12
+  S.z = z + dS * t;
+  S.s = s1;
+  return true;
+}
+
+// SPEC 5.2 UPDATE(0, m, sy2) then UPDATE(1, m, sz2)
+__device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, float sy2, float sz2) {
+  {
+    const float w = 1.0f / (S.c00 + sy2);                  // U1
+    const float res = ym - S.y;                            // U2
+    const float o0 = S.c00, o1 = S.c10, o2 = S.c20, o3 = S.c30, o4 = S.c40;  // U3
+    const float k0 = o0 * w, k1 = o1 * w, k2 = o2 * w, k3 = o3 * w, k4 = o4 * w;  // U4
+    S.y = S.y + k0 * res; S.z = S.z + k1 * res; S.s = S.s + k2 * res;        // U5
+    S.t = S.t + k3 * res; S.q = S.q + k4 * res;
+    S.c00 = S.c00 - k0 * o0;                               // U6
+    S.c10 = S.c10 - k1 * o0; S.c11 = S.c11 - k1 * o1;
+    S.c20 = S.c20 - k2 * o0; S.c21 = S.c21 - k2 * o1; S.c22 = S.c22 - k2 * o2;
+    S.c30 = S.c30 - k3 * o0; S.c31 = S.c31 - k3 * o1; S.c32 = S.c32 - k3 * o2; S.c33 = S.c33 - k3 * o3;
+    S.c40 = S.c40 - k4 * o0; S.c41 = S.c41 - k4 * o1; S.c42 = S.c42 - k4 * o2; S.c43 = S.c43 - k4 * o3;
+    S.c44 = S.c44 - k4 * o4;
+    S.chi2 = S.chi2 + (res * res) * w;                     // U7
+  }
+  {
+    const float w = 1.0f / (S.c11 + sz2);
+    const float res = zm - S.z;
+    const float o0 = S.c10, o1 = S.c11, o2 = S.c21, o3 = S.c31, o4 = S.c41;
+    const float k0 = o0 * w, k1 = o1 * w, k2 = o2 * w, k3 = o3 * w, k4 = o4 * w;
+    S.y = S.y + k0 * res; S.z = S.z + k1 * res; S.s = S.s + k2 * res;
+    S.t = S.t + k3 * res; S.q = S.q + k4 * res;
+    S.c00 = S.c00 - k0 * o0;
+    S.c10 = S.c10 - k1 * o0; S.c11 = S.c11 - k1 * o1;
+    S.c20 = S.c20 - k2 * o0; S.c21 = S.c21 - k2 * o1; S.c22 = S.c22 - k2 * o2;
+    S.c30 = S.c30 - k3 * o0; S.c31 = S.c31 - k3 * o1; S.c32 = S.c32 - k3 * o2; S.c33 = S.c33 - k3 * o3;
+    S.c40 = S.c40 - k4 * o0; S.c41 = S.c41 - k4 * o1; S.c42 = S.c42 - k4 * o2; S.c43 = S.c43 - k4 * o3;
+    S.c44 = S.c44 - k4 * o4;
+    S.chi2 = S.chi2 + (res * res) * w;
+  }
+  S.ndf += 2;
+}
+
+// SPEC 5.3 SEARCH (H1..H6) in row-block tr; returns the idx of the best cluster or -1.
+template <bool COUNT>
+__device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, uint32_t tr, int row, float z0,
+                                              uint32_t& n_cand) {
+  const float y = S.y, z = S.z;
+  const float ey = S.c00 + c.sy2, ez = S.c11 + c.sz2;                 // H1
+  const float hy2 = fminf(c.prm.accept_k2 * ey, c.smax2);              // H2
+  const float hz2 = fminf(c.prm.accept_k2 * ez, c.smax2);
+  const float wy = sqrtf(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrtf(fmaxf(hz2, 0.0f)) + kGridMargin;
+  const RowGrid g = c.rowgrid[tr];
+  const float y0 = -c.ymax[row];
+  const uint32_t* bins = c.bins + bins_base(c, tr, c.row_off[tr]);
+  const int iy0 = bin_coord(y - wy, y0, g.inv, g.ny), iy1 = bin_coord(y + wy, y0, g.inv, g.ny);
+  const int iz0 = bin_coord(z - wz, z0, g.inv, g.nz), iz1 = bin_coord(z + wz, z0, g.inv, g.nz);
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bi = 0u;
+  for (int iz = iz0; iz <= iz1; ++iz) {
+    const uint32_t b0 = bins[iz * g.ny + iy0], b1 = bins[iz * g.ny + iy1 + 1];
+    for (uint32_t i = b0; i < b1; ++i) {
+      const float2 p = c.yz[i];
+      if (COUNT) ++n_cand;
+      const float dy = p.x - y, dz = p.y - z;                          // H3
+      const float dy2 = dy * dy, dz2 = dz * dz;
+      if (!(dy2 <= hy2 && dz2 <= hz2)) continue;                       // H4
+      const float d = (dy2 * ez) + (dz2 * ey);                         // H5
+      bool take = !have || d < best;                                   // H6
+      if (have && d == best) take = c.gid[i] < c.gid[bi];
+      if (take) { have = true; best = d; bi = i; }
+    }
+  }
+  return have ? (int32_t)bi : -1;
+}
+
+enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4 };
+
+__device__ __forceinline__ size_t map_index(uint32_t t, int row, int n_rows) {
+  return ((size_t)(t >> 5) * (size_t)n_rows + (size_t)row) * 32u + (t & 31u);
+}
+
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
+  __shared__ float sX[kMaxRows];
+  const uint32_t n_trk = *c.n_tracklets;
+  if (blockIdx.x * kTrackletThreads >= n_trk) return;
+  for (int r = threadIdx.x; r < c.n_rows; r += kTrackletThreads) sX[r] = c.X[r];
+  __syncthreads();
+  const uint32_t t = blockIdx.x * kTrackletThreads + threadIdx.x;
+  if (t >= n_trk) return;
+  const int n_rows = c.n_rows;
+  const uint32_t h0 = c.trk_start[t];
+  const uint32_t tr0 = c.trk_tr[t];
+  const uint32_t task = tr0 / (uint32_t)n_rows;
+  const int r0 = (int)(tr0 - task * (uint32_t)n_rows);
+  const uint32_t tr_base = task * (uint32_t)n_rows;
+  const float z0 = side_z0(c, task);
+  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
+  const int max_gap = c.prm.max_row_gap;
+  int32_t* map = c.trk_map;
+
+  // K1 seed
+  TrackState S;
+  const uint32_t h1 = (uint32_t)c.clean_up[h0];
+  {
+    const float2 p0 = c.yz[h0], p1 = c.yz[h1];
+    const float dx = sX[r0 + 1] - sX[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
+    const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
+    S.y = p1.x; S.z = p1.y; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
+    S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
+    S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
+    S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
+    S.chi2 = 0.0f; S.ndf = -5;
+  }
+  map[map_index(t, r0, n_rows)] = (int32_t)h0;
+  map[map_index(t, r0 + 1, n_rows)] = (int32_t)h1;
+  int row_cur = r0 + 1, first_row = r0, last_row = r0 + 1, n_hits = 2, gap = 0;
+  int32_t last_hit = (int32_t)h1;
+  int32_t next_chain = c.clean_up[h1];
+  int r_down = 0;
+  int phase = next_chain >= 0 ? PH_CHAIN : PH_UP;
+  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_chain = 2u;
+
+  while (true) {
+    // which row does this step go to?
+    if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
+    if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
+    int rt;
+    if (phase <= PH_UP) rt = row_cur + 1;
+    else if (phase == PH_TURN) rt = last_row;
+    else if (phase == PH_DOWN) rt = r_down;
+    else rt = first_row;
+    bool ok = true;
+    if (rt != row_cur) {
+      ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
+      if (ok) row_cur = rt;
+      if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
+    }
+    if (phase == PH_FINISH) break;                                    // K6
+    if (phase == PH_TURN) {                                           // K4
+      const float f = c.prm.turn_cov_scale;
+      S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
+      S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
+      S.chi2 = 0.0f; S.ndf = -5; gap = 0;
+      if (row_cur == last_row) {
+        const float2 p = c.yz[last_hit];
+        update_hit(S, p.x, p.y, sy2, sz2);
+      }
+      r_down = last_row - 1;
+      phase = PH_DOWN;
+      continue;
+    }
+    if (!ok) {  // transport failed: K2/K3 -> turn-around, K5 -> finish
+      phase = (phase == PH_DOWN) ? PH_FINISH : PH_TURN;
+      continue;
+    }
+    int32_t hit = -1;
+    bool do_search = false;
+    if (phase == PH_CHAIN) hit = next_chain;                          // K2
+    else if (phase == PH_UP) do_search = true;                        // K3
+    else {                                                            // K5
+      if (rt >= r0) {
+        hit = map[map_index(t, rt, n_rows)];
+        do_search = hit < 0;
+      } else {
+        do_search = true;
+      }
+    }
+    if (do_search) {
+      if (COUNT) ++n_search;
+      hit = search_row<COUNT>(c, S, tr_base + (uint32_t)rt, rt, z0, n_cand);
+    }
+    if (hit >= 0) {
+      const float2 p = c.yz[hit];
+      update_hit(S, p.x, p.y, sy2, sz2);
+    }
+    if (phase == PH_CHAIN) {
+      map[map_index(t, rt, n_rows)] = hit;
+      last_row = rt; last_hit = hit; ++n_hits;
+      if (COUNT) ++n_chain;
+      next_chain = c.clean_up[hit];
+      if (next_chain < 0) { phase = PH_UP; gap = 0; }
+    } else if (phase == PH_UP) {
+      map[map_index(t, rt, n_rows)] = hit;
+      if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
+      else if (++gap > max_gap) phase = PH_TURN;
+    } else {  // PH_DOWN
+      if (do_search) {
+        map[map_index(t, rt, n_rows)] = hit;
+        if (hit >= 0) {
+          ++n_hits;
+          if (rt < first_row) { first_row = rt; gap = 0; }
+        } else if (rt < first_row) {
+          if (++gap > max_gap) phase = PH_FINISH;
+        }
+      }
+      --r_down;
+    }
+  }
+
+  // tracklet record
+  const uint32_t T = c.max_tracklets;
+  c.trk_rows[t] = first_row; c.trk_rows[T + t] = last_row; c.trk_rows[2u * T + t] = n_hits;
+  c.trk_ndf[t] = S.ndf;
+  float* st = c.trk_state + t;
+  st[0 * (size_t)T] = sX[row_cur];
+  st[1 * (size_t)T] = S.y; st[2 * (size_t)T] = S.z; st[3 * (size_t)T] = S.s; st[4 * (size_t)T] = S.t;
+  st[5 * (size_t)T] = S.q;
+  st[6 * (size_t)T] = S.c00; st[7 * (size_t)T] = S.c10; st[8 * (size_t)T] = S.c11; st[9 * (size_t)T] = S.c20;
+  st[10 * (size_t)T] = S.c21; st[11 * (size_t)T] = S.c22; st[12 * (size_t)T] = S.c30; st[13 * (size_t)T] = S.c31;
+  st[14 * (size_t)T] = S.c32; st[15 * (size_t)T] = S.c33; st[16 * (size_t)T] = S.c40; st[17 * (size_t)T] = S.c41;
+  st[18 * (size_t)T] = S.c42; st[19 * (size_t)T] = S.c43; st[20 * (size_t)T] = S.c44; st[21 * (size_t)T] = S.chi2;
+
+  // K7 ownership: longest tracklet wins, then the smaller start-hit gid
+  if (n_hits >= c.prm.min_track_hits) {
+    const unsigned long long key =
+        ((unsigned long long)(uint32_t)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - c.gid[h0]);
+    for (int r = first_row; r <= last_row; ++r) {
+      const int32_t m = map[map_index(t, r, n_rows)];
+      if (m >= 0) atomicMax(&c.owner[m], key);
+    }
+    if (COUNT) {
+      atomicAdd(&c.counters[CN_TRACKLETS_KEPT], 1ull);
+      atomicAdd(&c.counters[CN_TRACKLET_HITS], (unsigned long long)n_hits);
+    }
+  }
+  if (COUNT) {
+    atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
+    atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
+    atomicAdd(&c.counters[CN_CANDIDATES], (unsigned long long)n_cand);
+    atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
+  }
+}
+
+}  // namespace tpc
