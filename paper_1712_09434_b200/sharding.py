@@ -22,3 +22,17 @@ def shard_events(n_events: int, world_size: int, rank: int) -> List[int]:
 def merge_counts(per_rank: Sequence[Sequence[int]]) -> List[int]:
     """Element-wise sum of the per-rank (clusters, events, tracks, hits) tuples."""
     return [sum(col) for col in zip(*per_rank)]
+
+
+def gather_counts(mine: Sequence[int]) -> List[int]:
+    """Sum of the per-rank counters over the default process group (the ONLY exchange on the N > 1
+    path; reporting, not data).  Works on gloo (CPU tensors) and nccl (tensors on the current device)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [int(v) for v in mine]
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    mine_t = torch.tensor([int(v) for v in mine], dtype=torch.int64, device=dev)
+    parts = [torch.zeros_like(mine_t) for _ in range(dist.get_world_size())]
+    dist.all_gather(parts, mine_t)
+    return merge_counts([p.cpu().tolist() for p in parts])
