@@ -1,0 +1,337 @@
+"""bench.py - throughput of the TPC sector tracker hot path (a1..a7) on synthetic Pb-Pb-shaped batches.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--events E]
+
+A step is one pass of the whole hot path (one tpc_track_batch call: grid build, neighbour finder, cleaner,
+start hits, tracklet constructor, selector + output) over one batch.  Default workload: BASELINE.json
+configs[3], 16 central-Pb-Pb-like events = 576 sector tasks, about 40.7 M clusters, per GPU (weak scaling:
+every rank tracks its own 16 events, no data-path collective - DESIGN.md section 8).
+Prints ONE JSON line (rank 0).  DESIGN.md section 6 states the algorithmic-bytes formula used for `roofline`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tpc_clusters_tracked_per_s"
+UNIT = "clusters/s"
+FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3: the batch)")
+    ap.add_argument("--events", type=int, default=None, help="use only the first E events of the config")
+    ap.add_argument("--cpu-events", type=int, default=4, help="events in the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(config, n_events):
+    from tpc_workload.events import CONFIGS
+    return f"{CONFIGS[config]['name']}[{n_events} events]"
+
+
+def make_workload(config, n_events, rank):
+    """Seeded synthetic batch of this rank: the config's seeds shifted by 1000*rank (rank 0 = the config itself)."""
+    from tpc_workload.events import CONFIGS, generate_event, default_geometry, concat_batches
+    c = CONFIGS[config]
+    seeds = [s + 1000 * rank for s in (c["seeds"] if n_events is None else c["seeds"][:n_events])]
+    jobs = [(c["n_sectors"], c["spec"], s, i) for i, s in enumerate(seeds)]
+    workers = max(1, min(len(jobs), (os.cpu_count() or 1) // max(int(os.environ.get("WORLD_SIZE", "1")), 1), 16))
+    if workers > 1:
+        import multiprocessing as mp
+        from tpc_workload.events import _gen_one
+        with mp.get_context("fork").Pool(workers) as pool:
+            evs = pool.map(_gen_one, jobs)
+    else:
+        evs = [generate_event(default_geometry(n_sectors=j[0]), j[1], j[2], track_id_base=j[3] * 1_000_000) for j in jobs]
+    return evs[0] if len(evs) == 1 else concat_batches(evs)
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic bytes (SURVEY.md section 8(d) / DESIGN.md section 6), from the device counters
+# ---------------------------------------------------------------------------------------------
+def algorithmic_bytes(c):
+    N, B, T0, T = c["clusters"], c["bins"], c["start_hits"], c["tracklets_built"]
+    Hc, S, K, Ht = c["chain_hits"], c["searches"], c["candidates"], c["tracklet_hits"]
+    Ho, To = c["out_hits"], c["out_tracks"]
+    return {
+        "grid_build": 8 * N + 8 * N + 4 * N + 4 * B,
+        "neighbour_finder": 8 * N + 4 * B + 8 * N,
+        "cleaner": 8 * N,
+        "start_hits": 4 * T0,
+        "tracklet_constructor": 12 * Hc + 16 * S + 8 * K + 8 * Ht + 4 * Ht + 8 * Ht + 8 * N + 88 * T,
+        "selector_output": 4 * Ht + 8 * Ht + 4 * Ho + 100 * To,
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [ln.split(",") for ln in open(self.f.name).read().splitlines() if ln.count(",") >= 8]
+        os.unlink(self.f.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle, timed as it stands (cpu_baseline leg and --impl reference): the ONLY use of oracle/ here
+# ---------------------------------------------------------------------------------------------
+def time_oracle(batch, events):
+    """Single-threaded CPU oracle over the given events of ``batch``; returns (seconds, clusters)."""
+    import oracle
+    from tpc_workload import take_tasks
+    ns = batch.geometry.n_sectors
+    tasks = [e * ns + s for e in events for s in range(ns)]
+    sub, _ = take_tasks(batch, tasks)
+    prm = oracle.OracleParams(sigma_y=batch.sigma_y, sigma_z=batch.sigma_z)
+    t0 = time.perf_counter()
+    oracle.track(sub.geometry, sub.y, sub.z, sub.row_offsets, sub.n_tasks, params=prm)
+    return time.perf_counter() - t0, sub.n_clusters
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; one step = one event (36 sector tasks) of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from tpc_workload.events import CONFIGS
+    n_cfg = len(CONFIGS[args.config]["seeds"]) if args.events is None else args.events
+    n_gen = min(n_cfg, 4)
+    batch = make_workload(args.config, n_gen, 0)
+    for i in range(args.warmup):
+        time_oracle(batch, [i % n_gen])
+    tot_s, tot_c = 0.0, 0
+    for i in range(args.steps):
+        s, c = time_oracle(batch, [i % n_gen])
+        tot_s += s
+        tot_c += c
+    value = tot_c / tot_s
+    sample = f"one event (36 sector tasks) of the workload per step, events 0..{n_gen - 1} in turn"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, n_cfg), "step_sample": sample},
+        "events_per_s": args.steps / tot_s,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# the product arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the tracker has no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1712_09434_b200 import Tracker, TrackerParams
+    from paper_1712_09434_b200.build import build as build_cuda
+    from paper_1712_09434_b200.sharding import gather_counts
+    from tpc_workload.events import CONFIGS
+    if rank == 0:
+        build_cuda()
+    if world > 1:
+        dist.barrier()
+    n_cfg = len(CONFIGS[args.config]["seeds"]) if args.events is None else args.events
+    batch = make_workload(args.config, args.events, rank)
+    n, n_tasks, nr = batch.n_clusters, batch.n_tasks, batch.geometry.n_rows
+    n_events = batch.n_events
+
+    trk = Tracker(batch.geometry, TrackerParams(sigma_y=batch.sigma_y, sigma_z=batch.sigma_z))
+    y_h = torch.from_numpy(np.ascontiguousarray(batch.y)).pin_memory()
+    z_h = torch.from_numpy(np.ascontiguousarray(batch.z)).pin_memory()
+    ro_h = torch.from_numpy(batch.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()
+    y, z, ro = y_h.to(dev), z_h.to(dev), ro_h.to(dev)
+    out = trk.alloc_outputs(n, dev)
+    ws = trk.alloc_workspace(trk.workspace_bytes(n, n_tasks), dev)
+    stream = torch.cuda.current_stream(dev)
+
+    # one untimed counted pass: the counters of the algorithmic-bytes formula, and the result sizes
+    trk.enable_counters(True)
+    trk.track_batch(y, z, ro, n_tasks, out, ws)
+    counters = trk.read_counters(stream)
+    trk.enable_counters(False)
+    hdr = out.header.cpu().numpy().astype(np.int64)
+    if int(hdr[2]) != 0:
+        raise RuntimeError(f"tracker status bits {int(hdr[2])}: capacity overflow in the bench workload")
+    counters["out_tracks"], counters["out_hits"] = int(hdr[0]), int(hdr[1])
+    alg = algorithmic_bytes(counters)
+
+    for _ in range(args.warmup):
+        trk.track_batch(y, z, ro, n_tasks, out, ws)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    trk.enable_stage_timing(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        trk.track_batch(y, z, ro, n_tasks, out, ws)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    stage_ms, stage_calls = trk.read_stage_ms(stream)
+    trk.enable_stage_timing(False)
+    clocks = sampler.stop() if sampler else None
+
+    # end to end through tpc_track_batch_host: pinned host inputs -> device -> tracks back on the host
+    e2e = None
+    if not args.no_e2e:
+        out_h = trk.alloc_outputs(n, dev, pinned_host=True)
+        tcap, hcap = out_h.track_task.shape[0], out_h.hit_cluster.shape[0]
+        ws_h = trk.alloc_workspace(trk.host_workspace_bytes(n, n_tasks, 0, tcap, hcap), dev)
+        for _ in range(min(args.warmup, 2)):
+            up, down = trk.track_batch_host(y_h, z_h, ro_h, n_tasks, out_h, ws_h)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            up, down = trk.track_batch_host(y_h, z_h, ro_h, n_tasks, out_h, ws_h)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        e2e_ms = e0.elapsed_time(e1)
+        e2e = (e2e_ms, up, down)
+        del ws_h, out_h
+
+    # max over ranks, totals over ranks
+    if world > 1:
+        t = torch.tensor([ms_total, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, e2e_ms_max = float(t[0]), float(t[1])
+    else:
+        e2e_ms_max = e2e[0] if e2e else 0.0
+    tot = gather_counts([n, n_events, int(hdr[0]), int(hdr[1])])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak_gbs, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak_gbs, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    secs = ms_total / 1e3
+    ms_step = ms_total / args.steps
+    value = tot[0] * args.steps / secs
+    top = max(stage_ms, key=stage_ms.get)
+    top_gbs = alg[top] / (stage_ms[top] / 1e3) / 1e9 if stage_ms[top] > 0 else 0.0
+    path_bytes = sum(alg.values())
+    path_gbs = path_bytes / (ms_step / 1e3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config, n_cfg), "events_per_gpu": n_events,
+                   "sector_tasks_per_gpu": n_tasks, "clusters_per_gpu": n, "tracks_per_gpu": int(hdr[0]),
+                   "parallelism": f"events sharded over {world} GPU(s), no collective",
+                   "l2": "inputs (8 B/cluster) and every intermediate array are larger than the 126 MB L2"
+                         if 8 * n > 126e6 else "inputs smaller than L2: latency case, not the headline"},
+        "events_per_s": tot[1] * args.steps / secs,
+        "tracks_per_s": tot[2] * args.steps / secs,
+        "hbm_roofline_frac_path": path_gbs / peak_gbs,
+        "roofline": {"bound": "hbm", "kernel": top, "achieved": top_gbs, "peak": peak_gbs, "unit": "GB/s",
+                     "frac": top_gbs / peak_gbs, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg[top], "ms_per_launch": stage_ms[top],
+                     "share_of_step": stage_ms[top] / max(sum(stage_ms.values()), 1e-9)},
+        "roofline_path": {"bound": "hbm", "achieved": path_gbs, "peak": peak_gbs, "unit": "GB/s",
+                          "frac": path_gbs / peak_gbs, "algorithmic_bytes_per_step": path_bytes,
+                          "bytes_per_cluster": path_bytes / max(n, 1)},
+        "stages_ms": stage_ms, "stages_algorithmic_bytes": alg, "stage_calls_averaged": stage_calls,
+        "counters": counters,
+        "clocks": clocks,
+        "gpu_launches": trk.launches_per_batch() * args.steps,
+    }
+    if e2e:
+        line["e2e"] = {"value": tot[0] * args.steps / (e2e_ms_max / 1e3), "unit": UNIT,
+                       "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2],
+                       "ms_per_step": e2e_ms_max / args.steps, "api": "tpc_track_batch_host (pinned host buffers)"}
+    if world == 1 and not args.no_cpu_baseline:
+        ne = max(1, min(args.cpu_events, n_events))
+        s, c = time_oracle(batch, list(range(ne)))
+        line["cpu_baseline"] = {"value": c / s, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"first {ne} event(s) of the workload ({c} clusters), single thread, {s:.1f} s",
+                                "events_per_s": ne / s}
+    trk.close()
+    if world > 1:
+        dist.destroy_process_group()
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -181,6 +181,22 @@ int tpc_read_counters(tpc_tracker* tracker, void* cuda_stream, uint64_t* out);
 /* Number of kernels one tpc_track_batch call launches (debug kernels excluded). */
 int tpc_launches_per_batch(const tpc_tracker* tracker);
 
+/* Per-stage device times.  With stage timing on, tpc_track_batch records one
+ * CUDA event on cuda_stream before its first kernel and one after every stage
+ * (a ring of TPC_STAGE_RING calls; recording costs no kernel and no sync).
+ * tpc_read_stage_ms synchronises the stream, then writes to out_ms (HOST,
+ * [TPC_N_STAGES]) the MEAN duration in milliseconds of every stage over the
+ * calls recorded since timing was switched on (at most the last TPC_STAGE_RING)
+ * and to n_calls (HOST, may be NULL) how many calls that was.  Stage i is
+ * named tpc_stage_name(i) (static string, NULL beyond the last stage):
+ * 0 grid build (a1), 1 neighbour finder (a2), 2 cleaner (a3), 3 start hits (a4),
+ * 4 tracklet constructor (a5), 5 selector + output (a6, a7). */
+#define TPC_N_STAGES 6
+#define TPC_STAGE_RING 64
+void tpc_tracker_enable_stage_timing(tpc_tracker* tracker, int on);
+int tpc_read_stage_ms(tpc_tracker* tracker, void* cuda_stream, float* out_ms, uint32_t* n_calls);
+const char* tpc_stage_name(int stage);
+
 /* Text of the last error on this tracker (never NULL). With tracker == NULL: the
  * last error of tpc_tracker_create on this thread. */
 const char* tpc_last_error(const tpc_tracker* tracker);

@@ -123,6 +123,12 @@ def load_library():
     lib.tpc_read_counters.argtypes = [vp, vp, u64p]
     lib.tpc_launches_per_batch.restype = C.c_int
     lib.tpc_launches_per_batch.argtypes = [vp]
+    lib.tpc_tracker_enable_stage_timing.restype = None
+    lib.tpc_tracker_enable_stage_timing.argtypes = [vp, C.c_int]
+    lib.tpc_read_stage_ms.restype = C.c_int
+    lib.tpc_read_stage_ms.argtypes = [vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
+    lib.tpc_stage_name.restype = C.c_char_p
+    lib.tpc_stage_name.argtypes = [C.c_int]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_last_error.argtypes = [vp]
     _lib = lib
@@ -214,6 +220,19 @@ class Tracker:
         buf = (C.c_uint64 * len(COUNTER_NAMES))()
         self._check(self._lib.tpc_read_counters(self._h, _stream_ptr(stream), buf), "tpc_read_counters")
         return {n: int(v) for n, v in zip(COUNTER_NAMES, buf)}
+
+    def enable_stage_timing(self, on: bool):
+        self._lib.tpc_tracker_enable_stage_timing(self._h, 1 if on else 0)
+
+    def read_stage_ms(self, stream=None):
+        """({stage name: mean ms}, calls averaged) of the calls since enable_stage_timing(True); synchronises."""
+        names = []
+        while self._lib.tpc_stage_name(len(names)) is not None:
+            names.append(self._lib.tpc_stage_name(len(names)).decode())
+        buf = (C.c_float * len(names))()
+        n = C.c_uint32(0)
+        self._check(self._lib.tpc_read_stage_ms(self._h, _stream_ptr(stream), buf, C.byref(n)), "tpc_read_stage_ms")
+        return {k: float(v) for k, v in zip(names, buf)}, int(n.value)
 
     # ---- allocation helpers (torch = device memory only) ---------------------
     def alloc_outputs(self, n_clusters: int, device, track_capacity: Optional[int] = None,

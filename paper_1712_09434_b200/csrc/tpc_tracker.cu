@@ -29,6 +29,10 @@ struct tpc_tracker {
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
+  // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
+  bool timing_on = false;
+  std::vector<cudaEvent_t> ev;
+  uint32_t timed_calls = 0;
   std::string err;
 };
 
@@ -196,6 +200,7 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
 
 void tpc_tracker_destroy(tpc_tracker* t) {
   if (!t) return;
+  for (cudaEvent_t e : t->ev) cudaEventDestroy(e);
   if (t->d_tables) cudaFree(t->d_tables);
   if (t->d_counters) cudaFree(t->d_counters);
   delete t;
@@ -211,6 +216,39 @@ int tpc_launches_per_batch(const tpc_tracker*) { return 6; }
 
 void tpc_tracker_enable_counters(tpc_tracker* t, int on) {
   if (t) t->counters_on = on != 0;
+}
+
+void tpc_tracker_enable_stage_timing(tpc_tracker* t, int on) {
+  if (!t) return;
+  t->timing_on = on != 0;
+  t->timed_calls = 0;
+}
+
+const char* tpc_stage_name(int stage) {
+  static const char* const names[TPC_N_STAGES] = {"grid_build", "neighbour_finder", "cleaner", "start_hits",
+                                                  "tracklet_constructor", "selector_output"};
+  return stage >= 0 && stage < TPC_N_STAGES ? names[stage] : nullptr;
+}
+
+int tpc_read_stage_ms(tpc_tracker* t, void* cuda_stream, float* out_ms, uint32_t* n_calls) {
+  if (!t || !out_ms) return TPC_ERR_ARGUMENT;
+  cudaError_t e = cudaStreamSynchronize((cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_read_stage_ms: CUDA: %s", cudaGetErrorString(e));
+  const uint32_t n = t->timed_calls < TPC_STAGE_RING ? t->timed_calls : TPC_STAGE_RING;
+  double sum[TPC_N_STAGES] = {0};
+  for (uint32_t k = 0; k < n; ++k) {
+    const uint32_t slot = (t->timed_calls - 1 - k) % TPC_STAGE_RING;
+    const cudaEvent_t* ev = t->ev.data() + (size_t)slot * (TPC_N_STAGES + 1);
+    for (int i = 0; i < TPC_N_STAGES; ++i) {
+      float ms = 0.f;
+      e = cudaEventElapsedTime(&ms, ev[i], ev[i + 1]);
+      if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_read_stage_ms: CUDA: %s", cudaGetErrorString(e));
+      sum[i] += ms;
+    }
+  }
+  for (int i = 0; i < TPC_N_STAGES; ++i) out_ms[i] = n ? (float)(sum[i] / n) : 0.f;
+  if (n_calls) *n_calls = n;
+  return TPC_OK;
 }
 
 int tpc_read_counters(tpc_tracker* t, void* cuda_stream, uint64_t* out) {
@@ -249,21 +287,42 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (e == cudaSuccess && out->dbg_n_start_hits) e = cudaMemsetAsync(out->dbg_n_start_hits, 0, sizeof(uint32_t), s);
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch: CUDA memset: %s", cudaGetErrorString(e));
   const bool cnt = t->counters_on;
+  cudaEvent_t* ev = nullptr;  // stage marks of this call (nullptr: timing off)
+  if (t->timing_on) {
+    if (t->ev.empty()) {
+      t->ev.resize((size_t)TPC_STAGE_RING * (TPC_N_STAGES + 1));
+      for (cudaEvent_t& x : t->ev)
+        if (cudaEventCreate(&x) != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch: cudaEventCreate failed");
+    }
+    ev = t->ev.data() + (size_t)(t->timed_calls % TPC_STAGE_RING) * (TPC_N_STAGES + 1);
+    ++t->timed_calls;
+  }
+  int stage = 0;
+  auto mark = [&]() { if (ev) cudaEventRecord(ev[stage], s); ++stage; };
+  mark();
   if (c.n_tr > 0) {
     if (cnt) k_grid_build<true><<<c.n_tr, kGridThreads, 0, s>>>(c);                         // a1
     else k_grid_build<false><<<c.n_tr, kGridThreads, 0, s>>>(c);
+  }
+  mark();
+  if (c.n_tr > 0) {
     if (cnt) k_neighbours<true><<<c.n_tr, kNfThreads, 0, s>>>(c);                           // a2
     else k_neighbours<false><<<c.n_tr, kNfThreads, 0, s>>>(c);
   }
+  mark();
   if (c.n > 0) {
     k_clean<<<(c.n + kCleanThreads - 1) / kCleanThreads, kCleanThreads, 0, s>>>(c);         // a3
   }
+  mark();
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
   else k_seeds<false><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);
+  mark();
   const uint32_t trk_blocks = (T + kTrackletThreads - 1) / kTrackletThreads;
   if (cnt) k_tracklets<true><<<trk_blocks, kTrackletThreads, 0, s>>>(c);                    // a5
   else k_tracklets<false><<<trk_blocks, kTrackletThreads, 0, s>>>(c);
+  mark();
   k_select_output<<<cv.out_tiles, kOutThreads, 0, s>>>(c);                                  // a6 + a7
+  mark();
   if (c.n > 0 && (out->dbg_link_up || out->dbg_link_dn || out->dbg_clean_up || out->dbg_clean_dn ||
                   out->dbg_start_hits))
     k_debug_links<<<(c.n + 255) / 256, 256, 0, s>>>(c);

@@ -1,0 +1,230 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
+inputs.  Bar (BASELINE.json north_star): bit-exact neighbour links, cleaned links, start hits,
+tracklet row maps and per-track cluster index lists; fitted parameters, covariances and chi2 within
+RTOL = 1e-4 relative (both sides run the same non-contracted fp32 sequence of docs/ARITH_SPEC.md,
+so they are in fact expected to be bit-identical, which is reported but not required).
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from tpc_workload import generate_config, take_tasks, concat_batches, default_geometry
+from helpers import batch_from_rows
+import gpu_helpers as G
+
+pytestmark = pytest.mark.gpu
+RTOL = 1e-4  # north_star: "fitted track parameters and covariances must agree within 1e-4 relative"
+
+
+@pytest.fixture(scope="module")
+def cfg2():
+    return generate_config(2)
+
+
+# ---- element by element, whole configs ------------------------------------------------------
+@pytest.mark.parametrize("config", [0, 1])
+def test_small_configs_every_stage(config):
+    b = generate_config(config)
+    gpu = G.run_gpu(b)
+    ref = G.run_oracle(b)
+    dev = G.compare(gpu, ref, b.geometry.n_rows, rtol=RTOL)
+    assert ref.n_tracks > 0
+    print(f"config {config}: {b.n_clusters} clusters, {ref.n_tracks} tracks, deviations {dev}")
+
+
+def test_config2_central_event_every_stage(cfg2):
+    """One central event: 2.5 M clusters, 5 700 row blocks of 28..570 clusters (several tiles + ragged tails)."""
+    gpu = G.run_gpu(cfg2)
+    ref = G.run_oracle(cfg2)
+    dev = G.compare(gpu, ref, cfg2.geometry.n_rows, rtol=RTOL)
+    print(f"config 2: {cfg2.n_clusters} clusters, {ref.n_tracks} tracks, deviations {dev}")
+
+
+def test_config4_stress_every_stage():
+    """50 000 tracks, 20 % noise, wider errors: long candidate lists in both searches."""
+    b = generate_config(4)
+    gpu = G.run_gpu(b)
+    ref = G.run_oracle(b)
+    dev = G.compare(gpu, ref, b.geometry.n_rows, rtol=RTOL)
+    print(f"config 4: {b.n_clusters} clusters, {ref.n_tracks} tracks, deviations {dev}")
+
+
+# ---- the bench launch configuration at full size, sampled tasks -------------------------------
+def test_config3_full_batch_sampled_tasks():
+    """Config 3 exactly as bench.py runs it (16 events, 576 tasks, one call, no debug outputs, default
+    capacities).  Tasks are independent, so the oracle computes a sample of tasks
+    one by one and every track of those tasks must match; properties hold for all."""
+    b = generate_config(3, workers=8)
+    gpu = G.run_gpu(b, debug=False, debug_tracklets=False)
+    assert gpu["status"] == 0
+    nr = b.geometry.n_rows
+    # properties at full size: every cluster in at most one track, hits ascending by row, >= min hits
+    hits = gpu["hit_cluster"].astype(np.int64)
+    assert len(np.unique(hits)) == len(hits)
+    assert gpu["n_hits"] == len(hits) and int(gpu["track_nhits"].sum()) == len(hits)
+    assert int(gpu["track_nhits"].min()) >= 10
+    tr_of = np.searchsorted(b.row_offsets.astype(np.int64), hits, side="right") - 1
+    beg = gpu["track_hit_begin"].astype(np.int64)
+    seg = np.repeat(np.arange(len(beg)), gpu["track_nhits"].astype(np.int64))
+    assert np.array_equal(tr_of // nr, gpu["track_task"].astype(np.int64)[seg]), "a hit outside its track's task"
+    same = seg[1:] == seg[:-1]
+    assert np.all((tr_of[1:] > tr_of[:-1])[same]), "hits not in ascending row order"
+    # sampled tasks: first, last, one per event side, seeded extras
+    rng = np.random.Generator(np.random.PCG64(7))
+    tasks = sorted({0, b.n_tasks - 1, 17, 18, *rng.integers(0, b.n_tasks, 4).tolist()})
+    for task in tasks:
+        sub, sel = take_tasks(b, [task])
+        ref = G.run_oracle(sub, dump_tracklets=False)
+        m = gpu["track_task"] == task
+        got = {}
+        for t in np.nonzero(m)[0]:
+            h = gpu["hit_cluster"][beg[t]:beg[t] + int(gpu["track_nhits"][t])].astype(np.int64)
+            got[tuple(h.tolist())] = t
+        assert len(got) == ref.n_tracks, f"task {task}: gpu {len(got)} oracle {ref.n_tracks}"
+        for t in range(ref.n_tracks):
+            key = tuple(sel[ref.track_hits(t).astype(np.int64)].tolist())
+            assert key in got, f"task {task}: oracle track {t} missing on the GPU"
+            g = got[key]
+            assert gpu["track_ndf"][g] == ref.track_ndf[t]
+            rp, gp = ref.track_par[:, t].astype(np.float64), gpu["track_par"][:, g].astype(np.float64)
+            sig = np.sqrt(np.maximum(ref.track_cov[[0, 2, 5, 9, 14], t].astype(np.float64), 0))
+            assert np.all(np.abs(gp - rp) <= RTOL * np.maximum(np.abs(rp), sig))
+            rc, gc = ref.track_cov[:, t].astype(np.float64), gpu["track_cov"][:, g].astype(np.float64)
+            sc = np.array([sig[i] * sig[j] for i in range(5) for j in range(i + 1)])
+            assert np.all(np.abs(gc - rc) <= RTOL * np.maximum(np.abs(rc), sc))
+
+
+# ---- invariances on the GPU path ---------------------------------------------------------------
+def test_batch_equals_single_events():
+    """events on one GPU are independent - a batch of 3 gives the 3 single results."""
+    evs = [generate_config(1), generate_config(1)]
+    from tpc_workload.events import CONFIGS, generate_event
+    evs[1] = generate_event(default_geometry(), CONFIGS[1]["spec"], 77, track_id_base=1_000_000)
+    both = concat_batches(evs)
+    gb = G.run_gpu(both, debug=False, debug_tracklets=False)
+    base, tbase = 0, 0
+    got = set()
+    beg = gb["track_hit_begin"].astype(np.int64)
+    for t in range(gb["n_tracks"]):
+        got.add((int(gb["track_task"][t]), tuple(gb["hit_cluster"][beg[t]:beg[t] + int(gb["track_nhits"][t])].tolist())))
+    want = set()
+    for e in evs:
+        g1 = G.run_gpu(e, debug=False, debug_tracklets=False)
+        b1 = g1["track_hit_begin"].astype(np.int64)
+        for t in range(g1["n_tracks"]):
+            want.add((int(g1["track_task"][t]) + tbase,
+                      tuple((g1["hit_cluster"][b1[t]:b1[t] + int(g1["track_nhits"][t])].astype(np.int64) + base).tolist())))
+        base += e.n_clusters
+        tbase += e.n_tasks
+    assert got == want
+
+
+def test_result_independent_of_grid_bin_size():
+    """SPEC 2: the grid is acceleration only."""
+    b = generate_config(1)
+    ref = G.run_oracle(b)
+    for lo, hi in ((1.0, 5.0), (8.0, 50.0)):
+        gpu = G.run_gpu(b, params_over=dict(grid_bin_min=lo, grid_bin_max=hi))
+        G.compare(gpu, ref, b.geometry.n_rows, rtol=RTOL)
+
+
+def test_run_to_run_determinism_including_track_order(cfg2):
+    a = G.run_gpu(cfg2, debug=False, debug_tracklets=False)
+    c = G.run_gpu(cfg2, debug=False, debug_tracklets=False)
+    for k in ("track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_par", "track_cov",
+              "track_chi2", "hit_cluster"):
+        assert np.array_equal(a[k], c[k]), k
+
+
+# ---- edge cases ---------------------------------------------------------------------------------
+def test_empty_input_and_empty_tasks():
+    geom = default_geometry(n_sectors=2)
+    empty = batch_from_rows(geom, {}, n_tasks=2)
+    gpu = G.run_gpu(empty)
+    assert gpu["n_tracks"] == 0 and gpu["n_hits"] == 0 and gpu["status"] == 0 and gpu["n_tracklets"] == 0
+    # config 0 event in task 2 of 4, the other tasks empty
+    b0 = generate_config(0)
+    g4 = default_geometry(n_sectors=1)
+    nr = g4.n_rows
+    offs = np.concatenate([np.zeros(2 * nr, np.uint32), b0.row_offsets, np.full(nr, b0.n_clusters, np.uint32)])
+    import dataclasses
+    b = dataclasses.replace(b0, n_tasks=4, row_offsets=offs)
+    gpu = G.run_gpu(b)
+    ref = G.run_oracle(b)
+    G.compare(gpu, ref, nr, rtol=RTOL)
+    assert set(gpu["track_task"].tolist()) == {2}
+
+
+def test_hand_built_rows_ragged_and_ties():
+    """Three straight tracks in a 12-row detector, one with duplicated clusters (equal chi2 ties broken
+    by gid, SPEC 0), rows of 1..3 clusters."""
+    geom = default_geometry(n_sectors=1, n_rows=12)
+    pts = {}
+    for r in range(12):
+        x = float(geom.row_x[r])
+        row = [(0.01 * x, 0.5 * x), (-0.02 * x, 0.2 * x)]
+        if r % 2 == 0:
+            row.append((0.01 * x, 0.5 * x))  # exact duplicate: tie
+        if r >= 3:
+            row.append((5.0 + 0.03 * x, 0.9 * x))
+        pts[(0, r)] = row
+    b = batch_from_rows(geom, pts, n_tasks=1)
+    gpu = G.run_gpu(b)
+    ref = G.run_oracle(b)
+    G.compare(gpu, ref, 12, rtol=RTOL)
+    assert ref.n_tracks >= 2
+
+
+def test_overflow_sets_status_and_never_writes_out_of_bounds():
+    b = generate_config(0)
+    ref = G.run_oracle(b)
+    # tracklet capacity
+    gpu = G.run_gpu(b, debug=False, debug_tracklets=False, max_tracklets=16)
+    assert gpu["status"] & 1 and gpu["n_tracklets"] == 16
+    # track capacity: totals are still reported, only the first slots are written
+    gpu = G.run_gpu(b, debug=False, debug_tracklets=False, track_capacity=8)
+    assert gpu["status"] & 2 and gpu["n_tracks"] == ref.n_tracks
+    # hit capacity
+    gpu = G.run_gpu(b, debug=False, debug_tracklets=False, hit_capacity=100)
+    assert gpu["status"] & 4 and gpu["n_hits"] == len(ref.hit_cluster)
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    """tpc_track_batch_host (the e2e leg of bench.py) gives the same tracks as tpc_track_batch."""
+    import torch
+    from paper_1712_09434_b200 import Tracker
+    b = generate_config(1)
+    dev = torch.device("cuda:0")
+    trk = Tracker(b.geometry, G.tracker_params_for(b))
+    n = b.n_clusters
+    y = torch.from_numpy(np.ascontiguousarray(b.y)).pin_memory()
+    z = torch.from_numpy(np.ascontiguousarray(b.z)).pin_memory()
+    ro = torch.from_numpy(b.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()
+    out = trk.alloc_outputs(n, dev, pinned_host=True)
+    tcap, hcap = out.track_task.shape[0], out.hit_cluster.shape[0]
+    ws = trk.alloc_workspace(trk.host_workspace_bytes(n, b.n_tasks, 0, tcap, hcap), dev)
+    up, down = trk.track_batch_host(y, z, ro, b.n_tasks, out, ws)
+    h = out.header.numpy()
+    assert up == 8 * n + 4 * (b.n_tasks * b.geometry.n_rows + 1)
+    assert down == 16 + 104 * int(h[0]) + 4 * int(h[1])  # 6 words + 5 par + 15 cov per track
+    host = out.to_numpy()
+    trk.close()
+    ref = G.run_oracle(b, dump_tracklets=False)
+    G.compare(host, ref, b.geometry.n_rows, rtol=RTOL, check_tracklets=False)
+
+
+def test_counters_match_the_oracle_counters():
+    """The device counters feed the algorithmic-bytes formula of bench.py."""
+    b = generate_config(1)
+    gpu = G.run_gpu(b, counters=True)
+    ref = G.run_oracle(b)
+    c, o = gpu["counters"], ref.counters
+    assert c["clusters"] == o["clusters"]
+    assert c["start_hits"] == o["start_hits"]
+    assert c["tracklets_built"] == o["tracklets_built"]
+    assert c["tracklets_kept"] == o["tracklets_kept"]
+    assert c["chain_hits"] == o["chain_hits"]
+    assert c["searches"] == o["search_up"] + o["search_dn"]
+    assert c["tracklet_hits"] == o["tracklet_hits"]
+    assert c["row_steps"] == o["row_steps"]
