@@ -25,13 +25,23 @@ enum CounterId {
 static_assert(CN_COUNT == TPC_N_COUNTERS, "counter list and header disagree");
 
 // Grid of one (task,row): bin = iz*ny + iy, iy = clamp((y - y0)*inv), iz likewise.
-// 16 bytes so that one vector load fetches it.
-struct __align__(16) RowGrid {
-  float inv;   // 1 / bin size
-  int32_t ny;  // bins across y
-  int32_t nz;  // bins along z
-  int32_t pad;
+// 16 bytes so that one vector load fetches everything a search needs to know about a row.
+struct __align__(16) RowInfo {
+  float inv;          // 1 / bin size
+  uint32_t ny_nz;     // ny | nz << 16  (bins across y, along z; both <= kMaxBinsPerRow)
+  uint32_t bins_off;  // first entry of this row in Ctx::bins
+  uint32_t row_lo;    // idx of the first cluster of the row (= row_off[tr])
 };
+__device__ __forceinline__ int info_ny(const RowInfo& g) { return (int)(g.ny_nz & 0xFFFFu); }
+__device__ __forceinline__ int info_nz(const RowInfo& g) { return (int)(g.ny_nz >> 16); }
+__device__ __forceinline__ RowInfo load_row_info(const RowInfo* p) {
+  const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+  RowInfo g;
+  g.inv = __uint_as_float(v.x); g.ny_nz = v.y; g.bins_off = v.z; g.row_lo = v.w;
+  return g;
+}
+
+constexpr int kRecFloat4 = 7;  // tracklet record: 7 float4 = x, p[5], c[15], chi2, ndf, first_row, last_row, n_hits, 2 pad
 
 // Everything a kernel needs, passed by value (about 300 bytes of kernel parameters).
 struct Ctx {
@@ -49,19 +59,17 @@ struct Ctx {
   float2* yz;              // [n]  (y,z) in bin-sorted order: rows keep their [row_off[tr], row_off[tr+1]) range
   uint32_t* gid;           // [n]  idx -> gid (index in the input arrays)
   uint32_t* bins;          // [n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
-  RowGrid* rowgrid;        // [n_tr]
+  RowInfo* rowinfo;        // [n_tr]
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   unsigned long long* owner;  // [n] K7 ownership key
   uint32_t* trk_start;     // [max_tracklets] idx of the start hit
   uint32_t* trk_tr;        // [max_tracklets] task*n_rows + row of the start hit
-  int32_t* trk_map;        // [ceil(max_tracklets/32)][n_rows][32] idx or -1
-  int32_t* trk_rows;       // [3][max_tracklets] firstRow, lastRow, nHits
-  int32_t* trk_ndf;        // [max_tracklets]
-  float* trk_state;        // [22][max_tracklets] x, p[5], c[15], chi2
+  uint32_t* trk_hits;      // [max_tracklets][n_rows] hits of the tracklet as idx, ascending row, n_hits entries
+  float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
-  uint32_t* tickets;       // [4] dynamic tile counters: 0 seeds, 1 output, 2 finished output tiles
+  uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2 tracklet queue head, 3 largest row (clusters)
   uint32_t* n_tracklets;   // [1] tracklets built (clamped to max_tracklets)
   uint32_t max_tracklets;
   unsigned long long* counters;  // [CN_COUNT] or nullptr
@@ -81,6 +89,16 @@ __device__ __forceinline__ int bin_coord(float v, float v0, float inv, int n) {
 __device__ __forceinline__ float side_z0(const Ctx& c, uint32_t task) {
   const bool a_side = 2 * (int)(task % (uint32_t)c.n_sectors) < c.n_sectors;
   return a_side ? -1.0f : -(c.z_max + 1.0f);
+}
+
+// task*n_rows + row of idx h: last tr with row_off[tr] <= h
+__device__ __forceinline__ uint32_t find_tr(const Ctx& c, uint32_t h) {
+  uint32_t lo = 0u, hi = c.n_tr;  // row_off[lo] <= h < row_off[hi]
+  while (hi - lo > 1u) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (c.row_off[mid] <= h) lo = mid; else hi = mid;
+  }
+  return lo;
 }
 
 // ---------------------------------------------------------------------------

@@ -6,16 +6,21 @@
 
 namespace tpc {
 
-constexpr int kOutThreads = 128;
+constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
 
-// One thread per tracklet.  Pass 1 counts the hits the tracklet still owns (L1);
-// the block then takes its place in the output with an ordered chained scan over
-// (tracks, hits) packed as tracks<<32 | hits; pass 2 writes the track and its
-// hits as gids in ascending row order (L3).  Output order = tracklet order.
+// One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by one,
+// the 32 lanes testing 32 hits of the tracklet's list at a time (coalesced list read, 32 owner
+// gathers in flight) - L1: hit kept iff the tracklet still owns it; the keep masks stay in
+// shared memory.  The tile then takes its place in the output with an ordered chained scan over
+// (tracks, hits) packed as tracks<<32 | hits.  Pass 2: the warp writes each surviving track - its
+// record as SoA columns and its kept hits as gids in ascending row order (L3).
+// Output order = tracklet order.
 __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
+  extern __shared__ uint32_t s_keep[];  // [kOutThreads][words] keep masks
   __shared__ uint32_t s_warp[33];
   __shared__ uint32_t s_tile;
   __shared__ unsigned long long s_prefix;
+  constexpr unsigned FULL = 0xffffffffu;
   if (threadIdx.x == 0) s_tile = atomicAdd(&c.tickets[1], 1u);
   __syncthreads();
   const uint32_t tile = s_tile;
@@ -23,27 +28,32 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   // the grid covers max_tracklets; tiles past the last tracklet have nothing to add and nobody waits for them
   const uint32_t last_tile = n_trk > 0u ? (n_trk - 1u) / kOutThreads : 0u;
   if (tile > last_tile) return;
-  const uint32_t t = tile * kOutThreads + threadIdx.x;
-  const uint32_t T = c.max_tracklets;
-  const int n_rows = c.n_rows;
-  int first_row = 0, last_row = -1;
-  uint32_t kept = 0u;
-  unsigned long long key = 0ull;
-  if (t < n_trk) {
-    const int n_hits = c.trk_rows[2u * T + t];
-    if (n_hits >= c.prm.min_track_hits) {                              // K6
-      first_row = c.trk_rows[t];
-      last_row = c.trk_rows[T + t];
-      key = ((unsigned long long)(uint32_t)n_hits << 32) |
-            (unsigned long long)(0xFFFFFFFFu - c.gid[c.trk_start[t]]);
-      for (int r = first_row; r <= last_row; ++r) {
-        const int32_t m = c.trk_map[map_index(t, r, n_rows)];
-        if (m >= 0 && c.owner[m] == key) ++kept;                       // L1
-      }
+  const int n_rows = c.n_rows, words = (n_rows + 31) / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t t_warp = tile * kOutThreads + warp * 32;
+  const int min_hits = c.prm.min_track_hits;
+  uint32_t my_kept = 0u;  // lane j: hits tracklet t_warp + j still owns
+  for (int j = 0; j < 32; ++j) {
+    const uint32_t t = t_warp + j;
+    if (t >= n_trk) break;
+    const float4 r5 = c.trk_rec[(size_t)t * kRecFloat4 + 5];
+    const int n_hits = __float_as_int(r5.w);
+    if (n_hits < min_hits) continue;                                   // K6
+    const unsigned long long key = ((unsigned long long)(uint32_t)n_hits << 32) |
+                                   (unsigned long long)(0xFFFFFFFFu - c.gid[c.trk_start[t]]);
+    const uint32_t* hits = c.trk_hits + (size_t)t * (size_t)n_rows;
+    uint32_t kept = 0u;
+    for (int k0 = 0; k0 < n_hits; k0 += 32) {
+      const int k = k0 + lane;
+      const bool own = k < n_hits && c.owner[hits[k]] == key;          // L1
+      const unsigned mask = __ballot_sync(FULL, own);
+      if (lane == 0) s_keep[(warp * 32 + j) * words + (k0 >> 5)] = mask;
+      kept += __popc(mask);
     }
+    if (lane == j) my_kept = kept;
   }
-  const bool is_track = kept >= (uint32_t)c.prm.min_track_hits && kept > 0u;  // L2
-  const uint32_t my_hits = is_track ? kept : 0u;
+  const bool is_track = my_kept >= (uint32_t)min_hits && my_kept > 0u;  // L2
+  const uint32_t my_hits = is_track ? my_kept : 0u;
   uint32_t tot_tracks, tot_hits;
   const uint32_t ex_tracks = block_exclusive_scan(is_track ? 1u : 0u, s_warp, &tot_tracks);
   const uint32_t ex_hits = block_exclusive_scan(my_hits, s_warp, &tot_hits);
@@ -54,36 +64,40 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   }
   __syncthreads();
   const unsigned long long prefix = s_prefix;
-  if (is_track) {
-    const uint32_t slot = (uint32_t)(prefix >> 32) + ex_tracks;
-    const uint32_t hb = (uint32_t)(prefix & 0xFFFFFFFFull) + ex_hits;
-    const tpc_tracks& o = c.out;
-    if (slot >= o.track_capacity) {
-      atomicOr(&o.header[2], TPC_STATUS_TRACK_OVERFLOW);
-    } else {
-      const size_t cap = o.track_capacity;
+  const uint32_t my_slot = (uint32_t)(prefix >> 32) + ex_tracks;
+  const uint32_t my_hb = (uint32_t)(prefix & 0xFFFFFFFFull) + ex_hits;
+  const tpc_tracks& o = c.out;
+  const size_t cap = o.track_capacity;
+  unsigned status = 0u;
+  const unsigned tracks_here = __ballot_sync(FULL, is_track);
+  for (unsigned rest = tracks_here; rest; rest &= rest - 1u) {
+    const int j = __ffs(rest) - 1;
+    const uint32_t t = t_warp + j;
+    const uint32_t slot = __shfl_sync(FULL, my_slot, j), hb = __shfl_sync(FULL, my_hb, j);
+    const uint32_t kept = __shfl_sync(FULL, my_kept, j);
+    if (slot >= o.track_capacity) { status |= TPC_STATUS_TRACK_OVERFLOW; continue; }
+    // record -> SoA columns: lanes 0..22 carry x, p[5], c[15], chi2, ndf
+    const float v = lane < 28 ? reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4)[lane] : 0.0f;
+    if (lane == 0) {
+      o.track_x[slot] = v;
       o.track_task[slot] = c.trk_tr[t] / (uint32_t)n_rows;
       o.track_hit_begin[slot] = hb;
       o.track_nhits[slot] = kept;
-      o.track_ndf[slot] = c.trk_ndf[t];
-      const float* st = c.trk_state + t;
-      o.track_x[slot] = st[0];
-#pragma unroll
-      for (int j = 0; j < 5; ++j) o.track_par[(size_t)j * cap + slot] = st[(size_t)(1 + j) * T];
-#pragma unroll
-      for (int j = 0; j < 15; ++j) o.track_cov[(size_t)j * cap + slot] = st[(size_t)(6 + j) * T];
-      o.track_chi2[slot] = st[(size_t)21 * T];
-      if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) {
-        atomicOr(&o.header[2], TPC_STATUS_HIT_OVERFLOW);
-      } else {
-        uint32_t w = hb;
-        for (int r = first_row; r <= last_row; ++r) {
-          const int32_t m = c.trk_map[map_index(t, r, n_rows)];
-          if (m >= 0 && c.owner[m] == key) o.hit_cluster[w++] = c.gid[m];
-        }
-      }
+    } else if (lane <= 5) o.track_par[(size_t)(lane - 1) * cap + slot] = v;
+    else if (lane <= 20) o.track_cov[(size_t)(lane - 6) * cap + slot] = v;
+    else if (lane == 21) o.track_chi2[slot] = v;
+    else if (lane == 22) o.track_ndf[slot] = __float_as_int(v);
+    if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
+    const int n_hits = __float_as_int(__shfl_sync(FULL, v, 23));
+    const uint32_t* hits = c.trk_hits + (size_t)t * (size_t)n_rows;
+    uint32_t w = hb;
+    for (int k0 = 0; k0 < n_hits; k0 += 32) {
+      const unsigned mask = s_keep[(warp * 32 + j) * words + (k0 >> 5)];
+      if (mask & (1u << lane)) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = c.gid[hits[k0 + lane]];
+      w += __popc(mask);
     }
   }
+  if (status && lane == 0) atomicOr(&o.header[2], status);
   if (threadIdx.x == 0 && tile == last_tile) {  // the last tile knows the totals
     const unsigned long long all = prefix + agg;
     c.out.header[0] = (uint32_t)(all >> 32);
@@ -116,18 +130,20 @@ __global__ void k_debug_tracklets(const Ctx c) {
   const uint32_t n_trk = *c.n_tracklets;
   const tpc_tracks& o = c.out;
   if (t >= n_trk || t >= o.dbg_tracklet_capacity) return;
-  const uint32_t T = c.max_tracklets;
   const int n_rows = c.n_rows;
+  const float* rec = reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4);
+  const int n_hits = __float_as_int(rec[23]);
   if (o.dbg_tracklet_start) o.dbg_tracklet_start[t] = c.gid[c.trk_start[t]];
-  if (o.dbg_tracklet_nhits) o.dbg_tracklet_nhits[t] = (uint32_t)c.trk_rows[2u * T + t];
+  if (o.dbg_tracklet_nhits) o.dbg_tracklet_nhits[t] = (uint32_t)n_hits;
   if (o.dbg_tracklet_par)
-    for (int j = 0; j < 5; ++j) o.dbg_tracklet_par[(size_t)t * 5 + j] = c.trk_state[(size_t)(1 + j) * T + t];
+    for (int j = 0; j < 5; ++j) o.dbg_tracklet_par[(size_t)t * 5 + j] = rec[1 + j];
   if (o.dbg_tracklet_map) {
-    const int first_row = c.trk_rows[t], last_row = c.trk_rows[T + t];
-    for (int r = 0; r < n_rows; ++r) {
-      int32_t m = -1;
-      if (r >= first_row && r <= last_row) m = c.trk_map[map_index(t, r, n_rows)];
-      o.dbg_tracklet_map[(size_t)t * n_rows + r] = m >= 0 ? (int32_t)c.gid[m] : -1;
+    for (int r = 0; r < n_rows; ++r) o.dbg_tracklet_map[(size_t)t * n_rows + r] = -1;
+    const uint32_t tr_base = c.trk_tr[t] / (uint32_t)n_rows * (uint32_t)n_rows;
+    for (int k = 0; k < n_hits; ++k) {
+      const uint32_t m = c.trk_hits[(size_t)t * n_rows + k];
+      const uint32_t r = find_tr(c, m) - tr_base;
+      o.dbg_tracklet_map[(size_t)t * n_rows + r] = (int32_t)c.gid[m];
     }
   }
 }

@@ -2,20 +2,24 @@
 // track following"; L123: "in the track following phase, 1 GPU thread handles 1
 // track").  docs/ARITH_SPEC.md sections 5 (track model) and 6 (K1..K7).
 //
-// One thread per tracklet, the whole filter state (5 parameters, 15 covariance
-// entries, chi2) in registers.  The five passes of SPEC 6 (chain fit, up pass,
-// turn-around, down pass, finish) are ONE loop whose body is a single row step
+// One LANE per tracklet, the whole filter state (5 parameters, 15 covariance
+// entries, chi2) in registers, in a PERSISTENT kernel: a lane whose tracklet has
+// ended takes the next one from a global queue, so the 32 lanes of a warp stay
+// busy although tracklets live for 10..320 row steps.  The five passes of SPEC 6
+// (chain fit, up pass, turn-around, down pass, finish) are ONE loop whose body is
+// a single row step
 //     transport -> choose the hit (chain link / row map / search) -> update
-// with a per-thread phase, so that threads of a warp that are in different
-// passes still execute the same instructions.  Consecutive tracklets start in
-// the same (task,row) (start hits are compacted in idx order), so a warp walks
-// neighbouring rows and bins.
+// with a per-lane phase, so lanes in different passes execute the same
+// instructions.  The row -> hit map of the running tracklet lives in shared
+// memory as row-local indices (16 bit; 32 bit when a row holds >= 65535
+// clusters); when a tracklet ends the WARP writes its hit list, claims the hits
+// (K7, atomicMax) and stores its record cooperatively.
 #pragma once
 #include "device_common.cuh"
 
 namespace tpc {
 
-constexpr int kTrackletThreads = 128;
+constexpr int kTrackletThreads = 128;  // u16 row maps, n_rows <= 192; other shapes: tracklet_threads()
 
 struct TrackState {
   float y, z, s, t, q;  // SPEC 5: y, z, sinphi, dz/dl, q/pT
@@ -121,189 +125,251 @@ __device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, fl
   S.ndf += 2;
 }
 
-// SPEC 5.3 SEARCH (H1..H6) in row-block tr; returns the idx of the best cluster or -1.
+
+// SPEC 5.3 SEARCH (H1..H6) in the row described by g; returns the idx of the best cluster or -1.
+// One flat loop over the window; the bin bounds of the next z row are fetched one row ahead.
 template <bool COUNT>
-__device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, uint32_t tr, int row, float z0,
+__device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g, float y0, float z0,
                                               uint32_t& n_cand) {
   const float y = S.y, z = S.z;
   const float ey = S.c00 + c.sy2, ez = S.c11 + c.sz2;                 // H1
   const float hy2 = fminf(c.prm.accept_k2 * ey, c.smax2);              // H2
   const float hz2 = fminf(c.prm.accept_k2 * ez, c.smax2);
   const float wy = sqrtf(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrtf(fmaxf(hz2, 0.0f)) + kGridMargin;
-  const RowGrid g = c.rowgrid[tr];
-  const float y0 = -c.ymax[row];
-  const uint32_t* bins = c.bins + bins_base(c, tr, c.row_off[tr]);
-  const int iy0 = bin_coord(y - wy, y0, g.inv, g.ny), iy1 = bin_coord(y + wy, y0, g.inv, g.ny);
-  const int iz0 = bin_coord(z - wz, z0, g.inv, g.nz), iz1 = bin_coord(z + wz, z0, g.inv, g.nz);
+  const int ny = info_ny(g), nz = info_nz(g);
+  const int iy0 = bin_coord(y - wy, y0, g.inv, ny), iy1 = bin_coord(y + wy, y0, g.inv, ny);
+  const int iz0 = bin_coord(z - wz, z0, g.inv, nz), iz1 = bin_coord(z + wz, z0, g.inv, nz);
+  const uint32_t* bp = c.bins + g.bins_off + iz0 * ny;
+  int rows_left = iz1 - iz0;
+  uint32_t i = bp[iy0], e = bp[iy1 + 1], i2 = 0u, e2 = 0u;
+  if (rows_left > 0) { i2 = bp[ny + iy0]; e2 = bp[ny + iy1 + 1]; }
   bool have = false;
   float best = 0.0f;
   uint32_t bi = 0u;
-  for (int iz = iz0; iz <= iz1; ++iz) {
-    const uint32_t b0 = bins[iz * g.ny + iy0], b1 = bins[iz * g.ny + iy1 + 1];
-    for (uint32_t i = b0; i < b1; ++i) {
-      const float2 p = c.yz[i];
-      if (COUNT) ++n_cand;
-      const float dy = p.x - y, dz = p.y - z;                          // H3
-      const float dy2 = dy * dy, dz2 = dz * dz;
-      if (!(dy2 <= hy2 && dz2 <= hz2)) continue;                       // H4
+  while (true) {
+    if (i >= e) {
+      if (rows_left <= 0) break;
+      --rows_left;
+      bp += ny;
+      i = i2; e = e2;
+      if (rows_left > 0) { i2 = bp[ny + iy0]; e2 = bp[ny + iy1 + 1]; }
+      continue;
+    }
+    const float2 p = c.yz[i];
+    if (COUNT) ++n_cand;
+    const float dy = p.x - y, dz = p.y - z;                            // H3
+    const float dy2 = dy * dy, dz2 = dz * dz;
+    if (dy2 <= hy2 && dz2 <= hz2) {                                    // H4
       const float d = (dy2 * ez) + (dz2 * ey);                         // H5
       bool take = !have || d < best;                                   // H6
       if (have && d == best) take = c.gid[i] < c.gid[bi];
       if (take) { have = true; best = d; bi = i; }
     }
+    ++i;
   }
   return have ? (int32_t)bi : -1;
 }
 
-enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4 };
+enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4, PH_ENDED = 5, PH_FETCH = 6, PH_EXIT = 7 };
 
-__device__ __forceinline__ size_t map_index(uint32_t t, int row, int n_rows) {
-  return ((size_t)(t >> 5) * (size_t)n_rows + (size_t)row) * 32u + (t & 31u);
+// Threads per block and dynamic shared memory of k_tracklets for a detector of n_rows rows.
+__host__ __device__ inline int tracklet_threads(int n_rows, int map_bytes) {
+  const int per_thread = n_rows * map_bytes;
+  return per_thread <= 384 ? 128 : (per_thread <= 1024 ? 64 : 32);
+}
+__host__ __device__ inline size_t tracklet_smem(int n_rows, int map_bytes) {
+  return (size_t)((n_rows * 4 + 15) / 16 * 16) + (size_t)n_rows * map_bytes * tracklet_threads(n_rows, map_bytes);
 }
 
-template <bool COUNT>
+template <typename MapT, bool COUNT>
 __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
-  __shared__ float sX[kMaxRows];
-  const uint32_t n_trk = *c.n_tracklets;
-  if (blockIdx.x * kTrackletThreads >= n_trk) return;
-  for (int r = threadIdx.x; r < c.n_rows; r += kTrackletThreads) sX[r] = c.X[r];
+  extern __shared__ __align__(16) unsigned char trk_smem[];
+  constexpr MapT kNone = (MapT)~(MapT)0;
+  constexpr unsigned FULL = 0xffffffffu;
+  // rows of >= 65535 clusters need the 32-bit instantiation; exactly one of the two launches works
+  const bool big_rows = c.tickets[3] >= 0xFFFFu;
+  if (big_rows != (sizeof(MapT) == 4)) return;
+  const int n_rows = c.n_rows, nthr = (int)blockDim.x, tid = (int)threadIdx.x, lane = tid & 31;
+  float* sX = reinterpret_cast<float*>(trk_smem);
+  MapT* s_map = reinterpret_cast<MapT*>(trk_smem + (n_rows * 4 + 15) / 16 * 16);  // [n_rows][nthr]
+  for (int r = tid; r < n_rows; r += nthr) sX[r] = c.X[r];
   __syncthreads();
-  const uint32_t t = blockIdx.x * kTrackletThreads + threadIdx.x;
-  if (t >= n_trk) return;
-  const int n_rows = c.n_rows;
-  const uint32_t h0 = c.trk_start[t];
-  const uint32_t tr0 = c.trk_tr[t];
-  const uint32_t task = tr0 / (uint32_t)n_rows;
-  const int r0 = (int)(tr0 - task * (uint32_t)n_rows);
-  const uint32_t tr_base = task * (uint32_t)n_rows;
-  const float z0 = side_z0(c, task);
+  const uint32_t n_trk = *c.n_tracklets;
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
-  const int max_gap = c.prm.max_row_gap;
-  int32_t* map = c.trk_map;
+  const int max_gap = c.prm.max_row_gap, min_hits = c.prm.min_track_hits;
 
-  // K1 seed
   TrackState S;
-  const uint32_t h1 = (uint32_t)c.clean_up[h0];
-  {
-    const float2 p0 = c.yz[h0], p1 = c.yz[h1];
-    const float dx = sX[r0 + 1] - sX[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
-    const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
-    S.y = p1.x; S.z = p1.y; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
-    S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
-    S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
-    S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
-    S.chi2 = 0.0f; S.ndf = -5;
-  }
-  map[map_index(t, r0, n_rows)] = (int32_t)h0;
-  map[map_index(t, r0 + 1, n_rows)] = (int32_t)h1;
-  int row_cur = r0 + 1, first_row = r0, last_row = r0 + 1, n_hits = 2, gap = 0;
-  int32_t last_hit = (int32_t)h1;
-  int32_t next_chain = c.clean_up[h1];
-  int r_down = 0;
-  int phase = next_chain >= 0 ? PH_CHAIN : PH_UP;
-  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_chain = 2u;
+  S.y = S.z = S.s = S.t = S.q = 0.0f;
+  S.c00 = S.c10 = S.c11 = S.c20 = S.c21 = S.c22 = S.c30 = S.c31 = S.c32 = S.c33 = 0.0f;
+  S.c40 = S.c41 = S.c42 = S.c43 = S.c44 = 0.0f;
+  S.chi2 = 0.0f; S.ndf = -5;
+  uint32_t t = 0u, tr_base = 0u, h0 = 0u;
+  float z0 = 0.0f;
+  int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
+  int32_t last_hit = -1, next_chain = -1;
+  int phase = PH_FETCH;
+  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_chain = 0u, n_kept = 0u, n_kept_hits = 0u;
 
   while (true) {
-    // which row does this step go to?
-    if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
-    if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
-    int rt;
-    if (phase <= PH_UP) rt = row_cur + 1;
-    else if (phase == PH_TURN) rt = last_row;
-    else if (phase == PH_DOWN) rt = r_down;
-    else rt = first_row;
-    bool ok = true;
-    if (rt != row_cur) {
-      ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
-      if (ok) row_cur = rt;
-      if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
-    }
-    if (phase == PH_FINISH) break;                                    // K6
-    if (phase == PH_TURN) {                                           // K4
-      const float f = c.prm.turn_cov_scale;
-      S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
-      S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
-      S.chi2 = 0.0f; S.ndf = -5; gap = 0;
-      if (row_cur == last_row) {
-        const float2 p = c.yz[last_hit];
-        update_hit(S, p.x, p.y, sy2, sz2);
+    // (A) tracklets that ended in the last step: the warp stores them one by one (hit list in
+    //     ascending row order, K7 ownership claims, record)
+    unsigned ended = __ballot_sync(FULL, phase == PH_ENDED);
+    while (ended) {
+      const int L = __ffs(ended) - 1;
+      ended &= ended - 1u;
+      const uint32_t ft = __shfl_sync(FULL, t, L), ftr = __shfl_sync(FULL, tr_base, L);
+      const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
+      const int fn = __shfl_sync(FULL, n_hits, L);
+      const uint32_t fh0 = __shfl_sync(FULL, h0, L);
+      const int col = (tid & ~31) + L;
+      unsigned long long key = 0ull;
+      if (fn >= min_hits)  // K6, K7: longest tracklet wins, then the smaller start-hit gid
+        key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - c.gid[fh0]);
+      uint32_t* hits_out = c.trk_hits + (size_t)ft * (size_t)n_rows;
+      uint32_t wpos = 0u;
+      for (int rb = ffirst; rb <= flast; rb += 32) {
+        const int r = rb + lane;
+        bool has = false;
+        uint32_t idx = 0u;
+        if (r <= flast) {
+          const MapT m = s_map[r * nthr + col];
+          if (m != kNone) { has = true; idx = c.row_off[ftr + (uint32_t)r] + (uint32_t)m; }
+        }
+        const unsigned mask = __ballot_sync(FULL, has);
+        if (has) {
+          hits_out[wpos + __popc(mask & ((1u << lane) - 1u))] = idx;
+          if (key) atomicMax(&c.owner[idx], key);
+        }
+        wpos += __popc(mask);
       }
-      r_down = last_row - 1;
-      phase = PH_DOWN;
-      continue;
-    }
-    if (!ok) {  // transport failed: K2/K3 -> turn-around, K5 -> finish
-      phase = (phase == PH_DOWN) ? PH_FINISH : PH_TURN;
-      continue;
-    }
-    int32_t hit = -1;
-    bool do_search = false;
-    if (phase == PH_CHAIN) hit = next_chain;                          // K2
-    else if (phase == PH_UP) do_search = true;                        // K3
-    else {                                                            // K5
-      if (rt >= r0) {
-        hit = map[map_index(t, rt, n_rows)];
-        do_search = hit < 0;
-      } else {
-        do_search = true;
+      if (lane == L) {
+        float4* rec = c.trk_rec + (size_t)t * kRecFloat4;
+        rec[0] = make_float4(sX[row_cur], S.y, S.z, S.s);
+        rec[1] = make_float4(S.t, S.q, S.c00, S.c10);
+        rec[2] = make_float4(S.c11, S.c20, S.c21, S.c22);
+        rec[3] = make_float4(S.c30, S.c31, S.c32, S.c33);
+        rec[4] = make_float4(S.c40, S.c41, S.c42, S.c43);
+        rec[5] = make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits));
+        rec[6] = make_float4(__int_as_float(first_row), __int_as_float(last_row), 0.0f, 0.0f);
+        if (COUNT && key) { ++n_kept; n_kept_hits += (uint32_t)n_hits; }
+        phase = PH_FETCH;
       }
     }
-    if (do_search) {
-      if (COUNT) ++n_search;
-      hit = search_row<COUNT>(c, S, tr_base + (uint32_t)rt, rt, z0, n_cand);
-    }
-    if (hit >= 0) {
-      const float2 p = c.yz[hit];
-      update_hit(S, p.x, p.y, sy2, sz2);
-    }
-    if (phase == PH_CHAIN) {
-      map[map_index(t, rt, n_rows)] = hit;
-      last_row = rt; last_hit = hit; ++n_hits;
-      if (COUNT) ++n_chain;
-      next_chain = c.clean_up[hit];
-      if (next_chain < 0) { phase = PH_UP; gap = 0; }
-    } else if (phase == PH_UP) {
-      map[map_index(t, rt, n_rows)] = hit;
-      if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
-      else if (++gap > max_gap) phase = PH_TURN;
-    } else {  // PH_DOWN
-      if (do_search) {
-        map[map_index(t, rt, n_rows)] = hit;
-        if (hit >= 0) {
-          ++n_hits;
-          if (rt < first_row) { first_row = rt; gap = 0; }
-        } else if (rt < first_row) {
-          if (++gap > max_gap) phase = PH_FINISH;
+    // (B) lanes without a tracklet take the next ones from the queue (K1 seed)
+    const unsigned need = __ballot_sync(FULL, phase == PH_FETCH);
+    if (need) {
+      uint32_t base = 0u;
+      if (lane == 0) base = atomicAdd(&c.tickets[2], (uint32_t)__popc(need));
+      base = __shfl_sync(FULL, base, 0);
+      if (phase == PH_FETCH) {
+        t = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
+        if (t >= n_trk) {
+          phase = PH_EXIT;
+        } else {
+          h0 = c.trk_start[t];
+          const uint32_t tr0 = c.trk_tr[t];
+          const uint32_t task = tr0 / (uint32_t)n_rows;
+          r0 = (int)(tr0 - task * (uint32_t)n_rows);
+          tr_base = task * (uint32_t)n_rows;
+          z0 = side_z0(c, task);
+          const uint32_t h1 = (uint32_t)c.clean_up[h0];
+          const float2 p0 = c.yz[h0], p1 = c.yz[h1];
+          const float dx = sX[r0 + 1] - sX[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
+          const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
+          S.y = p1.x; S.z = p1.y; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
+          S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
+          S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
+          S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
+          S.chi2 = 0.0f; S.ndf = -5;
+          s_map[r0 * nthr + tid] = (MapT)(h0 - c.row_off[tr0]);
+          s_map[(r0 + 1) * nthr + tid] = (MapT)(h1 - c.row_off[tr0 + 1u]);
+          row_cur = r0 + 1; first_row = r0; last_row = r0 + 1; n_hits = 2; gap = 0; r_down = 0;
+          last_hit = (int32_t)h1;
+          next_chain = c.clean_up[h1];
+          phase = next_chain >= 0 ? PH_CHAIN : PH_UP;
+          if (COUNT) n_chain += 2u;
         }
       }
-      --r_down;
     }
-  }
-
-  // tracklet record
-  const uint32_t T = c.max_tracklets;
-  c.trk_rows[t] = first_row; c.trk_rows[T + t] = last_row; c.trk_rows[2u * T + t] = n_hits;
-  c.trk_ndf[t] = S.ndf;
-  float* st = c.trk_state + t;
-  st[0 * (size_t)T] = sX[row_cur];
-  st[1 * (size_t)T] = S.y; st[2 * (size_t)T] = S.z; st[3 * (size_t)T] = S.s; st[4 * (size_t)T] = S.t;
-  st[5 * (size_t)T] = S.q;
-  st[6 * (size_t)T] = S.c00; st[7 * (size_t)T] = S.c10; st[8 * (size_t)T] = S.c11; st[9 * (size_t)T] = S.c20;
-  st[10 * (size_t)T] = S.c21; st[11 * (size_t)T] = S.c22; st[12 * (size_t)T] = S.c30; st[13 * (size_t)T] = S.c31;
-  st[14 * (size_t)T] = S.c32; st[15 * (size_t)T] = S.c33; st[16 * (size_t)T] = S.c40; st[17 * (size_t)T] = S.c41;
-  st[18 * (size_t)T] = S.c42; st[19 * (size_t)T] = S.c43; st[20 * (size_t)T] = S.c44; st[21 * (size_t)T] = S.chi2;
-
-  // K7 ownership: longest tracklet wins, then the smaller start-hit gid
-  if (n_hits >= c.prm.min_track_hits) {
-    const unsigned long long key =
-        ((unsigned long long)(uint32_t)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - c.gid[h0]);
-    for (int r = first_row; r <= last_row; ++r) {
-      const int32_t m = map[map_index(t, r, n_rows)];
-      if (m >= 0) atomicMax(&c.owner[m], key);
-    }
-    if (COUNT) {
-      atomicAdd(&c.counters[CN_TRACKLETS_KEPT], 1ull);
-      atomicAdd(&c.counters[CN_TRACKLET_HITS], (unsigned long long)n_hits);
+    if (__ballot_sync(FULL, phase != PH_EXIT) == 0u) break;
+    // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping
+    if (phase <= PH_FINISH) {
+      if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
+      if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
+      int rt;
+      if (phase <= PH_UP) rt = row_cur + 1;
+      else if (phase == PH_TURN) rt = last_row;
+      else if (phase == PH_DOWN) rt = r_down;
+      else rt = first_row;
+      // the row's grid header does not depend on the state: its load overlaps the transport arithmetic
+      const RowInfo g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
+      bool ok = true;
+      if (rt != row_cur) {
+        ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
+        if (ok) row_cur = rt;
+        if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
+      }
+      int32_t hit = -1;
+      bool book = false, searched = false;
+      if (phase == PH_FINISH) {                                         // K6
+        phase = PH_ENDED;
+      } else if (phase == PH_TURN) {                                    // K4
+        const float f = c.prm.turn_cov_scale;
+        S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
+        S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
+        S.chi2 = 0.0f; S.ndf = -5; gap = 0;
+        if (row_cur == last_row) hit = last_hit;                        // the lastRow hit opens the down pass
+        r_down = last_row - 1;
+        phase = PH_DOWN;
+      } else if (!ok) {  // transport failed: K2/K3 -> turn-around, K5 -> finish
+        phase = (phase == PH_DOWN) ? PH_FINISH : PH_TURN;
+      } else {
+        book = true;
+        if (phase == PH_CHAIN) {                                        // K2
+          hit = next_chain;
+          next_chain = c.clean_up[hit];
+        } else if (phase == PH_UP) {                                    // K3
+          searched = true;
+        } else {                                                        // K5
+          searched = true;
+          if (rt >= r0) {
+            const MapT m = s_map[rt * nthr + tid];
+            if (m != kNone) { hit = (int32_t)(g.row_lo + (uint32_t)m); searched = false; }
+          }
+        }
+        if (searched) {
+          if (COUNT) ++n_search;
+          hit = search_row<COUNT>(c, S, g, -c.ymax[rt], z0, n_cand);
+        }
+      }
+      if (hit >= 0) {
+        const float2 p = c.yz[hit];
+        update_hit(S, p.x, p.y, sy2, sz2);
+      }
+      if (book) {
+        const MapT m = hit >= 0 ? (MapT)((uint32_t)hit - g.row_lo) : kNone;
+        if (phase == PH_CHAIN) {
+          s_map[rt * nthr + tid] = m;
+          last_row = rt; last_hit = hit; ++n_hits;
+          if (COUNT) ++n_chain;
+          if (next_chain < 0) { phase = PH_UP; gap = 0; }
+        } else if (phase == PH_UP) {
+          s_map[rt * nthr + tid] = m;
+          if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
+          else if (++gap > max_gap) phase = PH_TURN;
+        } else {  // PH_DOWN
+          if (searched) {
+            s_map[rt * nthr + tid] = m;
+            if (hit >= 0) {
+              ++n_hits;
+              if (rt < first_row) { first_row = rt; gap = 0; }
+            } else if (rt < first_row) {
+              if (++gap > max_gap) phase = PH_FINISH;
+            }
+          }
+          --r_down;
+        }
+      }
     }
   }
   if (COUNT) {
@@ -311,6 +377,8 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
     atomicAdd(&c.counters[CN_CANDIDATES], (unsigned long long)n_cand);
     atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
+    atomicAdd(&c.counters[CN_TRACKLETS_KEPT], (unsigned long long)n_kept);
+    atomicAdd(&c.counters[CN_TRACKLET_HITS], (unsigned long long)n_kept_hits);
   }
 }
 

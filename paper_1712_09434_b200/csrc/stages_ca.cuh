@@ -1,7 +1,7 @@
 // Cellular-Automaton stages of the TPC sector tracker (PAPER.md L121, L123:
 // "1 GPU thread handles 1 cluster" in the CA phase):
 //   a1 k_grid_build   - per (task,row) counting sort of the clusters into a y-z grid (SPEC 2)
-//   a2 k_neighbours   - best (up,down) pair by straight-line chi2 (SPEC 3, N1..N5)
+//   (a2, the neighbour finder, is in stage_neighbours.cuh)
 //   a3 k_clean        - keep a link iff reciprocated (SPEC 4, C1; C2 is evaluated where needed)
 //   a4 k_seeds        - start hits with a chain of >= min_seed_hits, compacted in idx order (S1..S3)
 #pragma once
@@ -19,20 +19,23 @@ namespace tpc {
 // ---------------------------------------------------------------------------
 constexpr int kGridThreads = 128;
 
-__device__ __forceinline__ RowGrid make_row_grid(const Ctx& c, int row, uint32_t n) {
+__device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, int row, uint32_t lo, uint32_t n) {
   const float W = 2.0f * c.ymax[row], L = c.z_max + 2.0f;
   float B = sqrtf((W * L) / (float)(n > 0u ? n : 1u));
   B = fminf(fmaxf(B, c.prm.grid_bin_min), c.prm.grid_bin_max);
-  RowGrid g;
+  RowInfo g;
+  int ny, nz;
   while (true) {
     g.inv = 1.0f / B;
-    g.ny = (int)(W * g.inv) + 1;
-    g.nz = (int)(L * g.inv) + 1;
-    const long long nb = (long long)g.ny * g.nz;
+    ny = (int)(W * g.inv) + 1;
+    nz = (int)(L * g.inv) + 1;
+    const long long nb = (long long)ny * nz;
     if (nb + 1 <= (long long)n + kBinPad && nb <= (long long)kMaxBinsPerRow) break;
     B = B * 1.25f;  // too many bins for the slot of this row: coarser grid
   }
-  g.pad = 0;
+  g.ny_nz = (uint32_t)ny | ((uint32_t)nz << 16);
+  g.bins_off = bins_base(c, tr, lo);
+  g.row_lo = lo;
   return g;
 }
 
@@ -44,15 +47,19 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   const int row = (int)(tr % (uint32_t)c.n_rows);
   const uint32_t task = tr / (uint32_t)c.n_rows;
   const uint32_t lo = c.row_off[tr], hi = c.row_off[tr + 1], n = hi - lo;
-  const RowGrid g = make_row_grid(c, row, n);
-  const int nb = g.ny * g.nz;
+  const RowInfo g = make_row_info(c, tr, row, lo, n);
+  const int g_ny = info_ny(g), g_nz = info_nz(g);
+  const int nb = g_ny * g_nz;
   const float y0 = -c.ymax[row], z0 = side_z0(c, task);
   const int tid = threadIdx.x;
-  if (tid == 0) c.rowgrid[tr] = g;
+  if (tid == 0) {
+    c.rowinfo[tr] = g;
+    if (n >= 0xFFFFu) atomicMax(&c.tickets[3], n);  // rows this large need the 32-bit row maps of a5
+  }
   for (int b = tid; b <= nb; b += kGridThreads) s_cnt[b] = 0u;
   __syncthreads();
   for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
-    const int bin = bin_coord(c.z[i], z0, g.inv, g.nz) * g.ny + bin_coord(c.y[i], y0, g.inv, g.ny);
+    const int bin = bin_coord(c.z[i], z0, g.inv, g_nz) * g_ny + bin_coord(c.y[i], y0, g.inv, g_ny);
     atomicAdd(&s_cnt[bin], 1u);
   }
   __syncthreads();
@@ -81,14 +88,14 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   uint32_t run = s_part[tid];
   for (int b = b0; b < b1; ++b) { const uint32_t t = s_cnt[b]; s_cnt[b] = run; run += t; }
   __syncthreads();
-  uint32_t* gbins = c.bins + bins_base(c, tr, lo);
+  uint32_t* gbins = c.bins + g.bins_off;
   for (int b = tid; b < nb; b += kGridThreads) gbins[b] = lo + s_cnt[b];
   if (tid == 0) gbins[nb] = hi;
   __syncthreads();
   // scatter; s_cnt[b] becomes the running end of bin b
   for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
     const float y = c.y[i], z = c.z[i];
-    const int bin = bin_coord(z, z0, g.inv, g.nz) * g.ny + bin_coord(y, y0, g.inv, g.ny);
+    const int bin = bin_coord(z, z0, g.inv, g_nz) * g_ny + bin_coord(y, y0, g.inv, g_ny);
     const uint32_t pos = lo + atomicAdd(&s_cnt[bin], 1u);
     c.yz[pos] = make_float2(y, z);
     c.gid[pos] = i;
@@ -112,92 +119,6 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
 }
 
 // ---------------------------------------------------------------------------
-// a2  neighbour finder (SPEC 3).  One block per (task,row); one thread per
-// cluster of the row, in idx order so that the lanes of a warp look at the same
-// few bins of rows r+1 and r-1.
-// ---------------------------------------------------------------------------
-constexpr int kNfThreads = 128;
-
-struct Window {  // bin range of one search window in one row
-  const uint32_t* bins;  // first bin of the row
-  int ny, iy0, iy1, iz0, iz1;
-};
-
-__device__ __forceinline__ Window make_window(const Ctx& c, uint32_t tr, int row, float z0, float ylo, float yhi,
-                                              float zlo, float zhi) {
-  const RowGrid g = c.rowgrid[tr];
-  const float y0 = -c.ymax[row];
-  Window w;
-  w.bins = c.bins + bins_base(c, tr, c.row_off[tr]);
-  w.ny = g.ny;
-  w.iy0 = bin_coord(ylo, y0, g.inv, g.ny);
-  w.iy1 = bin_coord(yhi, y0, g.inv, g.ny);
-  w.iz0 = bin_coord(zlo, z0, g.inv, g.nz);
-  w.iz1 = bin_coord(zhi, z0, g.inv, g.nz);
-  return w;
-}
-
-template <bool COUNT>
-__global__ void __launch_bounds__(kNfThreads) k_neighbours(const Ctx c) {
-  const uint32_t tr = blockIdx.x;
-  const int row = (int)(tr % (uint32_t)c.n_rows);
-  const uint32_t task = tr / (uint32_t)c.n_rows;
-  const uint32_t lo = c.row_off[tr], hi = c.row_off[tr + 1];
-  if (row == 0 || row == c.n_rows - 1) {  // SPEC 3: no links in the first and last row
-    for (uint32_t i = lo + threadIdx.x; i < hi; i += kNfThreads) { c.link_up[i] = -1; c.link_dn[i] = -1; }
-    return;
-  }
-  const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max, M = kGridMargin;
-  const float b = c.dx_dn[row], a_ = c.dx_up[row];                 // N4
-  const float ratio_up = c.ratio_up[row], ratio_dn = c.ratio_dn[row];
-  const float wy = c.wy, wz = c.wz;
-  const float z0 = side_z0(c, task);
-  unsigned long long n_pairs = 0ull;
-  for (uint32_t i = lo + threadIdx.x; i < hi; i += kNfThreads) {
-    const float2 h = c.yz[i];
-    const float y = h.x, z = h.y;
-    const float zu = z * ratio_up, zd = z * ratio_dn;              // N1
-    const Window wu = make_window(c, tr + 1, row + 1, z0, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M);
-    const Window wd = make_window(c, tr - 1, row - 1, z0, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M);
-    bool have = false;
-    float best = 0.0f;
-    uint32_t bu = 0u, bd = 0u, bgu = 0u, bgd = 0u;  // idx and gid of the best pair
-    for (int izu = wu.iz0; izu <= wu.iz1; ++izu) {
-      const uint32_t u0 = wu.bins[izu * wu.ny + wu.iy0], u1 = wu.bins[izu * wu.ny + wu.iy1 + 1];
-      for (uint32_t u = u0; u < u1; ++u) {
-        const float2 pu = c.yz[u];
-        if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) continue;   // N2
-        const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
-        for (int izd = wd.iz0; izd <= wd.iz1; ++izd) {
-          const uint32_t d0 = wd.bins[izd * wd.ny + wd.iy0], d1 = wd.bins[izd * wd.ny + wd.iy1 + 1];
-          for (uint32_t d = d0; d < d1; ++d) {
-            const float2 pd = c.yz[d];
-            if (!(fabsf(pd.x - y) <= HY && fabsf(pd.y - zd) <= HZ)) continue;  // N3
-            const float dy = ty - ((y - pd.x) * a_);                          // N4
-            const float dz = tz - ((z - pd.y) * a_);
-            const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
-            if (COUNT) ++n_pairs;
-            if (!(chi < CHI_MAX)) continue;                                   // N5
-            bool take = !have || chi < best;
-            if (have && chi == best) {  // tie: lexicographic (gid_u, gid_d)
-              const uint32_t gu = c.gid[u], gd = c.gid[d];
-              take = gu < bgu || (gu == bgu && gd < bgd);
-            }
-            if (take) {
-              have = true; best = chi; bu = u; bd = d;
-              bgu = c.gid[u]; bgd = c.gid[d];
-            }
-          }
-        }
-      }
-    }
-    c.link_up[i] = have ? (int32_t)bu : -1;
-    c.link_dn[i] = have ? (int32_t)bd : -1;
-  }
-  if (COUNT && n_pairs) atomicAdd(&c.counters[CN_NF_PAIRS], n_pairs);
-}
-
-// ---------------------------------------------------------------------------
 // a3  neighbour cleaner (SPEC 4, C1): clean_up[h] = up[h] iff dn[up[h]] == h.
 // One thread per cluster.  Also clears the ownership words of K7.
 // ---------------------------------------------------------------------------
@@ -218,16 +139,6 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 constexpr int kSeedThreads = 256;
 constexpr int kSeedItems = 4;
 constexpr uint32_t kSeedTile = kSeedThreads * kSeedItems;
-
-// task*n_rows + row of idx h: last tr with row_off[tr] <= h
-__device__ __forceinline__ uint32_t find_tr(const Ctx& c, uint32_t h) {
-  uint32_t lo = 0u, hi = c.n_tr;  // row_off[lo] <= h < row_off[hi]
-  while (hi - lo > 1u) {
-    const uint32_t mid = (lo + hi) >> 1;
-    if (c.row_off[mid] <= h) lo = mid; else hi = mid;
-  }
-  return lo;
-}
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {

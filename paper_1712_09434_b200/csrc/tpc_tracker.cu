@@ -15,6 +15,7 @@
 
 #include "../../include/tpc_tracker.h"
 #include "device_common.cuh"
+#include "stage_neighbours.cuh"
 #include "stage_output.cuh"
 #include "stage_tracklet.cuh"
 #include "stages_ca.cuh"
@@ -29,6 +30,10 @@ struct tpc_tracker {
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
+  // persistent tracklet kernel: [map width 16/32 bit][counters off/on] -> blocks that fit the device at once
+  int trk_threads[2] = {0, 0};
+  size_t trk_smem[2] = {0, 0};
+  int trk_grid[2][2] = {{0, 0}, {0, 0}};
   // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
   bool timing_on = false;
   std::vector<cudaEvent_t> ev;
@@ -61,8 +66,8 @@ uint32_t resolve_max_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tr
 
 // Offsets of every workspace array, in bytes.
 struct Carve {
-  size_t yz, gid, bins, rowgrid, link_up, link_dn, clean_up, owner, trk_start, trk_tr, trk_map, trk_rows, trk_ndf,
-      trk_state, zero_begin, scan_seed, scan_out, tickets, n_tracklets, zero_end, total;
+  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, owner, trk_start, trk_tr, trk_hits, trk_rec, zero_begin,
+      scan_seed, scan_out, tickets, n_tracklets, zero_end, total;
   uint32_t seed_tiles, out_tiles;
 };
 
@@ -74,18 +79,16 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
   c.yz = take(n4 * sizeof(float2));
   c.gid = take(n4 * sizeof(uint32_t));
-  c.bins = take(((size_t)n + n_tr * kBinPad + 1) * sizeof(uint32_t));
-  c.rowgrid = take((n_tr + 1) * sizeof(RowGrid));
+  c.bins = take(((size_t)n + n_tr * kBinPad + 16) * sizeof(uint32_t));  // + slack of the 16-byte aligned bulk copies
+  c.rowinfo = take((n_tr + 1) * sizeof(RowInfo));
   c.link_up = take(n4 * sizeof(int32_t));
   c.link_dn = take(n4 * sizeof(int32_t));
   c.clean_up = take(n4 * sizeof(int32_t));
   c.owner = take(n4 * sizeof(unsigned long long));
   c.trk_start = take((size_t)T * sizeof(uint32_t));
   c.trk_tr = take((size_t)T * sizeof(uint32_t));
-  c.trk_map = take(((size_t)T + 31) / 32 * 32 * n_rows * sizeof(int32_t));
-  c.trk_rows = take((size_t)3 * T * sizeof(int32_t));
-  c.trk_ndf = take((size_t)T * sizeof(int32_t));
-  c.trk_state = take((size_t)22 * T * sizeof(float));
+  c.trk_hits = take((size_t)T * n_rows * sizeof(uint32_t));
+  c.trk_rec = take((size_t)T * kRecFloat4 * sizeof(float4));
   c.seed_tiles = (uint32_t)(((size_t)n + kSeedTile - 1) / kSeedTile);
   if (c.seed_tiles == 0) c.seed_tiles = 1;
   c.out_tiles = (uint32_t)(((size_t)T + kOutThreads - 1) / kOutThreads);
@@ -93,7 +96,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.zero_begin = off;  // everything from here to zero_end is cleared by one memset per call
   c.scan_seed = take((size_t)c.seed_tiles * sizeof(unsigned long long));
   c.scan_out = take((size_t)c.out_tiles * sizeof(unsigned long long));
-  c.tickets = take(4 * sizeof(uint32_t));
+  c.tickets = take(8 * sizeof(uint32_t));
   c.n_tracklets = take(sizeof(uint32_t));
   c.zero_end = off;
   c.total = off;
@@ -124,12 +127,11 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.y = in->y; c.z = in->z; c.row_off = in->row_offsets;
   c.n = in->n_clusters; c.n_tasks = in->n_tasks; c.n_tr = in->n_tasks * (uint32_t)t->n_rows;
   c.yz = (float2*)(ws + cv.yz); c.gid = (uint32_t*)(ws + cv.gid); c.bins = (uint32_t*)(ws + cv.bins);
-  c.rowgrid = (RowGrid*)(ws + cv.rowgrid);
+  c.rowinfo = (RowInfo*)(ws + cv.rowinfo);
   c.link_up = (int32_t*)(ws + cv.link_up); c.link_dn = (int32_t*)(ws + cv.link_dn);
   c.clean_up = (int32_t*)(ws + cv.clean_up); c.owner = (unsigned long long*)(ws + cv.owner);
   c.trk_start = (uint32_t*)(ws + cv.trk_start); c.trk_tr = (uint32_t*)(ws + cv.trk_tr);
-  c.trk_map = (int32_t*)(ws + cv.trk_map); c.trk_rows = (int32_t*)(ws + cv.trk_rows);
-  c.trk_ndf = (int32_t*)(ws + cv.trk_ndf); c.trk_state = (float*)(ws + cv.trk_state);
+  c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
   c.max_tracklets = T;
@@ -194,6 +196,32 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
     cudaGetLastError();
     return rc;
   }
+  // launch shape of the persistent tracklet constructor: as many blocks as the device holds at once
+  int dev = 0, n_sm = 0;
+  e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  for (int w = 0; w < 2 && e == cudaSuccess; ++w) {
+    const int map_bytes = w ? 4 : 2;
+    t->trk_threads[w] = tracklet_threads(t->n_rows, map_bytes);
+    t->trk_smem[w] = tracklet_smem(t->n_rows, map_bytes);
+    for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
+      const void* fn = w ? (cnt ? (const void*)k_tracklets<uint32_t, true> : (const void*)k_tracklets<uint32_t, false>)
+                         : (cnt ? (const void*)k_tracklets<uint16_t, true> : (const void*)k_tracklets<uint16_t, false>);
+      e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->trk_smem[w]);
+      int per_sm = 0;
+      if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, t->trk_threads[w], t->trk_smem[w]);
+      t->trk_grid[w][cnt] = (per_sm > 0 ? per_sm : 1) * n_sm;
+    }
+  }
+  if (e != cudaSuccess) {
+    const int rc = fail(nullptr, TPC_ERR_CUDA, "tpc_tracker_create: CUDA: %s", cudaGetErrorString(e));
+    cudaFree(t->d_tables);
+    cudaFree(t->d_counters);
+    delete t;
+    cudaGetLastError();
+    return rc;
+  }
   *out = t;
   return TPC_OK;
 }
@@ -212,7 +240,7 @@ size_t tpc_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t
   return carve((uint32_t)t->n_rows, max_clusters, max_tasks, T).total;
 }
 
-int tpc_launches_per_batch(const tpc_tracker*) { return 6; }
+int tpc_launches_per_batch(const tpc_tracker*) { return 7; }  // a5 is launched in both row-map widths; one returns at once
 
 void tpc_tracker_enable_counters(tpc_tracker* t, int on) {
   if (t) t->counters_on = on != 0;
@@ -306,8 +334,8 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   }
   mark();
   if (c.n_tr > 0) {
-    if (cnt) k_neighbours<true><<<c.n_tr, kNfThreads, 0, s>>>(c);                           // a2
-    else k_neighbours<false><<<c.n_tr, kNfThreads, 0, s>>>(c);
+    if (cnt) k_neighbours<true><<<c.n_tr, kNfThreads, kNfSmemBytes, s>>>(c);                // a2
+    else k_neighbours<false><<<c.n_tr, kNfThreads, kNfSmemBytes, s>>>(c);
   }
   mark();
   if (c.n > 0) {
@@ -317,11 +345,17 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
   else k_seeds<false><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);
   mark();
-  const uint32_t trk_blocks = (T + kTrackletThreads - 1) / kTrackletThreads;
-  if (cnt) k_tracklets<true><<<trk_blocks, kTrackletThreads, 0, s>>>(c);                    // a5
-  else k_tracklets<false><<<trk_blocks, kTrackletThreads, 0, s>>>(c);
+  // a5: persistent, one launch per row-map width; the one that does not match the batch returns at once
+  if (cnt) {
+    k_tracklets<uint16_t, true><<<t->trk_grid[0][1], t->trk_threads[0], t->trk_smem[0], s>>>(c);
+    k_tracklets<uint32_t, true><<<t->trk_grid[1][1], t->trk_threads[1], t->trk_smem[1], s>>>(c);
+  } else {
+    k_tracklets<uint16_t, false><<<t->trk_grid[0][0], t->trk_threads[0], t->trk_smem[0], s>>>(c);
+    k_tracklets<uint32_t, false><<<t->trk_grid[1][0], t->trk_threads[1], t->trk_smem[1], s>>>(c);
+  }
   mark();
-  k_select_output<<<cv.out_tiles, kOutThreads, 0, s>>>(c);                                  // a6 + a7
+  const size_t keep_smem = (size_t)kOutThreads * ((size_t)(t->n_rows + 31) / 32) * sizeof(uint32_t);
+  k_select_output<<<cv.out_tiles, kOutThreads, keep_smem, s>>>(c);                          // a6 + a7
   mark();
   if (c.n > 0 && (out->dbg_link_up || out->dbg_link_dn || out->dbg_clean_up || out->dbg_clean_dn ||
                   out->dbg_start_hits))
