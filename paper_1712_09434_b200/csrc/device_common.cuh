@@ -41,6 +41,11 @@ __device__ __forceinline__ RowInfo load_row_info(const RowInfo* p) {
   return g;
 }
 
+// Seed record of a tracklet, 3 x 16 bytes, so that a5 starts a tracklet with ONE round of loads:
+//   [0] h0 (idx of the start hit), tr0 (task*n_rows + row of h0), h1 = clean_up[h0], h2 = clean_up[h1] (or -1)
+//   [1] y0, z0, y1, z1 (the (y,z) of h0 and h1 as float bits)
+//   [2] h0 - row_lo(tr0), h1 - row_lo(tr0+1) (row-local indices), gid(h0), 0
+constexpr int kSeedU4 = 3;
 constexpr int kRecFloat4 = 7;  // tracklet record: 7 float4 = x, p[5], c[15], chi2, ndf, first_row, last_row, n_hits, 2 pad
 
 // Everything a kernel needs, passed by value (about 300 bytes of kernel parameters).
@@ -63,8 +68,7 @@ struct Ctx {
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   unsigned long long* owner;  // [n] K7 ownership key
-  uint32_t* trk_start;     // [max_tracklets] idx of the start hit
-  uint32_t* trk_tr;        // [max_tracklets] task*n_rows + row of the start hit
+  uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)
   uint32_t* trk_hits;      // [max_tracklets][n_rows] hits of the tracklet as idx, ascending row, n_hits entries
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]

@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     const int n_hits = __float_as_int(r5.w);
     if (n_hits < min_hits) continue;                                   // K6
     const unsigned long long key = ((unsigned long long)(uint32_t)n_hits << 32) |
-                                   (unsigned long long)(0xFFFFFFFFu - c.gid[c.trk_start[t]]);
+                                   (unsigned long long)(0xFFFFFFFFu - c.trk_seed[(size_t)t * kSeedU4 + 2].z);
     const uint32_t* hits = c.trk_hits + (size_t)t * (size_t)n_rows;
     uint32_t kept = 0u;
     for (int k0 = 0; k0 < n_hits; k0 += 32) {
@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     const float v = lane < 28 ? reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4)[lane] : 0.0f;
     if (lane == 0) {
       o.track_x[slot] = v;
-      o.track_task[slot] = c.trk_tr[t] / (uint32_t)n_rows;
+      o.track_task[slot] = c.trk_seed[(size_t)t * kSeedU4].y / (uint32_t)n_rows;
       o.track_hit_begin[slot] = hb;
       o.track_nhits[slot] = kept;
     } else if (lane <= 5) o.track_par[(size_t)(lane - 1) * cap + slot] = v;
@@ -133,13 +133,13 @@ __global__ void k_debug_tracklets(const Ctx c) {
   const int n_rows = c.n_rows;
   const float* rec = reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4);
   const int n_hits = __float_as_int(rec[23]);
-  if (o.dbg_tracklet_start) o.dbg_tracklet_start[t] = c.gid[c.trk_start[t]];
+  if (o.dbg_tracklet_start) o.dbg_tracklet_start[t] = c.trk_seed[(size_t)t * kSeedU4 + 2].z;
   if (o.dbg_tracklet_nhits) o.dbg_tracklet_nhits[t] = (uint32_t)n_hits;
   if (o.dbg_tracklet_par)
     for (int j = 0; j < 5; ++j) o.dbg_tracklet_par[(size_t)t * 5 + j] = rec[1 + j];
   if (o.dbg_tracklet_map) {
     for (int r = 0; r < n_rows; ++r) o.dbg_tracklet_map[(size_t)t * n_rows + r] = -1;
-    const uint32_t tr_base = c.trk_tr[t] / (uint32_t)n_rows * (uint32_t)n_rows;
+    const uint32_t tr_base = c.trk_seed[(size_t)t * kSeedU4].y / (uint32_t)n_rows * (uint32_t)n_rows;
     for (int k = 0; k < n_hits; ++k) {
       const uint32_t m = c.trk_hits[(size_t)t * n_rows + k];
       const uint32_t r = find_tr(c, m) - tr_base;

@@ -126,46 +126,54 @@ __device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, fl
 }
 
 
-// SPEC 5.3 SEARCH (H1..H6) in the row described by g; returns the idx of the best cluster or -1.
-// One flat loop over the window; the bin bounds of the next z row are fetched one row ahead.
+// SPEC 5.3 SEARCH (H1..H6) in the row described by g; returns the idx of the best cluster or -1 and
+// its (y,z) in best_p.  The window covers 1..4 bin rows in z; two bin rows are handled per round: their
+// four bin bounds are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at
+// a time with all loads of a group in flight before the first is tested (the walk is latency bound).
+constexpr int kSearchUnroll = 4;
+
 template <bool COUNT>
 __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g, float y0, float z0,
-                                              uint32_t& n_cand) {
+                                              float2& best_p, uint32_t& n_cand) {
   const float y = S.y, z = S.z;
   const float ey = S.c00 + c.sy2, ez = S.c11 + c.sz2;                 // H1
   const float hy2 = fminf(c.prm.accept_k2 * ey, c.smax2);              // H2
   const float hz2 = fminf(c.prm.accept_k2 * ez, c.smax2);
   const float wy = sqrtf(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrtf(fmaxf(hz2, 0.0f)) + kGridMargin;
   const int ny = info_ny(g), nz = info_nz(g);
-  const int iy0 = bin_coord(y - wy, y0, g.inv, ny), iy1 = bin_coord(y + wy, y0, g.inv, ny);
+  const int iy0 = bin_coord(y - wy, y0, g.inv, ny), iy1 = bin_coord(y + wy, y0, g.inv, ny) + 1;
   const int iz0 = bin_coord(z - wz, z0, g.inv, nz), iz1 = bin_coord(z + wz, z0, g.inv, nz);
   const uint32_t* bp = c.bins + g.bins_off + iz0 * ny;
-  int rows_left = iz1 - iz0;
-  uint32_t i = bp[iy0], e = bp[iy1 + 1], i2 = 0u, e2 = 0u;
-  if (rows_left > 0) { i2 = bp[ny + iy0]; e2 = bp[ny + iy1 + 1]; }
   bool have = false;
   float best = 0.0f;
   uint32_t bi = 0u;
-  while (true) {
-    if (i >= e) {
-      if (rows_left <= 0) break;
-      --rows_left;
-      bp += ny;
-      i = i2; e = e2;
-      if (rows_left > 0) { i2 = bp[ny + iy0]; e2 = bp[ny + iy1 + 1]; }
-      continue;
+  for (int rows_left = iz1 - iz0 + 1; rows_left > 0; rows_left -= 2, bp += 2 * ny) {
+    const bool two = rows_left > 1;
+    const uint32_t i1 = __ldg(bp + iy0), e1 = __ldg(bp + iy1);
+    const uint32_t i2 = two ? __ldg(bp + ny + iy0) : 0u, e2 = two ? __ldg(bp + ny + iy1) : 0u;
+    const uint32_t n1 = e1 - i1, n_tot = n1 + (e2 - i2);
+    if (COUNT) n_cand += n_tot;
+    for (uint32_t k0 = 0u; k0 < n_tot; k0 += kSearchUnroll) {
+      uint32_t idx[kSearchUnroll];
+      float2 p[kSearchUnroll];
+#pragma unroll
+      for (int j = 0; j < kSearchUnroll; ++j) {
+        const uint32_t k = k0 + j;
+        idx[j] = k < n1 ? i1 + k : i2 + (k - n1);
+        p[j] = k < n_tot ? c.yz[idx[j]] : make_float2(0.0f, 0.0f);
+      }
+#pragma unroll
+      for (int j = 0; j < kSearchUnroll; ++j) {
+        const float dy = p[j].x - y, dz = p[j].y - z;                  // H3
+        const float dy2 = dy * dy, dz2 = dz * dz;
+        if (k0 + j < n_tot && dy2 <= hy2 && dz2 <= hz2) {              // H4
+          const float d = (dy2 * ez) + (dz2 * ey);                     // H5
+          bool take = !have || d < best;                               // H6
+          if (have && d == best) take = c.gid[idx[j]] < c.gid[bi];
+          if (take) { have = true; best = d; bi = idx[j]; best_p = p[j]; }
+        }
+      }
     }
-    const float2 p = c.yz[i];
-    if (COUNT) ++n_cand;
-    const float dy = p.x - y, dz = p.y - z;                            // H3
-    const float dy2 = dy * dy, dz2 = dz * dz;
-    if (dy2 <= hy2 && dz2 <= hz2) {                                    // H4
-      const float d = (dy2 * ez) + (dz2 * ey);                         // H5
-      bool take = !have || d < best;                                   // H6
-      if (have && d == best) take = c.gid[i] < c.gid[bi];
-      if (take) { have = true; best = d; bi = i; }
-    }
-    ++i;
   }
   return have ? (int32_t)bi : -1;
 }
@@ -177,8 +185,9 @@ __host__ __device__ inline int tracklet_threads(int n_rows, int map_bytes) {
   const int per_thread = n_rows * map_bytes;
   return per_thread <= 384 ? 128 : (per_thread <= 1024 ? 64 : 32);
 }
+__host__ __device__ inline size_t tracklet_tab_bytes(int n_rows) { return (size_t)((n_rows * 8 + 15) / 16 * 16); }
 __host__ __device__ inline size_t tracklet_smem(int n_rows, int map_bytes) {
-  return (size_t)((n_rows * 4 + 15) / 16 * 16) + (size_t)n_rows * map_bytes * tracklet_threads(n_rows, map_bytes);
+  return tracklet_tab_bytes(n_rows) + (size_t)n_rows * map_bytes * tracklet_threads(n_rows, map_bytes);
 }
 
 template <typename MapT, bool COUNT>
@@ -191,8 +200,9 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
   if (big_rows != (sizeof(MapT) == 4)) return;
   const int n_rows = c.n_rows, nthr = (int)blockDim.x, tid = (int)threadIdx.x, lane = tid & 31;
   float* sX = reinterpret_cast<float*>(trk_smem);
-  MapT* s_map = reinterpret_cast<MapT*>(trk_smem + (n_rows * 4 + 15) / 16 * 16);  // [n_rows][nthr]
-  for (int r = tid; r < n_rows; r += nthr) sX[r] = c.X[r];
+  float* sYmax = sX + n_rows;
+  MapT* s_map = reinterpret_cast<MapT*>(trk_smem + tracklet_tab_bytes(n_rows));  // [n_rows][nthr]
+  for (int r = tid; r < n_rows; r += nthr) { sX[r] = c.X[r]; sYmax[r] = c.ymax[r]; }
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
@@ -203,7 +213,7 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
   S.c00 = S.c10 = S.c11 = S.c20 = S.c21 = S.c22 = S.c30 = S.c31 = S.c32 = S.c33 = 0.0f;
   S.c40 = S.c41 = S.c42 = S.c43 = S.c44 = 0.0f;
   S.chi2 = 0.0f; S.ndf = -5;
-  uint32_t t = 0u, tr_base = 0u, h0 = 0u;
+  uint32_t t = 0u, tr_base = 0u, gid0 = 0u;
   float z0 = 0.0f;
   int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
   int32_t last_hit = -1, next_chain = -1;
@@ -220,11 +230,11 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
       const uint32_t ft = __shfl_sync(FULL, t, L), ftr = __shfl_sync(FULL, tr_base, L);
       const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
       const int fn = __shfl_sync(FULL, n_hits, L);
-      const uint32_t fh0 = __shfl_sync(FULL, h0, L);
+      const uint32_t fgid0 = __shfl_sync(FULL, gid0, L);
       const int col = (tid & ~31) + L;
       unsigned long long key = 0ull;
       if (fn >= min_hits)  // K6, K7: longest tracklet wins, then the smaller start-hit gid
-        key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - c.gid[fh0]);
+        key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
       uint32_t* hits_out = c.trk_hits + (size_t)ft * (size_t)n_rows;
       uint32_t wpos = 0u;
       for (int rb = ffirst; rb <= flast; rb += 32) {
@@ -255,7 +265,8 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
         phase = PH_FETCH;
       }
     }
-    // (B) lanes without a tracklet take the next ones from the queue (K1 seed)
+    // (B) lanes without a tracklet take the next ones from the queue (K1 seed); the seed record of a4
+    //     holds everything the seed needs, so a new tracklet costs one round of loads
     const unsigned need = __ballot_sync(FULL, phase == PH_FETCH);
     if (need) {
       uint32_t base = 0u;
@@ -266,51 +277,70 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
         if (t >= n_trk) {
           phase = PH_EXIT;
         } else {
-          h0 = c.trk_start[t];
-          const uint32_t tr0 = c.trk_tr[t];
+          const uint4* sr = c.trk_seed + (size_t)t * kSeedU4;
+          const uint4 q0 = __ldg(sr), q1 = __ldg(sr + 1), q2 = __ldg(sr + 2);
+          const uint32_t tr0 = q0.y;
           const uint32_t task = tr0 / (uint32_t)n_rows;
           r0 = (int)(tr0 - task * (uint32_t)n_rows);
           tr_base = task * (uint32_t)n_rows;
           z0 = side_z0(c, task);
-          const uint32_t h1 = (uint32_t)c.clean_up[h0];
-          const float2 p0 = c.yz[h0], p1 = c.yz[h1];
-          const float dx = sX[r0 + 1] - sX[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
+          gid0 = q2.z;
+          const float y0s = __uint_as_float(q1.x), z0s = __uint_as_float(q1.y);
+          const float y1s = __uint_as_float(q1.z), z1s = __uint_as_float(q1.w);
+          const float dx = sX[r0 + 1] - sX[r0], dy = y1s - y0s, dz = z1s - z0s;
           const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
-          S.y = p1.x; S.z = p1.y; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
+          S.y = y1s; S.z = z1s; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
           S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
           S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
           S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
           S.chi2 = 0.0f; S.ndf = -5;
-          s_map[r0 * nthr + tid] = (MapT)(h0 - c.row_off[tr0]);
-          s_map[(r0 + 1) * nthr + tid] = (MapT)(h1 - c.row_off[tr0 + 1u]);
+          s_map[r0 * nthr + tid] = (MapT)q2.x;
+          s_map[(r0 + 1) * nthr + tid] = (MapT)q2.y;
           row_cur = r0 + 1; first_row = r0; last_row = r0 + 1; n_hits = 2; gap = 0; r_down = 0;
-          last_hit = (int32_t)h1;
-          next_chain = c.clean_up[h1];
+          last_hit = (int32_t)q0.z;
+          next_chain = (int32_t)q0.w;
           phase = next_chain >= 0 ? PH_CHAIN : PH_UP;
           if (COUNT) n_chain += 2u;
         }
       }
     }
     if (__ballot_sync(FULL, phase != PH_EXIT) == 0u) break;
-    // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping
+    // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping.
+    //     The three parts are separated by warp barriers so that the lanes run each of them together
+    //     whatever their phase is.
+    int rt = 0;
+    uint32_t row_lo = 0u;
+    int32_t hit = -1;
+    float2 hp = make_float2(0.0f, 0.0f);
+    bool book = false, do_search = false;
+    RowInfo g;
+    g.inv = 0.0f; g.ny_nz = 0u; g.bins_off = 0u; g.row_lo = 0u;
     if (phase <= PH_FINISH) {
       if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
       if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
-      int rt;
       if (phase <= PH_UP) rt = row_cur + 1;
       else if (phase == PH_TURN) rt = last_row;
       else if (phase == PH_DOWN) rt = r_down;
       else rt = first_row;
-      // the row's grid header does not depend on the state: its load overlaps the transport arithmetic
-      const RowInfo g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
+      // loads that do not depend on the transported state are issued before the transport: the row's grid
+      // header, and the hit when it is known already (chain link, lastRow hit at the turn, row map)
+      g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
+      row_lo = g.row_lo;
+      int32_t known = -1;
+      if (phase == PH_CHAIN) known = next_chain;
+      else if (phase == PH_TURN) known = last_hit;
+      else if (phase == PH_DOWN && rt >= r0) {
+        const MapT m = s_map[rt * nthr + tid];
+        if (m != kNone) known = (int32_t)(row_lo + (uint32_t)m);
+      }
+      if (known >= 0) hp = c.yz[known];
+      if (phase == PH_CHAIN) next_chain = c.clean_up[known];            // K2: the link after this one
       bool ok = true;
       if (rt != row_cur) {
         ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
         if (ok) row_cur = rt;
         if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
       }
-      int32_t hit = -1;
-      bool book = false, searched = false;
       if (phase == PH_FINISH) {                                         // K6
         phase = PH_ENDED;
       } else if (phase == PH_TURN) {                                    // K4
@@ -318,57 +348,47 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
         S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
         S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
         S.chi2 = 0.0f; S.ndf = -5; gap = 0;
-        if (row_cur == last_row) hit = last_hit;                        // the lastRow hit opens the down pass
+        if (row_cur == last_row) hit = known;                           // the lastRow hit opens the down pass
         r_down = last_row - 1;
         phase = PH_DOWN;
       } else if (!ok) {  // transport failed: K2/K3 -> turn-around, K5 -> finish
         phase = (phase == PH_DOWN) ? PH_FINISH : PH_TURN;
       } else {
         book = true;
-        if (phase == PH_CHAIN) {                                        // K2
-          hit = next_chain;
-          next_chain = c.clean_up[hit];
-        } else if (phase == PH_UP) {                                    // K3
-          searched = true;
-        } else {                                                        // K5
-          searched = true;
-          if (rt >= r0) {
-            const MapT m = s_map[rt * nthr + tid];
-            if (m != kNone) { hit = (int32_t)(g.row_lo + (uint32_t)m); searched = false; }
+        if (phase == PH_UP || known < 0) do_search = true;              // K3, K5 without a map entry
+        else hit = known;                                               // K2, K5 with a map entry
+      }
+    }
+    __syncwarp();
+    if (do_search) {
+      if (COUNT) ++n_search;
+      hit = search_row<COUNT>(c, S, g, -sYmax[rt], z0, hp, n_cand);
+    }
+    __syncwarp();
+    if (hit >= 0) update_hit(S, hp.x, hp.y, sy2, sz2);
+    __syncwarp();
+    if (book) {
+      const MapT m = hit >= 0 ? (MapT)((uint32_t)hit - row_lo) : kNone;
+      if (phase == PH_CHAIN) {
+        s_map[rt * nthr + tid] = m;
+        last_row = rt; last_hit = hit; ++n_hits;
+        if (COUNT) ++n_chain;
+        if (next_chain < 0) { phase = PH_UP; gap = 0; }
+      } else if (phase == PH_UP) {
+        s_map[rt * nthr + tid] = m;
+        if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
+        else if (++gap > max_gap) phase = PH_TURN;
+      } else {  // PH_DOWN
+        if (do_search) {
+          s_map[rt * nthr + tid] = m;
+          if (hit >= 0) {
+            ++n_hits;
+            if (rt < first_row) { first_row = rt; gap = 0; }
+          } else if (rt < first_row) {
+            if (++gap > max_gap) phase = PH_FINISH;
           }
         }
-        if (searched) {
-          if (COUNT) ++n_search;
-          hit = search_row<COUNT>(c, S, g, -c.ymax[rt], z0, n_cand);
-        }
-      }
-      if (hit >= 0) {
-        const float2 p = c.yz[hit];
-        update_hit(S, p.x, p.y, sy2, sz2);
-      }
-      if (book) {
-        const MapT m = hit >= 0 ? (MapT)((uint32_t)hit - g.row_lo) : kNone;
-        if (phase == PH_CHAIN) {
-          s_map[rt * nthr + tid] = m;
-          last_row = rt; last_hit = hit; ++n_hits;
-          if (COUNT) ++n_chain;
-          if (next_chain < 0) { phase = PH_UP; gap = 0; }
-        } else if (phase == PH_UP) {
-          s_map[rt * nthr + tid] = m;
-          if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
-          else if (++gap > max_gap) phase = PH_TURN;
-        } else {  // PH_DOWN
-          if (searched) {
-            s_map[rt * nthr + tid] = m;
-            if (hit >= 0) {
-              ++n_hits;
-              if (rt < first_row) { first_row = rt; gap = 0; }
-            } else if (rt < first_row) {
-              if (++gap > max_gap) phase = PH_FINISH;
-            }
-          }
-          --r_down;
-        }
+        --r_down;
       }
     }
   }

@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 
 // ---------------------------------------------------------------------------
 // a4  start hits (S1) whose chain has >= min_seed_hits hits (S2, S3), written
-// in idx order to trk_start / trk_tr.  Tile = kSeedThreads * kSeedItems idx.
+// in idx order as seed records (trk_seed).  Tile = kSeedThreads * kSeedItems idx.
 // ---------------------------------------------------------------------------
 constexpr int kSeedThreads = 256;
 constexpr int kSeedItems = 4;
@@ -150,20 +150,31 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
   const uint32_t tile = s_tile;
   const uint32_t base = tile * kSeedTile + threadIdx.x * kSeedItems;
   uint32_t flags = 0u, n_s1 = 0u;
+  int32_t h1s[kSeedItems], h2s[kSeedItems];
+  // the four cleaned up-links and raw down-links of this thread: one 16-byte load each (arrays are padded)
+  int4 cu4 = make_int4(-1, -1, -1, -1), dn4 = make_int4(-1, -1, -1, -1);
+  if (base < c.n) {
+    cu4 = *reinterpret_cast<const int4*>(c.clean_up + base);
+    dn4 = *reinterpret_cast<const int4*>(c.link_dn + base);
+  }
+  const int32_t cu[kSeedItems] = {cu4.x, cu4.y, cu4.z, cu4.w}, dn[kSeedItems] = {dn4.x, dn4.y, dn4.z, dn4.w};
 #pragma unroll
   for (int k = 0; k < kSeedItems; ++k) {
     const uint32_t i = base + k;
-    if (i >= c.n) break;
-    int32_t h = c.clean_up[i];
+    h1s[k] = -1; h2s[k] = -1;
+    if (i >= c.n) continue;
+    int32_t h = cu[k];
     if (h < 0) continue;
-    const int32_t d = c.link_dn[i];
+    const int32_t d = dn[k];
     if (d >= 0 && c.link_up[d] == (int32_t)i) continue;  // clean_dn[i] >= 0 (C2): not a start hit
     if (COUNT) ++n_s1;
+    h1s[k] = h;
+    h = c.clean_up[h];
+    h2s[k] = h;
     int len = 2;
-    while (len < c.prm.min_seed_hits) {
+    while (h >= 0) {
+      if (++len >= c.prm.min_seed_hits) break;
       h = c.clean_up[h];
-      if (h < 0) break;
-      ++len;
     }
     if (len >= c.prm.min_seed_hits) flags |= 1u << k;
   }
@@ -180,8 +191,13 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
   for (int k = 0; k < kSeedItems; ++k) {
     if (!(flags & (1u << k))) continue;
     if (pos < c.max_tracklets) {
-      c.trk_start[pos] = base + k;
-      c.trk_tr[pos] = find_tr(c, base + k);
+      const uint32_t h0 = base + k, h1 = (uint32_t)h1s[k];
+      const uint32_t tr0 = find_tr(c, h0);
+      const float2 p0 = c.yz[h0], p1 = c.yz[h1];
+      uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
+      rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2s[k]);
+      rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));
+      rec[2] = make_uint4(h0 - c.row_off[tr0], h1 - c.row_off[tr0 + 1u], c.gid[h0], 0u);
     }
     ++pos;
   }

@@ -66,7 +66,7 @@ uint32_t resolve_max_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tr
 
 // Offsets of every workspace array, in bytes.
 struct Carve {
-  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, owner, trk_start, trk_tr, trk_hits, trk_rec, zero_begin,
+  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, owner, trk_seed, trk_hits, trk_rec, zero_begin,
       scan_seed, scan_out, tickets, n_tracklets, zero_end, total;
   uint32_t seed_tiles, out_tiles;
 };
@@ -85,8 +85,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.link_dn = take(n4 * sizeof(int32_t));
   c.clean_up = take(n4 * sizeof(int32_t));
   c.owner = take(n4 * sizeof(unsigned long long));
-  c.trk_start = take((size_t)T * sizeof(uint32_t));
-  c.trk_tr = take((size_t)T * sizeof(uint32_t));
+  c.trk_seed = take((size_t)T * kSeedU4 * sizeof(uint4));
   c.trk_hits = take((size_t)T * n_rows * sizeof(uint32_t));
   c.trk_rec = take((size_t)T * kRecFloat4 * sizeof(float4));
   c.seed_tiles = (uint32_t)(((size_t)n + kSeedTile - 1) / kSeedTile);
@@ -130,7 +129,7 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.rowinfo = (RowInfo*)(ws + cv.rowinfo);
   c.link_up = (int32_t*)(ws + cv.link_up); c.link_dn = (int32_t*)(ws + cv.link_dn);
   c.clean_up = (int32_t*)(ws + cv.clean_up); c.owner = (unsigned long long*)(ws + cv.owner);
-  c.trk_start = (uint32_t*)(ws + cv.trk_start); c.trk_tr = (uint32_t*)(ws + cv.trk_tr);
+  c.trk_seed = (uint4*)(ws + cv.trk_seed);
   c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
