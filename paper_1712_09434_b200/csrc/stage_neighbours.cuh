@@ -4,20 +4,21 @@
 // One block per (task,row).  The two neighbour rows r-1 and r+1 (their bin-sorted (y,z) pairs
 // and their bin tables, both contiguous in memory) are staged in shared memory with two TMA 1-D
 // bulk copies each (cp.async.bulk + mbarrier) when they fit; larger rows are read through L1.
-// A thread first collects the down candidates that pass N3 into a short list in shared memory
-// (stored as the products (y - y_d)*a_, (z - z_d)*a_ of N4), then walks its up window once and
-// pairs every up candidate that passes N2 with the list.  Both window walks are single flat
-// loops, so a warp runs max-over-lanes(candidates) iterations instead of the product of the
-// nested trip counts.
+// A thread owns one cluster and runs three flat loops, each entered by the whole warp together:
+// the down window (clusters that pass N3 go to a short list in shared memory, stored as the
+// products (y - y_d)*a_, (z - z_d)*a_ of N4), the up window (N2, list of (y_u - y)*b, (z_u - z)*b),
+// and the nu*nd pairs of the two lists (N4, N5).  A window is read as ONE virtual range over its
+// (at most two, else looped) bin rows, so a warp runs max-over-lanes(candidates) iterations of a
+// short body instead of nested loops.  A list overflow sends the cluster to the nested serial walk.
 #pragma once
 #include "device_common.cuh"
 
 namespace tpc {
 
 constexpr int kNfThreads = 128;
-constexpr int kNfList = 8;                    // down candidates a thread keeps; more -> nested fallback
-constexpr uint32_t kNfStageBytes = 24 * 1024;  // staged neighbour rows (both) must fit in this
-constexpr uint32_t kNfListBytes = kNfThreads * kNfList * 12;
+constexpr int kNfList = 8;                    // candidates per side a cluster keeps; more -> serial search
+constexpr uint32_t kNfStageBytes = 16 * 1024;  // staged neighbour rows (both) must fit in this
+constexpr uint32_t kNfListBytes = 2u * kNfThreads * kNfList * 12u;  // 2 sides x (py, pz, idx)[kNfList][threads]
 constexpr uint32_t kNfSmemBytes = 16 + kNfListBytes + kNfStageBytes;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -77,85 +78,142 @@ __device__ __forceinline__ void for_window(const RowView& v, float z0, float ylo
   }
 }
 
-// lexicographic (chi, gid_u, gid_d) comparison of N5; the gids are only loaded on an exact chi tie
-__device__ __forceinline__ bool nf_better(const Ctx& c, bool have, float chi, float best, uint32_t u, uint32_t d,
-                                          uint32_t bu, uint32_t bd) {
-  if (!have || chi < best) return true;
-  if (chi != best) return false;
-  const uint32_t gu = c.gid[u], gbu = c.gid[bu];
-  if (gu != gbu) return gu < gbu;
-  return c.gid[d] < c.gid[bd];
+
+// The exact serial search of one cluster (N1..N5 as written, ties by gid): nested walk of both windows.
+// Used for the rare clusters the cooperative search cannot decide (chi2 ties, list overflow).
+template <bool COUNT>
+__device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const RowView& vd, int row, float z0, float y,
+                                       float z, int32_t* out_up, int32_t* out_dn, unsigned long long* n_pairs) {
+  const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max, M = kGridMargin;
+  const float b = c.dx_dn[row], a_ = c.dx_up[row];  // N4
+  const float zu = z * c.ratio_up[row], zd = z * c.ratio_dn[row];  // N1
+  const float wy = c.wy, wz = c.wz;
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bu = 0u, bd = 0u;
+  for_window(vu, z0, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
+    if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) return;  // N2
+    const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
+    for_window(vd, z0, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, [&](uint32_t d, float2 pd) {
+      if (!(fabsf(pd.x - y) <= HY && fabsf(pd.y - zd) <= HZ)) return;  // N3
+      const float dy = ty - ((y - pd.x) * a_);  // N4
+      const float dz = tz - ((z - pd.y) * a_);
+      const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
+      if (COUNT) ++*n_pairs;
+      if (!(chi < CHI_MAX)) return;  // N5: lexicographic (chi, gid_u, gid_d)
+      bool take = !have || chi < best;
+      if (have && chi == best) {
+        const uint32_t gu = c.gid[u], gbu = c.gid[bu];
+        take = gu != gbu ? gu < gbu : c.gid[d] < c.gid[bd];
+      }
+      if (take) { have = true; best = chi; bu = u; bd = d; }
+    });
+  });
+  *out_up = have ? (int32_t)bu : -1;
+  *out_dn = have ? (int32_t)bd : -1;
+}
+
+// Window walk of one thread around (y, zc) (zc = the projected z of N1) in row view v: the clusters that
+// pass the window test are appended to the thread's list as ((p.x - y)*sgn*fac, (p.y - z)*sgn*fac, idx).
+// Returns the number that passed (entries beyond kNfList are not stored).
+__device__ __forceinline__ uint32_t nf_collect(const RowView& v, float z0, bool act, float y, float z, float zc,
+                                               float HY, float HZ, float sgn, float fac, float* l_y, float* l_z,
+                                               uint32_t* l_i) {
+  const float M = kGridMargin;
+  const int iy0 = bin_coord((y - HY) - M, v.y0, v.inv, v.ny), iy1 = bin_coord((y + HY) + M, v.y0, v.inv, v.ny) + 1;
+  const int iz0 = bin_coord((zc - HZ) - M, z0, v.inv, v.nz);
+  const int nzr = act ? bin_coord((zc + HZ) + M, z0, v.inv, v.nz) - iz0 + 1 : 0;
+  uint32_t n = 0u;
+  for (int r = 0; r < nzr; r += 2) {
+    const uint32_t* bp = v.bins + (iz0 + r) * v.ny;
+    const uint32_t i1 = bp[iy0], n1 = bp[iy1] - i1;
+    uint32_t i2 = 0u, n2 = 0u;
+    if (r + 1 < nzr) { i2 = bp[v.ny + iy0]; n2 = bp[v.ny + iy1] - i2; }
+    const uint32_t n_tot = n1 + n2;
+    for (uint32_t k = 0u; k < n_tot; ++k) {
+      const uint32_t idx = k < n1 ? i1 + k : i2 + (k - n1);
+      const float2 p = v.yz[idx - v.yz_base];
+      const float ry = p.x - y;
+      if (fabsf(ry) <= HY && fabsf(p.y - zc) <= HZ) {  // N2 / N3
+        if (n < (uint32_t)kNfList) {
+          // up: (y_u - y)*b, (z_u - z)*b.  down: (y - y_d)*a_, (z - z_d)*a_ (exact negation of the difference)
+          l_y[n * kNfThreads] = (sgn * ry) * fac;
+          l_z[n * kNfThreads] = (sgn * (p.y - z)) * fac;
+          l_i[n * kNfThreads] = idx;
+        }
+        ++n;
+      }
+    }
+  }
+  return n;
 }
 
 template <bool COUNT>
 __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const RowView& vd, int row, float z0,
-                                       uint32_t lo, uint32_t hi, float* s_py, float* s_pz, uint32_t* s_pi) {
-  const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max, M = kGridMargin;
+                                       uint32_t lo, uint32_t hi, unsigned char* list_smem) {
+  const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max;
   const float b = c.dx_dn[row], a_ = c.dx_up[row];  // N4
   const float ratio_up = c.ratio_up[row], ratio_dn = c.ratio_dn[row];
   const float wy = c.wy, wz = c.wz;
   const int tid = threadIdx.x;
+  float* d_y = reinterpret_cast<float*>(list_smem) + tid;  // [kNfList][kNfThreads] each, this thread's column
+  float* d_z = d_y + kNfList * kNfThreads;
+  uint32_t* d_i = reinterpret_cast<uint32_t*>(d_z + kNfList * kNfThreads);
+  float* u_y = reinterpret_cast<float*>(d_i + kNfList * kNfThreads);
+  float* u_z = u_y + kNfList * kNfThreads;
+  uint32_t* u_i = reinterpret_cast<uint32_t*>(u_z + kNfList * kNfThreads);
   unsigned long long n_pairs = 0ull;
-  for (uint32_t i = lo + tid; i < hi; i += kNfThreads) {
-    const float2 h = c.yz[i];
-    const float y = h.x, z = h.y;
+  for (uint32_t i0 = lo + (uint32_t)(tid & ~31); i0 < hi; i0 += kNfThreads) {  // warp-uniform trip count
+    const uint32_t i = i0 + (uint32_t)(tid & 31);
+    const bool act = i < hi;
+    float y = 0.0f, z = 0.0f;
+    if (act) { const float2 h = c.yz[i]; y = h.x; z = h.y; }
     const float zu = z * ratio_up, zd = z * ratio_dn;  // N1
-    // down candidates (N3)
-    int nd = 0;
-    for_window(vd, z0, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, [&](uint32_t d, float2 pd) {
-      if (!(fabsf(pd.x - y) <= HY && fabsf(pd.y - zd) <= HZ)) return;
-      if (nd < kNfList) {
-        s_py[nd * kNfThreads + tid] = (y - pd.x) * a_;
-        s_pz[nd * kNfThreads + tid] = (z - pd.y) * a_;
-        s_pi[nd * kNfThreads + tid] = d;
-      }
-      ++nd;
-    });
+    const uint32_t nd = nf_collect(vd, z0, act, y, z, zd, HY, HZ, -1.0f, a_, d_y, d_z, d_i);  // N3
+    __syncwarp();
+    const uint32_t nu = nd ? nf_collect(vu, z0, act, y, z, zu, HY, HZ, 1.0f, b, u_y, u_z, u_i) : 0u;  // N2
+    __syncwarp();
+    const bool overflow = nd > (uint32_t)kNfList || nu > (uint32_t)kNfList;
+    const uint32_t n_pr = overflow ? 0u : nu * nd;
+    const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 64, nd <= 8
+    if (COUNT) n_pairs += n_pr;
     bool have = false;
     float best = 0.0f;
     uint32_t bu = 0u, bd = 0u;
-    if (nd > 0 && nd <= kNfList) {
-      for_window(vu, z0, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
-        if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) return;  // N2
-        const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
-        if (COUNT) n_pairs += (unsigned)nd;
-        for (int k = 0; k < nd; ++k) {
-          const float dy = ty - s_py[k * kNfThreads + tid];  // N4
-          const float dz = tz - s_pz[k * kNfThreads + tid];
-          const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
-          if (!(chi < CHI_MAX)) continue;  // N5
-          const uint32_t d = s_pi[k * kNfThreads + tid];
-          if (nf_better(c, have, chi, best, u, d, bu, bd)) { have = true; best = chi; bu = u; bd = d; }
-        }
-      });
-    } else if (nd > kNfList) {  // list overflow: nested walk of both windows for this cluster
-      for_window(vu, z0, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
-        if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) return;
-        const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
-        for_window(vd, z0, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, [&](uint32_t d, float2 pd) {
-          if (!(fabsf(pd.x - y) <= HY && fabsf(pd.y - zd) <= HZ)) return;
-          const float dy = ty - ((y - pd.x) * a_);
-          const float dz = tz - ((z - pd.y) * a_);
-          const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
-          if (COUNT) ++n_pairs;
-          if (!(chi < CHI_MAX)) return;
-          if (nf_better(c, have, chi, best, u, d, bu, bd)) { have = true; best = chi; bu = u; bd = d; }
-        });
-      });
+    for (uint32_t k = 0u; k < n_pr; ++k) {
+      const uint32_t u = (k * magic) >> 16, d = k - u * nd;
+      const float dy = u_y[u * kNfThreads] - d_y[d * kNfThreads];  // N4
+      const float dz = u_z[u * kNfThreads] - d_z[d * kNfThreads];
+      const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
+      if (!(chi < CHI_MAX)) continue;  // N5: lexicographic (chi, gid_u, gid_d)
+      bool take = !have || chi < best;
+      if (have && chi == best) {
+        const uint32_t gu = c.gid[u_i[u * kNfThreads]], gbu = c.gid[u_i[bu * kNfThreads]];
+        take = gu != gbu ? gu < gbu : c.gid[d_i[d * kNfThreads]] < c.gid[d_i[bd * kNfThreads]];
+      }
+      if (take) { have = true; best = chi; bu = u; bd = d; }
     }
-    c.link_up[i] = have ? (int32_t)bu : -1;
-    c.link_dn[i] = have ? (int32_t)bd : -1;
+    __syncwarp();
+    if (act) {
+      int32_t up = -1, dn = -1;
+      if (overflow) {
+        nf_serial<COUNT>(c, vu, vd, row, z0, y, z, &up, &dn, &n_pairs);
+      } else if (have) {
+        up = (int32_t)u_i[bu * kNfThreads];
+        dn = (int32_t)d_i[bd * kNfThreads];
+      }
+      c.link_up[i] = up;
+      c.link_dn[i] = dn;
+    }
   }
   if (COUNT && n_pairs) atomicAdd(&c.counters[CN_NF_PAIRS], n_pairs);
 }
 
 template <bool COUNT>
-__global__ void __launch_bounds__(kNfThreads) k_neighbours(const Ctx c) {
+__global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant__ Ctx c) {
   extern __shared__ __align__(16) unsigned char nf_smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(nf_smem);
-  float* s_py = reinterpret_cast<float*>(nf_smem + 16);
-  float* s_pz = s_py + kNfThreads * kNfList;
-  uint32_t* s_pi = reinterpret_cast<uint32_t*>(s_pz + kNfThreads * kNfList);
+  unsigned char* list_smem = nf_smem + 16;
   unsigned char* stage = nf_smem + 16 + kNfListBytes;
 
   const uint32_t tr = blockIdx.x;
@@ -202,11 +260,11 @@ __global__ void __launch_bounds__(kNfThreads) k_neighbours(const Ctx c) {
     mbar_wait(bar, 0u);
     vu.yz = s_uyz; vu.yz_base = uya0; vu.bins = s_ub + (gu.bins_off - uba0);
     vd.yz = s_dyz; vd.yz_base = dya0; vd.bins = s_db + (gd.bins_off - dba0);
-    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, s_py, s_pz, s_pi);
+    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, list_smem);
   } else {
     vu.yz = c.yz; vu.yz_base = 0u; vu.bins = c.bins + gu.bins_off;
     vd.yz = c.yz; vd.yz_base = 0u; vd.bins = c.bins + gd.bins_off;
-    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, s_py, s_pz, s_pi);
+    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, list_smem);
   }
 }
 

@@ -199,6 +199,12 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
   int dev = 0, n_sm = 0;
   e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute((const void*)k_neighbours<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)kNfSmemBytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute((const void*)k_neighbours<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)kNfSmemBytes);
   for (int w = 0; w < 2 && e == cudaSuccess; ++w) {
     const int map_bytes = w ? 4 : 2;
     t->trk_threads[w] = tracklet_threads(t->n_rows, map_bytes);
