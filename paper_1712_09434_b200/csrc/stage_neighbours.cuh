@@ -9,7 +9,8 @@
 // products (y - y_d)*a_, (z - z_d)*a_ of N4), the up window (N2, list of (y_u - y)*b, (z_u - z)*b),
 // and the nu*nd pairs of the two lists (N4, N5).  A window is read as ONE virtual range over its
 // (at most two, else looped) bin rows, so a warp runs max-over-lanes(candidates) iterations of a
-// short body instead of nested loops.  A list overflow sends the cluster to the nested serial walk.
+// short branch-free body instead of nested loops.  A list overflow or two pairs of equal chi2 send the
+// cluster to the nested serial walk, which alone compares gids.
 #pragma once
 #include "device_common.cuh"
 
@@ -130,19 +131,21 @@ __device__ __forceinline__ uint32_t nf_collect(const RowView& v, float z0, bool 
     uint32_t i2 = 0u, n2 = 0u;
     if (r + 1 < nzr) { i2 = bp[v.ny + iy0]; n2 = bp[v.ny + iy1] - i2; }
     const uint32_t n_tot = n1 + n2;
+    const uint32_t skip = i2 - (i1 + n1);  // idx of candidate k >= n1 is i1 + k + skip
     for (uint32_t k = 0u; k < n_tot; ++k) {
-      const uint32_t idx = k < n1 ? i1 + k : i2 + (k - n1);
+      const uint32_t idx = i1 + k + (k < n1 ? 0u : skip);
       const float2 p = v.yz[idx - v.yz_base];
       const float ry = p.x - y;
-      if (fabsf(ry) <= HY && fabsf(p.y - zc) <= HZ) {  // N2 / N3
-        if (n < (uint32_t)kNfList) {
-          // up: (y_u - y)*b, (z_u - z)*b.  down: (y - y_d)*a_, (z - z_d)*a_ (exact negation of the difference)
-          l_y[n * kNfThreads] = (sgn * ry) * fac;
-          l_z[n * kNfThreads] = (sgn * (p.y - z)) * fac;
-          l_i[n * kNfThreads] = idx;
-        }
-        ++n;
+      const bool pass = (fabsf(ry) <= HY) & (fabsf(p.y - zc) <= HZ);  // N2 / N3
+      // stored whether it passes or not: a cluster that fails is overwritten by the next one (n stays)
+      if (n < (uint32_t)kNfList) {
+        const uint32_t slot = n * kNfThreads;
+        // up: (y_u - y)*b, (z_u - z)*b.  down: (y - y_d)*a_, (z - z_d)*a_ (exact negation of the difference)
+        l_y[slot] = (sgn * ry) * fac;
+        l_z[slot] = (sgn * (p.y - z)) * fac;
+        l_i[slot] = idx;
       }
+      n += pass ? 1u : 0u;
     }
   }
   return n;
@@ -177,26 +180,25 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     const uint32_t n_pr = overflow ? 0u : nu * nd;
     const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 64, nd <= 8
     if (COUNT) n_pairs += n_pr;
-    bool have = false;
-    float best = 0.0f;
+    float best = CHI_MAX;  // N5: only chi < CHI_MAX is eligible
     uint32_t bu = 0u, bd = 0u;
+    bool have = false, tie = false;
     for (uint32_t k = 0u; k < n_pr; ++k) {
       const uint32_t u = (k * magic) >> 16, d = k - u * nd;
       const float dy = u_y[u * kNfThreads] - d_y[d * kNfThreads];  // N4
       const float dz = u_z[u * kNfThreads] - d_z[d * kNfThreads];
       const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
-      if (!(chi < CHI_MAX)) continue;  // N5: lexicographic (chi, gid_u, gid_d)
-      bool take = !have || chi < best;
-      if (have && chi == best) {
-        const uint32_t gu = c.gid[u_i[u * kNfThreads]], gbu = c.gid[u_i[bu * kNfThreads]];
-        take = gu != gbu ? gu < gbu : c.gid[d_i[d * kNfThreads]] < c.gid[d_i[bd * kNfThreads]];
-      }
-      if (take) { have = true; best = chi; bu = u; bd = d; }
+      const bool lt = chi < best;
+      tie |= have & (chi == best);  // equal chi2: the gids decide (N5), left to the serial search
+      have |= lt;
+      best = lt ? chi : best;
+      bu = lt ? u : bu;
+      bd = lt ? d : bd;
     }
     __syncwarp();
     if (act) {
       int32_t up = -1, dn = -1;
-      if (overflow) {
+      if (overflow || tie) {
         nf_serial<COUNT>(c, vu, vd, row, z0, y, z, &up, &dn, &n_pairs);
       } else if (have) {
         up = (int32_t)u_i[bu * kNfThreads];

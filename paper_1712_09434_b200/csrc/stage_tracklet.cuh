@@ -126,10 +126,35 @@ __device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, fl
 }
 
 
-// SPEC 5.3 SEARCH (H1..H6) in the row described by g; returns the idx of the best cluster or -1 and
-// its (y,z) in best_p.  The window covers 1..4 bin rows in z; two bin rows are handled per round: their
-// four bin bounds are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at
-// a time with all loads of a group in flight before the first is tested (the walk is latency bound).
+// SPEC 5.3 SEARCH (H1..H6), exact and serial: one flat loop over the window, ties decided by gid.  The fast
+// search below hands over to this one when it meets two valid clusters with the same distance.
+__device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz, const uint32_t* __restrict__ gid,
+                                                  const uint32_t* bp, int ny, int iy0, int iy1, int n_zrows, float y,
+                                                  float z, float hy2, float hz2, float ey, float ez, float2* best_p) {
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bi = 0u;
+  for (int r = 0; r < n_zrows; ++r, bp += ny) {
+    for (uint32_t i = bp[iy0], e = bp[iy1]; i < e; ++i) {
+      const float2 p = yz[i];
+      const float dy = p.x - y, dz = p.y - z;                          // H3
+      const float dy2 = dy * dy, dz2 = dz * dz;
+      if (dy2 <= hy2 && dz2 <= hz2) {                                  // H4
+        const float d = (dy2 * ez) + (dz2 * ey);                       // H5
+        bool take = !have || d < best;                                 // H6
+        if (have && d == best) take = gid[i] < gid[bi];
+        if (take) { have = true; best = d; bi = i; *best_p = p; }
+      }
+    }
+  }
+  return have ? (int32_t)bi : -1;
+}
+
+// SPEC 5.3 SEARCH in the row described by g; returns the idx of the best cluster or -1 and its (y,z) in
+// best_p.  The window covers 1..4 bin rows in z; two bin rows are handled per round: their four bin bounds
+// are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at a time, all
+// loads of a group in flight before the first is tested (the walk is latency bound) and the tests written
+// without branches (lanes of a warp are at different candidates of different windows).
 constexpr int kSearchUnroll = 4;
 
 template <bool COUNT>
@@ -143,15 +168,18 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
   const int ny = info_ny(g), nz = info_nz(g);
   const int iy0 = bin_coord(y - wy, y0, g.inv, ny), iy1 = bin_coord(y + wy, y0, g.inv, ny) + 1;
   const int iz0 = bin_coord(z - wz, z0, g.inv, nz), iz1 = bin_coord(z + wz, z0, g.inv, nz);
-  const uint32_t* bp = c.bins + g.bins_off + iz0 * ny;
-  bool have = false;
-  float best = 0.0f;
-  uint32_t bi = 0u;
+  const uint32_t* bp0 = c.bins + g.bins_off + iz0 * ny;
+  const uint32_t* bp = bp0;
+  float best = __int_as_float(0x7f800000);  // +inf: a valid cluster at distance +inf counts as a tie
+  float bx = 0.0f, bz = 0.0f;
+  int32_t bi = -1;
+  bool tie = false;
   for (int rows_left = iz1 - iz0 + 1; rows_left > 0; rows_left -= 2, bp += 2 * ny) {
     const bool two = rows_left > 1;
     const uint32_t i1 = __ldg(bp + iy0), e1 = __ldg(bp + iy1);
     const uint32_t i2 = two ? __ldg(bp + ny + iy0) : 0u, e2 = two ? __ldg(bp + ny + iy1) : 0u;
     const uint32_t n1 = e1 - i1, n_tot = n1 + (e2 - i2);
+    const uint32_t skip = i2 - e1;  // idx of candidate k >= n1 is i1 + k + skip
     if (COUNT) n_cand += n_tot;
     for (uint32_t k0 = 0u; k0 < n_tot; k0 += kSearchUnroll) {
       uint32_t idx[kSearchUnroll];
@@ -159,23 +187,27 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
 #pragma unroll
       for (int j = 0; j < kSearchUnroll; ++j) {
         const uint32_t k = k0 + j;
-        idx[j] = k < n1 ? i1 + k : i2 + (k - n1);
+        idx[j] = i1 + k + (k < n1 ? 0u : skip);
         p[j] = k < n_tot ? c.yz[idx[j]] : make_float2(0.0f, 0.0f);
       }
 #pragma unroll
       for (int j = 0; j < kSearchUnroll; ++j) {
         const float dy = p[j].x - y, dz = p[j].y - z;                  // H3
         const float dy2 = dy * dy, dz2 = dz * dz;
-        if (k0 + j < n_tot && dy2 <= hy2 && dz2 <= hz2) {              // H4
-          const float d = (dy2 * ez) + (dz2 * ey);                     // H5
-          bool take = !have || d < best;                               // H6
-          if (have && d == best) take = c.gid[idx[j]] < c.gid[bi];
-          if (take) { have = true; best = d; bi = idx[j]; best_p = p[j]; }
-        }
+        const bool ok = (k0 + j < n_tot) & (dy2 <= hy2) & (dz2 <= hz2);  // H4
+        const float d = (dy2 * ez) + (dz2 * ey);                       // H5
+        const bool lt = ok & (d < best);                               // H6
+        tie |= ok & (d == best);
+        best = lt ? d : best;
+        bi = lt ? (int32_t)idx[j] : bi;
+        bx = lt ? p[j].x : bx;
+        bz = lt ? p[j].y : bz;
       }
     }
   }
-  return have ? (int32_t)bi : -1;
+  best_p = make_float2(bx, bz);
+  if (tie) bi = search_row_serial(c.yz, c.gid, bp0, ny, iy0, iy1, iz1 - iz0 + 1, y, z, hy2, hz2, ey, ez, &best_p);
+  return bi;
 }
 
 enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4, PH_ENDED = 5, PH_FETCH = 6, PH_EXIT = 7 };
