@@ -14,7 +14,8 @@
 namespace tpc {
 
 constexpr int kMaxRows = 1024;        // include/tpc_tracker.h: n_rows <= 1024
-constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at row_off[tr] + tr*kBinPad
+constexpr uint32_t kBinsPerCluster = 2;  // grid density: bins per cluster of a row (the clusters bunch at small |z|)
+constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at kBinsPerCluster*row_off[tr] + tr*kBinPad
 constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the grid build
 constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
 
@@ -24,20 +25,28 @@ enum CounterId {
 };
 static_assert(CN_COUNT == TPC_N_COUNTERS, "counter list and header disagree");
 
-// Grid of one (task,row): bin = iz*ny + iy, iy = clamp((y - y0)*inv), iz likewise.
-// 16 bytes so that one vector load fetches everything a search needs to know about a row.
+// Grid of one (task,row): bin = iz*ny + iy, iy = clamp((y - y0)*inv), iz likewise.  The grid spans the
+// bounding box of the row's clusters, not the geometric extent of the row: the clusters of a central event
+// fill a third of the drift length in the inner rows, and a grid over the whole row would put three of
+// them in every occupied bin.  Coordinates outside the box clamp to the edge bins (monotone), so a window's
+// bin range still holds every cluster inside the window.
+// 32 bytes = one sector: two vector loads fetch everything a search needs to know about a row.
 struct __align__(16) RowInfo {
   float inv;          // 1 / bin size
+  float y0, z0;       // origin of the grid
   uint32_t ny_nz;     // ny | nz << 16  (bins across y, along z; both <= kMaxBinsPerRow)
   uint32_t bins_off;  // first entry of this row in Ctx::bins
   uint32_t row_lo;    // idx of the first cluster of the row (= row_off[tr])
+  uint32_t pad0, pad1;
 };
 __device__ __forceinline__ int info_ny(const RowInfo& g) { return (int)(g.ny_nz & 0xFFFFu); }
 __device__ __forceinline__ int info_nz(const RowInfo& g) { return (int)(g.ny_nz >> 16); }
 __device__ __forceinline__ RowInfo load_row_info(const RowInfo* p) {
   const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+  const uint2 w = __ldg(reinterpret_cast<const uint2*>(p) + 2);
   RowInfo g;
-  g.inv = __uint_as_float(v.x); g.ny_nz = v.y; g.bins_off = v.z; g.row_lo = v.w;
+  g.inv = __uint_as_float(v.x); g.y0 = __uint_as_float(v.y); g.z0 = __uint_as_float(v.z); g.ny_nz = v.w;
+  g.bins_off = w.x; g.row_lo = w.y; g.pad0 = 0u; g.pad1 = 0u;
   return g;
 }
 
@@ -63,17 +72,18 @@ struct Ctx {
   // workspace (device); "idx" = position of a cluster in the bin-sorted order, the internal identity
   float2* yz;              // [n]  (y,z) in bin-sorted order: rows keep their [row_off[tr], row_off[tr+1]) range
   uint32_t* gid;           // [n]  idx -> gid (index in the input arrays)
-  uint32_t* bins;          // [n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
+  uint32_t* bins;          // [kBinsPerCluster*n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
   RowInfo* rowinfo;        // [n_tr]
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   unsigned long long* owner;  // [n] K7 ownership key
   uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)
-  uint32_t* trk_hits;      // [max_tracklets][n_rows] hits of the tracklet as idx, ascending row, n_hits entries
+  uint32_t* trk_hits;      // [max_tracklets][n_rows] row map of the tracklet: idx of its hit in that row or kNoHit;
+                           // valid for the rows first_row..last_row of the tracklet record
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
-  uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2 tracklet queue head, 3 largest row (clusters)
+  uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2 tracklet queue head
   uint32_t* n_tracklets;   // [1] tracklets built (clamped to max_tracklets)
   uint32_t max_tracklets;
   unsigned long long* counters;  // [CN_COUNT] or nullptr
@@ -82,17 +92,12 @@ struct Ctx {
 };
 
 __device__ __forceinline__ uint32_t bins_base(const Ctx& c, uint32_t tr, uint32_t row_lo) {
-  return row_lo + tr * kBinPad;
+  return kBinsPerCluster * row_lo + tr * kBinPad;
 }
 
 // Monotone clamped bin coordinate; the float is clamped before the conversion (SPEC 0).
 __device__ __forceinline__ int bin_coord(float v, float v0, float inv, int n) {
   return (int)fminf(fmaxf((v - v0) * inv, 0.0f), (float)(n - 1));
-}
-
-__device__ __forceinline__ float side_z0(const Ctx& c, uint32_t task) {
-  const bool a_side = 2 * (int)(task % (uint32_t)c.n_sectors) < c.n_sectors;
-  return a_side ? -1.0f : -(c.z_max + 1.0f);
 }
 
 // task*n_rows + row of idx h: last tr with row_off[tr] <= h

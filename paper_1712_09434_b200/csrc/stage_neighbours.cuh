@@ -53,16 +53,16 @@ struct RowView {
   const uint32_t* bins;  // first idx of bin b at bins[b]; bins[ny*nz] = end of the row
   uint32_t yz_base;
   int ny, nz;
-  float inv, y0;
+  float inv, y0, z0;
 };
 
 // Calls f(idx, (y,z)) for every cluster whose bin overlaps the window; one flat loop.
 template <class F>
-__device__ __forceinline__ void for_window(const RowView& v, float z0, float ylo, float yhi, float zlo, float zhi,
+__device__ __forceinline__ void for_window(const RowView& v, float ylo, float yhi, float zlo, float zhi,
                                            F&& f) {
   const int iy0 = bin_coord(ylo, v.y0, v.inv, v.ny), iy1 = bin_coord(yhi, v.y0, v.inv, v.ny);
-  int iz = bin_coord(zlo, z0, v.inv, v.nz);
-  const int iz1 = bin_coord(zhi, z0, v.inv, v.nz);
+  int iz = bin_coord(zlo, v.z0, v.inv, v.nz);
+  const int iz1 = bin_coord(zhi, v.z0, v.inv, v.nz);
   const uint32_t* bp = v.bins + iz * v.ny;
   uint32_t i = bp[iy0], e = bp[iy1 + 1];
   while (true) {
@@ -83,7 +83,7 @@ __device__ __forceinline__ void for_window(const RowView& v, float z0, float ylo
 // The exact serial search of one cluster (N1..N5 as written, ties by gid): nested walk of both windows.
 // Used for the rare clusters the cooperative search cannot decide (chi2 ties, list overflow).
 template <bool COUNT>
-__device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const RowView& vd, int row, float z0, float y,
+__device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const RowView& vd, int row, float y,
                                        float z, int32_t* out_up, int32_t* out_dn, unsigned long long* n_pairs) {
   const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max, M = kGridMargin;
   const float b = c.dx_dn[row], a_ = c.dx_up[row];  // N4
@@ -92,10 +92,10 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
   bool have = false;
   float best = 0.0f;
   uint32_t bu = 0u, bd = 0u;
-  for_window(vu, z0, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
+  for_window(vu, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
     if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) return;  // N2
     const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
-    for_window(vd, z0, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, [&](uint32_t d, float2 pd) {
+    for_window(vd, (y - HY) - M, (y + HY) + M, (zd - HZ) - M, (zd + HZ) + M, [&](uint32_t d, float2 pd) {
       if (!(fabsf(pd.x - y) <= HY && fabsf(pd.y - zd) <= HZ)) return;  // N3
       const float dy = ty - ((y - pd.x) * a_);  // N4
       const float dz = tz - ((z - pd.y) * a_);
@@ -117,13 +117,13 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
 // Window walk of one thread around (y, zc) (zc = the projected z of N1) in row view v: the clusters that
 // pass the window test are appended to the thread's list as ((p.x - y)*sgn*fac, (p.y - z)*sgn*fac, idx).
 // Returns the number that passed (entries beyond kNfList are not stored).
-__device__ __forceinline__ uint32_t nf_collect(const RowView& v, float z0, bool act, float y, float z, float zc,
+__device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float y, float z, float zc,
                                                float HY, float HZ, float sgn, float fac, float* l_y, float* l_z,
                                                uint32_t* l_i) {
   const float M = kGridMargin;
   const int iy0 = bin_coord((y - HY) - M, v.y0, v.inv, v.ny), iy1 = bin_coord((y + HY) + M, v.y0, v.inv, v.ny) + 1;
-  const int iz0 = bin_coord((zc - HZ) - M, z0, v.inv, v.nz);
-  const int nzr = act ? bin_coord((zc + HZ) + M, z0, v.inv, v.nz) - iz0 + 1 : 0;
+  const int iz0 = bin_coord((zc - HZ) - M, v.z0, v.inv, v.nz);
+  const int nzr = act ? bin_coord((zc + HZ) + M, v.z0, v.inv, v.nz) - iz0 + 1 : 0;
   uint32_t n = 0u;
   for (int r = 0; r < nzr; r += 2) {
     const uint32_t* bp = v.bins + (iz0 + r) * v.ny;
@@ -152,7 +152,7 @@ __device__ __forceinline__ uint32_t nf_collect(const RowView& v, float z0, bool 
 }
 
 template <bool COUNT>
-__device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const RowView& vd, int row, float z0,
+__device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const RowView& vd, int row,
                                        uint32_t lo, uint32_t hi, unsigned char* list_smem) {
   const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max;
   const float b = c.dx_dn[row], a_ = c.dx_up[row];  // N4
@@ -172,9 +172,9 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     float y = 0.0f, z = 0.0f;
     if (act) { const float2 h = c.yz[i]; y = h.x; z = h.y; }
     const float zu = z * ratio_up, zd = z * ratio_dn;  // N1
-    const uint32_t nd = nf_collect(vd, z0, act, y, z, zd, HY, HZ, -1.0f, a_, d_y, d_z, d_i);  // N3
+    const uint32_t nd = nf_collect(vd, act, y, z, zd, HY, HZ, -1.0f, a_, d_y, d_z, d_i);  // N3
     __syncwarp();
-    const uint32_t nu = nd ? nf_collect(vu, z0, act, y, z, zu, HY, HZ, 1.0f, b, u_y, u_z, u_i) : 0u;  // N2
+    const uint32_t nu = nd ? nf_collect(vu, act, y, z, zu, HY, HZ, 1.0f, b, u_y, u_z, u_i) : 0u;  // N2
     __syncwarp();
     const bool overflow = nd > (uint32_t)kNfList || nu > (uint32_t)kNfList;
     const uint32_t n_pr = overflow ? 0u : nu * nd;
@@ -199,7 +199,7 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     if (act) {
       int32_t up = -1, dn = -1;
       if (overflow || tie) {
-        nf_serial<COUNT>(c, vu, vd, row, z0, y, z, &up, &dn, &n_pairs);
+        nf_serial<COUNT>(c, vu, vd, row, y, z, &up, &dn, &n_pairs);
       } else if (have) {
         up = (int32_t)u_i[bu * kNfThreads];
         dn = (int32_t)d_i[bd * kNfThreads];
@@ -220,19 +220,17 @@ __global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant
 
   const uint32_t tr = blockIdx.x;
   const int row = (int)(tr % (uint32_t)c.n_rows);
-  const uint32_t task = tr / (uint32_t)c.n_rows;
   const uint32_t lo = c.row_off[tr], hi = c.row_off[tr + 1];
   if (hi == lo) return;
   if (row == 0 || row == c.n_rows - 1) {  // SPEC 3: no links in the first and last row
     for (uint32_t i = lo + threadIdx.x; i < hi; i += kNfThreads) { c.link_up[i] = -1; c.link_dn[i] = -1; }
     return;
   }
-  const float z0 = side_z0(c, task);
   const RowInfo gu = load_row_info(&c.rowinfo[tr + 1]), gd = load_row_info(&c.rowinfo[tr - 1]);
   const uint32_t u_hi = c.row_off[tr + 2];
   RowView vu, vd;
-  vu.ny = info_ny(gu); vu.nz = info_nz(gu); vu.inv = gu.inv; vu.y0 = -c.ymax[row + 1];
-  vd.ny = info_ny(gd); vd.nz = info_nz(gd); vd.inv = gd.inv; vd.y0 = -c.ymax[row - 1];
+  vu.ny = info_ny(gu); vu.nz = info_nz(gu); vu.inv = gu.inv; vu.y0 = gu.y0; vu.z0 = gu.z0;
+  vd.ny = info_ny(gd); vd.nz = info_nz(gd); vd.inv = gd.inv; vd.y0 = gd.y0; vd.z0 = gd.z0;
   // 16-byte aligned source ranges: (y,z) pairs [ya0, ya1) and bin entries [ba0, ba1) of both rows
   const uint32_t uya0 = gu.row_lo & ~1u, uya1 = (u_hi + 1u) & ~1u;
   const uint32_t dya0 = gd.row_lo & ~1u, dya1 = (lo + 1u) & ~1u;
@@ -262,11 +260,11 @@ __global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant
     mbar_wait(bar, 0u);
     vu.yz = s_uyz; vu.yz_base = uya0; vu.bins = s_ub + (gu.bins_off - uba0);
     vd.yz = s_dyz; vd.yz_base = dya0; vd.bins = s_db + (gd.bins_off - dba0);
-    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, list_smem);
+    nf_row<COUNT>(c, vu, vd, row, lo, hi, list_smem);
   } else {
     vu.yz = c.yz; vu.yz_base = 0u; vu.bins = c.bins + gu.bins_off;
     vd.yz = c.yz; vd.yz_base = 0u; vd.bins = c.bins + gd.bins_off;
-    nf_row<COUNT>(c, vu, vd, row, z0, lo, hi, list_smem);
+    nf_row<COUNT>(c, vu, vd, row, lo, hi, list_smem);
   }
 }
 

@@ -9,14 +9,14 @@ namespace tpc {
 constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
 
 // One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by one,
-// the 32 lanes testing 32 hits of the tracklet's list at a time (coalesced list read, 32 owner
+// the 32 lanes testing 32 rows of the tracklet's row map at a time (coalesced map read, 32 owner
 // gathers in flight) - L1: hit kept iff the tracklet still owns it; the keep masks stay in
 // shared memory.  The tile then takes its place in the output with an ordered chained scan over
 // (tracks, hits) packed as tracks<<32 | hits.  Pass 2: the warp writes each surviving track - its
 // record as SoA columns and its kept hits as gids in ascending row order (L3).
 // Output order = tracklet order.
 __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
-  extern __shared__ uint32_t s_keep[];  // [kOutThreads][words] keep masks
+  extern __shared__ uint32_t s_keep[];  // [kOutThreads][words] keep masks, bit k of word w = row first_row + 32 w + k
   __shared__ uint32_t s_warp[33];
   __shared__ uint32_t s_tile;
   __shared__ unsigned long long s_prefix;
@@ -32,22 +32,35 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t t_warp = tile * kOutThreads + warp * 32;
   const int min_hits = c.prm.min_track_hits;
+  // lane j holds what it needs of tracklet t_warp + j: n_hits, first/last row, start-hit gid
+  int my_n = 0, my_first = 0, my_last = -1;
+  uint32_t my_gid0 = 0u;
+  if (t_warp + lane < n_trk) {
+    const float4* rec = c.trk_rec + (size_t)(t_warp + lane) * kRecFloat4;
+    my_n = __float_as_int(__ldg(rec + 5).w);
+    const float4 r6 = __ldg(rec + 6);
+    my_first = __float_as_int(r6.x); my_last = __float_as_int(r6.y);
+    my_gid0 = __ldg(c.trk_seed + (size_t)(t_warp + lane) * kSeedU4 + 2).z;
+  }
   uint32_t my_kept = 0u;  // lane j: hits tracklet t_warp + j still owns
-  for (int j = 0; j < 32; ++j) {
+  for (unsigned rest = __ballot_sync(FULL, my_n >= min_hits); rest; rest &= rest - 1u) {  // K6
+    const int j = __ffs(rest) - 1;
     const uint32_t t = t_warp + j;
-    if (t >= n_trk) break;
-    const float4 r5 = c.trk_rec[(size_t)t * kRecFloat4 + 5];
-    const int n_hits = __float_as_int(r5.w);
-    if (n_hits < min_hits) continue;                                   // K6
+    const int n_hits = __shfl_sync(FULL, my_n, j), first = __shfl_sync(FULL, my_first, j);
+    const int last = __shfl_sync(FULL, my_last, j);
     const unsigned long long key = ((unsigned long long)(uint32_t)n_hits << 32) |
-                                   (unsigned long long)(0xFFFFFFFFu - c.trk_seed[(size_t)t * kSeedU4 + 2].z);
-    const uint32_t* hits = c.trk_hits + (size_t)t * (size_t)n_rows;
+                                   (unsigned long long)(0xFFFFFFFFu - __shfl_sync(FULL, my_gid0, j));
+    const uint32_t* map = c.trk_hits + (size_t)t * (size_t)n_rows;
     uint32_t kept = 0u;
-    for (int k0 = 0; k0 < n_hits; k0 += 32) {
-      const int k = k0 + lane;
-      const bool own = k < n_hits && c.owner[hits[k]] == key;          // L1
+    for (int rb = first; rb <= last; rb += 32) {
+      const int r = rb + lane;
+      bool own = false;
+      if (r <= last) {
+        const uint32_t idx = map[r];
+        own = idx != kNoHit && c.owner[idx] == key;                    // L1
+      }
       const unsigned mask = __ballot_sync(FULL, own);
-      if (lane == 0) s_keep[(warp * 32 + j) * words + (k0 >> 5)] = mask;
+      if (lane == 0) s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)] = mask;
       kept += __popc(mask);
     }
     if (lane == j) my_kept = kept;
@@ -75,6 +88,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     const uint32_t t = t_warp + j;
     const uint32_t slot = __shfl_sync(FULL, my_slot, j), hb = __shfl_sync(FULL, my_hb, j);
     const uint32_t kept = __shfl_sync(FULL, my_kept, j);
+    const int first = __shfl_sync(FULL, my_first, j), last = __shfl_sync(FULL, my_last, j);
     if (slot >= o.track_capacity) { status |= TPC_STATUS_TRACK_OVERFLOW; continue; }
     // record -> SoA columns: lanes 0..22 carry x, p[5], c[15], chi2, ndf
     const float v = lane < 28 ? reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4)[lane] : 0.0f;
@@ -88,12 +102,11 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     else if (lane == 21) o.track_chi2[slot] = v;
     else if (lane == 22) o.track_ndf[slot] = __float_as_int(v);
     if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
-    const int n_hits = __float_as_int(__shfl_sync(FULL, v, 23));
-    const uint32_t* hits = c.trk_hits + (size_t)t * (size_t)n_rows;
+    const uint32_t* map = c.trk_hits + (size_t)t * (size_t)n_rows;
     uint32_t w = hb;
-    for (int k0 = 0; k0 < n_hits; k0 += 32) {
-      const unsigned mask = s_keep[(warp * 32 + j) * words + (k0 >> 5)];
-      if (mask & (1u << lane)) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = c.gid[hits[k0 + lane]];
+    for (int rb = first; rb <= last; rb += 32) {
+      const unsigned mask = s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)];
+      if (mask & (1u << lane)) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = c.gid[map[rb + lane]];
       w += __popc(mask);
     }
   }
@@ -138,12 +151,10 @@ __global__ void k_debug_tracklets(const Ctx c) {
   if (o.dbg_tracklet_par)
     for (int j = 0; j < 5; ++j) o.dbg_tracklet_par[(size_t)t * 5 + j] = rec[1 + j];
   if (o.dbg_tracklet_map) {
-    for (int r = 0; r < n_rows; ++r) o.dbg_tracklet_map[(size_t)t * n_rows + r] = -1;
-    const uint32_t tr_base = c.trk_seed[(size_t)t * kSeedU4].y / (uint32_t)n_rows * (uint32_t)n_rows;
-    for (int k = 0; k < n_hits; ++k) {
-      const uint32_t m = c.trk_hits[(size_t)t * n_rows + k];
-      const uint32_t r = find_tr(c, m) - tr_base;
-      o.dbg_tracklet_map[(size_t)t * n_rows + r] = (int32_t)c.gid[m];
+    const int first = __float_as_int(rec[24]), last = __float_as_int(rec[25]);
+    for (int r = 0; r < n_rows; ++r) {
+      const uint32_t m = (r >= first && r <= last) ? c.trk_hits[(size_t)t * n_rows + r] : kNoHit;
+      o.dbg_tracklet_map[(size_t)t * n_rows + r] = m != kNoHit ? (int32_t)c.gid[m] : -1;
     }
   }
 }

@@ -10,16 +10,19 @@
 // a single row step
 //     transport -> choose the hit (chain link / row map / search) -> update
 // with a per-lane phase, so lanes in different passes execute the same
-// instructions.  The row -> hit map of the running tracklet lives in shared
-// memory as row-local indices (16 bit; 32 bit when a row holds >= 65535
-// clusters); when a tracklet ends the WARP writes its hit list, claims the hits
-// (K7, atomicMax) and stores its record cooperatively.
+// instructions.  The row -> hit map of a tracklet is its row of Ctx::trk_hits in
+// global memory (idx per pad row or kNoHit): written once per row step, read
+// back in the down pass ONE ROW AHEAD, so that together with the chain link and
+// the grid header every load a step needs is issued before the transport
+// arithmetic and none is waited for.  No shared memory besides the row table:
+// the registers alone bound the number of tracklets in flight.
 #pragma once
 #include "device_common.cuh"
 
 namespace tpc {
 
-constexpr int kTrackletThreads = 128;  // u16 row maps, n_rows <= 192; other shapes: tracklet_threads()
+constexpr int kTrackletThreads = 128;
+constexpr int kTrackletBlocksPerSm = 6;  // registers per thread <= 65536 / (128 * 6) = 85
 
 struct TrackState {
   float y, z, s, t, q;  // SPEC 5: y, z, sinphi, dz/dl, q/pT
@@ -158,7 +161,7 @@ __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz,
 constexpr int kSearchUnroll = 4;
 
 template <bool COUNT>
-__device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g, float y0, float z0,
+__device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g,
                                               float2& best_p, uint32_t& n_cand) {
   const float y = S.y, z = S.z;
   const float ey = S.c00 + c.sy2, ez = S.c11 + c.sz2;                 // H1
@@ -166,8 +169,8 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
   const float hz2 = fminf(c.prm.accept_k2 * ez, c.smax2);
   const float wy = sqrtf(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrtf(fmaxf(hz2, 0.0f)) + kGridMargin;
   const int ny = info_ny(g), nz = info_nz(g);
-  const int iy0 = bin_coord(y - wy, y0, g.inv, ny), iy1 = bin_coord(y + wy, y0, g.inv, ny) + 1;
-  const int iz0 = bin_coord(z - wz, z0, g.inv, nz), iz1 = bin_coord(z + wz, z0, g.inv, nz);
+  const int iy0 = bin_coord(y - wy, g.y0, g.inv, ny), iy1 = bin_coord(y + wy, g.y0, g.inv, ny) + 1;
+  const int iz0 = bin_coord(z - wz, g.z0, g.inv, nz), iz1 = bin_coord(z + wz, g.z0, g.inv, nz);
   const uint32_t* bp0 = c.bins + g.bins_off + iz0 * ny;
   const uint32_t* bp = bp0;
   float best = __int_as_float(0x7f800000);  // +inf: a valid cluster at distance +inf counts as a tie
@@ -212,29 +215,14 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
 
 enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4, PH_ENDED = 5, PH_FETCH = 6, PH_EXIT = 7 };
 
-// Threads per block and dynamic shared memory of k_tracklets for a detector of n_rows rows.
-__host__ __device__ inline int tracklet_threads(int n_rows, int map_bytes) {
-  const int per_thread = n_rows * map_bytes;
-  return per_thread <= 384 ? 128 : (per_thread <= 1024 ? 64 : 32);
-}
-__host__ __device__ inline size_t tracklet_tab_bytes(int n_rows) { return (size_t)((n_rows * 8 + 15) / 16 * 16); }
-__host__ __device__ inline size_t tracklet_smem(int n_rows, int map_bytes) {
-  return tracklet_tab_bytes(n_rows) + (size_t)n_rows * map_bytes * tracklet_threads(n_rows, map_bytes);
-}
+constexpr uint32_t kNoHit = 0xFFFFFFFFu;  // row map entry of a row without a hit
 
-template <typename MapT, bool COUNT>
-__global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
-  extern __shared__ __align__(16) unsigned char trk_smem[];
-  constexpr MapT kNone = (MapT)~(MapT)0;
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_tracklets(const Ctx c) {
+  extern __shared__ __align__(16) float sX[];  // [n_rows] x of the pad rows
   constexpr unsigned FULL = 0xffffffffu;
-  // rows of >= 65535 clusters need the 32-bit instantiation; exactly one of the two launches works
-  const bool big_rows = c.tickets[3] >= 0xFFFFu;
-  if (big_rows != (sizeof(MapT) == 4)) return;
   const int n_rows = c.n_rows, nthr = (int)blockDim.x, tid = (int)threadIdx.x, lane = tid & 31;
-  float* sX = reinterpret_cast<float*>(trk_smem);
-  float* sYmax = sX + n_rows;
-  MapT* s_map = reinterpret_cast<MapT*>(trk_smem + tracklet_tab_bytes(n_rows));  // [n_rows][nthr]
-  for (int r = tid; r < n_rows; r += nthr) { sX[r] = c.X[r]; sYmax[r] = c.ymax[r]; }
+  for (int r = tid; r < n_rows; r += nthr) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
@@ -246,43 +234,31 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
   S.c40 = S.c41 = S.c42 = S.c43 = S.c44 = 0.0f;
   S.chi2 = 0.0f; S.ndf = -5;
   uint32_t t = 0u, tr_base = 0u, gid0 = 0u;
-  float z0 = 0.0f;
+  uint32_t* map = c.trk_hits;  // row map of the running tracklet
   int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
   int32_t last_hit = -1, next_chain = -1;
+  uint32_t map_next = kNoHit;  // down pass: map[r_down], loaded one step ahead
   int phase = PH_FETCH;
   uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_chain = 0u, n_kept = 0u, n_kept_hits = 0u;
 
   while (true) {
-    // (A) tracklets that ended in the last step: the warp stores them one by one (hit list in
-    //     ascending row order, K7 ownership claims, record)
+    // (A) tracklets that ended in the last step: the warp claims their hits one tracklet at a time
+    //     (K7 ownership, 32 rows of the map per round), the lane stores the record
     unsigned ended = __ballot_sync(FULL, phase == PH_ENDED);
+    if (ended) __syncwarp();  // the map rows written by the ended lanes are read by the other lanes below
     while (ended) {
       const int L = __ffs(ended) - 1;
       ended &= ended - 1u;
-      const uint32_t ft = __shfl_sync(FULL, t, L), ftr = __shfl_sync(FULL, tr_base, L);
-      const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
       const int fn = __shfl_sync(FULL, n_hits, L);
-      const uint32_t fgid0 = __shfl_sync(FULL, gid0, L);
-      const int col = (tid & ~31) + L;
-      unsigned long long key = 0ull;
-      if (fn >= min_hits)  // K6, K7: longest tracklet wins, then the smaller start-hit gid
-        key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
-      uint32_t* hits_out = c.trk_hits + (size_t)ft * (size_t)n_rows;
-      uint32_t wpos = 0u;
-      for (int rb = ffirst; rb <= flast; rb += 32) {
-        const int r = rb + lane;
-        bool has = false;
-        uint32_t idx = 0u;
-        if (r <= flast) {
-          const MapT m = s_map[r * nthr + col];
-          if (m != kNone) { has = true; idx = c.row_off[ftr + (uint32_t)r] + (uint32_t)m; }
+      if (fn >= min_hits) {  // K6, K7: longest tracklet wins, then the smaller start-hit gid
+        const uint32_t ft = __shfl_sync(FULL, t, L), fgid0 = __shfl_sync(FULL, gid0, L);
+        const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
+        const unsigned long long key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
+        const uint32_t* fmap = c.trk_hits + (size_t)ft * (size_t)n_rows;
+        for (int r = ffirst + lane; r <= flast; r += 32) {
+          const uint32_t idx = fmap[r];
+          if (idx != kNoHit) atomicMax(&c.owner[idx], key);
         }
-        const unsigned mask = __ballot_sync(FULL, has);
-        if (has) {
-          hits_out[wpos + __popc(mask & ((1u << lane) - 1u))] = idx;
-          if (key) atomicMax(&c.owner[idx], key);
-        }
-        wpos += __popc(mask);
       }
       if (lane == L) {
         float4* rec = c.trk_rec + (size_t)t * kRecFloat4;
@@ -293,7 +269,7 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
         rec[4] = make_float4(S.c40, S.c41, S.c42, S.c43);
         rec[5] = make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits));
         rec[6] = make_float4(__int_as_float(first_row), __int_as_float(last_row), 0.0f, 0.0f);
-        if (COUNT && key) { ++n_kept; n_kept_hits += (uint32_t)n_hits; }
+        if (COUNT && n_hits >= min_hits) { ++n_kept; n_kept_hits += (uint32_t)n_hits; }
         phase = PH_FETCH;
       }
     }
@@ -315,8 +291,8 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
           const uint32_t task = tr0 / (uint32_t)n_rows;
           r0 = (int)(tr0 - task * (uint32_t)n_rows);
           tr_base = task * (uint32_t)n_rows;
-          z0 = side_z0(c, task);
           gid0 = q2.z;
+          map = c.trk_hits + (size_t)t * (size_t)n_rows;
           const float y0s = __uint_as_float(q1.x), z0s = __uint_as_float(q1.y);
           const float y1s = __uint_as_float(q1.z), z1s = __uint_as_float(q1.w);
           const float dx = sX[r0 + 1] - sX[r0], dy = y1s - y0s, dz = z1s - z0s;
@@ -326,8 +302,8 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
           S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
           S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
           S.chi2 = 0.0f; S.ndf = -5;
-          s_map[r0 * nthr + tid] = (MapT)q2.x;
-          s_map[(r0 + 1) * nthr + tid] = (MapT)q2.y;
+          map[r0] = q0.x;
+          map[r0 + 1] = q0.z;
           row_cur = r0 + 1; first_row = r0; last_row = r0 + 1; n_hits = 2; gap = 0; r_down = 0;
           last_hit = (int32_t)q0.z;
           next_chain = (int32_t)q0.w;
@@ -338,15 +314,14 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
     }
     if (__ballot_sync(FULL, phase != PH_EXIT) == 0u) break;
     // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping.
-    //     The three parts are separated by warp barriers so that the lanes run each of them together
+    //     The parts are separated by warp barriers so that the lanes run each of them together
     //     whatever their phase is.
     int rt = 0;
-    uint32_t row_lo = 0u;
     int32_t hit = -1;
     float2 hp = make_float2(0.0f, 0.0f);
     bool book = false, do_search = false;
     RowInfo g;
-    g.inv = 0.0f; g.ny_nz = 0u; g.bins_off = 0u; g.row_lo = 0u;
+    g.inv = 0.0f; g.y0 = 0.0f; g.z0 = 0.0f; g.ny_nz = 0u; g.bins_off = 0u; g.row_lo = 0u; g.pad0 = 0u; g.pad1 = 0u;
     if (phase <= PH_FINISH) {
       if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
       if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
@@ -354,19 +329,21 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
       else if (phase == PH_TURN) rt = last_row;
       else if (phase == PH_DOWN) rt = r_down;
       else rt = first_row;
-      // loads that do not depend on the transported state are issued before the transport: the row's grid
-      // header, and the hit when it is known already (chain link, lastRow hit at the turn, row map)
-      g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
-      row_lo = g.row_lo;
+      // Every load of this step whose address does not depend on the transported state is issued here,
+      // before the transport: the hit when it is known already (chain link, lastRow hit at the turn, row
+      // map entry fetched a step ago), the next chain link, the map entry of the next down row, and the
+      // row's grid header when a search may follow.
       int32_t known = -1;
       if (phase == PH_CHAIN) known = next_chain;
       else if (phase == PH_TURN) known = last_hit;
-      else if (phase == PH_DOWN && rt >= r0) {
-        const MapT m = s_map[rt * nthr + tid];
-        if (m != kNone) known = (int32_t)(row_lo + (uint32_t)m);
-      }
+      else if (phase == PH_DOWN && map_next != kNoHit) known = (int32_t)map_next;
       if (known >= 0) hp = c.yz[known];
       if (phase == PH_CHAIN) next_chain = c.clean_up[known];            // K2: the link after this one
+      if (phase == PH_TURN || phase == PH_DOWN) {                       // map entry of the row after this one
+        const int rn = (phase == PH_TURN ? last_row : rt) - 1;
+        map_next = rn >= r0 ? map[rn] : kNoHit;
+      }
+      if (phase == PH_UP || (phase == PH_DOWN && known < 0)) g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
       bool ok = true;
       if (rt != row_cur) {
         ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
@@ -394,25 +371,24 @@ __global__ void __launch_bounds__(kTrackletThreads) k_tracklets(const Ctx c) {
     __syncwarp();
     if (do_search) {
       if (COUNT) ++n_search;
-      hit = search_row<COUNT>(c, S, g, -sYmax[rt], z0, hp, n_cand);
+      hit = search_row<COUNT>(c, S, g, hp, n_cand);
     }
     __syncwarp();
     if (hit >= 0) update_hit(S, hp.x, hp.y, sy2, sz2);
     __syncwarp();
     if (book) {
-      const MapT m = hit >= 0 ? (MapT)((uint32_t)hit - row_lo) : kNone;
       if (phase == PH_CHAIN) {
-        s_map[rt * nthr + tid] = m;
+        map[rt] = (uint32_t)hit;
         last_row = rt; last_hit = hit; ++n_hits;
         if (COUNT) ++n_chain;
         if (next_chain < 0) { phase = PH_UP; gap = 0; }
       } else if (phase == PH_UP) {
-        s_map[rt * nthr + tid] = m;
+        map[rt] = (uint32_t)hit;  // -1 = kNoHit
         if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
         else if (++gap > max_gap) phase = PH_TURN;
       } else {  // PH_DOWN
         if (do_search) {
-          s_map[rt * nthr + tid] = m;
+          map[rt] = (uint32_t)hit;
           if (hit >= 0) {
             ++n_hits;
             if (rt < first_row) { first_row = rt; gap = 0; }

@@ -12,30 +12,34 @@ namespace tpc {
 // ---------------------------------------------------------------------------
 // a1  grid build.  One block per (task,row).  The grid is acceleration only
 // (SPEC 2): every later search applies the exact test to a superset, so the bin
-// size below is this implementation's own choice.  The clusters of a row are
+// size and the extent of the grid (the bounding box of the row's clusters) are this implementation's own choice.  The clusters of a row are
 // rewritten as float2 (y,z) in bin order ("idx" order) with idx -> gid beside;
 // inside a bin they are ordered by gid so that idx order, and with it the order
 // of start hits, tracklets and output tracks, is the same on every run.
 // ---------------------------------------------------------------------------
 constexpr int kGridThreads = 128;
 
-__device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, int row, uint32_t lo, uint32_t n) {
-  const float W = 2.0f * c.ymax[row], L = c.z_max + 2.0f;
-  float B = sqrtf((W * L) / (float)(n > 0u ? n : 1u));
+// Grid of a row with n clusters inside the box [ylo, yhi] x [zlo, zhi]: kBinsPerCluster bins per cluster.
+__device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint32_t lo, uint32_t n, float ylo,
+                                                 float yhi, float zlo, float zhi) {
+  const float W = fmaxf(yhi - ylo, 0.0f), L = fmaxf(zhi - zlo, 0.0f);
+  float B = sqrtf((W * L) / (float)(kBinsPerCluster * (n > 0u ? n : 1u)));
   B = fminf(fmaxf(B, c.prm.grid_bin_min), c.prm.grid_bin_max);
   RowInfo g;
   int ny, nz;
   while (true) {
     g.inv = 1.0f / B;
-    ny = (int)(W * g.inv) + 1;
-    nz = (int)(L * g.inv) + 1;
+    ny = (int)fminf(W * g.inv, 65000.0f) + 1;
+    nz = (int)fminf(L * g.inv, 65000.0f) + 1;
     const long long nb = (long long)ny * nz;
-    if (nb + 1 <= (long long)n + kBinPad && nb <= (long long)kMaxBinsPerRow) break;
+    if (nb + 1 <= (long long)kBinsPerCluster * n + kBinPad && nb <= (long long)kMaxBinsPerRow) break;
     B = B * 1.25f;  // too many bins for the slot of this row: coarser grid
   }
+  g.y0 = ylo; g.z0 = zlo;
   g.ny_nz = (uint32_t)ny | ((uint32_t)nz << 16);
   g.bins_off = bins_base(c, tr, lo);
   g.row_lo = lo;
+  g.pad0 = 0u; g.pad1 = 0u;
   return g;
 }
 
@@ -43,19 +47,34 @@ template <bool COUNT>
 __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   __shared__ uint32_t s_cnt[kMaxBinsPerRow + 1];
   __shared__ uint32_t s_part[kGridThreads];
+  __shared__ float s_box[4][kGridThreads / 32];
   const uint32_t tr = blockIdx.x;
-  const int row = (int)(tr % (uint32_t)c.n_rows);
-  const uint32_t task = tr / (uint32_t)c.n_rows;
   const uint32_t lo = c.row_off[tr], hi = c.row_off[tr + 1], n = hi - lo;
-  const RowInfo g = make_row_info(c, tr, row, lo, n);
+  const int tid = threadIdx.x;
+  // bounding box of the row's clusters
+  const float kInf = __int_as_float(0x7f800000);
+  float ylo = kInf, yhi = -kInf, zlo = kInf, zhi = -kInf;
+  for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
+    const float y = c.y[i], z = c.z[i];
+    ylo = fminf(ylo, y); yhi = fmaxf(yhi, y); zlo = fminf(zlo, z); zhi = fmaxf(zhi, z);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ylo = fminf(ylo, __shfl_xor_sync(0xffffffffu, ylo, o)); yhi = fmaxf(yhi, __shfl_xor_sync(0xffffffffu, yhi, o));
+    zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, o)); zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+  }
+  if ((tid & 31) == 0) { s_box[0][tid >> 5] = ylo; s_box[1][tid >> 5] = yhi; s_box[2][tid >> 5] = zlo; s_box[3][tid >> 5] = zhi; }
+  __syncthreads();
+#pragma unroll
+  for (int w = 0; w < kGridThreads / 32; ++w) {
+    ylo = fminf(ylo, s_box[0][w]); yhi = fmaxf(yhi, s_box[1][w]); zlo = fminf(zlo, s_box[2][w]); zhi = fmaxf(zhi, s_box[3][w]);
+  }
+  if (n == 0u) { ylo = yhi = zlo = zhi = 0.0f; }
+  const RowInfo g = make_row_info(c, tr, lo, n, ylo, yhi, zlo, zhi);
   const int g_ny = info_ny(g), g_nz = info_nz(g);
   const int nb = g_ny * g_nz;
-  const float y0 = -c.ymax[row], z0 = side_z0(c, task);
-  const int tid = threadIdx.x;
-  if (tid == 0) {
-    c.rowinfo[tr] = g;
-    if (n >= 0xFFFFu) atomicMax(&c.tickets[3], n);  // rows this large need the 32-bit row maps of a5
-  }
+  const float y0 = g.y0, z0 = g.z0;
+  if (tid == 0) c.rowinfo[tr] = g;
   for (int b = tid; b <= nb; b += kGridThreads) s_cnt[b] = 0u;
   __syncthreads();
   for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {

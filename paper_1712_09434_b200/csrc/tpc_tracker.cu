@@ -30,10 +30,9 @@ struct tpc_tracker {
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
-  // persistent tracklet kernel: [map width 16/32 bit][counters off/on] -> blocks that fit the device at once
-  int trk_threads[2] = {0, 0};
-  size_t trk_smem[2] = {0, 0};
-  int trk_grid[2][2] = {{0, 0}, {0, 0}};
+  // persistent tracklet kernel: [counters off/on] -> blocks that fit the device at once
+  size_t trk_smem = 0;
+  int trk_grid[2] = {0, 0};
   // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
   bool timing_on = false;
   std::vector<cudaEvent_t> ev;
@@ -79,7 +78,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
   c.yz = take(n4 * sizeof(float2));
   c.gid = take(n4 * sizeof(uint32_t));
-  c.bins = take(((size_t)n + n_tr * kBinPad + 16) * sizeof(uint32_t));  // + slack of the 16-byte aligned bulk copies
+  c.bins = take(((size_t)kBinsPerCluster * n + n_tr * kBinPad + 16) * sizeof(uint32_t));  // + slack of the 16-byte aligned bulk copies
   c.rowinfo = take((n_tr + 1) * sizeof(RowInfo));
   c.link_up = take(n4 * sizeof(int32_t));
   c.link_dn = take(n4 * sizeof(int32_t));
@@ -205,19 +204,12 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute((const void*)k_neighbours<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)kNfSmemBytes);
-  for (int w = 0; w < 2 && e == cudaSuccess; ++w) {
-    const int map_bytes = w ? 4 : 2;
-    t->trk_threads[w] = tracklet_threads(t->n_rows, map_bytes);
-    t->trk_smem[w] = tracklet_smem(t->n_rows, map_bytes);
-    for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
-      const void* fn = w ? (cnt ? (const void*)k_tracklets<uint32_t, true> : (const void*)k_tracklets<uint32_t, false>)
-                         : (cnt ? (const void*)k_tracklets<uint16_t, true> : (const void*)k_tracklets<uint16_t, false>);
-      e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t->trk_smem[w]);
-      int per_sm = 0;
-      if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, t->trk_threads[w], t->trk_smem[w]);
-      t->trk_grid[w][cnt] = (per_sm > 0 ? per_sm : 1) * n_sm;
-    }
+  t->trk_smem = (size_t)t->n_rows * sizeof(float);
+  for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
+    const void* fn = cnt ? (const void*)k_tracklets<true> : (const void*)k_tracklets<false>;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kTrackletThreads, t->trk_smem);
+    t->trk_grid[cnt] = (per_sm > 0 ? per_sm : 1) * n_sm;
   }
   if (e != cudaSuccess) {
     const int rc = fail(nullptr, TPC_ERR_CUDA, "tpc_tracker_create: CUDA: %s", cudaGetErrorString(e));
@@ -245,7 +237,7 @@ size_t tpc_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t
   return carve((uint32_t)t->n_rows, max_clusters, max_tasks, T).total;
 }
 
-int tpc_launches_per_batch(const tpc_tracker*) { return 7; }  // a5 is launched in both row-map widths; one returns at once
+int tpc_launches_per_batch(const tpc_tracker*) { return 6; }  // a1, a2, a3, a4, a5, a6+a7
 
 void tpc_tracker_enable_counters(tpc_tracker* t, int on) {
   if (t) t->counters_on = on != 0;
@@ -350,14 +342,9 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
   else k_seeds<false><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);
   mark();
-  // a5: persistent, one launch per row-map width; the one that does not match the batch returns at once
-  if (cnt) {
-    k_tracklets<uint16_t, true><<<t->trk_grid[0][1], t->trk_threads[0], t->trk_smem[0], s>>>(c);
-    k_tracklets<uint32_t, true><<<t->trk_grid[1][1], t->trk_threads[1], t->trk_smem[1], s>>>(c);
-  } else {
-    k_tracklets<uint16_t, false><<<t->trk_grid[0][0], t->trk_threads[0], t->trk_smem[0], s>>>(c);
-    k_tracklets<uint32_t, false><<<t->trk_grid[1][0], t->trk_threads[1], t->trk_smem[1], s>>>(c);
-  }
+  // a5: persistent, as many blocks as the device holds at once
+  if (cnt) k_tracklets<true><<<t->trk_grid[1], kTrackletThreads, t->trk_smem, s>>>(c);
+  else k_tracklets<false><<<t->trk_grid[0], kTrackletThreads, t->trk_smem, s>>>(c);
   mark();
   const size_t keep_smem = (size_t)kOutThreads * ((size_t)(t->n_rows + 31) / 32) * sizeof(uint32_t);
   k_select_output<<<cv.out_tiles, kOutThreads, keep_smem, s>>>(c);                          // a6 + a7
