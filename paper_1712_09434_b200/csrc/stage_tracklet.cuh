@@ -133,7 +133,7 @@ __device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, fl
 // search below hands over to this one when it meets two valid clusters with the same distance.
 __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz, const uint32_t* __restrict__ gid,
                                                   const uint32_t* bp, int ny, int iy0, int iy1, int n_zrows, float y,
-                                                  float z, float hy2, float hz2, float ey, float ez, float2* best_p) {
+                                                  float z, float hy2, float hz2, float ey, float ez) {
   bool have = false;
   float best = 0.0f;
   uint32_t bi = 0u;
@@ -146,7 +146,7 @@ __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz,
         const float d = (dy2 * ez) + (dz2 * ey);                       // H5
         bool take = !have || d < best;                                 // H6
         if (have && d == best) take = gid[i] < gid[bi];
-        if (take) { have = true; best = d; bi = i; *best_p = p; }
+        if (take) { have = true; best = d; bi = i; }
       }
     }
   }
@@ -208,8 +208,11 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
       }
     }
   }
+  if (tie) {  // the (y,z) is re-read here so that best_p never has its address taken (it stays in registers)
+    bi = search_row_serial(c.yz, c.gid, bp0, ny, iy0, iy1, iz1 - iz0 + 1, y, z, hy2, hz2, ey, ez);
+    if (bi >= 0) { const float2 p = c.yz[bi]; bx = p.x; bz = p.y; }
+  }
   best_p = make_float2(bx, bz);
-  if (tie) bi = search_row_serial(c.yz, c.gid, bp0, ny, iy0, iy1, iz1 - iz0 + 1, y, z, hy2, hz2, ey, ez, &best_p);
   return bi;
 }
 
