@@ -7,6 +7,7 @@
 namespace tpc {
 
 constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
+constexpr int kOutChunks = 5;     // 32-row chunks of a row map tested per round (159 rows = 5 chunks)
 
 // One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by one,
 // the 32 lanes testing 32 rows of the tracklet's row map at a time (coalesced map read, 32 owner
@@ -52,16 +53,23 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
                                    (unsigned long long)(0xFFFFFFFFu - __shfl_sync(FULL, my_gid0, j));
     const uint32_t* map = c.trk_hits + (size_t)t * (size_t)n_rows;
     uint32_t kept = 0u;
-    for (int rb = first; rb <= last; rb += 32) {
-      const int r = rb + lane;
-      bool own = false;
-      if (r <= last) {
-        const uint32_t idx = map[r];
-        own = idx != kNoHit && c.owner[idx] == key;                    // L1
+    // kOutChunks x 32 rows per round: all map loads of a round are issued together, then all owner gathers
+    for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
+      uint32_t idx[kOutChunks];
+      unsigned long long own[kOutChunks];
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) {
+        const int r = rb0 + 32 * q + lane;
+        idx[q] = r <= last ? map[r] : kNoHit;
       }
-      const unsigned mask = __ballot_sync(FULL, own);
-      if (lane == 0) s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)] = mask;
-      kept += __popc(mask);
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) own[q] = idx[q] != kNoHit ? c.owner[idx[q]] : 0ull;
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) {
+        const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit && own[q] == key);   // L1
+        if (lane == 0 && rb0 + 32 * q <= last) s_keep[(warp * 32 + j) * words + ((rb0 - first) >> 5) + q] = mask;
+        kept += __popc(mask);
+      }
     }
     if (lane == j) my_kept = kept;
   }

@@ -176,6 +176,29 @@ def test_hand_built_rows_ragged_and_ties():
     assert ref.n_tracks >= 2
 
 
+def test_rows_beyond_16_bit_indices():
+    """Maximum sizes: three adjacent rows of 70 000 clusters each (row-local indices need more than 16 bits; bins
+    hold ~17 clusters, so the candidate lists of the neighbour finder overflow and its serial search runs), next to
+    ordinary rows with three straight tracks."""
+    geom = default_geometry(n_sectors=1, n_rows=14)
+    rng = np.random.default_rng(7)
+    pts = {}
+    for r in range(14):
+        x = float(geom.row_x[r])
+        row = [(0.01 * x, 0.5 * x), (-0.02 * x, 0.2 * x), (3.0 + 0.03 * x, 0.9 * x)]
+        if 5 <= r <= 7:
+            w = x * float(geom.tan_half_angle)
+            yy = rng.uniform(-w, w, 70_000).astype(np.float32)
+            zz = rng.uniform(0.0, 250.0, 70_000).astype(np.float32)
+            row += list(zip(yy.tolist(), zz.tolist()))
+        pts[(0, r)] = row
+    b = batch_from_rows(geom, pts, n_tasks=1)
+    assert int(np.diff(b.row_offsets.astype(np.int64)).max()) > 65535
+    gpu = G.run_gpu(b, debug_tracklets=False)
+    ref = G.run_oracle(b, dump_tracklets=False)
+    G.compare(gpu, ref, 14, rtol=RTOL, check_tracklets=False)
+
+
 def test_overflow_sets_status_and_never_writes_out_of_bounds():
     b = generate_config(0)
     ref = G.run_oracle(b)
