@@ -27,6 +27,11 @@ if ROOT not in sys.path:
 METRIC = "tpc_clusters_tracked_per_s"
 UNIT = "clusters/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+# From the committed `ncu --set full` capture of the tracklet constructor on this workload
+# (profiles/r01_ncu_tracklets.md): DRAM bytes read + written and thread instructions executed per launch.
+NCU_TRACKLETS = {"workload": "config3_batch16_central", "dram_bytes": 12.996e9 + 3.166e9, "thread_inst": 149.5e9,
+                 "source": "profiles/r01_ncu_tracklets.md"}
+ALU_PEAK_THREAD_INST_PER_S = 148 * 4 * 32 * 1.965e9  # SMs x schedulers x lanes x SM clock
 
 
 def parse_args():
@@ -285,6 +290,7 @@ def run_ours(args):
     top_gbs = alg[top] / (stage_ms[top] / 1e3) / 1e9 if stage_ms[top] > 0 else 0.0
     path_bytes = sum(alg.values())
     path_gbs = path_bytes / (ms_step / 1e3) / 1e9
+    ncu_ok = top == "tracklet_constructor" and CONFIGS[args.config]["name"] == NCU_TRACKLETS["workload"] and args.events is None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -298,12 +304,20 @@ def run_ours(args):
         "tracks_per_s": tot[2] * args.steps / secs,
         "hbm_roofline_frac_path": path_gbs / peak_gbs,
         "roofline": {"bound": "hbm", "kernel": top, "achieved": top_gbs, "peak": peak_gbs, "unit": "GB/s",
-                     "frac": top_gbs / peak_gbs, "traffic": None, "peak_source": peak_src,
+                     "frac": top_gbs / peak_gbs, "traffic": NCU_TRACKLETS["dram_bytes"] if ncu_ok else None,
+                     "traffic_source": NCU_TRACKLETS["source"] if ncu_ok else None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg[top], "ms_per_launch": stage_ms[top],
                      "share_of_step": stage_ms[top] / max(sum(stage_ms.values()), 1e-9)},
         "roofline_path": {"bound": "hbm", "achieved": path_gbs, "peak": peak_gbs, "unit": "GB/s",
                           "frac": path_gbs / peak_gbs, "algorithmic_bytes_per_step": path_bytes,
                           "bytes_per_cluster": path_bytes / max(n, 1)},
+        # the dominant kernel is bound by plain (non-FMA) ALU issue, not by HBM: thread
+        # instructions per launch from the committed ncu capture over the live launch time, against the ALU ceiling
+        "alu": ({"bound": "alu", "kernel": top, "achieved": NCU_TRACKLETS["thread_inst"] / (stage_ms[top] / 1e3) / 1e12,
+                 "peak": ALU_PEAK_THREAD_INST_PER_S / 1e12, "unit": "T thread-instructions/s",
+                 "frac": NCU_TRACKLETS["thread_inst"] / (stage_ms[top] / 1e3) / ALU_PEAK_THREAD_INST_PER_S,
+                 "thread_inst_per_launch": NCU_TRACKLETS["thread_inst"], "source": NCU_TRACKLETS["source"]}
+                if ncu_ok else None),
         "stages_ms": stage_ms, "stages_algorithmic_bytes": alg, "stage_calls_averaged": stage_calls,
         "counters": counters,
         "clocks": clocks,

@@ -16,6 +16,8 @@ namespace tpc {
 constexpr int kMaxRows = 1024;        // include/tpc_tracker.h: n_rows <= 1024
 constexpr uint32_t kBinsPerCluster = 2;  // grid density: bins per cluster of a row (the clusters bunch at small |z|)
 constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at kBinsPerCluster*row_off[tr] + tr*kBinPad
+// entries of one tracklet's row map in Ctx::trk_hits: n_rows rounded up to whole 32-byte sectors
+__host__ __device__ inline size_t map_stride(int n_rows) { return (size_t)((n_rows + 7) & ~7); }
 constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the grid build
 constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
 
@@ -78,7 +80,7 @@ struct Ctx {
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   unsigned long long* owner;  // [n] K7 ownership key
   uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)
-  uint32_t* trk_hits;      // [max_tracklets][n_rows] row map of the tracklet: idx of its hit in that row or kNoHit;
+  uint32_t* trk_hits;      // [max_tracklets][map_stride(n_rows)] row map of the tracklet: idx of its hit in that row or kNoHit;
                            // valid for the rows first_row..last_row of the tracklet record
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     const int last = __shfl_sync(FULL, my_last, j);
     const unsigned long long key = ((unsigned long long)(uint32_t)n_hits << 32) |
                                    (unsigned long long)(0xFFFFFFFFu - __shfl_sync(FULL, my_gid0, j));
-    const uint32_t* map = c.trk_hits + (size_t)t * (size_t)n_rows;
+    const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t kept = 0u;
     // kOutChunks x 32 rows per round: all map loads of a round are issued together, then all owner gathers
     for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     else if (lane == 21) o.track_chi2[slot] = v;
     else if (lane == 22) o.track_ndf[slot] = __float_as_int(v);
     if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
-    const uint32_t* map = c.trk_hits + (size_t)t * (size_t)n_rows;
+    const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t w = hb;
     for (int rb = first; rb <= last; rb += 32) {
       const unsigned mask = s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)];
@@ -161,7 +161,7 @@ __global__ void k_debug_tracklets(const Ctx c) {
   if (o.dbg_tracklet_map) {
     const int first = __float_as_int(rec[24]), last = __float_as_int(rec[25]);
     for (int r = 0; r < n_rows; ++r) {
-      const uint32_t m = (r >= first && r <= last) ? c.trk_hits[(size_t)t * n_rows + r] : kNoHit;
+      const uint32_t m = (r >= first && r <= last) ? c.trk_hits[(size_t)t * map_stride(n_rows) + r] : kNoHit;
       o.dbg_tracklet_map[(size_t)t * n_rows + r] = m != kNoHit ? (int32_t)c.gid[m] : -1;
     }
   }

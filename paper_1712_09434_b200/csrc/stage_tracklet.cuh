@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
         const uint32_t ft = __shfl_sync(FULL, t, L), fgid0 = __shfl_sync(FULL, gid0, L);
         const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
         const unsigned long long key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
-        const uint32_t* fmap = c.trk_hits + (size_t)ft * (size_t)n_rows;
+        const uint32_t* fmap = c.trk_hits + (size_t)ft * map_stride(n_rows);
         for (int r = ffirst + lane; r <= flast; r += 32) {
           const uint32_t idx = fmap[r];
           if (idx != kNoHit) atomicMax(&c.owner[idx], key);
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
           r0 = (int)(tr0 - task * (uint32_t)n_rows);
           tr_base = task * (uint32_t)n_rows;
           gid0 = q2.z;
-          map = c.trk_hits + (size_t)t * (size_t)n_rows;
+          map = c.trk_hits + (size_t)t * map_stride(n_rows);
           const float y0s = __uint_as_float(q1.x), z0s = __uint_as_float(q1.y);
           const float y1s = __uint_as_float(q1.z), z1s = __uint_as_float(q1.w);
           const float dx = sX[r0 + 1] - sX[r0], dy = y1s - y0s, dz = z1s - z0s;

@@ -85,7 +85,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.clean_up = take(n4 * sizeof(int32_t));
   c.owner = take(n4 * sizeof(unsigned long long));
   c.trk_seed = take((size_t)T * kSeedU4 * sizeof(uint4));
-  c.trk_hits = take((size_t)T * n_rows * sizeof(uint32_t));
+  c.trk_hits = take((size_t)T * map_stride((int)n_rows) * sizeof(uint32_t));
   c.trk_rec = take((size_t)T * kRecFloat4 * sizeof(float4));
   c.seed_tiles = (uint32_t)(((size_t)n + kSeedTile - 1) / kSeedTile);
   if (c.seed_tiles == 0) c.seed_tiles = 1;
