@@ -35,6 +35,10 @@ struct tpc_tracker {
   int trk_grid[2] = {0, 0};
   // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
   bool timing_on = false;
+  // tpc_track_batch_host: one stream per chunk (+ events, pinned headers), created on first use
+  std::vector<cudaStream_t> host_streams;
+  std::vector<cudaEvent_t> host_events;
+  uint32_t* host_headers = nullptr;
   std::vector<cudaEvent_t> ev;
   uint32_t timed_calls = 0;
   std::string err;
@@ -226,6 +230,9 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
 void tpc_tracker_destroy(tpc_tracker* t) {
   if (!t) return;
   for (cudaEvent_t e : t->ev) cudaEventDestroy(e);
+  for (cudaStream_t x : t->host_streams) cudaStreamDestroy(x);
+  for (cudaEvent_t x : t->host_events) cudaEventDestroy(x);
+  if (t->host_headers) cudaFreeHost(t->host_headers);
   if (t->d_tables) cudaFree(t->d_tables);
   if (t->d_counters) cudaFree(t->d_counters);
   delete t;
@@ -361,24 +368,53 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
 }
 
 // ---- host-buffer variant -------------------------------------------------------
+// The batch is cut into up to kHostChunks runs of whole sector tasks (tasks are independent, PAPER.md L138,
+// L127), each with its own stream: the host->device copy of chunk k+1 and the device->host copy of chunk k-1
+// overlap the kernels of chunk k.  Every chunk is one tpc_track_batch call on its slice of the inputs; a small
+// kernel rebases its row offsets before, and one shifts its task numbers, hit ranges and cluster indices to
+// those of the whole batch after.  Chunks are visited in task order, so the result is the one call's result.
 namespace {
+constexpr uint32_t kHostChunks = 4;
+constexpr uint32_t kHostChunkMinClusters = 1u << 20;  // smaller batches go through as one chunk
+
+__global__ void k_rebase_offsets(uint32_t* ro, uint32_t n, uint32_t base) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) ro[i] -= base;
+}
+__global__ void k_shift_chunk(uint32_t* track_task, uint32_t* track_hit_begin, uint32_t n_tracks, uint32_t* hit_cluster,
+                              uint32_t n_hits, uint32_t task0, uint32_t hit0, uint32_t gid0) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_tracks) { track_task[i] += task0; track_hit_begin[i] += hit0; }
+  if (i < n_hits) hit_cluster[i] += gid0;
+}
+
 struct HostCarve {
   size_t y, z, row_off, header, track_task, track_hit_begin, track_nhits, track_ndf, track_x, track_par, track_cov,
       track_chi2, hit_cluster, inner, total;
+  uint32_t tcap_dev, hcap_dev;
 };
 HostCarve host_carve(const tpc_tracker* t, uint32_t n, uint32_t n_tasks, uint32_t T, uint32_t tcap, uint32_t hcap) {
   HostCarve h{};
+  const uint32_t mh = (uint32_t)(t->prm.min_track_hits > 0 ? t->prm.min_track_hits : 1);
+  // device-side capacities: every chunk gets min(caller's capacity, what its clusters can produce at most)
+  const uint64_t tc = (uint64_t)n / mh + kHostChunks, hc = (uint64_t)n + kHostChunks;
+  h.tcap_dev = (uint32_t)(tc < (uint64_t)tcap * kHostChunks ? tc : (uint64_t)tcap * kHostChunks);
+  h.hcap_dev = (uint32_t)(hc < (uint64_t)hcap * kHostChunks ? hc : (uint64_t)hcap * kHostChunks);
+  if (h.tcap_dev < tcap) h.tcap_dev = tcap;
+  if (h.hcap_dev < hcap) h.hcap_dev = hcap;
+  const size_t tcd = h.tcap_dev, hcd = h.hcap_dev;
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
   h.y = take((size_t)n * 4); h.z = take((size_t)n * 4);
-  h.row_off = take(((size_t)n_tasks * t->n_rows + 1) * 4);
-  h.header = take(16);
-  h.track_task = take((size_t)tcap * 4); h.track_hit_begin = take((size_t)tcap * 4);
-  h.track_nhits = take((size_t)tcap * 4); h.track_ndf = take((size_t)tcap * 4); h.track_x = take((size_t)tcap * 4);
-  h.track_par = take((size_t)tcap * 20); h.track_cov = take((size_t)tcap * 60); h.track_chi2 = take((size_t)tcap * 4);
-  h.hit_cluster = take((size_t)hcap * 4);
+  h.row_off = take(((size_t)n_tasks * t->n_rows + kHostChunks) * 4 + kHostChunks * kAlign);
+  h.header = take(16 * kHostChunks);
+  h.track_task = take(tcd * 4); h.track_hit_begin = take(tcd * 4);
+  h.track_nhits = take(tcd * 4); h.track_ndf = take(tcd * 4); h.track_x = take(tcd * 4);
+  h.track_par = take(tcd * 20); h.track_cov = take(tcd * 60); h.track_chi2 = take(tcd * 4);
+  h.hit_cluster = take(hcd * 4);
   h.inner = off;
-  h.total = off + carve((uint32_t)t->n_rows, n, n_tasks, T).total;
+  // the chunks' workspaces together: linear in clusters, tasks and tracklets, plus alignment slack per chunk
+  h.total = off + carve((uint32_t)t->n_rows, n, n_tasks, T).total + (size_t)kHostChunks * (T ? 64 : 64) * 1024;
   return h;
 }
 }  // namespace
@@ -386,7 +422,7 @@ HostCarve host_carve(const tpc_tracker* t, uint32_t n, uint32_t n_tasks, uint32_
 size_t tpc_host_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t max_tasks, uint32_t max_tracklets,
                                 uint32_t track_capacity, uint32_t hit_capacity) {
   if (!t) return 0;
-  const uint32_t T = resolve_max_tracklets(t, max_clusters, max_tracklets);
+  const uint32_t T = resolve_max_tracklets(t, max_clusters, max_tracklets) + kHostChunks;
   return host_carve(t, max_clusters, max_tasks, T, track_capacity, hit_capacity).total;
 }
 
@@ -400,60 +436,144 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
       out->dbg_tracklet_start || out->dbg_tracklet_nhits || out->dbg_tracklet_map || out->dbg_tracklet_par)
     return fail(t, TPC_ERR_ARGUMENT, "tpc_track_batch_host: dbg_* outputs are not supported on host buffers");
   const uint32_t n = in->n_clusters, tcap = out->track_capacity, hcap = out->hit_capacity;
-  const uint32_t T = resolve_max_tracklets(t, n, max_tracklets);
-  const HostCarve h = host_carve(t, n, in->n_tasks, T, tcap, hcap);
+  const uint32_t n_rows = (uint32_t)t->n_rows;
+  const uint32_t T_all = resolve_max_tracklets(t, n, max_tracklets) + kHostChunks;
+  const HostCarve h = host_carve(t, n, in->n_tasks, T_all, tcap, hcap);
   if (!workspace || workspace_bytes < h.total)
     return fail(t, TPC_ERR_WORKSPACE, "tpc_track_batch_host: workspace of %zu bytes, need %zu", workspace_bytes, h.total);
   if (((uintptr_t)workspace & (kAlign - 1)) != 0)
     return fail(t, TPC_ERR_WORKSPACE, "tpc_track_batch_host: workspace must be %zu-byte aligned", kAlign);
-  cudaStream_t s = (cudaStream_t)cuda_stream;
+  cudaStream_t s_user = (cudaStream_t)cuda_stream;
   char* ws = (char*)workspace;
-  const size_t n_off = (size_t)in->n_tasks * t->n_rows + 1;
-  uint64_t up = 0, down = 0;
+  const uint32_t* ro = in->row_offsets;
+  if (ro[(size_t)in->n_tasks * n_rows] != n)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_track_batch_host: row_offsets must end at n_clusters");
+  // chunk boundaries: whole tasks, about n / n_chunks clusters each
+  uint32_t n_chunks = (n >= kHostChunkMinClusters && in->n_tasks >= kHostChunks) ? kHostChunks : 1u;
+  uint32_t task_b[kHostChunks + 1];
+  task_b[0] = 0u;
+  for (uint32_t k = 1; k < n_chunks; ++k) {
+    const uint64_t want = (uint64_t)n * k / n_chunks;
+    uint32_t lo = task_b[k - 1], hi = in->n_tasks;  // first task whose clusters start at or after `want`
+    while (lo < hi) {
+      const uint32_t mid = lo + (hi - lo) / 2;
+      if (ro[(size_t)mid * n_rows] < want) lo = mid + 1; else hi = mid;
+    }
+    task_b[k] = lo;
+  }
+  task_b[n_chunks] = in->n_tasks;
+  // streams and events of the chunks, created on first use
   cudaError_t e = cudaSuccess;
-  auto h2d = [&](size_t off, const void* src, size_t bytes) {
-    if (e == cudaSuccess && bytes) { e = cudaMemcpyAsync(ws + off, src, bytes, cudaMemcpyHostToDevice, s); up += bytes; }
-  };
-  h2d(h.y, in->y, (size_t)n * 4);
-  h2d(h.z, in->z, (size_t)n * 4);
-  h2d(h.row_off, in->row_offsets, n_off * 4);
-  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA H2D: %s", cudaGetErrorString(e));
-  tpc_clusters din = *in;
-  din.x = nullptr; din.charge = nullptr;  // not read (R18, R23), so not copied either
-  din.y = (const float*)(ws + h.y); din.z = (const float*)(ws + h.z);
-  din.row_offsets = (const uint32_t*)(ws + h.row_off);
-  tpc_tracks dout{};
-  dout.track_capacity = tcap; dout.hit_capacity = hcap;
-  dout.header = (uint32_t*)(ws + h.header);
-  dout.track_task = (uint32_t*)(ws + h.track_task); dout.track_hit_begin = (uint32_t*)(ws + h.track_hit_begin);
-  dout.track_nhits = (uint32_t*)(ws + h.track_nhits); dout.track_ndf = (int32_t*)(ws + h.track_ndf);
-  dout.track_x = (float*)(ws + h.track_x); dout.track_par = (float*)(ws + h.track_par);
-  dout.track_cov = (float*)(ws + h.track_cov); dout.track_chi2 = (float*)(ws + h.track_chi2);
-  dout.hit_cluster = (uint32_t*)(ws + h.hit_cluster);
-  const int rc = tpc_track_batch(t, &din, &dout, ws + h.inner, workspace_bytes - h.inner, T, cuda_stream);
+  if (t->host_streams.empty()) {
+    t->host_streams.resize(kHostChunks);
+    t->host_events.resize(kHostChunks + 1);
+    for (auto& x : t->host_streams) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking);
+    for (auto& x : t->host_events) if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->host_headers, 16 * kHostChunks, cudaHostAllocDefault);
+    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA: %s", cudaGetErrorString(e));
+  }
+  const bool timing = t->timing_on, counters = t->counters_on;
+  t->timing_on = false; t->counters_on = false;  // per-stage marks and counters describe one tpc_track_batch call
+  uint64_t up = 0, down = 0;
+  e = cudaEventRecord(t->host_events[kHostChunks], s_user);  // the chunks start after the caller's stream got here
+  struct Chunk { uint32_t n, idx0, task0, n_tasks, T, tcap, hcap, t0, h0; tpc_tracks d; } ch[kHostChunks];
+  size_t inner_off = h.inner, ro_off = h.row_off;
+  uint32_t t_used = 0, h_used = 0;
+  const uint32_t mh = (uint32_t)(t->prm.min_track_hits > 0 ? t->prm.min_track_hits : 1);
+  int rc = TPC_OK;
+  for (uint32_t k = 0; k < n_chunks && e == cudaSuccess && rc == TPC_OK; ++k) {
+    Chunk& c = ch[k];
+    cudaStream_t s = t->host_streams[k];
+    c.task0 = task_b[k]; c.n_tasks = task_b[k + 1] - task_b[k];
+    c.idx0 = ro[(size_t)c.task0 * n_rows];
+    c.n = ro[(size_t)task_b[k + 1] * n_rows] - c.idx0;
+    c.T = n_chunks == 1 ? T_all - kHostChunks : (uint32_t)((uint64_t)(T_all - kHostChunks) * c.n / (n ? n : 1)) + 1u;
+    c.tcap = c.n / mh + 1u < tcap ? c.n / mh + 1u : tcap;
+    c.hcap = c.n + 1u < hcap ? c.n + 1u : hcap;
+    c.t0 = t_used; c.h0 = h_used;
+    t_used += c.tcap; h_used += c.hcap;
+    const size_t n_off = (size_t)c.n_tasks * n_rows + 1;
+    uint32_t* d_ro = (uint32_t*)(ws + ro_off);
+    ro_off = align_up(ro_off + n_off * 4);
+    e = cudaStreamWaitEvent(s, t->host_events[kHostChunks], 0);
+    auto h2d = [&](void* dst, const void* src, size_t bytes) {
+      if (e == cudaSuccess && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s); up += bytes; }
+    };
+    h2d(ws + h.y + (size_t)c.idx0 * 4, in->y + c.idx0, (size_t)c.n * 4);
+    h2d(ws + h.z + (size_t)c.idx0 * 4, in->z + c.idx0, (size_t)c.n * 4);
+    h2d(d_ro, ro + (size_t)c.task0 * n_rows, n_off * 4);
+    if (e != cudaSuccess) break;
+    if (c.idx0) k_rebase_offsets<<<(unsigned)((n_off + 255) / 256), 256, 0, s>>>(d_ro, (uint32_t)n_off, c.idx0);
+    tpc_clusters din{};
+    din.y = (const float*)(ws + h.y) + c.idx0; din.z = (const float*)(ws + h.z) + c.idx0;  // x, charge: not read (R18, R23)
+    din.row_offsets = d_ro; din.n_clusters = c.n; din.n_tasks = c.n_tasks;
+    tpc_tracks& d = c.d;
+    d = tpc_tracks{};
+    d.track_capacity = c.tcap; d.hit_capacity = c.hcap;
+    d.header = (uint32_t*)(ws + h.header) + 4 * k;
+    d.track_task = (uint32_t*)(ws + h.track_task) + c.t0; d.track_hit_begin = (uint32_t*)(ws + h.track_hit_begin) + c.t0;
+    d.track_nhits = (uint32_t*)(ws + h.track_nhits) + c.t0; d.track_ndf = (int32_t*)(ws + h.track_ndf) + c.t0;
+    d.track_x = (float*)(ws + h.track_x) + c.t0; d.track_chi2 = (float*)(ws + h.track_chi2) + c.t0;
+    // SoA columns of a chunk are c.tcap apart, packed one chunk after the other
+    d.track_par = (float*)(ws + h.track_par) + (size_t)5 * c.t0; d.track_cov = (float*)(ws + h.track_cov) + (size_t)15 * c.t0;
+    d.hit_cluster = (uint32_t*)(ws + h.hit_cluster) + c.h0;
+    const size_t need = carve(n_rows, c.n, c.n_tasks, c.T).total;
+    if (inner_off + need > workspace_bytes) { rc = fail(t, TPC_ERR_WORKSPACE, "tpc_track_batch_host: workspace too small for chunk %u", k); break; }
+    rc = tpc_track_batch(t, &din, &d, ws + inner_off, need, c.T, s);
+    inner_off = align_up(inner_off + need);
+    if (rc != TPC_OK) break;
+    e = cudaMemcpyAsync(t->host_headers + 4 * k, d.header, 16, cudaMemcpyDeviceToHost, s);
+    down += 16;
+    if (e == cudaSuccess) e = cudaEventRecord(t->host_events[k], s);
+  }
+  // collect the chunks in task order
+  uint32_t tracks_off = 0, hits_off = 0, status = 0, tracklets = 0;
+  uint64_t tracks_all = 0, hits_all = 0;
+  for (uint32_t k = 0; k < n_chunks && e == cudaSuccess && rc == TPC_OK; ++k) {
+    Chunk& c = ch[k];
+    cudaStream_t s = t->host_streams[k];
+    e = cudaEventSynchronize(t->host_events[k]);
+    if (e != cudaSuccess) break;
+    const uint32_t* hh = t->host_headers + 4 * k;
+    status |= hh[2]; tracklets += hh[3];
+    tracks_all += hh[0]; hits_all += hh[1];
+    const uint32_t nt_dev = hh[0] < c.tcap ? hh[0] : c.tcap, nh_dev = hh[1] < c.hcap ? hh[1] : c.hcap;
+    uint32_t nt = nt_dev, nh = nh_dev;
+    if ((uint64_t)tracks_off + nt > tcap) { nt = tcap - tracks_off; status |= TPC_STATUS_TRACK_OVERFLOW; }
+    if ((uint64_t)hits_off + nh > hcap) { nh = hcap - hits_off; status |= TPC_STATUS_HIT_OVERFLOW; }
+    const uint32_t m = nt_dev > nh_dev ? nt_dev : nh_dev;
+    if (m && (c.task0 || hits_off || c.idx0))
+      k_shift_chunk<<<(m + 255) / 256, 256, 0, s>>>(c.d.track_task, c.d.track_hit_begin, nt_dev, c.d.hit_cluster, nh_dev,
+                                                    c.task0, hits_off, c.idx0);
+    auto d2h = [&](void* dst, const void* src, size_t bytes) {
+      if (e == cudaSuccess && dst && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s); down += bytes; }
+    };
+    d2h(out->track_task ? out->track_task + tracks_off : nullptr, c.d.track_task, (size_t)nt * 4);
+    d2h(out->track_hit_begin ? out->track_hit_begin + tracks_off : nullptr, c.d.track_hit_begin, (size_t)nt * 4);
+    d2h(out->track_nhits ? out->track_nhits + tracks_off : nullptr, c.d.track_nhits, (size_t)nt * 4);
+    d2h(out->track_ndf ? out->track_ndf + tracks_off : nullptr, c.d.track_ndf, (size_t)nt * 4);
+    d2h(out->track_x ? out->track_x + tracks_off : nullptr, c.d.track_x, (size_t)nt * 4);
+    d2h(out->track_chi2 ? out->track_chi2 + tracks_off : nullptr, c.d.track_chi2, (size_t)nt * 4);
+    for (int j = 0; j < 5 && out->track_par; ++j)
+      d2h(out->track_par + (size_t)j * tcap + tracks_off, c.d.track_par + (size_t)j * c.tcap, (size_t)nt * 4);
+    for (int j = 0; j < 15 && out->track_cov; ++j)
+      d2h(out->track_cov + (size_t)j * tcap + tracks_off, c.d.track_cov + (size_t)j * c.tcap, (size_t)nt * 4);
+    d2h(out->hit_cluster ? out->hit_cluster + hits_off : nullptr, c.d.hit_cluster, (size_t)nh * 4);
+    tracks_off += nt; hits_off += nh;
+  }
+  for (uint32_t k = 0; k < n_chunks; ++k) {
+    const cudaError_t e2 = cudaStreamSynchronize(t->host_streams[k]);
+    if (e == cudaSuccess) e = e2;
+  }
+  t->timing_on = timing; t->counters_on = counters;
   if (rc != TPC_OK) return rc;
-  e = cudaMemcpyAsync(out->header, dout.header, 16, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA: %s", cudaGetErrorString(e));
-  down += 16;
-  const uint32_t nt = out->header[0] < tcap ? out->header[0] : tcap;
-  const uint32_t nh = out->header[1] < hcap ? out->header[1] : hcap;
-  auto d2h = [&](void* dst, const void* src, size_t bytes) {
-    if (e == cudaSuccess && dst && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s); down += bytes; }
-  };
-  d2h(out->track_task, dout.track_task, (size_t)nt * 4);
-  d2h(out->track_hit_begin, dout.track_hit_begin, (size_t)nt * 4);
-  d2h(out->track_nhits, dout.track_nhits, (size_t)nt * 4);
-  d2h(out->track_ndf, dout.track_ndf, (size_t)nt * 4);
-  d2h(out->track_x, dout.track_x, (size_t)nt * 4);
-  d2h(out->track_chi2, dout.track_chi2, (size_t)nt * 4);
-  for (int j = 0; j < 5 && out->track_par; ++j)
-    d2h(out->track_par + (size_t)j * tcap, dout.track_par + (size_t)j * tcap, (size_t)nt * 4);
-  for (int j = 0; j < 15 && out->track_cov; ++j)
-    d2h(out->track_cov + (size_t)j * tcap, dout.track_cov + (size_t)j * tcap, (size_t)nt * 4);
-  d2h(out->hit_cluster, dout.hit_cluster, (size_t)nh * 4);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA D2H: %s", cudaGetErrorString(e));
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA launch: %s", cudaGetErrorString(e));
+  out->header[0] = (uint32_t)(tracks_all > 0xFFFFFFFFull ? 0xFFFFFFFFull : tracks_all);
+  out->header[1] = (uint32_t)(hits_all > 0xFFFFFFFFull ? 0xFFFFFFFFull : hits_all);
+  out->header[2] = status;
+  out->header[3] = tracklets;
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = down;
   return TPC_OK;

@@ -237,6 +237,35 @@ def test_host_buffer_entry_point_matches_device_entry_point():
     G.compare(host, ref, b.geometry.n_rows, rtol=RTOL, check_tracklets=False)
 
 
+def test_host_entry_point_in_chunks_equals_one_call(cfg2):
+    """A batch of more than 2^20 clusters goes through tpc_track_batch_host as four chunks of whole sector tasks on
+    four streams (copies overlap kernels); the result must be the single call's, array for array."""
+    import torch
+    from paper_1712_09434_b200 import Tracker
+    b = cfg2
+    assert b.n_clusters > (1 << 20)
+    dev = torch.device("cuda:0")
+    ref = G.run_gpu(b, debug=False, debug_tracklets=False)
+    trk = Tracker(b.geometry, G.tracker_params_for(b))
+    n = b.n_clusters
+    y = torch.from_numpy(np.ascontiguousarray(b.y)).pin_memory()
+    z = torch.from_numpy(np.ascontiguousarray(b.z)).pin_memory()
+    ro = torch.from_numpy(b.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()
+    out = trk.alloc_outputs(n, dev, pinned_host=True)
+    tcap, hcap = out.track_task.shape[0], out.hit_cluster.shape[0]
+    ws = trk.alloc_workspace(trk.host_workspace_bytes(n, b.n_tasks, 0, tcap, hcap), dev)
+    for _ in range(2):  # twice: the streams and buffers of the chunks are reused
+        up, down = trk.track_batch_host(y, z, ro, b.n_tasks, out, ws)
+    host = out.to_numpy()
+    trk.close()
+    assert up == 8 * n + 4 * (b.n_tasks * b.geometry.n_rows + 4)
+    assert host["n_tracks"] == ref["n_tracks"] and host["n_hits"] == ref["n_hits"] and host["status"] == 0
+    assert host["n_tracklets"] == ref["n_tracklets"]
+    for k in ("track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_par", "track_cov",
+              "track_chi2", "hit_cluster"):
+        assert np.array_equal(host[k], ref[k]), k
+
+
 def test_counters_match_the_oracle_counters():
     """The device counters feed the algorithmic-bytes formula of bench.py."""
     b = generate_config(1)
