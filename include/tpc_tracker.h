@@ -159,7 +159,13 @@ int tpc_track_batch(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_trac
  * the device, runs a1..a8, copies the header and the used part of every
  * non-NULL output back, and synchronises.  workspace is DEVICE memory of at
  * least tpc_host_workspace_bytes(...).  dbg_* pointers must be NULL.
- * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied. */
+ * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied.
+ * A batch of 2^20 clusters or more is cut into four runs of whole sector tasks
+ * (tasks are independent), each on a stream of its own, so
+ * that the copies of one run overlap the kernels of another; the result is
+ * the single call's (same tracks, same order).  The streams belong to the
+ * tracker; work queued on cuda_stream before the call is waited for.  For
+ * fastest copies the host buffers should be page-locked. */
 size_t tpc_host_workspace_bytes(const tpc_tracker* tracker, uint32_t max_clusters, uint32_t max_tasks,
                                 uint32_t max_tracklets, uint32_t track_capacity, uint32_t hit_capacity);
 int tpc_track_batch_host(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_tracks* tracks,
