@@ -328,18 +328,14 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
     if (phase <= PH_FINISH) {
       if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
       if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
-      if (phase <= PH_UP) rt = row_cur + 1;
-      else if (phase == PH_TURN) rt = last_row;
-      else if (phase == PH_DOWN) rt = r_down;
-      else rt = first_row;
+      const bool p_chain = phase == PH_CHAIN, p_turn = phase == PH_TURN, p_down = phase == PH_DOWN;
+      rt = phase <= PH_UP ? row_cur + 1 : (p_turn ? last_row : (p_down ? r_down : first_row));
       // Every load of this step whose address does not depend on the transported state is issued here,
       // before the transport: the hit when it is known already (chain link, lastRow hit at the turn, row
       // map entry fetched a step ago), the next chain link, the map entry of the next down row, and the
       // row's grid header when a search may follow.
-      int32_t known = -1;
-      if (phase == PH_CHAIN) known = next_chain;
-      else if (phase == PH_TURN) known = last_hit;
-      else if (phase == PH_DOWN && map_next != kNoHit) known = (int32_t)map_next;
+      const int32_t known = p_chain ? next_chain
+                                    : (p_turn ? last_hit : ((p_down & (map_next != kNoHit)) ? (int32_t)map_next : -1));
       if (known >= 0) hp = c.yz[known];
       if (phase == PH_CHAIN) next_chain = c.clean_up[known];            // K2: the link after this one
       if (phase == PH_TURN || phase == PH_DOWN) {                       // map entry of the row after this one
@@ -379,28 +375,20 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
     __syncwarp();
     if (hit >= 0) update_hit(S, hp.x, hp.y, sy2, sz2);
     __syncwarp();
-    if (book) {
-      if (phase == PH_CHAIN) {
-        map[rt] = (uint32_t)hit;
-        last_row = rt; last_hit = hit; ++n_hits;
-        if (COUNT) ++n_chain;
-        if (next_chain < 0) { phase = PH_UP; gap = 0; }
-      } else if (phase == PH_UP) {
-        map[rt] = (uint32_t)hit;  // -1 = kNoHit
-        if (hit >= 0) { last_row = rt; last_hit = hit; ++n_hits; gap = 0; }
-        else if (++gap > max_gap) phase = PH_TURN;
-      } else {  // PH_DOWN
-        if (do_search) {
-          map[rt] = (uint32_t)hit;
-          if (hit >= 0) {
-            ++n_hits;
-            if (rt < first_row) { first_row = rt; gap = 0; }
-          } else if (rt < first_row) {
-            if (++gap > max_gap) phase = PH_FINISH;
-          }
-        }
-        --r_down;
-      }
+    if (book) {  // chain fit, up pass or down pass, transport done: record the row, count hits and gaps (no branches:
+                 // the lanes of a warp are in different passes)
+      const bool is_up = phase == PH_UP, is_dn = phase == PH_DOWN, got = hit >= 0;
+      const bool decided = !is_dn | do_search;                  // this step decided the row's map entry
+      const bool gap_row = is_up | (is_dn & do_search & (rt < first_row));  // rows whose hits / misses drive the gap
+      if (decided) map[rt] = (uint32_t)hit;                     // -1 = kNoHit
+      n_hits += (decided & got) ? 1 : 0;
+      if (COUNT && phase == PH_CHAIN) ++n_chain;
+      if (!is_dn & got) { last_row = rt; last_hit = hit; }
+      if (gap_row & got & is_dn) first_row = rt;
+      gap = gap_row ? (got ? 0 : gap + 1) : gap;
+      if (gap_row & !got & (gap > max_gap)) phase = is_up ? PH_TURN : PH_FINISH;   // K3 / K5 stop
+      if (phase == PH_CHAIN && next_chain < 0) { phase = PH_UP; gap = 0; }          // K2 -> K3
+      r_down -= is_dn ? 1 : 0;
     }
   }
   if (COUNT) {
