@@ -349,23 +349,23 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
         if (ok) row_cur = rt;
         if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
       }
-      if (phase == PH_FINISH) {                                         // K6
-        phase = PH_ENDED;
-      } else if (phase == PH_TURN) {                                    // K4
+      // what the step does next, by phase, without branches (the lanes of a warp are in different passes)
+      const bool p_fin = phase == PH_FINISH;
+      if (p_turn) {                                                       // K4: C <- C * turn_cov_scale (once per tracklet)
         const float f = c.prm.turn_cov_scale;
         S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
         S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
-        S.chi2 = 0.0f; S.ndf = -5; gap = 0;
-        if (row_cur == last_row) hit = known;                           // the lastRow hit opens the down pass
-        r_down = last_row - 1;
-        phase = PH_DOWN;
-      } else if (!ok) {  // transport failed: K2/K3 -> turn-around, K5 -> finish
-        phase = (phase == PH_DOWN) ? PH_FINISH : PH_TURN;
-      } else {
-        book = true;
-        if (phase == PH_UP || known < 0) do_search = true;              // K3, K5 without a map entry
-        else hit = known;                                               // K2, K5 with a map entry
       }
+      S.chi2 = p_turn ? 0.0f : S.chi2;
+      S.ndf = p_turn ? -5 : S.ndf;
+      gap = p_turn ? 0 : gap;
+      r_down = p_turn ? last_row - 1 : r_down;
+      book = ok & !p_fin & !p_turn;                                       // K2, K3, K5 with the transport done
+      do_search = book & ((phase == PH_UP) | (known < 0));                // K3, K5 without a map entry
+      // the hit is known: K2, K5 with a map entry, K4 (the lastRow hit opens the down pass)
+      hit = ((book & !do_search) | (p_turn & (row_cur == last_row))) ? known : -1;
+      // K6 finish -> ended; K4 -> down pass; failed transport: K2/K3 -> turn-around, K5 -> finish
+      phase = p_fin ? PH_ENDED : (p_turn ? PH_DOWN : (ok ? phase : (p_down ? PH_FINISH : PH_TURN)));
     }
     __syncwarp();
     if (do_search) {
