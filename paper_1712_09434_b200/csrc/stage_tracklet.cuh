@@ -129,6 +129,12 @@ __device__ __forceinline__ void update_hit(TrackState& S, float ym, float zm, fl
 }
 
 
+__device__ __forceinline__ float sqrt_approx(float v) {
+  float r;
+  asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+
 // SPEC 5.3 SEARCH (H1..H6), exact and serial: one flat loop over the window, ties decided by gid.  The fast
 // search below hands over to this one when it meets two valid clusters with the same distance.
 __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz, const uint32_t* __restrict__ gid,
@@ -158,7 +164,7 @@ __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz,
 // are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at a time, all
 // loads of a group in flight before the first is tested (the walk is latency bound) and the tests written
 // without branches (lanes of a warp are at different candidates of different windows).
-constexpr int kSearchUnroll = 4;
+constexpr int kSearchUnroll = 2;
 
 template <bool COUNT>
 __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g,
@@ -167,7 +173,9 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
   const float ey = S.c00 + c.sy2, ez = S.c11 + c.sz2;                 // H1
   const float hy2 = fminf(c.prm.accept_k2 * ey, c.smax2);              // H2
   const float hz2 = fminf(c.prm.accept_k2 * ez, c.smax2);
-  const float wy = sqrtf(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrtf(fmaxf(hz2, 0.0f)) + kGridMargin;
+  // half widths of the grid window: acceleration only (SPEC 2), so the approximate square root (about 1 ulp) will
+  // do - kGridMargin is four orders of magnitude larger than its error
+  const float wy = sqrt_approx(fmaxf(hy2, 0.0f)) + kGridMargin, wz = sqrt_approx(fmaxf(hz2, 0.0f)) + kGridMargin;
   const int ny = info_ny(g), nz = info_nz(g);
   const int iy0 = bin_coord(y - wy, g.y0, g.inv, ny), iy1 = bin_coord(y + wy, g.y0, g.inv, ny) + 1;
   const int iz0 = bin_coord(z - wz, g.z0, g.inv, nz), iz1 = bin_coord(z + wz, g.z0, g.inv, nz);
