@@ -118,7 +118,7 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
 // pass the window test are appended to the thread's list as ((p.x - y)*sgn*fac, (p.y - z)*sgn*fac, idx).
 // Returns the number that passed (entries beyond kNfList are not stored).
 __device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float y, float z, float zc,
-                                               float HY, float HZ, float sgn, float fac, float* l_y, float* l_z,
+                                               float HY, float HZ, float sgn, float fac, float2* l_p,
                                                uint32_t* l_i) {
   const float M = kGridMargin;
   const int iy0 = bin_coord((y - HY) - M, v.y0, v.inv, v.ny), iy1 = bin_coord((y + HY) + M, v.y0, v.inv, v.ny) + 1;
@@ -141,8 +141,7 @@ __device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float
       if (n < (uint32_t)kNfList) {
         const uint32_t slot = n * kNfThreads;
         // up: (y_u - y)*b, (z_u - z)*b.  down: (y - y_d)*a_, (z - z_d)*a_ (exact negation of the difference)
-        l_y[slot] = (sgn * ry) * fac;
-        l_z[slot] = (sgn * (p.y - z)) * fac;
+        l_p[slot] = make_float2((sgn * ry) * fac, (sgn * (p.y - z)) * fac);
         l_i[slot] = idx;
       }
       n += pass ? 1u : 0u;
@@ -159,12 +158,10 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
   const float ratio_up = c.ratio_up[row], ratio_dn = c.ratio_dn[row];
   const float wy = c.wy, wz = c.wz;
   const int tid = threadIdx.x;
-  float* d_y = reinterpret_cast<float*>(list_smem) + tid;  // [kNfList][kNfThreads] each, this thread's column
-  float* d_z = d_y + kNfList * kNfThreads;
-  uint32_t* d_i = reinterpret_cast<uint32_t*>(d_z + kNfList * kNfThreads);
-  float* u_y = reinterpret_cast<float*>(d_i + kNfList * kNfThreads);
-  float* u_z = u_y + kNfList * kNfThreads;
-  uint32_t* u_i = reinterpret_cast<uint32_t*>(u_z + kNfList * kNfThreads);
+  float2* d_p = reinterpret_cast<float2*>(list_smem) + tid;  // [kNfList][kNfThreads] each, this thread's column
+  float2* u_p = d_p + kNfList * kNfThreads;
+  uint32_t* d_i = reinterpret_cast<uint32_t*>(reinterpret_cast<float2*>(list_smem) + 2 * kNfList * kNfThreads) + tid;
+  uint32_t* u_i = d_i + kNfList * kNfThreads;
   unsigned long long n_pairs = 0ull;
   for (uint32_t i0 = lo + (uint32_t)(tid & ~31); i0 < hi; i0 += kNfThreads) {  // warp-uniform trip count
     const uint32_t i = i0 + (uint32_t)(tid & 31);
@@ -172,29 +169,29 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     float y = 0.0f, z = 0.0f;
     if (act) { const float2 h = c.yz[i]; y = h.x; z = h.y; }
     const float zu = z * ratio_up, zd = z * ratio_dn;  // N1
-    const uint32_t nd = nf_collect(vd, act, y, z, zd, HY, HZ, -1.0f, a_, d_y, d_z, d_i);  // N3
+    const uint32_t nd = nf_collect(vd, act, y, z, zd, HY, HZ, -1.0f, a_, d_p, d_i);  // N3
     __syncwarp();
-    const uint32_t nu = nd ? nf_collect(vu, act, y, z, zu, HY, HZ, 1.0f, b, u_y, u_z, u_i) : 0u;  // N2
+    const uint32_t nu = nd ? nf_collect(vu, act, y, z, zu, HY, HZ, 1.0f, b, u_p, u_i) : 0u;  // N2
     __syncwarp();
     const bool overflow = nd > (uint32_t)kNfList || nu > (uint32_t)kNfList;
     const uint32_t n_pr = overflow ? 0u : nu * nd;
     const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 64, nd <= 8
     if (COUNT) n_pairs += n_pr;
     float best = CHI_MAX;  // N5: only chi < CHI_MAX is eligible
-    uint32_t bu = 0u, bd = 0u;
-    bool have = false, tie = false;
+    uint32_t bk = 0u;
+    bool tie = false;
     for (uint32_t k = 0u; k < n_pr; ++k) {
       const uint32_t u = (k * magic) >> 16, d = k - u * nd;
-      const float dy = u_y[u * kNfThreads] - d_y[d * kNfThreads];  // N4
-      const float dz = u_z[u * kNfThreads] - d_z[d * kNfThreads];
+      const float2 pu = u_p[u * kNfThreads], pd = d_p[d * kNfThreads];
+      const float dy = pu.x - pd.x, dz = pu.y - pd.y;  // N4
       const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
       const bool lt = chi < best;
-      tie |= have & (chi == best);  // equal chi2: the gids decide (N5), left to the serial search
-      have |= lt;
+      tie |= chi == best;  // equal chi2 (or chi2 == CHI_MAX exactly): the gids decide (N5), left to the serial search
       best = lt ? chi : best;
-      bu = lt ? u : bu;
-      bd = lt ? d : bd;
+      bk = lt ? k : bk;
     }
+    const bool have = best < CHI_MAX;
+    const uint32_t bu = (bk * magic) >> 16, bd = bk - bu * nd;
     __syncwarp();
     if (act) {
       int32_t up = -1, dn = -1;
