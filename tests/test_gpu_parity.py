@@ -266,6 +266,35 @@ def test_host_entry_point_in_chunks_equals_one_call(cfg2):
         assert np.array_equal(host[k], ref[k]), k
 
 
+def test_host_entry_point_in_chunks_overflow_is_reported(cfg2):
+    """Capacities far too small, through the chunked host path: totals are still the true ones, status bits are
+    set, only the first slots are written (and they are the single call's first tracks)."""
+    import torch
+    from paper_1712_09434_b200 import Tracker
+    b = cfg2
+    dev = torch.device("cuda:0")
+    ref = G.run_gpu(b, debug=False, debug_tracklets=False)
+    trk = Tracker(b.geometry, G.tracker_params_for(b))
+    n = b.n_clusters
+    y = torch.from_numpy(np.ascontiguousarray(b.y)).pin_memory()
+    z = torch.from_numpy(np.ascontiguousarray(b.z)).pin_memory()
+    ro = torch.from_numpy(b.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()
+    out = trk.alloc_outputs(n, dev, pinned_host=True, track_capacity=8, hit_capacity=100)
+    ws = trk.alloc_workspace(trk.host_workspace_bytes(n, b.n_tasks, 0, 8, 100), dev)
+    trk.track_batch_host(y, z, ro, b.n_tasks, out, ws)
+    h = out.header.numpy()
+    assert int(h[0]) == ref["n_tracks"] and int(h[1]) == ref["n_hits"] and int(h[3]) == ref["n_tracklets"]
+    assert int(h[2]) & 2 and int(h[2]) & 4
+    assert np.array_equal(out.track_task.numpy()[:8], ref["track_task"][:8])
+    assert np.array_equal(out.track_nhits.numpy()[:8], ref["track_nhits"][:8])
+    hb, nh = out.track_hit_begin.numpy()[:8].astype(np.int64), out.track_nhits.numpy()[:8].astype(np.int64)
+    assert np.array_equal(hb, ref["track_hit_begin"][:8])
+    for t in range(8):  # include/tpc_tracker.h: a track is valid iff its hits fit the hit capacity
+        if hb[t] + nh[t] <= 100:
+            assert np.array_equal(out.hit_cluster.numpy()[hb[t]:hb[t] + nh[t]], ref["hit_cluster"][hb[t]:hb[t] + nh[t]])
+    trk.close()
+
+
 def test_counters_match_the_oracle_counters():
     """The device counters feed the algorithmic-bytes formula of bench.py."""
     b = generate_config(1)
