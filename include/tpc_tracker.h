@@ -161,6 +161,7 @@ int tpc_track_batch(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_trac
  * least tpc_host_workspace_bytes(...).  dbg_* pointers must be NULL.
  * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied.
  * A batch of 2^20 clusters or more is cut into four runs of whole sector tasks
+ * (at about 12, 45 and 80 % of the clusters)
  * (tasks are independent), each on a stream of its own, so
  * that the copies of one run overlap the kernels of another; the result is
  * the single call's (same tracks, same order).  The streams belong to the
