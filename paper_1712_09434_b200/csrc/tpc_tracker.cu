@@ -369,8 +369,8 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
 
 // ---- host-buffer variant -------------------------------------------------------
 // The batch is cut into up to kHostChunks runs of whole sector tasks (tasks are independent, PAPER.md L138,
-// L127), each with its own stream: the host->device copy of chunk k+1 and the device->host copy of chunk k-1
-// overlap the kernels of chunk k.  Every chunk is one tpc_track_batch call on its slice of the inputs; a small
+// L127) and three streams - copies in, kernels, copies out - are used: the host->device copy of chunk k+1 and the
+// device->host copy of chunk k-1 overlap the kernels of chunk k.  Every chunk is one tpc_track_batch call on its slice of the inputs; a small
 // kernel rebases its row offsets before, and one shifts its task numbers, hit ranges and cluster indices to
 // those of the whole batch after.  Chunks are visited in task order, so the result is the one call's result.
 namespace {
@@ -469,7 +469,7 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   cudaError_t e = cudaSuccess;
   if (t->host_streams.empty()) {
     t->host_streams.resize(kHostChunks);
-    t->host_events.resize(kHostChunks + 1);
+    t->host_events.resize(2 * kHostChunks + 1);  // [k] chunk k computed, [kHostChunks] start, [kHostChunks + 1 + k] chunk k copied in
     for (auto& x : t->host_streams) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking);
     for (auto& x : t->host_events) if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->host_headers, 16 * kHostChunks, cudaHostAllocDefault);
@@ -484,9 +484,15 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   uint32_t t_used = 0, h_used = 0;
   const uint32_t mh = (uint32_t)(t->prm.min_track_hits > 0 ? t->prm.min_track_hits : 1);
   int rc = TPC_OK;
+  // three streams: copies in, kernels, copies out.  The kernels of the chunks run one after the other - run side by
+  // side, two persistent tracklet constructors slow each other down more than the overlap gains (measured:
+  // 16.5 ms against 14.6 ms for the two halves of config 3).
+  cudaStream_t s_in = t->host_streams[0], s_cmp = t->host_streams[1], s_out = t->host_streams[2];
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s_in, t->host_events[kHostChunks], 0);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s_cmp, t->host_events[kHostChunks], 0);
   for (uint32_t k = 0; k < n_chunks && e == cudaSuccess && rc == TPC_OK; ++k) {
     Chunk& c = ch[k];
-    cudaStream_t s = t->host_streams[k];
+    cudaStream_t s = s_cmp;
     c.task0 = task_b[k]; c.n_tasks = task_b[k + 1] - task_b[k];
     c.idx0 = ro[(size_t)c.task0 * n_rows];
     c.n = ro[(size_t)task_b[k + 1] * n_rows] - c.idx0;
@@ -498,13 +504,14 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
     const size_t n_off = (size_t)c.n_tasks * n_rows + 1;
     uint32_t* d_ro = (uint32_t*)(ws + ro_off);
     ro_off = align_up(ro_off + n_off * 4);
-    e = cudaStreamWaitEvent(s, t->host_events[kHostChunks], 0);
     auto h2d = [&](void* dst, const void* src, size_t bytes) {
-      if (e == cudaSuccess && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s); up += bytes; }
+      if (e == cudaSuccess && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s_in); up += bytes; }
     };
     h2d(ws + h.y + (size_t)c.idx0 * 4, in->y + c.idx0, (size_t)c.n * 4);
     h2d(ws + h.z + (size_t)c.idx0 * 4, in->z + c.idx0, (size_t)c.n * 4);
     h2d(d_ro, ro + (size_t)c.task0 * n_rows, n_off * 4);
+    if (e == cudaSuccess) e = cudaEventRecord(t->host_events[kHostChunks + 1 + k], s_in);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_cmp, t->host_events[kHostChunks + 1 + k], 0);
     if (e != cudaSuccess) break;
     if (c.idx0) k_rebase_offsets<<<(unsigned)((n_off + 255) / 256), 256, 0, s>>>(d_ro, (uint32_t)n_off, c.idx0);
     tpc_clusters din{};
@@ -534,8 +541,9 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   uint64_t tracks_all = 0, hits_all = 0;
   for (uint32_t k = 0; k < n_chunks && e == cudaSuccess && rc == TPC_OK; ++k) {
     Chunk& c = ch[k];
-    cudaStream_t s = t->host_streams[k];
+    cudaStream_t s = s_out;
     e = cudaEventSynchronize(t->host_events[k]);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, t->host_events[k], 0);
     if (e != cudaSuccess) break;
     const uint32_t* hh = t->host_headers + 4 * k;
     status |= hh[2]; tracklets += hh[3];
@@ -564,7 +572,7 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
     d2h(out->hit_cluster ? out->hit_cluster + hits_off : nullptr, c.d.hit_cluster, (size_t)nh * 4);
     tracks_off += nt; hits_off += nh;
   }
-  for (uint32_t k = 0; k < n_chunks; ++k) {
+  for (uint32_t k = 0; k < 3; ++k) {
     const cudaError_t e2 = cudaStreamSynchronize(t->host_streams[k]);
     if (e == cudaSuccess) e = e2;
   }
