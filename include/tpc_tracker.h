@@ -161,12 +161,12 @@ int tpc_track_batch(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_trac
  * least tpc_host_workspace_bytes(...).  dbg_* pointers must be NULL.
  * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied.
  * A batch of 2^20 clusters or more is cut into four runs of whole sector tasks
- * (at about 12, 45 and 80 % of the clusters)
- * (tasks are independent), each on a stream of its own, so
- * that the copies of one run overlap the kernels of another; the result is
- * the single call's (same tracks, same order).  The streams belong to the
- * tracker; work queued on cuda_stream before the call is waited for.  For
- * fastest copies the host buffers should be page-locked. */
+ * (at about 12, 45 and 80 % of the clusters; tasks are independent, PAPER.md
+ * L138/L127) and pipelined over three streams of the tracker's own - copies
+ * in, kernels, copies out - so that the copies of one run overlap the kernels
+ * of another; the result is the single call's (same tracks, same order).
+ * Work queued on cuda_stream before the call is waited for.  For fastest
+ * copies the host buffers should be page-locked. */
 size_t tpc_host_workspace_bytes(const tpc_tracker* tracker, uint32_t max_clusters, uint32_t max_tasks,
                                 uint32_t max_tracklets, uint32_t track_capacity, uint32_t hit_capacity);
 int tpc_track_batch_host(tpc_tracker* tracker, const tpc_clusters* clusters, tpc_tracks* tracks,
