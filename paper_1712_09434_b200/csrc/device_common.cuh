@@ -187,36 +187,4 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
   return r;
 }
 
-// ---------------------------------------------------------------------------
-// Warp-cooperative work distribution.  Lane L brings n work items; the sum(n)
-// items of the warp are numbered lane by lane and handed out 32 at a time, so
-// every lane gets one item per round whoever owns it (the per-lane trip counts
-// of the searches differ by an order of magnitude; this evens them out).
-// f(valid, owner, k) is called by all 32 lanes together: item k of lane `owner`.
-// ---------------------------------------------------------------------------
-template <class F>
-__device__ __forceinline__ void warp_items(uint32_t n, F&& f) {
-  constexpr unsigned FULL = 0xffffffffu;
-  const int lane = threadIdx.x & 31;
-  uint32_t incl = n;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const uint32_t t = __shfl_up_sync(FULL, incl, o);
-    if (lane >= o) incl += t;
-  }
-  const uint32_t total = __shfl_sync(FULL, incl, 31);
-  const uint32_t excl = incl - n;
-  for (uint32_t w0 = 0u; w0 < total; w0 += 32u) {
-    const uint32_t w = w0 + (uint32_t)lane;
-    int o = 0;  // number of lanes whose items all come before w = the owner of w
-#pragma unroll
-    for (int s = 16; s > 0; s >>= 1) {
-      const uint32_t pr = __shfl_sync(FULL, incl, o + s - 1);
-      if (pr <= w) o += s;
-    }
-    const uint32_t k = w - __shfl_sync(FULL, excl, o);
-    f(w < total, o, k);
-  }
-}
-
 }  // namespace tpc
