@@ -120,9 +120,26 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
     c.gid[pos] = i;
   }
   __syncthreads();
-  // order every bin by gid (bins hold about one cluster; insertion sort)
+  // order every bin by gid.  Bins hold about half a cluster; those with 2..4 are sorted in registers - their gids
+  // are read together, ordered by a 5-exchange network, and (y,z) is re-read from the input by gid - so that a bin
+  // costs one round of loads instead of a chain of them; larger bins take the insertion sort.
   for (int b = tid; b < nb; b += kGridThreads) {
     const uint32_t e = lo + s_cnt[b], s = lo + (b > 0 ? s_cnt[b - 1] : 0u);
+    const uint32_t m = e - s;
+    if (m < 2u) continue;
+    if (m <= 4u) {
+      const uint32_t o0 = c.gid[s], o1 = c.gid[s + 1], o2 = m > 2u ? c.gid[s + 2] : 0xFFFFFFFFu;
+      const uint32_t o3 = m > 3u ? c.gid[s + 3] : 0xFFFFFFFFu;
+      uint32_t g0 = o0, g1 = o1, g2 = o2, g3 = o3, t;
+#define TPC_CSWAP(a, b) t = min(a, b); b = max(a, b); a = t;
+      TPC_CSWAP(g0, g1) TPC_CSWAP(g2, g3) TPC_CSWAP(g0, g2) TPC_CSWAP(g1, g3) TPC_CSWAP(g1, g2)
+#undef TPC_CSWAP
+      if (g0 != o0) { c.gid[s] = g0; c.yz[s] = make_float2(c.y[g0], c.z[g0]); }
+      if (g1 != o1) { c.gid[s + 1] = g1; c.yz[s + 1] = make_float2(c.y[g1], c.z[g1]); }
+      if (g2 != o2) { c.gid[s + 2] = g2; c.yz[s + 2] = make_float2(c.y[g2], c.z[g2]); }
+      if (g3 != o3) { c.gid[s + 3] = g3; c.yz[s + 3] = make_float2(c.y[g3], c.z[g3]); }
+      continue;
+    }
     for (uint32_t i = s + 1; i < e; ++i) {
       const uint32_t gi = c.gid[i];
       const float2 vi = c.yz[i];
