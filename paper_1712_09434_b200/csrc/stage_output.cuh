@@ -112,10 +112,23 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
     const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t w = hb;
-    for (int rb = first; rb <= last; rb += 32) {
-      const unsigned mask = s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)];
-      if (mask & (1u << lane)) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = c.gid[map[rb + lane]];
-      w += __popc(mask);
+    // as in pass 1: the map loads of kOutChunks chunks together, then their gid gathers, then the stores
+    for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
+      unsigned mask[kOutChunks];
+      uint32_t idx[kOutChunks], g[kOutChunks];
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) {
+        const int rb = rb0 + 32 * q;
+        mask[q] = rb <= last ? s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)] : 0u;
+        idx[q] = (mask[q] >> lane) & 1u ? map[rb + lane] : 0u;
+      }
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) g[q] = (mask[q] >> lane) & 1u ? c.gid[idx[q]] : 0u;
+#pragma unroll
+      for (int q = 0; q < kOutChunks; ++q) {
+        if ((mask[q] >> lane) & 1u) o.hit_cluster[w + __popc(mask[q] & ((1u << lane) - 1u))] = g[q];
+        w += __popc(mask[q]);
+      }
     }
   }
   if (status && lane == 0) atomicOr(&o.header[2], status);
