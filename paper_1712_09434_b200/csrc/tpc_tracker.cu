@@ -414,7 +414,7 @@ HostCarve host_carve(const tpc_tracker* t, uint32_t n, uint32_t n_tasks, uint32_
   h.hit_cluster = take(hcd * 4);
   h.inner = off;
   // the chunks' workspaces together: linear in clusters, tasks and tracklets, plus alignment slack per chunk
-  h.total = off + carve((uint32_t)t->n_rows, n, n_tasks, T).total + (size_t)kHostChunks * (T ? 64 : 64) * 1024;
+  h.total = off + carve((uint32_t)t->n_rows, n, n_tasks, T).total + (size_t)kHostChunks * 64 * 1024;
   return h;
 }
 }  // namespace
