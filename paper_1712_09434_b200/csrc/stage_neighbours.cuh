@@ -18,7 +18,7 @@ namespace tpc {
 
 constexpr int kNfThreads = 128;
 constexpr int kNfList = 8;                    // candidates per side a cluster keeps; more -> serial search
-constexpr uint32_t kNfStageBytes = 16 * 1024;  // staged neighbour rows (both) must fit in this
+constexpr uint32_t kNfStageBytes = 18 * 1024 + 512;  // staged neighbour rows (both) must fit in this
 constexpr uint32_t kNfListBytes = 2u * kNfThreads * kNfList * 12u;  // 2 sides x (py, pz, idx)[kNfList][threads]
 constexpr uint32_t kNfSmemBytes = 16 + kNfListBytes + kNfStageBytes;
 
