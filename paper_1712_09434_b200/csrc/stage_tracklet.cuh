@@ -160,7 +160,7 @@ __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz,
 }
 
 // SPEC 5.3 SEARCH in the row described by g; returns the idx of the best cluster or -1 and its (y,z) in
-// best_p.  The window covers 1..4 bin rows in z; two bin rows are handled per round: their four bin bounds
+// best_p.  The window covers 1..4 bin rows in z, almost always 1 or 2: the four bin bounds of two rows
 // are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at a time, all
 // loads of a group in flight before the first is tested (the walk is latency bound) and the tests written
 // without branches (lanes of a warp are at different candidates of different windows).
@@ -179,14 +179,14 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
   const int ny = info_ny(g), nz = info_nz(g);
   const int iy0 = bin_coord(y - wy, g.y0, g.inv, ny), iy1 = bin_coord(y + wy, g.y0, g.inv, ny) + 1;
   const int iz0 = bin_coord(z - wz, g.z0, g.inv, nz), iz1 = bin_coord(z + wz, g.z0, g.inv, nz);
-  const uint32_t* bp0 = c.bins + g.bins_off + iz0 * ny;
-  const uint32_t* bp = bp0;
+  const uint32_t* bp = c.bins + g.bins_off + iz0 * ny;
   float best = __int_as_float(0x7f800000);  // +inf: a valid cluster at distance +inf counts as a tie
   float bx = 0.0f, bz = 0.0f;
   int32_t bi = -1;
-  bool tie = false;
-  for (int rows_left = iz1 - iz0 + 1; rows_left > 0; rows_left -= 2, bp += 2 * ny) {
-    const bool two = rows_left > 1;
+  const int n_zrows = iz1 - iz0 + 1;
+  bool tie = n_zrows > 2;  // a window over 3 or 4 bin rows (6 in a million) is left to the serial search as well
+  {
+    const bool two = n_zrows > 1;
     const uint32_t i1 = __ldg(bp + iy0), e1 = __ldg(bp + iy1);
     const uint32_t i2 = two ? __ldg(bp + ny + iy0) : 0u, e2 = two ? __ldg(bp + ny + iy1) : 0u;
     const uint32_t n1 = e1 - i1, n_tot = n1 + (e2 - i2);
@@ -217,7 +217,7 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
     }
   }
   if (tie) {  // the (y,z) is re-read here so that best_p never has its address taken (it stays in registers)
-    bi = search_row_serial(c.yz, c.gid, bp0, ny, iy0, iy1, iz1 - iz0 + 1, y, z, hy2, hz2, ey, ez);
+    bi = search_row_serial(c.yz, c.gid, bp, ny, iy0, iy1, n_zrows, y, z, hy2, hz2, ey, ez);
     if (bi >= 0) { const float2 p = c.yz[bi]; bx = p.x; bz = p.y; }
   }
   best_p = make_float2(bx, bz);
