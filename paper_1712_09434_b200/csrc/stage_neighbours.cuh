@@ -17,10 +17,12 @@
 namespace tpc {
 
 constexpr int kNfThreads = 128;
-constexpr int kNfList = 8;                    // candidates per side a cluster keeps; more -> serial search
+constexpr int kNfList = 8;                    // candidates per side a cluster keeps (more -> serial search) at the
+constexpr int kNfListDense = 16;              // density of a central event / in denser batches (host's choice)
+constexpr uint32_t kNfDenseRow = 900;         // mean clusters per row from which the deeper lists are used
 constexpr uint32_t kNfStageBytes = 18 * 1024 + 512;  // staged neighbour rows (both) must fit in this
-constexpr uint32_t kNfListBytes = 2u * kNfThreads * kNfList * 12u;  // 2 sides x (py, pz, idx)[kNfList][threads]
-constexpr uint32_t kNfSmemBytes = 16 + kNfListBytes + kNfStageBytes;
+__host__ __device__ constexpr uint32_t nf_list_bytes(int list) { return 2u * kNfThreads * (uint32_t)list * 12u; }  // 2 sides x (py, pz, idx)
+__host__ __device__ constexpr uint32_t nf_smem_bytes(int list) { return 16u + nf_list_bytes(list) + kNfStageBytes; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -116,7 +118,8 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
 
 // Window walk of one thread around (y, zc) (zc = the projected z of N1) in row view v: the clusters that
 // pass the window test are appended to the thread's list as ((p.x - y)*sgn*fac, (p.y - z)*sgn*fac, idx).
-// Returns the number that passed (entries beyond kNfList are not stored).
+// Returns the number that passed (entries beyond LIST are not stored).
+template <int LIST>
 __device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float y, float z, float zc,
                                                float HY, float HZ, float sgn, float fac, float2* l_p,
                                                uint32_t* l_i) {
@@ -138,7 +141,7 @@ __device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float
       const float ry = p.x - y;
       const bool pass = (fabsf(ry) <= HY) & (fabsf(p.y - zc) <= HZ);  // N2 / N3
       // stored whether it passes or not: a cluster that fails is overwritten by the next one (n stays)
-      if (n < (uint32_t)kNfList) {
+      if (n < (uint32_t)LIST) {
         const uint32_t slot = n * kNfThreads;
         // up: (y_u - y)*b, (z_u - z)*b.  down: (y - y_d)*a_, (z - z_d)*a_ (exact negation of the difference)
         l_p[slot] = make_float2((sgn * ry) * fac, (sgn * (p.y - z)) * fac);
@@ -150,7 +153,7 @@ __device__ __forceinline__ uint32_t nf_collect(const RowView& v, bool act, float
   return n;
 }
 
-template <bool COUNT>
+template <bool COUNT, int LIST>
 __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const RowView& vd, int row,
                                        uint32_t lo, uint32_t hi, unsigned char* list_smem) {
   const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max;
@@ -158,10 +161,10 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
   const float ratio_up = c.ratio_up[row], ratio_dn = c.ratio_dn[row];
   const float wy = c.wy, wz = c.wz;
   const int tid = threadIdx.x;
-  float2* d_p = reinterpret_cast<float2*>(list_smem) + tid;  // [kNfList][kNfThreads] each, this thread's column
-  float2* u_p = d_p + kNfList * kNfThreads;
-  uint32_t* d_i = reinterpret_cast<uint32_t*>(reinterpret_cast<float2*>(list_smem) + 2 * kNfList * kNfThreads) + tid;
-  uint32_t* u_i = d_i + kNfList * kNfThreads;
+  float2* d_p = reinterpret_cast<float2*>(list_smem) + tid;  // [LIST][kNfThreads] each, this thread's column
+  float2* u_p = d_p + LIST * kNfThreads;
+  uint32_t* d_i = reinterpret_cast<uint32_t*>(reinterpret_cast<float2*>(list_smem) + 2 * LIST * kNfThreads) + tid;
+  uint32_t* u_i = d_i + LIST * kNfThreads;
   unsigned long long n_pairs = 0ull;
   for (uint32_t i0 = lo + (uint32_t)(tid & ~31); i0 < hi; i0 += kNfThreads) {  // warp-uniform trip count
     const uint32_t i = i0 + (uint32_t)(tid & 31);
@@ -169,13 +172,13 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     float y = 0.0f, z = 0.0f;
     if (act) { const float2 h = c.yz[i]; y = h.x; z = h.y; }
     const float zu = z * ratio_up, zd = z * ratio_dn;  // N1
-    const uint32_t nd = nf_collect(vd, act, y, z, zd, HY, HZ, -1.0f, a_, d_p, d_i);  // N3
+    const uint32_t nd = nf_collect<LIST>(vd, act, y, z, zd, HY, HZ, -1.0f, a_, d_p, d_i);  // N3
     __syncwarp();
-    const uint32_t nu = nd ? nf_collect(vu, act, y, z, zu, HY, HZ, 1.0f, b, u_p, u_i) : 0u;  // N2
+    const uint32_t nu = nd ? nf_collect<LIST>(vu, act, y, z, zu, HY, HZ, 1.0f, b, u_p, u_i) : 0u;  // N2
     __syncwarp();
-    const bool overflow = nd > (uint32_t)kNfList || nu > (uint32_t)kNfList;
+    const bool overflow = nd > (uint32_t)LIST || nu > (uint32_t)LIST;
     const uint32_t n_pr = overflow ? 0u : nu * nd;
-    const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 64, nd <= 8
+    const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 256, nd <= 16
     if (COUNT) n_pairs += n_pr;
     float best = CHI_MAX;  // N5: only chi < CHI_MAX is eligible
     uint32_t bk = 0u;
@@ -208,12 +211,12 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
   if (COUNT && n_pairs) atomicAdd(&c.counters[CN_NF_PAIRS], n_pairs);
 }
 
-template <bool COUNT>
+template <bool COUNT, int LIST>
 __global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant__ Ctx c) {
   extern __shared__ __align__(16) unsigned char nf_smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(nf_smem);
   unsigned char* list_smem = nf_smem + 16;
-  unsigned char* stage = nf_smem + 16 + kNfListBytes;
+  unsigned char* stage = nf_smem + 16 + nf_list_bytes(LIST);
 
   const uint32_t tr = blockIdx.x;
   const int row = (int)(tr % (uint32_t)c.n_rows);
@@ -257,11 +260,11 @@ __global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant
     mbar_wait(bar, 0u);
     vu.yz = s_uyz; vu.yz_base = uya0; vu.bins = s_ub + (gu.bins_off - uba0);
     vd.yz = s_dyz; vd.yz_base = dya0; vd.bins = s_db + (gd.bins_off - dba0);
-    nf_row<COUNT>(c, vu, vd, row, lo, hi, list_smem);
+    nf_row<COUNT, LIST>(c, vu, vd, row, lo, hi, list_smem);
   } else {
     vu.yz = c.yz; vu.yz_base = 0u; vu.bins = c.bins + gu.bins_off;
     vd.yz = c.yz; vd.yz_base = 0u; vd.bins = c.bins + gd.bins_off;
-    nf_row<COUNT>(c, vu, vd, row, lo, hi, list_smem);
+    nf_row<COUNT, LIST>(c, vu, vd, row, lo, hi, list_smem);
   }
 }
 

@@ -203,11 +203,17 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
   e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute((const void*)k_neighbours<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)kNfSmemBytes);
+    e = cudaFuncSetAttribute((const void*)k_neighbours<false, kNfList>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)nf_smem_bytes(kNfList));
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute((const void*)k_neighbours<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)kNfSmemBytes);
+    e = cudaFuncSetAttribute((const void*)k_neighbours<true, kNfList>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)nf_smem_bytes(kNfList));
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute((const void*)k_neighbours<false, kNfListDense>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)nf_smem_bytes(kNfListDense));
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute((const void*)k_neighbours<true, kNfListDense>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)nf_smem_bytes(kNfListDense));
   t->trk_smem = (size_t)t->n_rows * sizeof(float);
   for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
     const void* fn = cnt ? (const void*)k_tracklets<true> : (const void*)k_tracklets<false>;
@@ -338,8 +344,15 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   }
   mark();
   if (c.n_tr > 0) {
-    if (cnt) k_neighbours<true><<<c.n_tr, kNfThreads, kNfSmemBytes, s>>>(c);                // a2
-    else k_neighbours<false><<<c.n_tr, kNfThreads, kNfSmemBytes, s>>>(c);
+    // deeper candidate lists where the rows are dense (more than kNfDenseRow clusters per row on average)
+    const bool dense = (uint64_t)c.n > (uint64_t)kNfDenseRow * c.n_tr;
+    if (dense) {
+      if (cnt) k_neighbours<true, kNfListDense><<<c.n_tr, kNfThreads, nf_smem_bytes(kNfListDense), s>>>(c);   // a2
+      else k_neighbours<false, kNfListDense><<<c.n_tr, kNfThreads, nf_smem_bytes(kNfListDense), s>>>(c);
+    } else {
+      if (cnt) k_neighbours<true, kNfList><<<c.n_tr, kNfThreads, nf_smem_bytes(kNfList), s>>>(c);             // a2
+      else k_neighbours<false, kNfList><<<c.n_tr, kNfThreads, nf_smem_bytes(kNfList), s>>>(c);
+    }
   }
   mark();
   if (c.n > 0) {
