@@ -295,6 +295,43 @@ def test_host_entry_point_in_chunks_overflow_is_reported(cfg2):
     trk.close()
 
 
+def test_host_entry_point_chunks_with_one_heavy_task():
+    """Chunk boundaries fall on whole tasks: a batch whose clusters sit almost all in one task leaves chunks empty.
+    The chunked host path must still give the device path's result."""
+    import torch
+    from paper_1712_09434_b200 import Tracker
+    geom = default_geometry(n_sectors=1, n_rows=20)
+    rng = np.random.default_rng(11)
+    pts = {}
+    for r in range(20):
+        x = float(geom.row_x[r])
+        pts[(0, r)] = [(0.01 * x, 0.5 * x), (-0.02 * x, 0.2 * x)]
+        pts[(3, r)] = [(0.02 * x, 0.3 * x)]
+        w = x * float(geom.tan_half_angle)
+        yy = rng.uniform(-w, w, 60_000).astype(np.float32)
+        zz = rng.uniform(0.0, 250.0, 60_000).astype(np.float32)
+        pts[(2, r)] = [(3.0 + 0.03 * x, 0.9 * x)] + list(zip(yy.tolist(), zz.tolist()))
+    b = batch_from_rows(geom, pts, n_tasks=5)  # task 1 and 4 empty, task 2 holds 1.2 M clusters
+    assert b.n_clusters > (1 << 20)
+    dev = torch.device("cuda:0")
+    ref = G.run_gpu(b, debug=False, debug_tracklets=False)
+    trk = Tracker(b.geometry, G.tracker_params_for(b))
+    n = b.n_clusters
+    y = torch.from_numpy(np.ascontiguousarray(b.y)).pin_memory()
+    z = torch.from_numpy(np.ascontiguousarray(b.z)).pin_memory()
+    ro = torch.from_numpy(b.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()
+    out = trk.alloc_outputs(n, dev, pinned_host=True)
+    ws = trk.alloc_workspace(trk.host_workspace_bytes(n, b.n_tasks, 0, out.track_task.shape[0], out.hit_cluster.shape[0]), dev)
+    trk.track_batch_host(y, z, ro, b.n_tasks, out, ws)
+    host = out.to_numpy()
+    trk.close()
+    assert host["n_tracks"] == ref["n_tracks"] and host["n_hits"] == ref["n_hits"] and host["status"] == ref["status"] == 0
+    assert ref["n_tracks"] >= 4
+    for k in ("track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_par", "track_cov",
+              "track_chi2", "hit_cluster"):
+        assert np.array_equal(host[k], ref[k]), k
+
+
 def test_counters_match_the_oracle_counters():
     """The device counters feed the algorithmic-bytes formula of bench.py."""
     b = generate_config(1)
