@@ -227,6 +227,7 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
 enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4, PH_ENDED = 5, PH_FETCH = 6, PH_EXIT = 7 };
 
 constexpr uint32_t kNoHit = 0xFFFFFFFFu;  // row map entry of a row without a hit
+constexpr int kClaimChunks = 5;           // 32-row chunks of a map row claimed per round (159 rows = 5 chunks)
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_tracklets(const Ctx c) {
@@ -266,9 +267,16 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
         const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
         const unsigned long long key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
         const uint32_t* fmap = c.trk_hits + (size_t)ft * map_stride(n_rows);
-        for (int r = ffirst + lane; r <= flast; r += 32) {
-          const uint32_t idx = fmap[r];
-          if (idx != kNoHit) atomicMax(&c.owner[idx], key);
+        for (int rb = ffirst; rb <= flast; rb += 32 * kClaimChunks) {  // the map loads of a round together, then the claims
+          uint32_t idx[kClaimChunks];
+#pragma unroll
+          for (int q = 0; q < kClaimChunks; ++q) {
+            const int r = rb + 32 * q + lane;
+            idx[q] = r <= flast ? fmap[r] : kNoHit;
+          }
+#pragma unroll
+          for (int q = 0; q < kClaimChunks; ++q)
+            if (idx[q] != kNoHit) atomicMax(&c.owner[idx[q]], key);
         }
       }
       if (lane == L) {
