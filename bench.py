@@ -29,7 +29,7 @@ UNIT = "clusters/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 # From the committed `ncu --set full` capture of the tracklet constructor on this workload
 # (profiles/r01_ncu_tracklets.md): DRAM bytes read + written and thread instructions executed per launch.
-NCU_TRACKLETS = {"workload": "config3_batch16_central", "dram_bytes": 12.934e9 + 3.147e9, "thread_inst": 145.7e9,
+NCU_TRACKLETS = {"workload": "config3_batch16_central", "dram_bytes": 13.030e9 + 3.172e9, "thread_inst": 146.5e9,
                  "source": "profiles/r01_ncu_tracklets.md"}
 ALU_PEAK_THREAD_INST_PER_S = 148 * 4 * 32 * 1.965e9  # SMs x schedulers x lanes x SM clock
 
