@@ -3,6 +3,10 @@
     python -m oracle.build
 
 Flags: -O2, no fast-math, no FMA contraction (docs/ARITH_SPEC.md section 0).
+
+TPC_ORACLE_SANITIZE=1 builds (and loads) a second library with -fsanitize=address,undefined instead; run the CPU
+suite on it with  LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)"
+(the summary of such a run is kept in profiles/).
 """
 from __future__ import annotations
 
@@ -17,12 +21,16 @@ FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-
 
 
 def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
-        return LIB
-    cmd = ["g++", *FLAGS, SRC, "-o", LIB]
+    lib, flags = LIB, FLAGS
+    if os.environ.get("TPC_ORACLE_SANITIZE") == "1":
+        lib = os.path.join(HERE, "libtpc_oracle_asan.so")
+        flags = [*FLAGS, "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+    if (not force and os.path.exists(lib)
+            and os.path.getmtime(lib) >= os.path.getmtime(SRC)):
+        return lib
+    cmd = ["g++", *flags, SRC, "-o", lib]
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -429,17 +429,18 @@ int run(const OGeometry* g, float bz, const OParams* p, uint32_t n, uint32_t nt,
   std::vector<int32_t> up(n), dn(n), cu(n), cd(n);
   O.neighbours(up.data(), dn.data(), use_grid_nf != 0);
   O.clean(up.data(), dn.data(), cu.data(), cd.data());
-  if (o->link_up) std::memcpy(o->link_up, up.data(), n * 4);
-  if (o->link_dn) std::memcpy(o->link_dn, dn.data(), n * 4);
-  if (o->clean_up) std::memcpy(o->clean_up, cu.data(), n * 4);
-  if (o->clean_dn) std::memcpy(o->clean_dn, cd.data(), n * 4);
+  // (memcpy of zero bytes from an empty vector's null data() is undefined: found by UBSan, hence the n > 0 tests)
+  if (o->link_up && n) std::memcpy(o->link_up, up.data(), n * 4);
+  if (o->link_dn && n) std::memcpy(o->link_dn, dn.data(), n * 4);
+  if (o->clean_up && n) std::memcpy(o->clean_up, cu.data(), n * 4);
+  if (o->clean_dn && n) std::memcpy(o->clean_dn, cd.data(), n * 4);
   // S1 start hits, ascending gid
   std::vector<uint32_t> starts;
   for (uint32_t h = 0; h < n; ++h)
     if (cu[h] >= 0 && cd[h] < 0) starts.push_back(h);
   O.cnt[CN_START_HITS] = starts.size();
   o->n_start_hits = (uint32_t)starts.size();
-  if (o->start_hits) std::memcpy(o->start_hits, starts.data(), starts.size() * 4);
+  if (o->start_hits && !starts.empty()) std::memcpy(o->start_hits, starts.data(), starts.size() * 4);
   // task,row of a gid
   std::vector<uint32_t> tr_of(n);
   for (size_t tr = 0; tr < (size_t)nt * nr; ++tr)

@@ -155,51 +155,57 @@ def test_start_hits_one_per_chain(cfg0, cfg1):
 def test_noiseless_helices_recovered_fp64():
     """north_star: every cluster collected, fitted parameters = truth to 1e-5 (fp64 instantiation)."""
     rng = np.random.default_rng(11)
-    b = single_track_events(24, rng, pt_range=(0.3, 5.0), sigma_y=0.0, sigma_z=0.0)
+    b = single_track_events(80, rng, pt_range=(0.3, 5.0), sigma_y=0.0, sigma_z=0.0)
     # the generator's exact fp64 crossings (truth_state) are the input: no fp32 rounding of y, z
     res = oracle.track(b.geometry, b.truth_state[:, 0].copy(), b.truth_state[:, 1].copy(), b.row_offsets, b.n_tasks,
                        precision="f64")
-    _check_recovery(b, res, rtol=1e-5)
+    _check_recovery(b, res, rtol=1e-5, short_sigma_frac=2e-3)
 
 
 def test_noiseless_helices_recovered_fp32():
+    """the fp32 instantiation reaches ~2e-5 on long legs; held to 1e-4."""
     rng = np.random.default_rng(11)
-    b = single_track_events(24, rng, pt_range=(0.3, 5.0), sigma_y=0.0, sigma_z=0.0)
+    b = single_track_events(80, rng, pt_range=(0.3, 5.0), sigma_y=0.0, sigma_z=0.0)
     res = run(b)
-    _check_recovery(b, res, rtol=2e-4)
+    _check_recovery(b, res, rtol=1e-4, short_sigma_frac=2e-2)
 
 
-def _check_recovery(b, res, rtol):
+def _check_recovery(b, res, rtol, short_sigma_frac):
+    """SURVEY 8(c) 'Whole O5': EVERY leg with >= MIN_HITS (10) rows and |sin phi| < 0.95 is collected with every
+    cluster, exactly once.  Parameters: legs of >= 40 rows equal the truth to rtol; shorter fragments (10..39 rows:
+    sector-crossing stubs, sigma(q/pT) > 1 c/GeV) are held to short_sigma_frac of their OWN fitted error instead -
+    the turn-around keeps 1/turn_cov_scale = 1 % of the up pass's estimate (K4, reading R15: scale, do not
+    re-initialise), and on a 10-row lever arm that estimate still carries the q = 0 linearisation of the seed:
+    measured fp64 2.7e-3 relative = 1e-3 sigma on 10..19 rows, 7e-5 on 20..39, 2.8e-6 on 40..79, 8e-7 beyond
+    (D10)."""
     nr = b.geometry.n_rows
     tr = np.repeat(np.arange(len(b.row_offsets) - 1), np.diff(b.row_offsets.astype(np.int64)))
     task_of, row_of = tr // nr, tr % nr
-    n_checked = 0
+    n_long, n_short = 0, 0
     tracks_by_task = {}
     for t in range(res.n_tracks):
         tracks_by_task.setdefault(int(res.track_task[t]), []).append(t)
     for task in np.unique(task_of):
         for leg in (0, 1):
             sel = np.nonzero((task_of == task) & (b.truth_leg == leg))[0]
-            # fragments shorter than 40 rows have almost no lever arm for q/pT (sigma(q/pT) > 1 c/GeV): their
-            # estimate keeps ~1 % of the up pass's linearisation error after the C x100 turn-around (K4), which
-            # is far below their own error but above 1e-5 - DESIGN.md section 4, reading R15.
-            if len(sel) < 40:
-                continue
-            # the leg must be contiguous in rows and away from the sin(phi) limit to be fully collectable
-            rows = np.sort(row_of[sel])
-            if not (np.diff(rows) == 1).all() or np.abs(b.truth_state[sel, 2]).max() > 0.9:
+            if len(sel) < 10 or np.abs(b.truth_state[sel, 2]).max() >= 0.95:
                 continue
             cand = [t for t in tracks_by_task.get(int(task), []) if set(res.track_hits(t)) == set(sel)]
-            assert len(cand) == 1, f"task {task} leg {leg}: clusters not collected exactly once"
+            assert len(cand) == 1, f"task {task} leg {leg} ({len(sel)} rows): clusters not collected exactly once"
             t = cand[0]
             first = sel[np.argmin(row_of[sel])]
             truth = b.truth_state[first].copy()
             got = res.track_par[:, t].astype(np.float64)
             assert float(res.track_x[t]) == float(b.geometry.row_x[row_of[first]])
-            scale = np.array([max(abs(truth[0]), 1.0), max(abs(truth[1]), 1.0), 1.0, 1.0, max(abs(truth[4]), 1.0)])
-            np.testing.assert_array_less(np.abs(got - truth) / scale, rtol)
-            n_checked += 1
-    assert n_checked >= 20
+            if len(sel) >= 40:
+                scale = np.array([max(abs(truth[0]), 1.0), max(abs(truth[1]), 1.0), 1.0, 1.0, max(abs(truth[4]), 1.0)])
+                np.testing.assert_array_less(np.abs(got - truth) / scale, rtol)
+                n_long += 1
+            else:
+                sig = np.sqrt(res.track_cov[[0, 2, 5, 9, 14], t].astype(np.float64))
+                np.testing.assert_array_less(np.abs(got - truth), short_sigma_frac * sig)
+                n_short += 1
+    assert n_long >= 80 and n_short >= 8
 
 
 def test_fit_equals_weighted_linear_regression_when_bz_zero():
@@ -247,12 +253,13 @@ def test_fit_equals_weighted_linear_regression_when_bz_zero():
         assert res.track_ndf[t] == 2 * len(hits) - 5
 
 
-@pytest.mark.parametrize("bz,prec", [(5.0, "f32"), (5.0, "f64"), (0.0, "f32")])
-def test_unit_pulls(bz, prec):
-    """north_star: the Kalman fit of straight lines and helices has unbiased, unit-width pulls."""
+@pytest.mark.parametrize("bz,prec,n_ev", [(5.0, "f32", 4000), (5.0, "f64", 2000), (0.0, "f32", 2000)])
+def test_unit_pulls(bz, prec, n_ev):
+    """north_star / SURVEY 8(c): the Kalman fit of straight lines and helices has unbiased, unit-width pulls:
+    |mean| < 0.05, width 1 +- 0.1, on thousands of tracks (statistical error of a mean over 2000: 0.022)."""
     g = dataclasses.replace(default_geometry(), bz_kgauss=bz)
     rng = np.random.default_rng(21)
-    b = single_track_events(400, rng, pt_range=(0.4, 5.0), geom=g)
+    b = single_track_events(n_ev, rng, pt_range=(0.4, 5.0), geom=g)
     dt = np.float32 if prec == "f32" else np.float64
     res = oracle.track(g, b.y.astype(dt), b.z.astype(dt), b.row_offsets, b.n_tasks, precision=prec)
     nr = g.n_rows
@@ -272,12 +279,12 @@ def test_unit_pulls(bz, prec):
         pulls.append((par - truth) / np.sqrt(var))
         chi.append(float(res.track_chi2[t]) / int(res.track_ndf[t]))
     pulls = np.array(pulls)
-    assert len(pulls) > 300
+    assert len(pulls) > 0.9 * n_ev
     n_par = 5 if bz != 0.0 else 4  # q/pT has no information at Bz = 0
     for j in range(n_par):
-        assert abs(pulls[:, j].mean()) < 0.12, (j, pulls[:, j].mean())
-        assert abs(pulls[:, j].std() - 1.0) < 0.12, (j, pulls[:, j].std())
-    assert abs(np.mean(chi) - 1.0) < 0.03
+        assert abs(pulls[:, j].mean()) < 0.05, (j, pulls[:, j].mean())
+        assert abs(pulls[:, j].std() - 1.0) < 0.1, (j, pulls[:, j].std())
+    assert abs(np.mean(chi) - 1.0) < 0.02
 
 
 # ---------------------------------------------------------------- selector / output
