@@ -27,11 +27,26 @@ if ROOT not in sys.path:
 METRIC = "tpc_clusters_tracked_per_s"
 UNIT = "clusters/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
-# From the committed `ncu --set full` capture of the tracklet constructor on this workload
-# (profiles/r01_ncu_tracklets.md): DRAM bytes read + written and thread instructions executed per launch.
-NCU_TRACKLETS = {"workload": "config3_batch16_central", "dram_bytes": 13.030e9 + 3.172e9, "thread_inst": 146.5e9,
-                 "source": "profiles/r01_ncu_tracklets.md"}
+# ncu figures of the dominant kernel (DRAM bytes, thread instructions per launch) are NOT constants of this file:
+# bench_profile.py writes them from an `ncu --set full` capture into profiles/r02_ncu_kernels.json together with a
+# hash of the CUDA sources they were measured on; they are reported only while that hash is the built sources' hash.
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "r02_ncu_kernels.json")
 ALU_PEAK_THREAD_INST_PER_S = 148 * 4 * 32 * 1.965e9  # SMs x schedulers x lanes x SM clock
+
+
+def load_ncu_summary(workload):
+    """{stage name: {"dram_bytes", "thread_inst", ...}} from the committed ncu summary, or {} when it is absent,
+    was taken on another workload, or the CUDA sources have changed since (stale numbers are not reported)."""
+    from bench_profile import source_hash
+    try:
+        d = json.load(open(NCU_SUMMARY))
+    except (OSError, ValueError):
+        return {}, "no ncu summary"
+    if d.get("workload") != workload:
+        return {}, f"ncu summary is for {d.get('workload')}"
+    if d.get("source_hash") != source_hash():
+        return {}, "ncu summary is older than the CUDA sources (hash differs)"
+    return d.get("kernels", {}), os.path.relpath(NCU_SUMMARY, ROOT)
 
 
 def parse_args():
@@ -45,6 +60,10 @@ def parse_args():
     ap.add_argument("--cpu-events", type=int, default=4, help="events in the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-workers", type=int, default=0, help="worker processes of the all-cores cpu_baseline leg (0 = all)")
+    ap.add_argument("--dry-run", action="store_true",
+                    help="control flow only (rendezvous, barriers, MAX-reduce, counter gather) on the gloo backend with "
+                         "no CUDA call and no tracking; prints a line marked dry_run with value null (used by the CPU tests)")
     return ap.parse_args()
 
 
@@ -143,6 +162,48 @@ def time_oracle(batch, events):
     return time.perf_counter() - t0, sub.n_clusters
 
 
+def _oracle_one_task(task):
+    import oracle
+    from tpc_workload import take_tasks
+    b = _POOL_BATCH
+    sub, _ = take_tasks(b, [task])
+    oracle.track(sub.geometry, sub.y, sub.z, sub.row_offsets, sub.n_tasks,
+                 params=oracle.OracleParams(sigma_y=b.sigma_y, sigma_z=b.sigma_z))
+    return sub.n_clusters
+
+
+_POOL_BATCH = None
+
+
+def time_oracle_all_cores(batch, workers=0):
+    """The oracle as it stands over every (event, sector) task of ``batch``, one task per worker process at a time
+    (tasks are independent; the oracle itself stays single-threaded).  Returns (s, clusters, workers)."""
+    global _POOL_BATCH
+    import multiprocessing as mp
+    import oracle  # noqa: F401  (builds the library before the fork)
+    oracle.oracle._load()
+    cores = len(os.sched_getaffinity(0))
+    workers = workers or cores
+    _POOL_BATCH = batch
+    with mp.get_context("fork").Pool(workers) as pool:
+        pool.map(_oracle_one_task, range(min(workers, batch.n_tasks)), chunksize=1)  # warm the workers
+        t0 = time.perf_counter()
+        done = pool.map(_oracle_one_task, range(batch.n_tasks), chunksize=1)
+        s = time.perf_counter() - t0
+    _POOL_BATCH = None
+    return s, int(sum(done)), workers
+
+
+def cpu_model():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores; one step = one event (36 sector tasks) of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -178,12 +239,49 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------
 # the product arm
 # ---------------------------------------------------------------------------------------------
-def run_ours(args):
+def reduce_over_ranks(ms_pair, counts, dev):
+    """The ONLY exchanges of the N > 1 path (reporting, not data): MAX over ranks of the timed durations and the
+    sum of (clusters, events, tracks, hits).  dev = a CUDA device under nccl, None under gloo."""
     import torch
     import torch.distributed as dist
+    from paper_1712_09434_b200.sharding import gather_counts
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        t = torch.tensor(list(ms_pair), dtype=torch.float64, device=dev if dev is not None else "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_pair = [float(v) for v in t.cpu()]
+    return ms_pair, gather_counts(counts)
+
+
+def run_dry(args, rank, world):
+    """--dry-run: the control flow of run_ours (rendezvous, barriers, MAX-reduce, counter gather, rank-0 print)
+    on gloo, with no CUDA call and NO tracking.  The line carries "dry_run": true and "value": null."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    fake_ms, fake_counts = [10.0 + rank, 20.0 + rank], [1000 * (rank + 1), 1, 10 * (rank + 1), 100 * (rank + 1)]
+    if world > 1:
+        dist.barrier()
+    ms, tot = reduce_over_ranks(fake_ms, fake_counts, None)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world,
+                          "max_ms_over_ranks": ms, "summed_counts": tot}))
+    return 0
+
+
+def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with one rank per GPU")
+    if args.dry_run:
+        return run_dry(args, rank, world)
+    import torch
+    import torch.distributed as dist
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the tracker has no CPU path")
     torch.cuda.set_device(local)
@@ -192,7 +290,6 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     from paper_1712_09434_b200 import Tracker, TrackerParams
     from paper_1712_09434_b200.build import build as build_cuda
-    from paper_1712_09434_b200.sharding import gather_counts
     from tpc_workload.events import CONFIGS
     if rank == 0:
         build_cuda()
@@ -266,13 +363,8 @@ def run_ours(args):
         del ws_h, out_h
 
     # max over ranks, totals over ranks
-    if world > 1:
-        t = torch.tensor([ms_total, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, e2e_ms_max = float(t[0]), float(t[1])
-    else:
-        e2e_ms_max = e2e[0] if e2e else 0.0
-    tot = gather_counts([n, n_events, int(hdr[0]), int(hdr[1])])
+    (ms_total, e2e_ms_max), tot = reduce_over_ranks([ms_total, e2e[0] if e2e else 0.0],
+                                                    [n, n_events, int(hdr[0]), int(hdr[1])], dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -290,7 +382,8 @@ def run_ours(args):
     top_gbs = alg[top] / (stage_ms[top] / 1e3) / 1e9 if stage_ms[top] > 0 else 0.0
     path_bytes = sum(alg.values())
     path_gbs = path_bytes / (ms_step / 1e3) / 1e9
-    ncu_ok = top == "tracklet_constructor" and CONFIGS[args.config]["name"] == NCU_TRACKLETS["workload"] and args.events is None
+    ncu_all, ncu_src = load_ncu_summary(CONFIGS[args.config]["name"] if args.events is None else "partial")
+    ncu = ncu_all.get(top)  # None unless the committed capture was taken on exactly these sources and this workload
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -304,8 +397,8 @@ def run_ours(args):
         "tracks_per_s": tot[2] * args.steps / secs,
         "hbm_roofline_frac_path": path_gbs / peak_gbs,
         "roofline": {"bound": "hbm", "kernel": top, "achieved": top_gbs, "peak": peak_gbs, "unit": "GB/s",
-                     "frac": top_gbs / peak_gbs, "traffic": NCU_TRACKLETS["dram_bytes"] if ncu_ok else None,
-                     "traffic_source": NCU_TRACKLETS["source"] if ncu_ok else None, "peak_source": peak_src,
+                     "frac": top_gbs / peak_gbs, "traffic": ncu.get("dram_bytes") if ncu else None,
+                     "traffic_source": ncu_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg[top], "ms_per_launch": stage_ms[top],
                      "note": "the metric asks for the HBM fraction; this kernel is bound by plain-ALU issue, see \"alu\"",
                      "share_of_step": stage_ms[top] / max(sum(stage_ms.values()), 1e-9)},
@@ -314,11 +407,11 @@ def run_ours(args):
                           "bytes_per_cluster": path_bytes / max(n, 1)},
         # the dominant kernel is bound by plain (non-FMA) ALU issue, not by HBM: thread
         # instructions per launch from the committed ncu capture over the live launch time, against the ALU ceiling
-        "alu": ({"bound": "alu", "kernel": top, "achieved": NCU_TRACKLETS["thread_inst"] / (stage_ms[top] / 1e3) / 1e12,
+        "alu": ({"bound": "alu", "kernel": top, "achieved": ncu["thread_inst"] / (stage_ms[top] / 1e3) / 1e12,
                  "peak": ALU_PEAK_THREAD_INST_PER_S / 1e12, "unit": "T thread-instructions/s",
-                 "frac": NCU_TRACKLETS["thread_inst"] / (stage_ms[top] / 1e3) / ALU_PEAK_THREAD_INST_PER_S,
-                 "thread_inst_per_launch": NCU_TRACKLETS["thread_inst"], "source": NCU_TRACKLETS["source"]}
-                if ncu_ok else None),
+                 "frac": ncu["thread_inst"] / (stage_ms[top] / 1e3) / ALU_PEAK_THREAD_INST_PER_S,
+                 "thread_inst_per_launch": ncu["thread_inst"], "source": ncu_src}
+                if ncu and "thread_inst" in ncu else None),
         "stages_ms": stage_ms, "stages_algorithmic_bytes": alg, "stage_calls_averaged": stage_calls,
         "counters": counters,
         "clocks": clocks,
@@ -329,11 +422,18 @@ def run_ours(args):
                        "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2],
                        "ms_per_step": e2e_ms_max / args.steps, "api": "tpc_track_batch_host (pinned host buffers)"}
     if world == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands, (i) over all host cores, one (event, sector) task per worker process at a time, on
+        # every event of the workload, (ii) on one thread on the first events
+        s_all, c_all, workers = time_oracle_all_cores(batch, args.cpu_workers)
         ne = max(1, min(args.cpu_events, n_events))
-        s, c = time_oracle(batch, list(range(ne)))
-        line["cpu_baseline"] = {"value": c / s, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"first {ne} event(s) of the workload ({c} clusters), single thread, {s:.1f} s",
-                                "events_per_s": ne / s}
+        s1, c1 = time_oracle(batch, list(range(ne)))
+        line["cpu_baseline"] = {
+            "value": c_all / s_all, "unit": UNIT, "cores": workers, "kind": "oracle",
+            "sample": f"all {n_events} event(s) of the workload ({c_all} clusters, {n_tasks} sector tasks), one task per "
+                      f"worker process, {workers} workers, {s_all:.1f} s",
+            "events_per_s": n_events / s_all, "cores_available": len(os.sched_getaffinity(0)), "cpu_model": cpu_model(),
+            "single_thread": {"value": c1 / s1, "unit": UNIT, "cores": 1,
+                              "sample": f"first {ne} event(s) ({c1} clusters), one thread, {s1:.1f} s"}}
     trk.close()
     if world > 1:
         dist.destroy_process_group()
@@ -341,8 +441,22 @@ def run_ours(args):
     return 0
 
 
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) outside a launcher: start N ranks, one per GPU, as the driver would."""
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return relaunch_under_torchrun(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -127,3 +127,41 @@ def test_sharding_world_size_2_gloo(tmp_path):
     for p, o in zip(procs, outs):
         assert p.returncode == 0, o
         assert "ok" in o
+
+
+def test_bench_gpus_2_launches_two_ranks_dry_run():
+    """`python bench.py --gpus 2` starts two ranks by itself (torch.distributed.run, 127.0.0.1) and its control flow -
+    rendezvous, barriers, MAX-reduce of the durations, gather of the counters, rank-0 print - runs on gloo with
+    --dry-run (no CUDA call, no tracking: the line says dry_run and carries no value)."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run"], env=env,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout  # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["dry_run"] is True and d["value"] is None and d["n_gpus"] == 2
+    assert d["max_ms_over_ranks"] == [11.0, 21.0]          # max over ranks of (10 + rank, 20 + rank)
+    assert d["summed_counts"] == [3000, 2, 30, 300]        # sums over ranks
+    # a rank count that contradicts --gpus is refused, not silently reported
+    env2 = dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--dry-run"], env=env2,
+                       capture_output=True, text=True, timeout=120)
+    assert r.returncode != 0 and "WORLD_SIZE" in r.stderr
+
+
+def test_ncu_summary_is_tied_to_the_source_hash(tmp_path, monkeypatch):
+    """bench.py reports ncu figures only while the CUDA sources still hash to what the capture was taken on."""
+    import json
+    import bench
+    import bench_profile
+    f = tmp_path / "k.json"
+    monkeypatch.setattr(bench, "NCU_SUMMARY", str(f))
+    assert bench.load_ncu_summary("w")[0] == {}
+    f.write_text(json.dumps({"workload": "w", "source_hash": bench_profile.source_hash(),
+                             "kernels": {"tracklet_constructor": {"dram_bytes": 1.0}}}))
+    assert bench.load_ncu_summary("w")[0]["tracklet_constructor"]["dram_bytes"] == 1.0
+    assert bench.load_ncu_summary("other")[0] == {}
+    f.write_text(json.dumps({"workload": "w", "source_hash": "stale", "kernels": {"tracklet_constructor": {}}}))
+    assert bench.load_ncu_summary("w")[0] == {}
