@@ -20,6 +20,7 @@ constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at kBinsPerC
 __host__ __device__ inline size_t map_stride(int n_rows) { return (size_t)((n_rows + 7) & ~7); }
 constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the grid build
 constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
+constexpr float kCoordClamp = 1.0e5f; // grid extents only: coordinates beyond +-1 km (or non-finite) count as this
 
 enum CounterId {
   CN_CLUSTERS = 0, CN_BINS, CN_START_HITS, CN_TRACKLETS_BUILT, CN_TRACKLETS_KEPT, CN_CHAIN_HITS, CN_SEARCHES,

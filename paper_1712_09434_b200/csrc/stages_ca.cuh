@@ -26,14 +26,17 @@ __device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint
   float B = sqrtf((W * L) / (float)(kBinsPerCluster * (n > 0u ? n : 1u)));
   B = fminf(fmaxf(B, c.prm.grid_bin_min), c.prm.grid_bin_max);
   RowInfo g;
-  int ny, nz;
-  while (true) {
+  int ny = 1, nz = 1;
+  // The box is finite (the caller clamps every coordinate to +-kCoordClamp), so a few dozen coarsening steps
+  // always end; the iteration bound only guards against parameters that make B non-finite: then one bin.
+  for (int it = 0; it < 96; ++it) {
     g.inv = 1.0f / B;
-    ny = (int)fminf(W * g.inv, 65000.0f) + 1;
-    nz = (int)fminf(L * g.inv, 65000.0f) + 1;
+    ny = (int)fminf(fmaxf(W * g.inv, 0.0f), 65000.0f) + 1;
+    nz = (int)fminf(fmaxf(L * g.inv, 0.0f), 65000.0f) + 1;
     const long long nb = (long long)ny * nz;
     if (nb + 1 <= (long long)kBinsPerCluster * n + kBinPad && nb <= (long long)kMaxBinsPerRow) break;
     B = B * 1.25f;  // too many bins for the slot of this row: coarser grid
+    if (it == 95) { ny = 1; nz = 1; g.inv = 0.0f; }
   }
   g.y0 = ylo; g.z0 = zlo;
   g.ny_nz = (uint32_t)ny | ((uint32_t)nz << 16);
@@ -55,7 +58,9 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   const float kInf = __int_as_float(0x7f800000);
   float ylo = kInf, yhi = -kInf, zlo = kInf, zhi = -kInf;
   for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
-    const float y = c.y[i], z = c.z[i];
+    // non-finite coordinates (outside the contract, R27) must not make the box infinite: +-Inf is clamped, NaN
+    // is dropped by fminf/fmaxf; such a cluster lands in an edge bin and never passes an exact window test
+    const float y = fminf(fmaxf(c.y[i], -kCoordClamp), kCoordClamp), z = fminf(fmaxf(c.z[i], -kCoordClamp), kCoordClamp);
     ylo = fminf(ylo, y); yhi = fmaxf(yhi, y); zlo = fminf(zlo, z); zhi = fmaxf(zhi, z);
   }
 #pragma unroll
@@ -69,7 +74,7 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   for (int w = 0; w < kGridThreads / 32; ++w) {
     ylo = fminf(ylo, s_box[0][w]); yhi = fmaxf(yhi, s_box[1][w]); zlo = fminf(zlo, s_box[2][w]); zhi = fmaxf(zhi, s_box[3][w]);
   }
-  if (n == 0u) { ylo = yhi = zlo = zhi = 0.0f; }
+  if (n == 0u || !(ylo <= yhi) || !(zlo <= zhi)) { ylo = yhi = zlo = zhi = 0.0f; }  // empty row, or NaN only
   const RowInfo g = make_row_info(c, tr, lo, n, ylo, yhi, zlo, zhi);
   const int g_ny = info_ny(g), g_nz = info_nz(g);
   const int nb = g_ny * g_nz;
