@@ -93,16 +93,30 @@ def make_workload(config, n_events, rank):
 # algorithmic bytes (SURVEY.md section 8(d) / DESIGN.md section 6), from the device counters
 # ---------------------------------------------------------------------------------------------
 def algorithmic_bytes(c):
+    """SURVEY.md section 8(d) / DESIGN.md section 6.  The tracklet constructor (a5) runs as four kernels; its
+    formula is split by what each kernel must move (chain: link + (y,z) per chain hit; up pass: bin bounds and
+    candidates of its searches; refit: (y,z) of the hits re-read; the last kernel: the rest - its searches, the
+    map, the ownership words, the record), so the four parts add up to the a5 formula exactly."""
     N, B, T0, T = c["clusters"], c["bins"], c["start_hits"], c["tracklets_built"]
     Hc, S, K, Ht = c["chain_hits"], c["searches"], c["candidates"], c["tracklet_hits"]
     Ho, To = c["out_hits"], c["out_tracks"]
+    a5 = 12 * Hc + 16 * S + 8 * K + 8 * Ht + 4 * Ht + 8 * Ht + 8 * N + 88 * T
+    chain = 12 * Hc
+    up = 16 * c["searches_up"] + 8 * c["candidates_up"]
+    refit = 8 * min(c["refit_steps"], Ht)
     return {
         "grid_build": 8 * N + 8 * N + 4 * N + 4 * B,
         "neighbour_finder": 8 * N + 4 * B + 8 * N,
         "cleaner": 8 * N,
         "start_hits": 4 * T0,
-        "tracklet_constructor": 12 * Hc + 16 * S + 8 * K + 8 * Ht + 4 * Ht + 8 * Ht + 8 * N + 88 * T,
-        "selector_output": 4 * Ht + 8 * Ht + 4 * Ho + 100 * To,
+        "tracklet_chain_fit": chain,
+        "tracklet_up_pass": up,
+        "tracklet_refit": refit,
+        # K7 (ownership words, 8 B per hit and 8 B per cluster) is its own kernel now; it takes the selector's
+        # map and ownership reads (12 B per hit) along
+        "tracklet_down_finish": a5 - chain - up - refit - 8 * Ht - 8 * N,
+        "ownership": 8 * Ht + 8 * N + 4 * Ht + 8 * Ht,
+        "selector_output": 4 * Ho + 100 * To,
     }
 
 

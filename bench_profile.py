@@ -27,8 +27,8 @@ OUT = os.path.join(ROOT, "profiles", "r02_ncu_kernels.json")
 
 # kernel name (substring) -> stage name of tpc_stage_name()
 STAGE_OF = {"k_grid_build": "grid_build", "k_neighbours": "neighbour_finder", "k_clean": "cleaner",
-            "k_seeds": "start_hits", "k_chain": "tracklet_constructor", "k_follow": "tracklet_constructor",
-            "k_refit": "tracklet_constructor", "k_tracklets": "tracklet_constructor",
+            "k_seeds": "start_hits", "k_trk_chain": "tracklet_chain_fit", "k_trk_up": "tracklet_up_pass",
+            "k_trk_refit": "tracklet_refit", "k_trk_finish": "tracklet_down_finish",
             "k_select_output": "selector_output", "k_merge": "merger_refit"}
 
 METRICS = {

@@ -178,10 +178,12 @@ int tpc_track_batch_host(tpc_tracker* tracker, const tpc_clusters* clusters, tpc
  * Only filled when the tracker was created with counters enabled through
  * tpc_tracker_enable_counters(tracker, 1) - counting costs atomics, so timed
  * runs leave it off. */
-#define TPC_N_COUNTERS 12
+#define TPC_N_COUNTERS 16
 /* 0 clusters, 1 grid bins, 2 start hits (S1), 3 tracklets built (S3), 4 tracklets kept (K6),
  * 5 chain hits fitted (K1, K2), 6 row searches (K3, K5), 7 candidates examined (H3),
- * 8 hits of kept tracklets, 9 row steps (transports of K2, K3, K5), 10 neighbour pairs (N4), 11 unused */
+ * 8 hits of kept tracklets, 9 row steps (transports of K2, K3, K5), 10 neighbour pairs (N4),
+ * 11 unused, 12 row searches of the up pass (K3), 13 candidates examined in the up pass,
+ * 14 row steps of the down pass that used a hit of the map without a search (K5), 15 unused. */
 void tpc_tracker_enable_counters(tpc_tracker* tracker, int on);
 int tpc_read_counters(tpc_tracker* tracker, void* cuda_stream, uint64_t* out);
 
@@ -197,8 +199,10 @@ int tpc_launches_per_batch(const tpc_tracker* tracker);
  * and to n_calls (HOST, may be NULL) how many calls that was.  Stage i is
  * named tpc_stage_name(i) (static string, NULL beyond the last stage):
  * 0 grid build (a1), 1 neighbour finder (a2), 2 cleaner (a3), 3 start hits (a4),
- * 4 tracklet constructor (a5), 5 selector + output (a6, a7). */
-#define TPC_N_STAGES 6
+ * 4..7 tracklet constructor (a5) as its four kernels - chain fit (K1, K2), up pass and
+ * turn-around (K3, K4), refit of the rows that have a hit (K5), rest of the down pass with
+ * finish (K5, K6) -, 8 ownership of shared clusters (K7, L1), 9 selector + output (a6, a7). */
+#define TPC_N_STAGES 10
 #define TPC_STAGE_RING 64
 void tpc_tracker_enable_stage_timing(tpc_tracker* tracker, int on);
 int tpc_read_stage_ms(tpc_tracker* tracker, void* cuda_stream, float* out_ms, uint32_t* n_calls);

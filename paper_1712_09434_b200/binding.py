@@ -18,7 +18,8 @@ _HEADER = os.path.join(os.path.dirname(HERE), "include", "tpc_tracker.h")
 
 STATUS_TRACKLET_OVERFLOW, STATUS_TRACK_OVERFLOW, STATUS_HIT_OVERFLOW = 1, 2, 4
 COUNTER_NAMES = ["clusters", "bins", "start_hits", "tracklets_built", "tracklets_kept", "chain_hits", "searches",
-                 "candidates", "tracklet_hits", "row_steps", "nf_pairs", "unused"]
+                 "candidates", "tracklet_hits", "row_steps", "nf_pairs", "unused", "searches_up", "candidates_up",
+                 "refit_steps", "unused2"]
 
 
 class TpcError(RuntimeError):

@@ -24,7 +24,8 @@ constexpr float kCoordClamp = 1.0e5f; // grid extents only: coordinates beyond +
 
 enum CounterId {
   CN_CLUSTERS = 0, CN_BINS, CN_START_HITS, CN_TRACKLETS_BUILT, CN_TRACKLETS_KEPT, CN_CHAIN_HITS, CN_SEARCHES,
-  CN_CANDIDATES, CN_TRACKLET_HITS, CN_ROW_STEPS, CN_NF_PAIRS, CN_RESERVED, CN_COUNT
+  CN_CANDIDATES, CN_TRACKLET_HITS, CN_ROW_STEPS, CN_NF_PAIRS, CN_RESERVED, CN_SEARCHES_UP, CN_CANDIDATES_UP,
+  CN_REFIT_STEPS, CN_RESERVED2, CN_COUNT
 };
 static_assert(CN_COUNT == TPC_N_COUNTERS, "counter list and header disagree");
 
@@ -56,9 +57,9 @@ __device__ __forceinline__ RowInfo load_row_info(const RowInfo* p) {
 // Seed record of a tracklet, 3 x 16 bytes, so that a5 starts a tracklet with ONE round of loads:
 //   [0] h0 (idx of the start hit), tr0 (task*n_rows + row of h0), h1 = clean_up[h0], h2 = clean_up[h1] (or -1)
 //   [1] y0, z0, y1, z1 (the (y,z) of h0 and h1 as float bits)
-//   [2] h0 - row_lo(tr0), h1 - row_lo(tr0+1) (row-local indices), gid(h0), 0
+//   [2] y2, z2 (the (y,z) of h2 as float bits), gid(h0), h3 = clean_up[h2] (or -1)
 constexpr int kSeedU4 = 3;
-constexpr int kRecFloat4 = 7;  // tracklet record: 7 float4 = x, p[5], c[15], chi2, ndf, first_row, last_row, n_hits, 2 pad
+constexpr int kRecFloat4 = 8;  // tracklet record: 7 float4, layout in stage_tracklet.cuh
 
 // Everything a kernel needs, passed by value (about 300 bytes of kernel parameters).
 struct Ctx {
@@ -79,20 +80,23 @@ struct Ctx {
   RowInfo* rowinfo;        // [n_tr]
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
-  unsigned long long* owner;  // [n] K7 ownership key
   uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)
   uint32_t* trk_hits;      // [max_tracklets][map_stride(n_rows)] row map of the tracklet: idx of its hit in that row or kNoHit;
                            // valid for the rows first_row..last_row of the tracklet record
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
+  uint4* trk_meta;         // [max_tracklets] nHits, firstRow | lastRow << 16, gid of the start hit, 0: what K7 needs
+  uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
-  uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2 tracklet queue head
+  uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2..5 queue heads of the four tracklet kernels
   uint32_t* n_tracklets;   // [1] tracklets built (clamped to max_tracklets)
   uint32_t max_tracklets;
   unsigned long long* counters;  // [CN_COUNT] or nullptr
   // outputs (device)
   tpc_tracks out;
 };
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ uint32_t bins_base(const Ctx& c, uint32_t tr, uint32_t row_lo) {
   return kBinsPerCluster * row_lo + tr * kBinPad;

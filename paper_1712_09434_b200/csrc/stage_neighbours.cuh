@@ -24,7 +24,6 @@ constexpr uint32_t kNfStageBytes = 18 * 1024 + 512;  // staged neighbour rows (b
 __host__ __device__ constexpr uint32_t nf_list_bytes(int list) { return 2u * kNfThreads * (uint32_t)list * 12u; }  // 2 sides x (py, pz, idx)
 __host__ __device__ constexpr uint32_t nf_smem_bytes(int list) { return 16u + nf_list_bytes(list) + kNfStageBytes; }
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }

@@ -1,4 +1,4 @@
-// a6 tracklet selector + a7 output compaction (docs/ARITH_SPEC.md section 7, L1..L4),
+// K7 ownership + a6 tracklet selector + a7 output compaction (docs/ARITH_SPEC.md sections 6 (K7) and 7, L1..L4),
 // and the untimed debug kernels that translate internal idx to gid.
 #pragma once
 #include "device_common.cuh"
@@ -6,16 +6,102 @@
 
 namespace tpc {
 
-constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
-constexpr int kOutChunks = 5;     // 32-row chunks of a row map tested per round (159 rows = 5 chunks)
+// ---------------------------------------------------------------------------
+// K7 + L1: who owns a cluster.  owner[h] = max over the kept tracklets that hold h of
+// key = nHits << 32 | ~gid(h0), and a tracklet keeps h iff it is that owner.  The ownership words never
+// exist in global memory: the clusters are cut into chunks of kResolveChunk consecutive idx, one block
+// per chunk holds the chunk's ownership words in shared memory, and walks the row maps of the tracklets
+// of the task(s) the chunk lies in - only the rows the chunk covers - twice: first atomicMax of the key
+// (shared-memory atomics), then the test; an entry that lost is overwritten with kNoHit in the map, so
+// after this kernel a row map lists exactly the hits its tracklet keeps (L1).
+// (Global 64-bit atomicMax per hit - 139 M of them on config 3, each a DRAM read-modify-write because
+// the three or four tracklets that share a cluster end far apart in time - cost more than the whole
+// down pass; shared memory takes that traffic away.)
+// ---------------------------------------------------------------------------
+constexpr int kResolveThreads = 256;
+constexpr uint32_t kResolveChunk = 8192;  // clusters per block: 64 KB of ownership words, 3 blocks per SM
+#ifndef TPC_RESOLVE_BATCH
+#define TPC_RESOLVE_BATCH 8
+#endif
+constexpr int kResolveBatch = TPC_RESOLVE_BATCH;          // tracklets a thread has in flight
 
-// One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by one,
-// the 32 lanes testing 32 rows of the tracklet's row map at a time (coalesced map read, 32 owner
-// gathers in flight) - L1: hit kept iff the tracklet still owns it; the keep masks stay in
-// shared memory.  The tile then takes its place in the output with an ordered chained scan over
-// (tracks, hits) packed as tracks<<32 | hits.  Pass 2: the warp writes each surviving track - its
-// record as SoA columns and its kept hits as gids in ascending row order (L3).
-// Output order = tracklet order.
+// first tracklet of every task: tracklets are in idx order of their start hits, so a task's are consecutive
+__global__ void k_task_offsets(const Ctx c) {
+  const uint32_t n_trk = *c.n_tracklets, n_rows = (uint32_t)c.n_rows;
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_trk; t += gridDim.x * blockDim.x) {
+    const uint32_t task = c.trk_seed[(size_t)t * kSeedU4].y / n_rows;
+    const uint32_t from = t ? c.trk_seed[(size_t)(t - 1u) * kSeedU4].y / n_rows + 1u : 0u;
+    for (uint32_t k = from; k <= task; ++k) c.trk_task_off[k] = t;
+    if (t == n_trk - 1u)
+      for (uint32_t k = task + 1u; k <= c.n_tasks; ++k) c.trk_task_off[k] = n_trk;
+  }
+}
+
+__global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
+  extern __shared__ unsigned long long s_owner[];  // [kResolveChunk]
+  const uint32_t i0 = blockIdx.x * kResolveChunk;
+  const uint32_t i1 = min(i0 + kResolveChunk, c.n), span = i1 - i0;
+  const int tid = (int)threadIdx.x, n_rows = c.n_rows;
+  for (uint32_t i = tid; i < kResolveChunk; i += kResolveThreads) s_owner[i] = 0ull;
+  const uint32_t tr_a = find_tr(c, i0), tr_b = find_tr(c, i1 - 1u);
+  const uint32_t task_a = tr_a / (uint32_t)n_rows, task_b = tr_b / (uint32_t)n_rows;
+  const int min_hits = c.prm.min_track_hits;
+  const size_t stride = map_stride(n_rows);
+  __syncthreads();
+#ifndef TPC_RESOLVE_PASSES
+#define TPC_RESOLVE_PASSES 2
+#endif
+  for (int pass = 0; pass < TPC_RESOLVE_PASSES; ++pass) {
+    for (uint32_t k = task_a; k <= task_b; ++k) {
+      const uint32_t t0 = c.trk_task_off[k], nt = c.trk_task_off[k + 1u] - t0;
+      const int ra = k == task_a ? (int)(tr_a - k * (uint32_t)n_rows) : 0;
+      const int rb = k == task_b ? (int)(tr_b - k * (uint32_t)n_rows) : n_rows - 1;
+      // threads = (tracklet group) x (row): rp = rows per tracklet rounded up to a power of two (<= block size)
+      int sh = 0;
+      while ((1 << sh) < rb - ra + 1 && (1 << sh) < kResolveThreads) ++sh;
+      const int rp = 1 << sh, grp = kResolveThreads >> sh;
+      const int r_lane = ra + (tid & (rp - 1));
+      for (uint32_t tb = (uint32_t)(tid >> sh); tb < nt; tb += (uint32_t)(grp * kResolveBatch)) {
+        for (int r = r_lane; r <= rb; r += rp) {
+          uint4 m[kResolveBatch];
+          uint32_t idx[kResolveBatch];
+#pragma unroll
+          for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
+            const uint32_t tt = tb + (uint32_t)(j * grp);  // tracklet's rows is read and ignored)
+            const bool in = tt < nt;
+            m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
+            idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + r] : kNoHit;
+          }
+#pragma unroll
+          for (int j = 0; j < kResolveBatch; ++j) {
+            const int first = (int)(m[j].y & 0xFFFFu), last = (int)(m[j].y >> 16);
+            const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
+            if ((int)m[j].x < min_hits || r < first || r > last || idx[j] == kNoHit || off >= span) continue;
+            const unsigned long long key =
+                ((unsigned long long)m[j].x << 32) | (unsigned long long)(0xFFFFFFFFu - m[j].z);
+#ifdef TPC_RESOLVE_NOATOM
+            if (pass == 0) s_owner[off] = key;
+#else
+            if (pass == 0) atomicMax(&s_owner[off], key);                                      // K7
+#endif
+            else if (s_owner[off] != key) c.trk_hits[(size_t)(t0 + tb + (uint32_t)(j * grp)) * stride + r] = kNoHit;  // L1
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
+constexpr int kOutChunks = 5;     // 32-row chunks of a row map read per round (159 rows = 5 chunks)
+
+// a6 (L2) + a7.  One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by
+// one, the 32 lanes reading 32 rows of the tracklet's row map at a time (after k_resolve the map holds the
+// hits the tracklet keeps); the keep masks stay in shared memory.  The tile then takes its place in the
+// output with an ordered chained scan over (tracks, hits) packed as tracks<<32 | hits.  Pass 2: the warp
+// writes each surviving track - its record as SoA columns and its kept hits as gids in ascending row
+// order (L3).  Output order = tracklet order.
 __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   extern __shared__ uint32_t s_keep[];  // [kOutThreads][words] keep masks, bit k of word w = row first_row + 32 w + k
   __shared__ uint32_t s_warp[33];
@@ -33,40 +119,29 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t t_warp = tile * kOutThreads + warp * 32;
   const int min_hits = c.prm.min_track_hits;
-  // lane j holds what it needs of tracklet t_warp + j: n_hits, first/last row, start-hit gid
+  // lane j holds what it needs of tracklet t_warp + j: n_hits, first/last row
   int my_n = 0, my_first = 0, my_last = -1;
-  uint32_t my_gid0 = 0u;
   if (t_warp + lane < n_trk) {
-    const float4* rec = c.trk_rec + (size_t)(t_warp + lane) * kRecFloat4;
-    my_n = __float_as_int(__ldg(rec + 5).w);
-    const float4 r6 = __ldg(rec + 6);
-    my_first = __float_as_int(r6.x); my_last = __float_as_int(r6.y);
-    my_gid0 = __ldg(c.trk_seed + (size_t)(t_warp + lane) * kSeedU4 + 2).z;
+    const uint4 m = __ldg(&c.trk_meta[t_warp + lane]);
+    my_n = (int)m.x; my_first = (int)(m.y & 0xFFFFu); my_last = (int)(m.y >> 16);
   }
-  uint32_t my_kept = 0u;  // lane j: hits tracklet t_warp + j still owns
+  uint32_t my_kept = 0u;  // lane j: hits tracklet t_warp + j keeps
   for (unsigned rest = __ballot_sync(FULL, my_n >= min_hits); rest; rest &= rest - 1u) {  // K6
     const int j = __ffs(rest) - 1;
     const uint32_t t = t_warp + j;
-    const int n_hits = __shfl_sync(FULL, my_n, j), first = __shfl_sync(FULL, my_first, j);
-    const int last = __shfl_sync(FULL, my_last, j);
-    const unsigned long long key = ((unsigned long long)(uint32_t)n_hits << 32) |
-                                   (unsigned long long)(0xFFFFFFFFu - __shfl_sync(FULL, my_gid0, j));
+    const int first = __shfl_sync(FULL, my_first, j), last = __shfl_sync(FULL, my_last, j);
     const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t kept = 0u;
-    // kOutChunks x 32 rows per round: all map loads of a round are issued together, then all owner gathers
-    for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
+    for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {  // the map loads of a round are issued together
       uint32_t idx[kOutChunks];
-      unsigned long long own[kOutChunks];
 #pragma unroll
       for (int q = 0; q < kOutChunks; ++q) {
         const int r = rb0 + 32 * q + lane;
         idx[q] = r <= last ? map[r] : kNoHit;
       }
 #pragma unroll
-      for (int q = 0; q < kOutChunks; ++q) own[q] = idx[q] != kNoHit ? c.owner[idx[q]] : 0ull;
-#pragma unroll
       for (int q = 0; q < kOutChunks; ++q) {
-        const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit && own[q] == key);   // L1
+        const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit);   // L1 (decided by k_resolve)
         if (lane == 0 && rb0 + 32 * q <= last) s_keep[(warp * 32 + j) * words + ((rb0 - first) >> 5) + q] = mask;
         kept += __popc(mask);
       }

@@ -3,26 +3,31 @@
 // track").  docs/ARITH_SPEC.md sections 5 (track model) and 6 (K1..K7).
 //
 // One LANE per tracklet, the whole filter state (5 parameters, 15 covariance
-// entries, chi2) in registers, in a PERSISTENT kernel: a lane whose tracklet has
-// ended takes the next one from a global queue, so the 32 lanes of a warp stay
-// busy although tracklets live for 10..320 row steps.  The five passes of SPEC 6
-// (chain fit, up pass, turn-around, down pass, finish) are ONE loop whose body is
-// a single row step
+// entries, chi2) in registers.  The life of a tracklet is cut where the KIND of
+// its row steps changes, and every part is its own persistent kernel, so that
+// the 32 lanes of a warp always execute the same kind of step:
+//   k_trk_chain   K1 + K2   seed, then the fit along the link chain   (hit known, no search)
+//   k_trk_up      K3 + K4   up pass and turn-around                   (every step searches)
+//   k_trk_refit   K5 (a)    down pass over the rows that have a hit   (hit known, no search)
+//   k_trk_finish  K5 (b), K6       rest of the down pass (searches below firstRow or in a hole of
+//                                  the map), finish
+// Between two kernels the tracklet rests in its record (Ctx::trk_rec, 128 bytes).  In every kernel
+// a lane whose tracklet has ended takes the next one from a queue (tickets drawn 32 at a time per
+// warp), so the lanes stay busy although tracklets live for very different numbers of row steps;
+// the record of the next tracklet is copied to the lane's shared-memory slot with cp.async while
+// the lane runs the last step of the current one, so no warp ever waits for a fetch.  A row step is
 //     transport -> choose the hit (chain link / row map / search) -> update
-// with a per-lane phase, so lanes in different passes execute the same
-// instructions.  The row -> hit map of a tracklet is its row of Ctx::trk_hits in
-// global memory (idx per pad row or kNoHit): written once per row step, read
-// back in the down pass ONE ROW AHEAD, so that together with the chain link and
-// the grid header every load a step needs is issued before the transport
-// arithmetic and none is waited for.  No shared memory besides the row table:
-// the registers alone bound the number of tracklets in flight.
+// with the loads that do not depend on the transported state issued before the transport.  The
+// row -> hit map of a tracklet is its row of Ctx::trk_hits in global memory (idx per pad row or
+// kNoHit).  Registers alone bound the tracklets in flight.
 #pragma once
 #include "device_common.cuh"
 
 namespace tpc {
 
 constexpr int kTrackletThreads = 128;
-constexpr int kTrackletBlocksPerSm = 6;  // registers per thread <= 65536 / (128 * 6) = 85
+constexpr int kFitBlocksPerSm = 8;     // k_trk_chain, k_trk_refit: registers per thread <= 65536 / (128 * 8) = 64
+constexpr int kSearchBlocksPerSm = 6;  // k_trk_up, k_trk_finish:  <= 85
 
 struct TrackState {
   float y, z, s, t, q;  // SPEC 5: y, z, sinphi, dz/dl, q/pT
@@ -224,164 +229,295 @@ __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S,
   return bi;
 }
 
-enum Phase { PH_CHAIN = 0, PH_UP = 1, PH_TURN = 2, PH_DOWN = 3, PH_FINISH = 4, PH_ENDED = 5, PH_FETCH = 6, PH_EXIT = 7 };
 
 constexpr uint32_t kNoHit = 0xFFFFFFFFu;  // row map entry of a row without a hit
-constexpr int kClaimChunks = 5;           // 32-row chunks of a map row claimed per round (159 rows = 5 chunks)
 
-template <bool COUNT>
-__global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_tracklets(const Ctx c) {
-  extern __shared__ __align__(16) float sX[];  // [n_rows] x of the pad rows
-  constexpr unsigned FULL = 0xffffffffu;
-  const int n_rows = c.n_rows, nthr = (int)blockDim.x, tid = (int)threadIdx.x, lane = tid & 31;
-  for (int r = tid; r < n_rows; r += nthr) sX[r] = c.X[r];
-  __syncthreads();
-  const uint32_t n_trk = *c.n_tracklets;
-  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
-  const int max_gap = c.prm.max_row_gap, min_hits = c.prm.min_track_hits;
+// Tracklet record (Ctx::trk_rec), 32 words: [0] x, [1..5] p, [6..20] C, [21] chi2, [22] ndf, [23] nHits,
+// [24] firstRow, [25] lastRow, [26] rows packed (below), [27] task*n_rows, [28] ia, [29] ib, [30..31] unused.
+// Words 0..25 are what the selector and the output read once k_trk_finish has stored them; between the
+// kernels the record carries the tracklet.
+//   pack = row_cur | (r_down + 1) << 10 | r0 << 20 | skip_up << 30       (n_rows <= 1024)
+// row_cur = row the state is at, r_down = next row of the down pass (-1: none left), r0 = row of the start
+// hit, skip_up = the chain fit ended with a failed transport (K2 -> K4).
+//   ia, ib: what the next kernel would otherwise have to load after the record (a second round trip):
+//   chain -> up: ia = hit of lastRow;  up -> refit: ia = map[r_down], ib = map[r_down - 1];
+//   refit -> finish: ia = map[r_down]   (kNoHit where the row is below r0)
+__device__ __forceinline__ uint32_t pack_rows(int row_cur, int r_down, int r0, bool skip_up) {
+  return (uint32_t)row_cur | ((uint32_t)(r_down + 1) << 10) | ((uint32_t)r0 << 20) | (skip_up ? 1u << 30 : 0u);
+}
+__device__ __forceinline__ void store_rec(float4* rec, const TrackState& S, float x, int n_hits, int first_row,
+                                          int last_row, uint32_t pack, uint32_t tr_base, uint32_t ia, uint32_t ib) {
+  rec[0] = make_float4(x, S.y, S.z, S.s);
+  rec[1] = make_float4(S.t, S.q, S.c00, S.c10);
+  rec[2] = make_float4(S.c11, S.c20, S.c21, S.c22);
+  rec[3] = make_float4(S.c30, S.c31, S.c32, S.c33);
+  rec[4] = make_float4(S.c40, S.c41, S.c42, S.c43);
+  rec[5] = make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits));
+  rec[6] = make_float4(__int_as_float(first_row), __int_as_float(last_row), __uint_as_float(pack),
+                       __uint_as_float(tr_base));
+  rec[7] = make_float4(__uint_as_float(ia), __uint_as_float(ib), 0.0f, 0.0f);
+}
+// rec: the lane's shared-memory copy of the record
+__device__ __forceinline__ void load_rec(const float4* rec, TrackState& S, int& n_hits, int& first_row,
+                                         int& last_row, uint32_t& pack, uint32_t& tr_base, uint32_t& ia,
+                                         uint32_t& ib) {
+  const float4 a0 = rec[0], a1 = rec[1], a2 = rec[2], a3 = rec[3], a4 = rec[4], a5 = rec[5], a6 = rec[6], a7 = rec[7];
+  S.y = a0.y; S.z = a0.z; S.s = a0.w;
+  S.t = a1.x; S.q = a1.y; S.c00 = a1.z; S.c10 = a1.w;
+  S.c11 = a2.x; S.c20 = a2.y; S.c21 = a2.z; S.c22 = a2.w;
+  S.c30 = a3.x; S.c31 = a3.y; S.c32 = a3.z; S.c33 = a3.w;
+  S.c40 = a4.x; S.c41 = a4.y; S.c42 = a4.z; S.c43 = a4.w;
+  S.c44 = a5.x; S.chi2 = a5.y; S.ndf = __float_as_int(a5.z); n_hits = __float_as_int(a5.w);
+  first_row = __float_as_int(a6.x); last_row = __float_as_int(a6.y);
+  pack = __float_as_uint(a6.z); tr_base = __float_as_uint(a6.w);
+  ia = __float_as_uint(a7.x); ib = __float_as_uint(a7.y);
+}
 
-  TrackState S;
+// ---- the queue of a tracklet kernel -------------------------------------------------------------------
+// Tickets are drawn kPoolBatch at a time per warp (one atomic per batch instead of one per fetch); the
+// lanes in `need` get consecutive tickets.  A ticket >= the number of tracklets means the queue is empty.
+constexpr uint32_t kPoolBatch = 32;
+struct TicketPool { uint32_t next, end; };
+__device__ __forceinline__ uint32_t pool_take(TicketPool& p, uint32_t* head, unsigned need, int lane) {
+  const uint32_t cnt = (uint32_t)__popc(need), have = p.end - p.next;
+  const uint32_t rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
+  if (cnt <= have) {
+    const uint32_t tk = p.next + rank;
+    p.next += cnt;
+    return tk;
+  }
+  uint32_t base = 0u;
+  if (lane == 0) base = atomicAdd(head, kPoolBatch);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  const uint32_t tk = rank < have ? p.next + rank : base + (rank - have);
+  p.next = base + (cnt - have);
+  p.end = base + kPoolBatch;
+  return tk;
+}
+// Asynchronous copy of n16 x 16 bytes, global -> this lane's slot in shared memory (no register is the
+// target, so the warp goes on; the lane reads the slot one loop iteration later).
+__device__ __forceinline__ void prefetch_slot(void* slot, const void* src, int n16) {
+  const uint32_t d = smem_u32(slot);
+  for (int k = 0; k < n16; ++k)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + 16u * (uint32_t)k),
+                 "l"(reinterpret_cast<const char*>(src) + 16 * k)
+                 : "memory");
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void prefetch_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+enum LaneState { LN_IDLE = 0, LN_RUN = 1, LN_EXIT = 2 };
+enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };  // ISSUED this iteration, READY from the next on
+
+// The fetch protocol of a lane, the same in all four kernels (macro-free: three calls per loop iteration):
+//   fetch_request: lanes that are idle, or run the last step of their tracklet (`ending`), and have nothing
+//                  requested draw a ticket and start the copy of that tracklet's record to their slot;
+//   (the kernel's own "consume" block turns an idle lane with a READY slot into a running one);
+//   fetch_advance: ISSUED -> READY at the end of the iteration.
+__device__ __forceinline__ void fetch_request(TicketPool& pool, uint32_t* head, bool want, int lane, uint32_t n_trk,
+                                              int& pf, uint32_t& t_next, void* slot, const void* src_base,
+                                              size_t src_stride, int n16) {
+  const unsigned need = __ballot_sync(0xffffffffu, want);
+  if (need) {
+    const uint32_t tk = pool_take(pool, head, need, lane);
+    if (want) {
+      if (tk >= n_trk) {
+        pf = PF_DRAINED;
+      } else {
+        t_next = tk;
+        prefetch_slot(slot, reinterpret_cast<const char*>(src_base) + (size_t)tk * src_stride, n16);
+        pf = PF_ISSUED;
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void zero_state(TrackState& S) {
   S.y = S.z = S.s = S.t = S.q = 0.0f;
   S.c00 = S.c10 = S.c11 = S.c20 = S.c21 = S.c22 = S.c30 = S.c31 = S.c32 = S.c33 = 0.0f;
   S.c40 = S.c41 = S.c42 = S.c43 = S.c44 = 0.0f;
   S.chi2 = 0.0f; S.ndf = -5;
-  uint32_t t = 0u, tr_base = 0u, gid0 = 0u;
-  uint32_t* map = c.trk_hits;  // row map of the running tracklet
-  int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
-  int32_t last_hit = -1, next_chain = -1;
-  uint32_t map_next = kNoHit;  // down pass: map[r_down], loaded one step ahead
-  int phase = PH_FETCH;
-  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_chain = 0u, n_kept = 0u, n_kept_hits = 0u;
+}
 
+// shared memory of a tracklet kernel: [n_rows floats, padded to 16 bytes][blockDim.x slots of SLOT16 x 16 bytes]
+__host__ __device__ inline size_t trk_smem_bytes(int n_rows, int slot16) {
+  return (size_t)((n_rows + 3) & ~3) * sizeof(float) + (size_t)kTrackletThreads * slot16 * 16;
+}
+
+// ---------------------------------------------------------------------------
+// K1 seed + K2 chain fit.  Every step: transport one row up, update with the chain hit.  The hit two links
+// ahead and the (y,z) of the next one are requested before the transport, so no step waits for a load.
+// ---------------------------------------------------------------------------
+constexpr int kChainSlot16 = kSeedU4;
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain(const Ctx c) {
+  extern __shared__ __align__(16) float sX[];  // [n_rows] x of the pad rows, then the slots
+  constexpr unsigned FULL = 0xffffffffu;
+  const int n_rows = c.n_rows, lane = (int)threadIdx.x & 31;
+  uint4* slot = reinterpret_cast<uint4*>(sX + ((n_rows + 3) & ~3)) + (size_t)threadIdx.x * kChainSlot16;
+  for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
+  __syncthreads();
+  const uint32_t n_trk = *c.n_tracklets;
+  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
+  TrackState S;
+  zero_state(S);
+  uint32_t t = 0u, t_next = 0u, tr_base = 0u;
+  uint32_t* map = c.trk_hits;
+  int r0 = 0, row_cur = 0, n_hits = 0;
+  int32_t h_cur = -1, h_next = -1, h_last = -1;  // chain hit of the next step, the one after it, the last one fitted
+  float2 p_cur = make_float2(0.0f, 0.0f);
+  int st = LN_IDLE, pf = PF_NONE;
+  TicketPool pool{0u, 0u};
+  uint32_t n_steps = 0u, n_chain = 0u;
   while (true) {
-    // (A) tracklets that ended in the last step: the warp claims their hits one tracklet at a time
-    //     (K7 ownership, 32 rows of the map per round), the lane stores the record
-    unsigned ended = __ballot_sync(FULL, phase == PH_ENDED);
-    if (ended) __syncwarp();  // the map rows written by the ended lanes are read by the other lanes below
-    while (ended) {
-      const int L = __ffs(ended) - 1;
-      ended &= ended - 1u;
-      const int fn = __shfl_sync(FULL, n_hits, L);
-      if (fn >= min_hits) {  // K6, K7: longest tracklet wins, then the smaller start-hit gid
-        const uint32_t ft = __shfl_sync(FULL, t, L), fgid0 = __shfl_sync(FULL, gid0, L);
-        const int ffirst = __shfl_sync(FULL, first_row, L), flast = __shfl_sync(FULL, last_row, L);
-        const unsigned long long key = ((unsigned long long)(uint32_t)fn << 32) | (unsigned long long)(0xFFFFFFFFu - fgid0);
-        const uint32_t* fmap = c.trk_hits + (size_t)ft * map_stride(n_rows);
-        for (int rb = ffirst; rb <= flast; rb += 32 * kClaimChunks) {  // the map loads of a round together, then the claims
-          uint32_t idx[kClaimChunks];
-#pragma unroll
-          for (int q = 0; q < kClaimChunks; ++q) {
-            const int r = rb + 32 * q + lane;
-            idx[q] = r <= flast ? fmap[r] : kNoHit;
-          }
-#pragma unroll
-          for (int q = 0; q < kClaimChunks; ++q)
-            if (idx[q] != kNoHit) atomicMax(&c.owner[idx[q]], key);
-        }
-      }
-      if (lane == L) {
-        float4* rec = c.trk_rec + (size_t)t * kRecFloat4;
-        rec[0] = make_float4(sX[row_cur], S.y, S.z, S.s);
-        rec[1] = make_float4(S.t, S.q, S.c00, S.c10);
-        rec[2] = make_float4(S.c11, S.c20, S.c21, S.c22);
-        rec[3] = make_float4(S.c30, S.c31, S.c32, S.c33);
-        rec[4] = make_float4(S.c40, S.c41, S.c42, S.c43);
-        rec[5] = make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits));
-        rec[6] = make_float4(__int_as_float(first_row), __int_as_float(last_row), 0.0f, 0.0f);
-        if (COUNT && n_hits >= min_hits) { ++n_kept; n_kept_hits += (uint32_t)n_hits; }
-        phase = PH_FETCH;
+    fetch_request(pool, &c.tickets[2], (st == LN_IDLE || (st == LN_RUN && h_next < 0)) && pf == PF_NONE, lane, n_trk,
+                  pf, t_next, slot, c.trk_seed, sizeof(uint4) * kSeedU4, kChainSlot16);
+    if (st == LN_IDLE) {
+      if (pf == PF_READY) {
+        prefetch_wait();
+        const uint4 q0 = slot[0], q1 = slot[1], q2 = slot[2];
+        t = t_next;
+        const uint32_t tr0 = q0.y;
+        const uint32_t task = tr0 / (uint32_t)n_rows;
+        r0 = (int)(tr0 - task * (uint32_t)n_rows);
+        tr_base = task * (uint32_t)n_rows;
+        map = c.trk_hits + (size_t)t * map_stride(n_rows);
+        h_last = (int32_t)q0.z;
+        h_cur = (int32_t)q0.w;
+        h_next = (int32_t)q2.w;
+        p_cur = make_float2(__uint_as_float(q2.x), __uint_as_float(q2.y));
+        const float y0s = __uint_as_float(q1.x), z0s = __uint_as_float(q1.y);
+        const float y1s = __uint_as_float(q1.z), z1s = __uint_as_float(q1.w);
+        const float dx = sX[r0 + 1] - sX[r0], dy = y1s - y0s, dz = z1s - z0s;       // K1
+        const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
+        S.y = y1s; S.z = z1s; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
+        S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
+        S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
+        S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
+        S.chi2 = 0.0f; S.ndf = -5;
+        map[r0] = q0.x;
+        map[r0 + 1] = q0.z;
+        row_cur = r0 + 1; n_hits = 2;
+        if (COUNT) n_chain += 2u;
+        st = LN_RUN; pf = PF_NONE;
+      } else if (pf == PF_DRAINED) {
+        st = LN_EXIT;
       }
     }
-    // (B) lanes without a tracklet take the next ones from the queue (K1 seed); the seed record of a4
-    //     holds everything the seed needs, so a new tracklet costs one round of loads
-    const unsigned need = __ballot_sync(FULL, phase == PH_FETCH);
-    if (need) {
-      uint32_t base = 0u;
-      if (lane == 0) base = atomicAdd(&c.tickets[2], (uint32_t)__popc(need));
-      base = __shfl_sync(FULL, base, 0);
-      if (phase == PH_FETCH) {
-        t = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
-        if (t >= n_trk) {
-          phase = PH_EXIT;
-        } else {
-          const uint4* sr = c.trk_seed + (size_t)t * kSeedU4;
-          const uint4 q0 = __ldg(sr), q1 = __ldg(sr + 1), q2 = __ldg(sr + 2);
-          const uint32_t tr0 = q0.y;
-          const uint32_t task = tr0 / (uint32_t)n_rows;
-          r0 = (int)(tr0 - task * (uint32_t)n_rows);
-          tr_base = task * (uint32_t)n_rows;
-          gid0 = q2.z;
-          map = c.trk_hits + (size_t)t * map_stride(n_rows);
-          const float y0s = __uint_as_float(q1.x), z0s = __uint_as_float(q1.y);
-          const float y1s = __uint_as_float(q1.z), z1s = __uint_as_float(q1.w);
-          const float dx = sX[r0 + 1] - sX[r0], dy = y1s - y0s, dz = z1s - z0s;
-          const float ri = 1.0f / sqrtf(dx * dx + dy * dy);
-          S.y = y1s; S.z = z1s; S.s = dy * ri; S.t = dz * ri; S.q = 0.0f;
-          S.c00 = sy2; S.c10 = 0.0f; S.c11 = sz2; S.c20 = 0.0f; S.c21 = 0.0f; S.c22 = c.prm.c0_sinphi;
-          S.c30 = 0.0f; S.c31 = 0.0f; S.c32 = 0.0f; S.c33 = c.prm.c0_dzds;
-          S.c40 = 0.0f; S.c41 = 0.0f; S.c42 = 0.0f; S.c43 = 0.0f; S.c44 = c.prm.c0_qpt;
-          S.chi2 = 0.0f; S.ndf = -5;
-          map[r0] = q0.x;
-          map[r0 + 1] = q0.z;
-          row_cur = r0 + 1; first_row = r0; last_row = r0 + 1; n_hits = 2; gap = 0; r_down = 0;
-          last_hit = (int32_t)q0.z;
-          next_chain = (int32_t)q0.w;
-          phase = next_chain >= 0 ? PH_CHAIN : PH_UP;
-          if (COUNT) n_chain += 2u;
-        }
+    if (pf == PF_ISSUED) pf = PF_READY;
+    if (__ballot_sync(FULL, st != LN_EXIT) == 0u) break;
+    bool ok = true;
+    const bool step = st == LN_RUN && h_cur >= 0;
+    int32_t h_n2 = -1;
+    float2 p_next = make_float2(0.0f, 0.0f);
+    if (step) {                                                        // K2
+      if (h_next >= 0) { p_next = c.yz[h_next]; h_n2 = c.clean_up[h_next]; }
+      ok = transport(S, sX[row_cur + 1] - sX[row_cur], a, max_sin);
+      if (COUNT) ++n_steps;
+    }
+    __syncwarp();
+    if (step && ok) {
+      update_hit(S, p_cur.x, p_cur.y, sy2, sz2);
+      ++row_cur;
+      map[row_cur] = (uint32_t)h_cur;
+      ++n_hits;
+      if (COUNT) ++n_chain;
+      h_last = h_cur;
+      h_cur = h_next; p_cur = p_next; h_next = h_n2;
+    }
+    if (st == LN_RUN && (h_cur < 0 || !ok)) {  // end of the chain, or K2's failed transport (-> K4, no up pass)
+      store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, r0, row_cur,
+                pack_rows(row_cur, row_cur - 1, r0, !ok), tr_base, (uint32_t)h_last, 0u);
+      st = LN_IDLE;
+    }
+  }
+  if (COUNT) {
+    atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
+    atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// K3 up pass + K4 turn-around.  Every step of the up pass searches; the turn-around is the same step
+// shape (transport to lastRow, no search, update with the hit of lastRow), so it runs with the others.
+// ---------------------------------------------------------------------------
+constexpr int kRecSlot16 = kRecFloat4;
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up(const Ctx c) {
+  extern __shared__ __align__(16) float sX[];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int n_rows = c.n_rows, lane = (int)threadIdx.x & 31;
+  float4* slot = reinterpret_cast<float4*>(sX + ((n_rows + 3) & ~3)) + (size_t)threadIdx.x * kRecSlot16;
+  for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
+  __syncthreads();
+  const uint32_t n_trk = *c.n_tracklets;
+  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
+  const int max_gap = c.prm.max_row_gap;
+  TrackState S;
+  zero_state(S);
+  uint32_t t = 0u, t_next = 0u, tr_base = 0u;
+  uint32_t* map = c.trk_hits;
+  int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0;
+  int32_t last_hit = -1;
+  bool turn = false;  // this lane's next step is the turn-around (its last step here)
+  int st = LN_IDLE, pf = PF_NONE;
+  TicketPool pool{0u, 0u};
+  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u;
+  while (true) {
+    if (st == LN_RUN && row_cur + 1 >= n_rows) turn = true;            // K3 ran off the last row
+    fetch_request(pool, &c.tickets[3], (st == LN_IDLE || (st == LN_RUN && turn)) && pf == PF_NONE, lane, n_trk, pf,
+                  t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
+    if (st == LN_IDLE) {
+      if (pf == PF_READY) {
+        prefetch_wait();
+        uint32_t pack, ia, ib;
+        load_rec(slot, S, n_hits, first_row, last_row, pack, tr_base, ia, ib);
+        t = t_next;
+        row_cur = (int)(pack & 1023u); r0 = (int)((pack >> 20) & 1023u);
+        map = c.trk_hits + (size_t)t * map_stride(n_rows);
+        last_hit = (int32_t)ia;
+        turn = (((pack >> 30) & 1u) != 0u) | (row_cur + 1 >= n_rows);
+        gap = 0;
+        st = LN_RUN; pf = PF_NONE;
+      } else if (pf == PF_DRAINED) {
+        st = LN_EXIT;
       }
     }
-    if (__ballot_sync(FULL, phase != PH_EXIT) == 0u) break;
-    // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping.
-    //     The parts are separated by warp barriers so that the lanes run each of them together
-    //     whatever their phase is.
+    if (pf == PF_ISSUED) pf = PF_READY;
+    if (__ballot_sync(FULL, st != LN_EXIT) == 0u) break;
+    const bool run = st == LN_RUN;
     int rt = 0;
     int32_t hit = -1;
     float2 hp = make_float2(0.0f, 0.0f);
-    bool book = false, do_search = false;
+    bool do_search = false, p_turn = false;
+    uint32_t ia = kNoHit, ib = kNoHit;  // turn-around: map[lastRow - 1], map[lastRow - 2] for the refit kernel
     RowInfo g;
     g.inv = 0.0f; g.y0 = 0.0f; g.z0 = 0.0f; g.ny_nz = 0u; g.bins_off = 0u; g.row_lo = 0u; g.pad0 = 0u; g.pad1 = 0u;
-    if (phase <= PH_FINISH) {
-      if (phase == PH_UP && row_cur + 1 >= n_rows) phase = PH_TURN;     // K3 ran off the last row
-      if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
-      const bool p_chain = phase == PH_CHAIN, p_turn = phase == PH_TURN, p_down = phase == PH_DOWN;
-      rt = phase <= PH_UP ? row_cur + 1 : (p_turn ? last_row : (p_down ? r_down : first_row));
-      // Every load of this step whose address does not depend on the transported state is issued here,
-      // before the transport: the hit when it is known already (chain link, lastRow hit at the turn, row
-      // map entry fetched a step ago), the next chain link, the map entry of the next down row, and the
-      // row's grid header when a search may follow.
-      const int32_t known = p_chain ? next_chain
-                                    : (p_turn ? last_hit : ((p_down & (map_next != kNoHit)) ? (int32_t)map_next : -1));
-      if (known >= 0) hp = c.yz[known];
-      if (phase == PH_CHAIN) next_chain = c.clean_up[known];            // K2: the link after this one
-      if (phase == PH_TURN || phase == PH_DOWN) {                       // map entry of the row after this one
-        const int rn = (phase == PH_TURN ? last_row : rt) - 1;
-        map_next = rn >= r0 ? map[rn] : kNoHit;
+    if (run) {
+      p_turn = turn;
+      rt = p_turn ? last_row : row_cur + 1;
+      if (p_turn) {
+        hp = c.yz[last_hit];
+        if (last_row - 1 >= r0) ia = map[last_row - 1];
+        if (last_row - 2 >= r0) ib = map[last_row - 2];
+      } else {
+        g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
       }
-      if (phase == PH_UP || (phase == PH_DOWN && known < 0)) g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
       bool ok = true;
       if (rt != row_cur) {
         ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
         if (ok) row_cur = rt;
-        if (COUNT && phase != PH_TURN && phase != PH_FINISH) ++n_steps;
+        if (COUNT && !p_turn) ++n_steps;
       }
-      // what the step does next, by phase, without branches (the lanes of a warp are in different passes)
-      const bool p_fin = phase == PH_FINISH;
-      if (p_turn) {                                                       // K4: C <- C * turn_cov_scale (once per tracklet)
+      if (p_turn) {                                                    // K4: C <- C * turn_cov_scale
         const float f = c.prm.turn_cov_scale;
         S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
         S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
+        S.chi2 = 0.0f; S.ndf = -5;
+        hit = row_cur == last_row ? last_hit : -1;                     // the hit of lastRow opens the down pass
       }
-      S.chi2 = p_turn ? 0.0f : S.chi2;
-      S.ndf = p_turn ? -5 : S.ndf;
-      gap = p_turn ? 0 : gap;
-      r_down = p_turn ? last_row - 1 : r_down;
-      book = ok & !p_fin & !p_turn;                                       // K2, K3, K5 with the transport done
-      do_search = book & ((phase == PH_UP) | (known < 0));                // K3, K5 without a map entry
-      // the hit is known: K2, K5 with a map entry, K4 (the lastRow hit opens the down pass)
-      hit = ((book & !do_search) | (p_turn & (row_cur == last_row))) ? known : -1;
-      // K6 finish -> ended; K4 -> down pass; failed transport: K2/K3 -> turn-around, K5 -> finish
-      phase = p_fin ? PH_ENDED : (p_turn ? PH_DOWN : (ok ? phase : (p_down ? PH_FINISH : PH_TURN)));
+      do_search = ok & !p_turn;
+      turn = turn | !ok;                                               // K3: failed transport -> turn-around
     }
     __syncwarp();
     if (do_search) {
@@ -391,27 +527,229 @@ __global__ void __launch_bounds__(kTrackletThreads, kTrackletBlocksPerSm) k_trac
     __syncwarp();
     if (hit >= 0) update_hit(S, hp.x, hp.y, sy2, sz2);
     __syncwarp();
-    if (book) {  // chain fit, up pass or down pass, transport done: record the row, count hits and gaps (no branches:
-                 // the lanes of a warp are in different passes)
-      const bool is_up = phase == PH_UP, is_dn = phase == PH_DOWN, got = hit >= 0;
-      const bool decided = !is_dn | do_search;                  // this step decided the row's map entry
-      const bool gap_row = is_up | (is_dn & do_search & (rt < first_row));  // rows whose hits / misses drive the gap
-      if (decided) map[rt] = (uint32_t)hit;                     // -1 = kNoHit
-      n_hits += (decided & got) ? 1 : 0;
-      if (COUNT && phase == PH_CHAIN) ++n_chain;
-      if (!is_dn & got) { last_row = rt; last_hit = hit; }
-      if (gap_row & got & is_dn) first_row = rt;
-      gap = gap_row ? (got ? 0 : gap + 1) : gap;
-      if (gap_row & !got & (gap > max_gap)) phase = is_up ? PH_TURN : PH_FINISH;   // K3 / K5 stop
-      if (phase == PH_CHAIN && next_chain < 0) { phase = PH_UP; gap = 0; }          // K2 -> K3
-      r_down -= is_dn ? 1 : 0;
+    if (do_search) {                                                   // K3 bookkeeping
+      const bool got = hit >= 0;
+      map[rt] = (uint32_t)hit;                                         // -1 = kNoHit
+      n_hits += got ? 1 : 0;
+      last_row = got ? rt : last_row;
+      last_hit = got ? hit : last_hit;
+      gap = got ? 0 : gap + 1;
+      turn = turn | (gap > max_gap);
+    }
+    if (p_turn) {
+      store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
+                pack_rows(row_cur, last_row - 1, r0, false), tr_base, ia, ib);
+      st = LN_IDLE;
     }
   }
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
     atomicAdd(&c.counters[CN_CANDIDATES], (unsigned long long)n_cand);
-    atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
+    atomicAdd(&c.counters[CN_SEARCHES_UP], (unsigned long long)n_search);
+    atomicAdd(&c.counters[CN_CANDIDATES_UP], (unsigned long long)n_cand);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// K5, first part: the down pass as long as the row has a hit in the map (no search): transport one row
+// down, update with the hit.  Map entry two rows ahead and (y,z) one row ahead are requested before the
+// transport.  The lane stops in front of the first row without a hit (a hole of the map, or firstRow - 1)
+// or of a transport that fails; k_trk_finish goes on from there.
+// ---------------------------------------------------------------------------
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit(const Ctx c) {
+  extern __shared__ __align__(16) float sX[];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int n_rows = c.n_rows, lane = (int)threadIdx.x & 31;
+  float4* slot = reinterpret_cast<float4*>(sX + ((n_rows + 3) & ~3)) + (size_t)threadIdx.x * kRecSlot16;
+  for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
+  __syncthreads();
+  const uint32_t n_trk = *c.n_tracklets;
+  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
+  TrackState S;
+  zero_state(S);
+  uint32_t t = 0u, t_next = 0u, tr_base = 0u;
+  const uint32_t* map = c.trk_hits;
+  int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, r_down = 0;
+  uint32_t m_cur = kNoHit, m_next = kNoHit;  // map[r_down], map[r_down - 1]
+  float2 p_cur = make_float2(0.0f, 0.0f);
+  int st = LN_IDLE, pf = PF_NONE;
+  TicketPool pool{0u, 0u};
+  uint32_t n_steps = 0u;
+  while (true) {
+    fetch_request(pool, &c.tickets[4], (st == LN_IDLE || (st == LN_RUN && m_next == kNoHit)) && pf == PF_NONE, lane,
+                  n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
+    if (st == LN_IDLE) {
+      if (pf == PF_READY) {
+        prefetch_wait();
+        uint32_t pack;
+        load_rec(slot, S, n_hits, first_row, last_row, pack, tr_base, m_cur, m_next);
+        t = t_next;
+        row_cur = (int)(pack & 1023u); r_down = (int)((pack >> 10) & 1023u) - 1; r0 = (int)((pack >> 20) & 1023u);
+        map = c.trk_hits + (size_t)t * map_stride(n_rows);
+        if (m_cur != kNoHit) p_cur = c.yz[m_cur];  // needed after the first transport only
+        st = LN_RUN; pf = PF_NONE;
+      } else if (pf == PF_DRAINED) {
+        st = LN_EXIT;
+      }
+    }
+    if (pf == PF_ISSUED) pf = PF_READY;
+    if (__ballot_sync(FULL, st != LN_EXIT) == 0u) break;
+    bool ok = true;
+    const bool step = st == LN_RUN && m_cur != kNoHit;
+    uint32_t m_n2 = kNoHit;
+    float2 p_next = make_float2(0.0f, 0.0f);
+    if (step) {
+      if (m_next != kNoHit) p_next = c.yz[m_next];
+      if (r_down - 2 >= r0) m_n2 = map[r_down - 2];
+      ok = transport(S, sX[r_down] - sX[row_cur], a, max_sin);
+    }
+    __syncwarp();
+    if (step && ok) {
+      update_hit(S, p_cur.x, p_cur.y, sy2, sz2);
+      if (COUNT) ++n_steps;
+      row_cur = r_down;
+      --r_down;
+      m_cur = m_next; p_cur = p_next; m_next = m_n2;
+    }
+    if (st == LN_RUN && (m_cur == kNoHit || !ok)) {
+      store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
+                pack_rows(row_cur, r_down, r0, false), tr_base, m_cur, 0u);
+      st = LN_IDLE;
+    }
+  }
+  if (COUNT) {
+    atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
+    atomicAdd(&c.counters[CN_REFIT_STEPS], (unsigned long long)n_steps);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// K5, rest: rows below firstRow (every step searches) and what follows a hole of the map inside
+// [firstRow, lastRow] (search in the hole, known hits after it); K6 finish (the same step shape: transport to
+// firstRow, nothing else).  K7 (ownership) is k_resolve in stage_output.cuh.
+// ---------------------------------------------------------------------------
+enum Phase { PH_DOWN = 0, PH_FINISH = 1, PH_ENDED = 2, PH_IDLE = 3, PH_EXIT = 4 };
+constexpr int kFinishSlot16 = kRecFloat4 + 1;  // the record and the third quarter of the seed record (gid of the start hit)
+
+template <bool COUNT>
+__global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_finish(const Ctx c) {
+  extern __shared__ __align__(16) float sX[];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int n_rows = c.n_rows, lane = (int)threadIdx.x & 31;
+  float4* slot = reinterpret_cast<float4*>(sX + ((n_rows + 3) & ~3)) + (size_t)threadIdx.x * kFinishSlot16;
+  for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
+  __syncthreads();
+  const uint32_t n_trk = *c.n_tracklets;
+  const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
+  const int max_gap = c.prm.max_row_gap;
+  [[maybe_unused]] const int min_hits = c.prm.min_track_hits;
+  TrackState S;
+  zero_state(S);
+  uint32_t t = 0u, t_next = 0u, tr_base = 0u, gid0 = 0u;
+  uint32_t* map = c.trk_hits;
+  int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
+  uint32_t map_next = kNoHit;  // map[r_down], loaded one step ahead
+  int phase = PH_IDLE, pf = PF_NONE;
+  TicketPool pool{0u, 0u};
+  uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_kept = 0u, n_kept_hits = 0u;
+  while (true) {
+    // (A) tracklets that ended in the last step: the record, and what the ownership kernel (K7) needs
+    if (phase == PH_ENDED) {
+      store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, sX[row_cur], n_hits, first_row, last_row, 0u, tr_base, 0u, 0u);
+      c.trk_meta[t] = make_uint4((uint32_t)n_hits, (uint32_t)first_row | ((uint32_t)last_row << 16), gid0, 0u);
+      if (COUNT && n_hits >= min_hits) { ++n_kept; n_kept_hits += (uint32_t)n_hits; }
+      phase = PH_IDLE;
+    }
+    // (B) the next tracklets: requested while the lane runs its finish step, taken over here
+    {
+      const bool want = (phase == PH_IDLE || phase == PH_FINISH || (phase == PH_DOWN && r_down < 0)) && pf == PF_NONE;
+      const unsigned need = __ballot_sync(FULL, want);
+      if (need) {
+        const uint32_t tk = pool_take(pool, &c.tickets[5], need, lane);
+        if (want) {
+          if (tk >= n_trk) {
+            pf = PF_DRAINED;
+          } else {
+            t_next = tk;
+            prefetch_slot(slot, c.trk_rec + (size_t)tk * kRecFloat4, kRecFloat4);
+            prefetch_slot(slot + kRecFloat4, c.trk_seed + (size_t)tk * kSeedU4 + 2, 1);
+            pf = PF_ISSUED;
+          }
+        }
+      }
+    }
+    if (phase == PH_IDLE) {
+      if (pf == PF_READY) {
+        prefetch_wait();
+        uint32_t pack, ib;
+        load_rec(slot, S, n_hits, first_row, last_row, pack, tr_base, map_next, ib);
+        gid0 = __float_as_uint(slot[kRecFloat4].z);
+        t = t_next;
+        row_cur = (int)(pack & 1023u); r_down = (int)((pack >> 10) & 1023u) - 1; r0 = (int)((pack >> 20) & 1023u);
+        map = c.trk_hits + (size_t)t * map_stride(n_rows);
+        gap = 0;
+        phase = PH_DOWN; pf = PF_NONE;
+      } else if (pf == PF_DRAINED) {
+        phase = PH_EXIT;
+      }
+    }
+    if (pf == PF_ISSUED) pf = PF_READY;
+    if (__ballot_sync(FULL, phase != PH_EXIT) == 0u) break;
+    // (C) one row step of every running lane: transport -> choose the hit -> update -> bookkeeping
+    int rt = 0;
+    int32_t hit = -1;
+    float2 hp = make_float2(0.0f, 0.0f);
+    bool book = false, do_search = false;
+    RowInfo g;
+    g.inv = 0.0f; g.y0 = 0.0f; g.z0 = 0.0f; g.ny_nz = 0u; g.bins_off = 0u; g.row_lo = 0u; g.pad0 = 0u; g.pad1 = 0u;
+    if (phase <= PH_FINISH) {
+      if (phase == PH_DOWN && r_down < 0) phase = PH_FINISH;            // K5 ran off row 0
+      const bool p_down = phase == PH_DOWN, p_fin = phase == PH_FINISH;
+      rt = p_down ? r_down : first_row;
+      const int32_t known = (p_down & (map_next != kNoHit)) ? (int32_t)map_next : -1;
+      if (known >= 0) hp = c.yz[known];
+      if (p_down) {                                                     // map entry of the row after this one
+        const int rn = rt - 1;
+        map_next = rn >= r0 ? map[rn] : kNoHit;
+      }
+      if (p_down && known < 0) g = load_row_info(&c.rowinfo[tr_base + (uint32_t)rt]);
+      bool ok = true;
+      if (rt != row_cur) {
+        ok = transport(S, sX[rt] - sX[row_cur], a, max_sin);
+        if (ok) row_cur = rt;
+        if (COUNT && p_down) ++n_steps;
+      }
+      book = ok & p_down;
+      do_search = book & (known < 0);
+      hit = (book & !do_search) ? known : -1;
+      // K6 finish -> ended; failed transport in K5 -> finish
+      phase = p_fin ? PH_ENDED : (ok ? phase : PH_FINISH);
+    }
+    __syncwarp();
+    if (do_search) {
+      if (COUNT) ++n_search;
+      hit = search_row<COUNT>(c, S, g, hp, n_cand);
+    }
+    __syncwarp();
+    if (hit >= 0) update_hit(S, hp.x, hp.y, sy2, sz2);
+    __syncwarp();
+    if (book) {
+      const bool got = hit >= 0;
+      const bool gap_row = do_search & (rt < first_row);                // rows whose hits / misses drive the gap
+      if (do_search) map[rt] = (uint32_t)hit;                           // -1 = kNoHit
+      n_hits += (do_search & got) ? 1 : 0;
+      if (gap_row & got) first_row = rt;
+      gap = gap_row ? (got ? 0 : gap + 1) : gap;
+      if (gap_row & !got & (gap > max_gap)) phase = PH_FINISH;          // K5 stop
+      --r_down;
+    }
+  }
+  if (COUNT) {
+    atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
+    atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
+    atomicAdd(&c.counters[CN_CANDIDATES], (unsigned long long)n_cand);
     atomicAdd(&c.counters[CN_TRACKLETS_KEPT], (unsigned long long)n_kept);
     atomicAdd(&c.counters[CN_TRACKLET_HITS], (unsigned long long)n_kept_hits);
   }

@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
 
 // ---------------------------------------------------------------------------
 // a3  neighbour cleaner (SPEC 4, C1): clean_up[h] = up[h] iff dn[up[h]] == h.
-// One thread per cluster.  Also clears the ownership words of K7.
+// One thread per cluster.
 // ---------------------------------------------------------------------------
 constexpr int kCleanThreads = 256;
 
@@ -170,7 +170,6 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
   if (i >= c.n) return;
   const int32_t u = c.link_up[i];
   c.clean_up[i] = (u >= 0 && c.link_dn[u] == (int32_t)i) ? u : -1;
-  c.owner[i] = 0ull;
 }
 
 // ---------------------------------------------------------------------------
@@ -191,7 +190,7 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
   const uint32_t tile = s_tile;
   const uint32_t base = tile * kSeedTile + threadIdx.x * kSeedItems;
   uint32_t flags = 0u, n_s1 = 0u;
-  int32_t h1s[kSeedItems], h2s[kSeedItems];
+  int32_t h1s[kSeedItems], h2s[kSeedItems], h3s[kSeedItems];
   // the four cleaned up-links and raw down-links of this thread: one 16-byte load each (arrays are padded)
   int4 cu4 = make_int4(-1, -1, -1, -1), dn4 = make_int4(-1, -1, -1, -1);
   if (base < c.n) {
@@ -202,20 +201,20 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
 #pragma unroll
   for (int k = 0; k < kSeedItems; ++k) {
     const uint32_t i = base + k;
-    h1s[k] = -1; h2s[k] = -1;
+    h1s[k] = -1; h2s[k] = -1; h3s[k] = -1;
     if (i >= c.n) continue;
-    int32_t h = cu[k];
-    if (h < 0) continue;
+    const int32_t h1 = cu[k];
+    if (h1 < 0) continue;
     const int32_t d = dn[k];
     if (d >= 0 && c.link_up[d] == (int32_t)i) continue;  // clean_dn[i] >= 0 (C2): not a start hit
     if (COUNT) ++n_s1;
-    h1s[k] = h;
-    h = c.clean_up[h];
-    h2s[k] = h;
-    int len = 2;
-    while (h >= 0) {
-      if (++len >= c.prm.min_seed_hits) break;
+    const int32_t h2 = c.clean_up[h1];
+    int32_t h = h2 >= 0 ? c.clean_up[h2] : -1;           // h3
+    h1s[k] = h1; h2s[k] = h2; h3s[k] = h;
+    int len = 2 + (h2 >= 0 ? 1 : 0) + (h >= 0 ? 1 : 0);  // S2: hits of the chain, counted up to min_seed_hits
+    while (len < c.prm.min_seed_hits && h >= 0) {
       h = c.clean_up[h];
+      if (h >= 0) ++len;
     }
     if (len >= c.prm.min_seed_hits) flags |= 1u << k;
   }
@@ -235,10 +234,11 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
       const uint32_t h0 = base + k, h1 = (uint32_t)h1s[k];
       const uint32_t tr0 = find_tr(c, h0);
       const float2 p0 = c.yz[h0], p1 = c.yz[h1];
+      const float2 p2 = h2s[k] >= 0 ? c.yz[h2s[k]] : make_float2(0.0f, 0.0f);
       uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
       rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2s[k]);
       rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));
-      rec[2] = make_uint4(h0 - c.row_off[tr0], h1 - c.row_off[tr0 + 1u], c.gid[h0], 0u);
+      rec[2] = make_uint4(__float_as_uint(p2.x), __float_as_uint(p2.y), c.gid[h0], (uint32_t)h3s[k]);
     }
     ++pos;
   }

@@ -30,9 +30,10 @@ struct tpc_tracker {
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
-  // persistent tracklet kernel: [counters off/on] -> blocks that fit the device at once
-  size_t trk_smem = 0;
-  int trk_grid[2] = {0, 0};
+  // persistent tracklet kernels (chain, up, refit, finish): [kernel][counters off/on] -> blocks that fit the device at once
+  int n_sm = 0;
+  size_t trk_smem[4] = {0, 0, 0, 0};
+  int trk_grid[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
   bool timing_on = false;
   // tpc_track_batch_host: one stream per chunk (+ events, pinned headers), created on first use
@@ -69,8 +70,8 @@ uint32_t resolve_max_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tr
 
 // Offsets of every workspace array, in bytes.
 struct Carve {
-  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, owner, trk_seed, trk_hits, trk_rec, zero_begin,
-      scan_seed, scan_out, tickets, n_tracklets, zero_end, total;
+  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
+      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, zero_end, total;
   uint32_t seed_tiles, out_tiles;
 };
 
@@ -87,10 +88,10 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.link_up = take(n4 * sizeof(int32_t));
   c.link_dn = take(n4 * sizeof(int32_t));
   c.clean_up = take(n4 * sizeof(int32_t));
-  c.owner = take(n4 * sizeof(unsigned long long));
   c.trk_seed = take((size_t)T * kSeedU4 * sizeof(uint4));
   c.trk_hits = take((size_t)T * map_stride((int)n_rows) * sizeof(uint32_t));
   c.trk_rec = take((size_t)T * kRecFloat4 * sizeof(float4));
+  c.trk_meta = take((size_t)T * sizeof(uint4));
   c.seed_tiles = (uint32_t)(((size_t)n + kSeedTile - 1) / kSeedTile);
   if (c.seed_tiles == 0) c.seed_tiles = 1;
   c.out_tiles = (uint32_t)(((size_t)T + kOutThreads - 1) / kOutThreads);
@@ -100,6 +101,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.scan_out = take((size_t)c.out_tiles * sizeof(unsigned long long));
   c.tickets = take(8 * sizeof(uint32_t));
   c.n_tracklets = take(sizeof(uint32_t));
+  c.trk_task_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
   c.zero_end = off;
   c.total = off;
   return c;
@@ -131,9 +133,10 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.yz = (float2*)(ws + cv.yz); c.gid = (uint32_t*)(ws + cv.gid); c.bins = (uint32_t*)(ws + cv.bins);
   c.rowinfo = (RowInfo*)(ws + cv.rowinfo);
   c.link_up = (int32_t*)(ws + cv.link_up); c.link_dn = (int32_t*)(ws + cv.link_dn);
-  c.clean_up = (int32_t*)(ws + cv.clean_up); c.owner = (unsigned long long*)(ws + cv.owner);
+  c.clean_up = (int32_t*)(ws + cv.clean_up);
   c.trk_seed = (uint4*)(ws + cv.trk_seed);
   c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
+  c.trk_meta = (uint4*)(ws + cv.trk_meta); c.trk_task_off = (uint32_t*)(ws + cv.trk_task_off);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
   c.max_tracklets = T;
@@ -214,13 +217,22 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute((const void*)k_neighbours<true, kNfListDense>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)nf_smem_bytes(kNfListDense));
-  t->trk_smem = (size_t)t->n_rows * sizeof(float);
-  for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
-    const void* fn = cnt ? (const void*)k_tracklets<true> : (const void*)k_tracklets<false>;
-    int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kTrackletThreads, t->trk_smem);
-    t->trk_grid[cnt] = (per_sm > 0 ? per_sm : 1) * n_sm;
-  }
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute((const void*)k_resolve, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(kResolveChunk * sizeof(unsigned long long)));
+  t->n_sm = n_sm;
+  const int trk_slot16[4] = {kChainSlot16, kRecSlot16, kRecSlot16, kFinishSlot16};
+  for (int k = 0; k < 4; ++k) t->trk_smem[k] = trk_smem_bytes(t->n_rows, trk_slot16[k]);
+  const void* trk_fn[4][2] = {{(const void*)k_trk_chain<false>, (const void*)k_trk_chain<true>},
+                               {(const void*)k_trk_up<false>, (const void*)k_trk_up<true>},
+                               {(const void*)k_trk_refit<false>, (const void*)k_trk_refit<true>},
+                               {(const void*)k_trk_finish<false>, (const void*)k_trk_finish<true>}};
+  for (int k = 0; k < 4; ++k)
+    for (int cnt = 0; cnt < 2 && e == cudaSuccess; ++cnt) {
+      int per_sm = 0;
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trk_fn[k][cnt], kTrackletThreads, t->trk_smem[k]);
+      t->trk_grid[k][cnt] = (per_sm > 0 ? per_sm : 1) * n_sm;
+    }
   if (e != cudaSuccess) {
     const int rc = fail(nullptr, TPC_ERR_CUDA, "tpc_tracker_create: CUDA: %s", cudaGetErrorString(e));
     cudaFree(t->d_tables);
@@ -250,7 +262,7 @@ size_t tpc_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t
   return carve((uint32_t)t->n_rows, max_clusters, max_tasks, T).total;
 }
 
-int tpc_launches_per_batch(const tpc_tracker*) { return 6; }  // a1, a2, a3, a4, a5, a6+a7
+int tpc_launches_per_batch(const tpc_tracker*) { return 11; }  // a1, a2, a3, a4, a5 (4 kernels), K7 (2), a6+a7
 
 void tpc_tracker_enable_counters(tpc_tracker* t, int on) {
   if (t) t->counters_on = on != 0;
@@ -264,7 +276,8 @@ void tpc_tracker_enable_stage_timing(tpc_tracker* t, int on) {
 
 const char* tpc_stage_name(int stage) {
   static const char* const names[TPC_N_STAGES] = {"grid_build", "neighbour_finder", "cleaner", "start_hits",
-                                                  "tracklet_constructor", "selector_output"};
+                                                  "tracklet_chain_fit", "tracklet_up_pass", "tracklet_refit",
+                                                  "tracklet_down_finish", "ownership", "selector_output"};
   return stage >= 0 && stage < TPC_N_STAGES ? names[stage] : nullptr;
 }
 
@@ -362,9 +375,26 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
   else k_seeds<false><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);
   mark();
-  // a5: persistent, as many blocks as the device holds at once
-  if (cnt) k_tracklets<true><<<t->trk_grid[1], kTrackletThreads, t->trk_smem, s>>>(c);
-  else k_tracklets<false><<<t->trk_grid[0], kTrackletThreads, t->trk_smem, s>>>(c);
+  // a5: four persistent kernels, each with as many blocks as the device holds at once
+  if (cnt) k_trk_chain<true><<<t->trk_grid[0][1], kTrackletThreads, t->trk_smem[0], s>>>(c);
+  else k_trk_chain<false><<<t->trk_grid[0][0], kTrackletThreads, t->trk_smem[0], s>>>(c);
+  mark();
+  if (cnt) k_trk_up<true><<<t->trk_grid[1][1], kTrackletThreads, t->trk_smem[1], s>>>(c);
+  else k_trk_up<false><<<t->trk_grid[1][0], kTrackletThreads, t->trk_smem[1], s>>>(c);
+  mark();
+  if (cnt) k_trk_refit<true><<<t->trk_grid[2][1], kTrackletThreads, t->trk_smem[2], s>>>(c);
+  else k_trk_refit<false><<<t->trk_grid[2][0], kTrackletThreads, t->trk_smem[2], s>>>(c);
+  mark();
+  if (cnt) k_trk_finish<true><<<t->trk_grid[3][1], kTrackletThreads, t->trk_smem[3], s>>>(c);
+  else k_trk_finish<false><<<t->trk_grid[3][0], kTrackletThreads, t->trk_smem[3], s>>>(c);
+  mark();
+  if (out->dbg_tracklet_capacity &&  // the row maps before the ownership kernel removes the hits a tracklet loses
+      (out->dbg_tracklet_start || out->dbg_tracklet_nhits || out->dbg_tracklet_map || out->dbg_tracklet_par))
+    k_debug_tracklets<<<(out->dbg_tracklet_capacity + 127) / 128, 128, 0, s>>>(c);
+  if (c.n > 0) {                                                                            // K7 + L1
+    k_task_offsets<<<2 * t->n_sm, 256, 0, s>>>(c);
+    k_resolve<<<(c.n + kResolveChunk - 1) / kResolveChunk, kResolveThreads, kResolveChunk * sizeof(unsigned long long), s>>>(c);
+  }
   mark();
   const size_t keep_smem = (size_t)kOutThreads * ((size_t)(t->n_rows + 31) / 32) * sizeof(uint32_t);
   k_select_output<<<cv.out_tiles, kOutThreads, keep_smem, s>>>(c);                          // a6 + a7
@@ -372,9 +402,6 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (c.n > 0 && (out->dbg_link_up || out->dbg_link_dn || out->dbg_clean_up || out->dbg_clean_dn ||
                   out->dbg_start_hits))
     k_debug_links<<<(c.n + 255) / 256, 256, 0, s>>>(c);
-  if (out->dbg_tracklet_capacity &&
-      (out->dbg_tracklet_start || out->dbg_tracklet_nhits || out->dbg_tracklet_map || out->dbg_tracklet_par))
-    k_debug_tracklets<<<(out->dbg_tracklet_capacity + 127) / 128, 128, 0, s>>>(c);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;

@@ -160,8 +160,8 @@ def test_ncu_summary_is_tied_to_the_source_hash(tmp_path, monkeypatch):
     monkeypatch.setattr(bench, "NCU_SUMMARY", str(f))
     assert bench.load_ncu_summary("w")[0] == {}
     f.write_text(json.dumps({"workload": "w", "source_hash": bench_profile.source_hash(),
-                             "kernels": {"tracklet_constructor": {"dram_bytes": 1.0}}}))
-    assert bench.load_ncu_summary("w")[0]["tracklet_constructor"]["dram_bytes"] == 1.0
+                             "kernels": {"tracklet_up_pass": {"dram_bytes": 1.0}}}))
+    assert bench.load_ncu_summary("w")[0]["tracklet_up_pass"]["dram_bytes"] == 1.0
     assert bench.load_ncu_summary("other")[0] == {}
-    f.write_text(json.dumps({"workload": "w", "source_hash": "stale", "kernels": {"tracklet_constructor": {}}}))
+    f.write_text(json.dumps({"workload": "w", "source_hash": "stale", "kernels": {"tracklet_up_pass": {}}}))
     assert bench.load_ncu_summary("w")[0] == {}
