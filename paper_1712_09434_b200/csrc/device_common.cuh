@@ -78,6 +78,7 @@ struct Ctx {
   uint32_t* gid;           // [n]  idx -> gid (index in the input arrays)
   uint32_t* bins;          // [kBinsPerCluster*n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
   RowInfo* rowinfo;        // [n_tr]
+  uint32_t* tile_tr;       // [seed_tiles] task*n_rows + row that holds idx = tile * 1024 (written by a1 for a4)
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)
@@ -85,6 +86,7 @@ struct Ctx {
                            // valid for the rows first_row..last_row of the tracklet record
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   uint4* trk_meta;         // [max_tracklets] nHits, firstRow | lastRow << 16, gid of the start hit, 0: what K7 needs
+  uint32_t* trk_kept;      // [max_tracklets] hits the tracklet keeps (L1), counted by k_resolve; cleared per call
   uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]

@@ -48,43 +48,45 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
   const int min_hits = c.prm.min_track_hits;
   const size_t stride = map_stride(n_rows);
   __syncthreads();
-#ifndef TPC_RESOLVE_PASSES
-#define TPC_RESOLVE_PASSES 2
-#endif
-  for (int pass = 0; pass < TPC_RESOLVE_PASSES; ++pass) {
+  for (int pass = 0; pass < 2; ++pass) {
     for (uint32_t k = task_a; k <= task_b; ++k) {
       const uint32_t t0 = c.trk_task_off[k], nt = c.trk_task_off[k + 1u] - t0;
-      const int ra = k == task_a ? (int)(tr_a - k * (uint32_t)n_rows) : 0;
-      const int rb = k == task_b ? (int)(tr_b - k * (uint32_t)n_rows) : n_rows - 1;
-      // threads = (tracklet group) x (row): rp = rows per tracklet rounded up to a power of two (<= block size)
-      int sh = 0;
-      while ((1 << sh) < rb - ra + 1 && (1 << sh) < kResolveThreads) ++sh;
-      const int rp = 1 << sh, grp = kResolveThreads >> sh;
-      const int r_lane = ra + (tid & (rp - 1));
-      for (uint32_t tb = (uint32_t)(tid >> sh); tb < nt; tb += (uint32_t)(grp * kResolveBatch)) {
-        for (int r = r_lane; r <= rb; r += rp) {
-          uint4 m[kResolveBatch];
-          uint32_t idx[kResolveBatch];
+      const uint32_t ra = k == task_a ? tr_a - k * (uint32_t)n_rows : 0u;
+      const uint32_t rb = k == task_b ? tr_b - k * (uint32_t)n_rows : (uint32_t)n_rows - 1u;
+      // the (tracklet, row) pairs of this task and these rows, row fastest: thread tid takes the pairs
+      // tid, tid + 256, ...; (tt, rr) is stepped without a division
+      const uint32_t R = rb - ra + 1u, step_t = kResolveThreads / R, step_r = kResolveThreads % R;
+      uint32_t tt = (uint32_t)tid / R, rr = (uint32_t)tid % R;
+      while (__any_sync(0xffffffffu, tt < nt)) {
+        uint4 m[kResolveBatch];
+        uint32_t idx[kResolveBatch], ts[kResolveBatch], rs[kResolveBatch];
 #pragma unroll
-          for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
-            const uint32_t tt = tb + (uint32_t)(j * grp);  // tracklet's rows is read and ignored)
-            const bool in = tt < nt;
-            m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
-            idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + r] : kNoHit;
-          }
+        for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
+          ts[j] = tt; rs[j] = ra + rr;             // tracklet's rows is read and ignored)
+          const bool in = tt < nt;
+          m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
+          idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + rs[j]] : kNoHit;
+          tt += step_t; rr += step_r;
+          if (rr >= R) { rr -= R; ++tt; }
+        }
 #pragma unroll
-          for (int j = 0; j < kResolveBatch; ++j) {
-            const int first = (int)(m[j].y & 0xFFFFu), last = (int)(m[j].y >> 16);
-            const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
-            if ((int)m[j].x < min_hits || r < first || r > last || idx[j] == kNoHit || off >= span) continue;
-            const unsigned long long key =
-                ((unsigned long long)m[j].x << 32) | (unsigned long long)(0xFFFFFFFFu - m[j].z);
-#ifdef TPC_RESOLVE_NOATOM
-            if (pass == 0) s_owner[off] = key;
-#else
-            if (pass == 0) atomicMax(&s_owner[off], key);                                      // K7
-#endif
-            else if (s_owner[off] != key) c.trk_hits[(size_t)(t0 + tb + (uint32_t)(j * grp)) * stride + r] = kNoHit;  // L1
+        for (int j = 0; j < kResolveBatch; ++j) {
+          const uint32_t first = m[j].y & 0xFFFFu, last = m[j].y >> 16;
+          const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
+          const bool mine = (int)m[j].x >= min_hits && rs[j] >= first && rs[j] <= last && idx[j] != kNoHit && off < span;
+          const unsigned long long key =
+              ((unsigned long long)m[j].x << 32) | (unsigned long long)(0xFFFFFFFFu - m[j].z);
+          if (pass == 0) {
+            if (mine) atomicMax(&s_owner[off], key);                                           // K7
+          } else {
+            const bool kept = mine && s_owner[off] == key;                                       // L1
+            if (mine && !kept) c.trk_hits[(size_t)(t0 + ts[j]) * stride + rs[j]] = kNoHit;
+            // hits a tracklet keeps, counted per tracklet: the lanes of a warp that hold the same tracklet add once
+            const unsigned act = __ballot_sync(0xffffffffu, kept);
+            if (kept) {
+              const unsigned same = __match_any_sync(act, ts[j]);
+              if ((same & ((1u << (tid & 31)) - 1u)) == 0u) atomicAdd(&c.trk_kept[t0 + ts[j]], (uint32_t)__popc(same));
+            }
           }
         }
       }
@@ -96,14 +98,12 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
 constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
 constexpr int kOutChunks = 5;     // 32-row chunks of a row map read per round (159 rows = 5 chunks)
 
-// a6 (L2) + a7.  One tile = 128 consecutive tracklets.  Pass 1: every WARP walks its 32 tracklets one by
-// one, the 32 lanes reading 32 rows of the tracklet's row map at a time (after k_resolve the map holds the
-// hits the tracklet keeps); the keep masks stay in shared memory.  The tile then takes its place in the
-// output with an ordered chained scan over (tracks, hits) packed as tracks<<32 | hits.  Pass 2: the warp
-// writes each surviving track - its record as SoA columns and its kept hits as gids in ascending row
-// order (L3).  Output order = tracklet order.
+// a6 (L2) + a7.  One tile = 128 consecutive tracklets; k_resolve has counted the hits every tracklet keeps
+// (L1) and left exactly those in its row map.  The tile takes its place in the output with an ordered
+// chained scan over (tracks, hits) packed as tracks<<32 | hits; then every warp writes its surviving
+// tracks one by one - the record as SoA columns and the kept hits as gids in ascending row order (L3).
+// Output order = tracklet order.
 __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
-  extern __shared__ uint32_t s_keep[];  // [kOutThreads][words] keep masks, bit k of word w = row first_row + 32 w + k
   __shared__ uint32_t s_warp[33];
   __shared__ uint32_t s_tile;
   __shared__ unsigned long long s_prefix;
@@ -115,38 +115,17 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   // the grid covers max_tracklets; tiles past the last tracklet have nothing to add and nobody waits for them
   const uint32_t last_tile = n_trk > 0u ? (n_trk - 1u) / kOutThreads : 0u;
   if (tile > last_tile) return;
-  const int n_rows = c.n_rows, words = (n_rows + 31) / 32;
+  const int n_rows = c.n_rows;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t t_warp = tile * kOutThreads + warp * 32;
   const int min_hits = c.prm.min_track_hits;
-  // lane j holds what it needs of tracklet t_warp + j: n_hits, first/last row
-  int my_n = 0, my_first = 0, my_last = -1;
+  // lane j holds what it needs of tracklet t_warp + j
+  int my_first = 0, my_last = -1;
+  uint32_t my_kept = 0u;
   if (t_warp + lane < n_trk) {
     const uint4 m = __ldg(&c.trk_meta[t_warp + lane]);
-    my_n = (int)m.x; my_first = (int)(m.y & 0xFFFFu); my_last = (int)(m.y >> 16);
-  }
-  uint32_t my_kept = 0u;  // lane j: hits tracklet t_warp + j keeps
-  for (unsigned rest = __ballot_sync(FULL, my_n >= min_hits); rest; rest &= rest - 1u) {  // K6
-    const int j = __ffs(rest) - 1;
-    const uint32_t t = t_warp + j;
-    const int first = __shfl_sync(FULL, my_first, j), last = __shfl_sync(FULL, my_last, j);
-    const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
-    uint32_t kept = 0u;
-    for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {  // the map loads of a round are issued together
-      uint32_t idx[kOutChunks];
-#pragma unroll
-      for (int q = 0; q < kOutChunks; ++q) {
-        const int r = rb0 + 32 * q + lane;
-        idx[q] = r <= last ? map[r] : kNoHit;
-      }
-#pragma unroll
-      for (int q = 0; q < kOutChunks; ++q) {
-        const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit);   // L1 (decided by k_resolve)
-        if (lane == 0 && rb0 + 32 * q <= last) s_keep[(warp * 32 + j) * words + ((rb0 - first) >> 5) + q] = mask;
-        kept += __popc(mask);
-      }
-    }
-    if (lane == j) my_kept = kept;
+    my_first = (int)(m.y & 0xFFFFu); my_last = (int)(m.y >> 16);
+    my_kept = c.trk_kept[t_warp + lane];
   }
   const bool is_track = my_kept >= (uint32_t)min_hits && my_kept > 0u;  // L2
   const uint32_t my_hits = is_track ? my_kept : 0u;
@@ -187,22 +166,21 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
     const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t w = hb;
-    // as in pass 1: the map loads of kOutChunks chunks together, then their gid gathers, then the stores
+    // the map loads of kOutChunks chunks together, then their gid gathers, then the stores
     for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
-      unsigned mask[kOutChunks];
       uint32_t idx[kOutChunks], g[kOutChunks];
 #pragma unroll
       for (int q = 0; q < kOutChunks; ++q) {
-        const int rb = rb0 + 32 * q;
-        mask[q] = rb <= last ? s_keep[(warp * 32 + j) * words + ((rb - first) >> 5)] : 0u;
-        idx[q] = (mask[q] >> lane) & 1u ? map[rb + lane] : 0u;
+        const int r = rb0 + 32 * q + lane;
+        idx[q] = r <= last ? map[r] : kNoHit;
       }
 #pragma unroll
-      for (int q = 0; q < kOutChunks; ++q) g[q] = (mask[q] >> lane) & 1u ? c.gid[idx[q]] : 0u;
+      for (int q = 0; q < kOutChunks; ++q) g[q] = idx[q] != kNoHit ? c.gid[idx[q]] : 0u;
 #pragma unroll
       for (int q = 0; q < kOutChunks; ++q) {
-        if ((mask[q] >> lane) & 1u) o.hit_cluster[w + __popc(mask[q] & ((1u << lane) - 1u))] = g[q];
-        w += __popc(mask[q]);
+        const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit);
+        if (idx[q] != kNoHit) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = g[q];
+        w += __popc(mask);
       }
     }
   }

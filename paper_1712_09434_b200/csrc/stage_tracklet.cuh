@@ -26,8 +26,14 @@
 namespace tpc {
 
 constexpr int kTrackletThreads = 128;
-constexpr int kFitBlocksPerSm = 8;     // k_trk_chain, k_trk_refit: registers per thread <= 65536 / (128 * 8) = 64
-constexpr int kSearchBlocksPerSm = 6;  // k_trk_up, k_trk_finish:  <= 85
+#ifndef TPC_FIT_BLOCKS
+#define TPC_FIT_BLOCKS 7
+#endif
+#ifndef TPC_SEARCH_BLOCKS
+#define TPC_SEARCH_BLOCKS 6
+#endif
+constexpr int kFitBlocksPerSm = TPC_FIT_BLOCKS;     // k_trk_chain, k_trk_refit: registers per thread <= 65536 / (128 * 8) = 64
+constexpr int kSearchBlocksPerSm = TPC_SEARCH_BLOCKS;  // k_trk_up, k_trk_finish:  <= 85
 
 struct TrackState {
   float y, z, s, t, q;  // SPEC 5: y, z, sinphi, dz/dl, q/pT
@@ -169,7 +175,10 @@ __device__ __noinline__ int32_t search_row_serial(const float2* __restrict__ yz,
 // are loaded together, then their candidates are read as ONE virtual range, kSearchUnroll at a time, all
 // loads of a group in flight before the first is tested (the walk is latency bound) and the tests written
 // without branches (lanes of a warp are at different candidates of different windows).
-constexpr int kSearchUnroll = 2;
+#ifndef TPC_SEARCH_UNROLL
+#define TPC_SEARCH_UNROLL 2
+#endif
+constexpr int kSearchUnroll = TPC_SEARCH_UNROLL;
 
 template <bool COUNT>
 __device__ __forceinline__ int32_t search_row(const Ctx& c, const TrackState& S, const RowInfo g,
@@ -245,17 +254,24 @@ constexpr uint32_t kNoHit = 0xFFFFFFFFu;  // row map entry of a row without a hi
 __device__ __forceinline__ uint32_t pack_rows(int row_cur, int r_down, int r0, bool skip_up) {
   return (uint32_t)row_cur | ((uint32_t)(r_down + 1) << 10) | ((uint32_t)r0 << 20) | (skip_up ? 1u << 30 : 0u);
 }
+#ifdef TPC_STREAM_STORES
+#define TPC_ST4(p, v) __stcs((p), (v))
+#define TPC_ST1(p, v) __stcs((p), (v))
+#else
+#define TPC_ST4(p, v) (*(p) = (v))
+#define TPC_ST1(p, v) (*(p) = (v))
+#endif
 __device__ __forceinline__ void store_rec(float4* rec, const TrackState& S, float x, int n_hits, int first_row,
                                           int last_row, uint32_t pack, uint32_t tr_base, uint32_t ia, uint32_t ib) {
-  rec[0] = make_float4(x, S.y, S.z, S.s);
-  rec[1] = make_float4(S.t, S.q, S.c00, S.c10);
-  rec[2] = make_float4(S.c11, S.c20, S.c21, S.c22);
-  rec[3] = make_float4(S.c30, S.c31, S.c32, S.c33);
-  rec[4] = make_float4(S.c40, S.c41, S.c42, S.c43);
-  rec[5] = make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits));
-  rec[6] = make_float4(__int_as_float(first_row), __int_as_float(last_row), __uint_as_float(pack),
-                       __uint_as_float(tr_base));
-  rec[7] = make_float4(__uint_as_float(ia), __uint_as_float(ib), 0.0f, 0.0f);
+  TPC_ST4(rec + 0, make_float4(x, S.y, S.z, S.s));
+  TPC_ST4(rec + 1, make_float4(S.t, S.q, S.c00, S.c10));
+  TPC_ST4(rec + 2, make_float4(S.c11, S.c20, S.c21, S.c22));
+  TPC_ST4(rec + 3, make_float4(S.c30, S.c31, S.c32, S.c33));
+  TPC_ST4(rec + 4, make_float4(S.c40, S.c41, S.c42, S.c43));
+  TPC_ST4(rec + 5, make_float4(S.c44, S.chi2, __int_as_float(S.ndf), __int_as_float(n_hits)));
+  TPC_ST4(rec + 6, make_float4(__int_as_float(first_row), __int_as_float(last_row), __uint_as_float(pack),
+                               __uint_as_float(tr_base)));
+  TPC_ST4(rec + 7, make_float4(__uint_as_float(ia), __uint_as_float(ib), 0.0f, 0.0f));
 }
 // rec: the lane's shared-memory copy of the record
 __device__ __forceinline__ void load_rec(const float4* rec, TrackState& S, int& n_hits, int& first_row,
@@ -529,7 +545,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     __syncwarp();
     if (do_search) {                                                   // K3 bookkeeping
       const bool got = hit >= 0;
-      map[rt] = (uint32_t)hit;                                         // -1 = kNoHit
+      TPC_ST1(map + rt, (uint32_t)hit);                                // -1 = kNoHit
       n_hits += got ? 1 : 0;
       last_row = got ? rt : last_row;
       last_hit = got ? hit : last_hit;
@@ -738,7 +754,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
     if (book) {
       const bool got = hit >= 0;
       const bool gap_row = do_search & (rt < first_row);                // rows whose hits / misses drive the gap
-      if (do_search) map[rt] = (uint32_t)hit;                           // -1 = kNoHit
+      if (do_search) TPC_ST1(map + rt, (uint32_t)hit);                  // -1 = kNoHit
       n_hits += (do_search & got) ? 1 : 0;
       if (gap_row & got) first_row = rt;
       gap = gap_row ? (got ? 0 : gap + 1) : gap;

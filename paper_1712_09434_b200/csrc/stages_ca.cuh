@@ -18,6 +18,7 @@ namespace tpc {
 // of start hits, tracklets and output tracks, is the same on every run.
 // ---------------------------------------------------------------------------
 constexpr int kGridThreads = 128;
+constexpr uint32_t kSeedTileIdx = 1024;  // = kSeedTile below
 
 // Grid of a row with n clusters inside the box [ylo, yhi] x [zlo, zhi]: kBinsPerCluster bins per cluster.
 __device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint32_t lo, uint32_t n, float ylo,
@@ -79,7 +80,11 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   const int g_ny = info_ny(g), g_nz = info_nz(g);
   const int nb = g_ny * g_nz;
   const float y0 = g.y0, z0 = g.z0;
-  if (tid == 0) c.rowinfo[tr] = g;
+  if (tid == 0) {
+    c.rowinfo[tr] = g;
+    // the row that holds the first idx of every tile of the start-hit finder (a4)
+    for (uint32_t k = (lo + kSeedTileIdx - 1u) / kSeedTileIdx; k * kSeedTileIdx < hi; ++k) c.tile_tr[k] = tr;
+  }
   for (int b = tid; b <= nb; b += kGridThreads) s_cnt[b] = 0u;
   __syncthreads();
   for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
@@ -175,74 +180,117 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 // ---------------------------------------------------------------------------
 // a4  start hits (S1) whose chain has >= min_seed_hits hits (S2, S3), written
 // in idx order as seed records (trk_seed).  Tile = kSeedThreads * kSeedItems idx.
+// Three steps per tile: every thread tests its four clusters for S1 (two 16-byte loads and the four
+// link gathers of C2 in flight together); the tile's start hits (about one cluster in twenty) are
+// compacted in order into shared memory and each is walked by a thread of its own (S2: the four or
+// five dependent link loads of a chain run side by side instead of up to four chains per thread one
+// after the other); those with a long enough chain are compacted again, the tile takes its place in
+// the output (chained scan with decoupled look-back), and the threads write the seed records.
 // ---------------------------------------------------------------------------
 constexpr int kSeedThreads = 256;
 constexpr int kSeedItems = 4;
 constexpr uint32_t kSeedTile = kSeedThreads * kSeedItems;
+static_assert(kSeedTile == kSeedTileIdx, "k_grid_build notes the row of every tile start");
+constexpr int kSeedRows = 96;  // row offsets of the tile kept in shared memory (a tile of a central event spans 3 rows)
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
   __shared__ uint32_t s_warp[33];
-  __shared__ uint32_t s_tile;
+  __shared__ uint32_t s_tile, s_tr;
   __shared__ unsigned long long s_prefix;
-  if (threadIdx.x == 0) s_tile = atomicAdd(&c.tickets[0], 1u);
+  __shared__ uint16_t s_cand[kSeedTile];        // start hits of the tile (idx - tile base), in idx order
+  __shared__ int32_t s_h[3][kSeedTile];         // h1, h2, h3 of candidate j
+  __shared__ uint32_t s_rowoff[kSeedRows + 1];  // row_off[s_tr + j]
+  const int tid = (int)threadIdx.x;
+  if (tid == 0) {
+    s_tile = atomicAdd(&c.tickets[0], 1u);
+    s_tr = c.tile_tr[s_tile];
+  }
   __syncthreads();
-  const uint32_t tile = s_tile;
-  const uint32_t base = tile * kSeedTile + threadIdx.x * kSeedItems;
-  uint32_t flags = 0u, n_s1 = 0u;
-  int32_t h1s[kSeedItems], h2s[kSeedItems], h3s[kSeedItems];
-  // the four cleaned up-links and raw down-links of this thread: one 16-byte load each (arrays are padded)
+  const uint32_t tile = s_tile, tile_base = tile * kSeedTile;
+  const uint32_t tr_tile = s_tr;
+  if (tid <= kSeedRows) s_rowoff[tid] = c.row_off[min(tr_tile + (uint32_t)tid, c.n_tr)];
+  const uint32_t base = tile_base + (uint32_t)tid * kSeedItems;
+  // S1: cleaned up-link present, cleaned down-link absent
   int4 cu4 = make_int4(-1, -1, -1, -1), dn4 = make_int4(-1, -1, -1, -1);
-  if (base < c.n) {
+  if (base < c.n) {  // arrays are padded to whole groups of four
     cu4 = *reinterpret_cast<const int4*>(c.clean_up + base);
     dn4 = *reinterpret_cast<const int4*>(c.link_dn + base);
   }
   const int32_t cu[kSeedItems] = {cu4.x, cu4.y, cu4.z, cu4.w}, dn[kSeedItems] = {dn4.x, dn4.y, dn4.z, dn4.w};
+  int32_t back[kSeedItems];
 #pragma unroll
-  for (int k = 0; k < kSeedItems; ++k) {
-    const uint32_t i = base + k;
-    h1s[k] = -1; h2s[k] = -1; h3s[k] = -1;
-    if (i >= c.n) continue;
-    const int32_t h1 = cu[k];
-    if (h1 < 0) continue;
-    const int32_t d = dn[k];
-    if (d >= 0 && c.link_up[d] == (int32_t)i) continue;  // clean_dn[i] >= 0 (C2): not a start hit
-    if (COUNT) ++n_s1;
+  for (int k = 0; k < kSeedItems; ++k)  // (the padding behind the last cluster holds anything)
+    back[k] = (base + k < c.n && cu[k] >= 0 && dn[k] >= 0) ? c.link_up[dn[k]] : -1;
+  uint32_t s1 = 0u;
+#pragma unroll
+  for (int k = 0; k < kSeedItems; ++k)
+    if (base + k < c.n && cu[k] >= 0 && !(dn[k] >= 0 && back[k] == (int32_t)(base + k))) s1 |= 1u << k;  // C2
+  uint32_t n_cand;
+  uint32_t at = block_exclusive_scan(__popc(s1), s_warp, &n_cand);
+#pragma unroll
+  for (int k = 0; k < kSeedItems; ++k)
+    if (s1 & (1u << k)) {
+      s_cand[at] = (uint16_t)(tid * kSeedItems + k);
+      s_h[0][at] = cu[k];
+      ++at;
+    }
+  __syncthreads();
+  // S2, S3: one start hit per thread (loop: a tile can hold more start hits than threads)
+  const int min_seed = c.prm.min_seed_hits;
+  uint32_t keep = 0u;  // bit q: candidate tid + q*kSeedThreads has a long enough chain
+  for (uint32_t j = (uint32_t)tid, q = 0u; j < n_cand; j += kSeedThreads, ++q) {
+    const int32_t h1 = s_h[0][j];
     const int32_t h2 = c.clean_up[h1];
-    int32_t h = h2 >= 0 ? c.clean_up[h2] : -1;           // h3
-    h1s[k] = h1; h2s[k] = h2; h3s[k] = h;
-    int len = 2 + (h2 >= 0 ? 1 : 0) + (h >= 0 ? 1 : 0);  // S2: hits of the chain, counted up to min_seed_hits
-    while (len < c.prm.min_seed_hits && h >= 0) {
+    int32_t h = h2 >= 0 ? c.clean_up[h2] : -1;  // h3
+    s_h[1][j] = h2; s_h[2][j] = h;
+    int len = 2 + (h2 >= 0 ? 1 : 0) + (h >= 0 ? 1 : 0);  // hits of the chain, counted up to min_seed_hits
+    while (len < min_seed && h >= 0) {
       h = c.clean_up[h];
       if (h >= 0) ++len;
     }
-    if (len >= c.prm.min_seed_hits) flags |= 1u << k;
+    if (len >= min_seed) keep |= 1u << q;
   }
-  uint32_t total;
-  const uint32_t excl = block_exclusive_scan(__popc(flags), s_warp, &total);
-  if (threadIdx.x < 32) {
+  // ordered compaction of the kept candidates: candidate order is j = tid + q*kSeedThreads, so the scan runs
+  // once per q (one round for a tile with up to kSeedThreads start hits)
+  uint32_t excl[kSeedItems], total = 0u;
+  for (uint32_t q = 0u; q * kSeedThreads < n_cand || q == 0u; ++q) {
+    uint32_t tq;
+    excl[q] = total + block_exclusive_scan((keep >> q) & 1u, s_warp, &tq);
+    total += tq;
+  }
+  if (tid < 32) {
     const unsigned long long p = lookback_exclusive(c.scan_seed, tile, (unsigned long long)total);
-    if (threadIdx.x == 0) s_prefix = p;
+    if (tid == 0) s_prefix = p;
   }
   __syncthreads();
   const unsigned long long prefix = s_prefix;
-  uint32_t pos = (uint32_t)prefix + excl;
-#pragma unroll
-  for (int k = 0; k < kSeedItems; ++k) {
-    if (!(flags & (1u << k))) continue;
-    if (pos < c.max_tracklets) {
-      const uint32_t h0 = base + k, h1 = (uint32_t)h1s[k];
-      const uint32_t tr0 = find_tr(c, h0);
-      const float2 p0 = c.yz[h0], p1 = c.yz[h1];
-      const float2 p2 = h2s[k] >= 0 ? c.yz[h2s[k]] : make_float2(0.0f, 0.0f);
-      uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
-      rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2s[k]);
-      rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));
-      rec[2] = make_uint4(__float_as_uint(p2.x), __float_as_uint(p2.y), c.gid[h0], (uint32_t)h3s[k]);
+  for (uint32_t j = (uint32_t)tid, q = 0u; j < n_cand; j += kSeedThreads, ++q) {
+    if (!((keep >> q) & 1u)) continue;
+    const unsigned long long pos = prefix + excl[q];
+    if (pos >= c.max_tracklets) continue;
+    const uint32_t h0 = tile_base + s_cand[j], h1 = (uint32_t)s_h[0][j];
+    const int32_t h2 = s_h[1][j], h3 = s_h[2][j];
+    uint32_t tr0;
+    if (h0 < s_rowoff[kSeedRows]) {  // last of the staged rows with row_off <= h0
+      int lo = 0, hi = kSeedRows;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (s_rowoff[mid] <= h0) lo = mid; else hi = mid;
+      }
+      tr0 = tr_tile + (uint32_t)lo;
+    } else {
+      tr0 = find_tr(c, h0);
     }
-    ++pos;
+    const float2 p0 = c.yz[h0], p1 = c.yz[h1];
+    const float2 p2 = h2 >= 0 ? c.yz[h2] : make_float2(0.0f, 0.0f);
+    const uint32_t g0 = c.gid[h0];
+    uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
+    rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2);
+    rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));
+    rec[2] = make_uint4(__float_as_uint(p2.x), __float_as_uint(p2.y), g0, (uint32_t)h3);
   }
-  if (threadIdx.x == 0 && tile == gridDim.x - 1) {  // the last tile knows the total
+  if (tid == 0 && tile == gridDim.x - 1) {  // the last tile knows the total
     const unsigned long long all = prefix + total;
     if (all > c.max_tracklets) atomicOr(&c.out.header[2], TPC_STATUS_TRACKLET_OVERFLOW);
     const uint32_t built = (uint32_t)(all > c.max_tracklets ? c.max_tracklets : all);
@@ -250,7 +298,10 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
     c.out.header[3] = built;
     if (COUNT) atomicAdd(&c.counters[CN_TRACKLETS_BUILT], (unsigned long long)built);
   }
-  if (COUNT && n_s1) atomicAdd(&c.counters[CN_START_HITS], (unsigned long long)n_s1);
+  if (COUNT) {
+    const uint32_t n_s1 = __popc(s1);
+    if (n_s1) atomicAdd(&c.counters[CN_START_HITS], (unsigned long long)n_s1);
+  }
 }
 
 }  // namespace tpc

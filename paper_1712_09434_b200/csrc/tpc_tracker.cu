@@ -8,6 +8,7 @@
 
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -30,6 +31,7 @@ struct tpc_tracker {
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
+  bool debug_sync = false;  // TPC_DEBUG_SYNC=1: synchronise after every stage and name the stage that failed
   // persistent tracklet kernels (chain, up, refit, finish): [kernel][counters off/on] -> blocks that fit the device at once
   int n_sm = 0;
   size_t trk_smem[4] = {0, 0, 0, 0};
@@ -70,8 +72,8 @@ uint32_t resolve_max_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tr
 
 // Offsets of every workspace array, in bytes.
 struct Carve {
-  size_t yz, gid, bins, rowinfo, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
-      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, zero_end, total;
+  size_t yz, gid, bins, rowinfo, tile_tr, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
+      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, trk_kept, zero_end, total;
   uint32_t seed_tiles, out_tiles;
 };
 
@@ -85,6 +87,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.gid = take(n4 * sizeof(uint32_t));
   c.bins = take(((size_t)kBinsPerCluster * n + n_tr * kBinPad + 16) * sizeof(uint32_t));  // + slack of the 16-byte aligned bulk copies
   c.rowinfo = take((n_tr + 1) * sizeof(RowInfo));
+  c.tile_tr = take((((size_t)n + kSeedTile - 1) / kSeedTile + 1) * sizeof(uint32_t));
   c.link_up = take(n4 * sizeof(int32_t));
   c.link_dn = take(n4 * sizeof(int32_t));
   c.clean_up = take(n4 * sizeof(int32_t));
@@ -102,6 +105,7 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.tickets = take(8 * sizeof(uint32_t));
   c.n_tracklets = take(sizeof(uint32_t));
   c.trk_task_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
+  c.trk_kept = take((size_t)T * sizeof(uint32_t));
   c.zero_end = off;
   c.total = off;
   return c;
@@ -131,12 +135,13 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.y = in->y; c.z = in->z; c.row_off = in->row_offsets;
   c.n = in->n_clusters; c.n_tasks = in->n_tasks; c.n_tr = in->n_tasks * (uint32_t)t->n_rows;
   c.yz = (float2*)(ws + cv.yz); c.gid = (uint32_t*)(ws + cv.gid); c.bins = (uint32_t*)(ws + cv.bins);
-  c.rowinfo = (RowInfo*)(ws + cv.rowinfo);
+  c.rowinfo = (RowInfo*)(ws + cv.rowinfo); c.tile_tr = (uint32_t*)(ws + cv.tile_tr);
   c.link_up = (int32_t*)(ws + cv.link_up); c.link_dn = (int32_t*)(ws + cv.link_dn);
   c.clean_up = (int32_t*)(ws + cv.clean_up);
   c.trk_seed = (uint4*)(ws + cv.trk_seed);
   c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
   c.trk_meta = (uint4*)(ws + cv.trk_meta); c.trk_task_off = (uint32_t*)(ws + cv.trk_task_off);
+  c.trk_kept = (uint32_t*)(ws + cv.trk_kept);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
   c.max_tracklets = T;
@@ -176,6 +181,10 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
                 "min_track_hits >= 1, max_row_gap >= 0");
   }
   t->n_sectors = g->n_sectors; t->n_rows = g->n_rows; t->z_max = g->z_max; t->bz = bz_kgauss;
+  {
+    const char* dbg = getenv("TPC_DEBUG_SYNC");
+    t->debug_sync = dbg && dbg[0] == '1';
+  }
   const int n = g->n_rows;
   std::vector<float> tab((size_t)6 * n, 0.f);
   float *X = tab.data(), *ymax = X + n, *dx_up = X + 2 * n, *dx_dn = X + 3 * n, *ratio_up = X + 4 * n,
@@ -201,6 +210,9 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
     cudaGetLastError();
     return rc;
   }
+#ifdef TPC_L2_FETCH
+  cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, TPC_L2_FETCH);
+#endif
   // launch shape of the persistent tracklet constructor: as many blocks as the device holds at once
   int dev = 0, n_sm = 0;
   e = cudaGetDevice(&dev);
@@ -348,8 +360,16 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
     ev = t->ev.data() + (size_t)(t->timed_calls % TPC_STAGE_RING) * (TPC_N_STAGES + 1);
     ++t->timed_calls;
   }
-  int stage = 0;
-  auto mark = [&]() { if (ev) cudaEventRecord(ev[stage], s); ++stage; };
+  int stage = 0, bad_stage = -1;
+  cudaError_t bad = cudaSuccess;
+  auto mark = [&]() {
+    if (ev) cudaEventRecord(ev[stage], s);
+    if (t->debug_sync && bad == cudaSuccess && stage > 0) {
+      bad = cudaStreamSynchronize(s);
+      if (bad != cudaSuccess) bad_stage = stage - 1;
+    }
+    ++stage;
+  };
   mark();
   if (c.n_tr > 0) {
     if (cnt) k_grid_build<true><<<c.n_tr, kGridThreads, 0, s>>>(c);                         // a1
@@ -396,12 +416,13 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
     k_resolve<<<(c.n + kResolveChunk - 1) / kResolveChunk, kResolveThreads, kResolveChunk * sizeof(unsigned long long), s>>>(c);
   }
   mark();
-  const size_t keep_smem = (size_t)kOutThreads * ((size_t)(t->n_rows + 31) / 32) * sizeof(uint32_t);
-  k_select_output<<<cv.out_tiles, kOutThreads, keep_smem, s>>>(c);                          // a6 + a7
+  k_select_output<<<cv.out_tiles, kOutThreads, 0, s>>>(c);                          // a6 + a7
   mark();
   if (c.n > 0 && (out->dbg_link_up || out->dbg_link_dn || out->dbg_clean_up || out->dbg_clean_dn ||
                   out->dbg_start_hits))
     k_debug_links<<<(c.n + 255) / 256, 256, 0, s>>>(c);
+  if (bad != cudaSuccess)
+    return fail(t, TPC_ERR_CUDA, "tpc_track_batch: stage %s: %s", tpc_stage_name(bad_stage), cudaGetErrorString(bad));
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;
