@@ -53,6 +53,7 @@ extern "C" {
 #define TPC_STATUS_TRACKLET_OVERFLOW 1u /* more tracklets than max_tracklets: the surplus was not built */
 #define TPC_STATUS_TRACK_OVERFLOW 2u    /* more tracks than track_capacity: the surplus was not written */
 #define TPC_STATUS_HIT_OVERFLOW 4u      /* more hits than hit_capacity: tracks that do not fit dropped  */
+#define TPC_STATUS_TASK_TOO_LARGE 8u    /* a sector task holds 2^27 clusters or more: it gives no tracks */
 
 /* Detector geometry (SPEC 1).  HOST memory; copied by tpc_tracker_create. */
 typedef struct {

@@ -8,22 +8,30 @@ namespace tpc {
 
 // ---------------------------------------------------------------------------
 // K7 + L1: who owns a cluster.  owner[h] = max over the kept tracklets that hold h of
-// key = nHits << 32 | ~gid(h0), and a tracklet keeps h iff it is that owner.  The ownership words never
-// exist in global memory: the clusters are cut into chunks of kResolveChunk consecutive idx, one block
-// per chunk holds the chunk's ownership words in shared memory, and walks the row maps of the tracklets
-// of the task(s) the chunk lies in - only the rows the chunk covers - twice: first atomicMax of the key
-// (shared-memory atomics), then the test; an entry that lost is overwritten with kNoHit in the map, so
-// after this kernel a row map lists exactly the hits its tracklet keeps (L1).
+// (nHits, ~gid(h0)), and a tracklet keeps h iff it is that owner.  The ownership words never exist in
+// global memory: the clusters are cut into chunks of kResolveChunk consecutive idx, one block per chunk
+// holds the chunk's ownership words in shared memory.  Pass 1 walks the row maps of the tracklets of the
+// task(s) the chunk lies in - only the rows the chunk covers - and takes atomicMax (shared-memory
+// atomics) of
+//     key = nHits << 53 | (2^27 - 1 - (gid(h0) - first gid of the task)) << 26 | tracklet index in the task
+// which orders like (nHits, ~gid(h0)) because a start hit has one tracklet, and names the winner.
+// Pass 2 walks the chunk's CLUSTERS: the winner's map entry gets kOwnedBit and its count of kept hits
+// goes up by one.  After this kernel a tracklet keeps exactly the flagged entries of its map (L1).
 // (Global 64-bit atomicMax per hit - 139 M of them on config 3, each a DRAM read-modify-write because
 // the three or four tracklets that share a cluster end far apart in time - cost more than the whole
 // down pass; shared memory takes that traffic away.)
+// A task with 2^27 clusters or more (fifty times the whole config-3 batch in one sector) does not fit
+// the key: its tracklets keep nothing and TPC_STATUS_TASK_TOO_LARGE is set.
 // ---------------------------------------------------------------------------
 constexpr int kResolveThreads = 256;
 constexpr uint32_t kResolveChunk = 8192;  // clusters per block: 64 KB of ownership words, 3 blocks per SM
 #ifndef TPC_RESOLVE_BATCH
 #define TPC_RESOLVE_BATCH 8
 #endif
-constexpr int kResolveBatch = TPC_RESOLVE_BATCH;          // tracklets a thread has in flight
+constexpr int kResolveBatch = TPC_RESOLVE_BATCH;  // (tracklet, row) pairs a thread has in flight
+constexpr int kResolveRows = 512;                 // row offsets of the chunk kept in shared memory
+constexpr uint32_t kOwnedBit = 0x80000000u;       // map entry: the tracklet keeps this hit (idx < 2^31)
+constexpr uint32_t kKeyGidBits = 27, kKeyTrkBits = 26;
 
 // first tracklet of every task: tracklets are in idx order of their start hits, so a task's are consecutive
 __global__ void k_task_offsets(const Ctx c) {
@@ -39,59 +47,78 @@ __global__ void k_task_offsets(const Ctx c) {
 
 __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
   extern __shared__ unsigned long long s_owner[];  // [kResolveChunk]
+  __shared__ uint32_t s_rowoff[kResolveRows + 1];
   const uint32_t i0 = blockIdx.x * kResolveChunk;
   const uint32_t i1 = min(i0 + kResolveChunk, c.n), span = i1 - i0;
   const int tid = (int)threadIdx.x, n_rows = c.n_rows;
   for (uint32_t i = tid; i < kResolveChunk; i += kResolveThreads) s_owner[i] = 0ull;
   const uint32_t tr_a = find_tr(c, i0), tr_b = find_tr(c, i1 - 1u);
   const uint32_t task_a = tr_a / (uint32_t)n_rows, task_b = tr_b / (uint32_t)n_rows;
+  const bool rows_staged = tr_b - tr_a < (uint32_t)kResolveRows;
+  if (rows_staged)
+    for (uint32_t j = tid; j <= tr_b - tr_a + 1u; j += kResolveThreads) s_rowoff[j] = c.row_off[tr_a + j];
   const int min_hits = c.prm.min_track_hits;
   const size_t stride = map_stride(n_rows);
   __syncthreads();
-  for (int pass = 0; pass < 2; ++pass) {
-    for (uint32_t k = task_a; k <= task_b; ++k) {
-      const uint32_t t0 = c.trk_task_off[k], nt = c.trk_task_off[k + 1u] - t0;
-      const uint32_t ra = k == task_a ? tr_a - k * (uint32_t)n_rows : 0u;
-      const uint32_t rb = k == task_b ? tr_b - k * (uint32_t)n_rows : (uint32_t)n_rows - 1u;
-      // the (tracklet, row) pairs of this task and these rows, row fastest: thread tid takes the pairs
-      // tid, tid + 256, ...; (tt, rr) is stepped without a division
-      const uint32_t R = rb - ra + 1u, step_t = kResolveThreads / R, step_r = kResolveThreads % R;
-      uint32_t tt = (uint32_t)tid / R, rr = (uint32_t)tid % R;
-      while (__any_sync(0xffffffffu, tt < nt)) {
-        uint4 m[kResolveBatch];
-        uint32_t idx[kResolveBatch], ts[kResolveBatch], rs[kResolveBatch];
+  // pass 1 (K7): the (tracklet, row) pairs of every task of the chunk, rows of the chunk only, row fastest:
+  // thread tid takes the pairs tid, tid + 256, ...; (tt, rr) is stepped without a division
+  for (uint32_t k = task_a; k <= task_b; ++k) {
+    const uint32_t t0 = c.trk_task_off[k], nt = c.trk_task_off[k + 1u] - t0;
+    const uint32_t gid_lo = c.row_off[k * (uint32_t)n_rows], gid_hi = c.row_off[(k + 1u) * (uint32_t)n_rows];
+    if (gid_hi - gid_lo >= (1u << kKeyGidBits)) {
+      if (tid == 0) atomicOr(&c.out.header[2], TPC_STATUS_TASK_TOO_LARGE);
+      continue;
+    }
+    const uint32_t ra = k == task_a ? tr_a - k * (uint32_t)n_rows : 0u;
+    const uint32_t rb = k == task_b ? tr_b - k * (uint32_t)n_rows : (uint32_t)n_rows - 1u;
+    const uint32_t R = rb - ra + 1u, step_t = kResolveThreads / R, step_r = kResolveThreads % R;
+    uint32_t tt = (uint32_t)tid / R, rr = (uint32_t)tid % R;
+    while (__any_sync(0xffffffffu, tt < nt)) {
+      uint4 m[kResolveBatch];
+      uint32_t idx[kResolveBatch], ts[kResolveBatch], rs[kResolveBatch];
 #pragma unroll
-        for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
-          ts[j] = tt; rs[j] = ra + rr;             // tracklet's rows is read and ignored)
-          const bool in = tt < nt;
-          m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
-          idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + rs[j]] : kNoHit;
-          tt += step_t; rr += step_r;
-          if (rr >= R) { rr -= R; ++tt; }
-        }
+      for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
+        ts[j] = tt; rs[j] = ra + rr;             // tracklet's rows is read and ignored)
+        const bool in = tt < nt;
+        m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
+        idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + rs[j]] : kNoHit;
+        tt += step_t; rr += step_r;
+        if (rr >= R) { rr -= R; ++tt; }
+      }
 #pragma unroll
-        for (int j = 0; j < kResolveBatch; ++j) {
-          const uint32_t first = m[j].y & 0xFFFFu, last = m[j].y >> 16;
-          const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
-          const bool mine = (int)m[j].x >= min_hits && rs[j] >= first && rs[j] <= last && idx[j] != kNoHit && off < span;
-          const unsigned long long key =
-              ((unsigned long long)m[j].x << 32) | (unsigned long long)(0xFFFFFFFFu - m[j].z);
-          if (pass == 0) {
-            if (mine) atomicMax(&s_owner[off], key);                                           // K7
-          } else {
-            const bool kept = mine && s_owner[off] == key;                                       // L1
-            if (mine && !kept) c.trk_hits[(size_t)(t0 + ts[j]) * stride + rs[j]] = kNoHit;
-            // hits a tracklet keeps, counted per tracklet: the lanes of a warp that hold the same tracklet add once
-            const unsigned act = __ballot_sync(0xffffffffu, kept);
-            if (kept) {
-              const unsigned same = __match_any_sync(act, ts[j]);
-              if ((same & ((1u << (tid & 31)) - 1u)) == 0u) atomicAdd(&c.trk_kept[t0 + ts[j]], (uint32_t)__popc(same));
-            }
-          }
+      for (int j = 0; j < kResolveBatch; ++j) {
+        const uint32_t first = m[j].y & 0xFFFFu, last = m[j].y >> 16;
+        const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
+        if ((int)m[j].x >= min_hits && rs[j] >= first && rs[j] <= last && idx[j] != kNoHit && off < span) {
+          const unsigned long long key = ((unsigned long long)m[j].x << (kKeyGidBits + kKeyTrkBits)) |
+                                         ((unsigned long long)(((1u << kKeyGidBits) - 1u) - (m[j].z - gid_lo)) << kKeyTrkBits) |
+                                         (unsigned long long)ts[j];
+          atomicMax(&s_owner[off], key);
         }
       }
     }
-    __syncthreads();
+  }
+  __syncthreads();
+  // pass 2 (L1): every owned cluster of the chunk marks its entry in the winner's map
+  for (uint32_t off = (uint32_t)tid; off < span; off += kResolveThreads) {
+    const unsigned long long key = s_owner[off];
+    if (key == 0ull) continue;
+    const uint32_t h = i0 + off;
+    uint32_t tr;
+    if (rows_staged) {  // last staged row with row_off <= h
+      uint32_t lo = 0u, hi = tr_b - tr_a + 1u;
+      while (hi - lo > 1u) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (s_rowoff[mid] <= h) lo = mid; else hi = mid;
+      }
+      tr = tr_a + lo;
+    } else {
+      tr = find_tr(c, h);
+    }
+    const uint32_t task = tr / (uint32_t)n_rows, row = tr - task * (uint32_t)n_rows;
+    const uint32_t t = c.trk_task_off[task] + (uint32_t)(key & ((1ull << kKeyTrkBits) - 1ull));
+    c.trk_hits[(size_t)t * stride + row] = h | kOwnedBit;
+    atomicAdd(&c.trk_kept[t], 1u);
   }
 }
 
@@ -99,7 +126,7 @@ constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklet
 constexpr int kOutChunks = 5;     // 32-row chunks of a row map read per round (159 rows = 5 chunks)
 
 // a6 (L2) + a7.  One tile = 128 consecutive tracklets; k_resolve has counted the hits every tracklet keeps
-// (L1) and left exactly those in its row map.  The tile takes its place in the output with an ordered
+// (L1) and flagged exactly those in its row map.  The tile takes its place in the output with an ordered
 // chained scan over (tracks, hits) packed as tracks<<32 | hits; then every warp writes its surviving
 // tracks one by one - the record as SoA columns and the kept hits as gids in ascending row order (L3).
 // Output order = tracklet order.
@@ -170,9 +197,10 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
       uint32_t idx[kOutChunks], g[kOutChunks];
 #pragma unroll
-      for (int q = 0; q < kOutChunks; ++q) {
+      for (int q = 0; q < kOutChunks; ++q) {  // kept (L1): the entry carries kOwnedBit
         const int r = rb0 + 32 * q + lane;
-        idx[q] = r <= last ? map[r] : kNoHit;
+        const uint32_t e = r <= last ? map[r] : kNoHit;
+        idx[q] = (e != kNoHit && (e & kOwnedBit)) ? (e & ~kOwnedBit) : kNoHit;
       }
 #pragma unroll
       for (int q = 0; q < kOutChunks; ++q) g[q] = idx[q] != kNoHit ? c.gid[idx[q]] : 0u;
