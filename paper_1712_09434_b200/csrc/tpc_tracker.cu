@@ -70,6 +70,14 @@ uint32_t resolve_max_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tr
   return n / m + 1u;  // chains are vertex disjoint and hold >= min_seed_hits clusters each (S2, S3)
 }
 
+// tpc_track_batch_host: tracklet slots of all chunks together.  Every chunk gets min(max_tracklets, what its
+// clusters can seed at most), so a chunk never overflows while the whole batch would have fitted.
+uint32_t host_total_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tracklets, uint32_t chunks) {
+  const uint64_t worst = (uint64_t)resolve_max_tracklets(t, n, 0u) + chunks;
+  const uint64_t want = max_tracklets ? (uint64_t)max_tracklets * chunks : worst;
+  return (uint32_t)(want < worst ? want : worst);
+}
+
 // Offsets of every workspace array, in bytes.
 struct Carve {
   size_t yz, gid, bins, rowinfo, tile_tr, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
@@ -353,9 +361,13 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   cudaEvent_t* ev = nullptr;  // stage marks of this call (nullptr: timing off)
   if (t->timing_on) {
     if (t->ev.empty()) {
-      t->ev.resize((size_t)TPC_STAGE_RING * (TPC_N_STAGES + 1));
+      t->ev.resize((size_t)TPC_STAGE_RING * (TPC_N_STAGES + 1), nullptr);
       for (cudaEvent_t& x : t->ev)
-        if (cudaEventCreate(&x) != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch: cudaEventCreate failed");
+        if (cudaEventCreate(&x) != cudaSuccess) {
+          for (cudaEvent_t& y : t->ev) if (y) cudaEventDestroy(y);
+          t->ev.clear();
+          return fail(t, TPC_ERR_CUDA, "tpc_track_batch: cudaEventCreate failed");
+        }
     }
     ev = t->ev.data() + (size_t)(t->timed_calls % TPC_STAGE_RING) * (TPC_N_STAGES + 1);
     ++t->timed_calls;
@@ -483,7 +495,7 @@ HostCarve host_carve(const tpc_tracker* t, uint32_t n, uint32_t n_tasks, uint32_
 size_t tpc_host_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t max_tasks, uint32_t max_tracklets,
                                 uint32_t track_capacity, uint32_t hit_capacity) {
   if (!t) return 0;
-  const uint32_t T = resolve_max_tracklets(t, max_clusters, max_tracklets) + kHostChunks;
+  const uint32_t T = host_total_tracklets(t, max_clusters, max_tracklets, kHostChunks);
   return host_carve(t, max_clusters, max_tasks, T, track_capacity, hit_capacity).total;
 }
 
@@ -498,7 +510,7 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
     return fail(t, TPC_ERR_ARGUMENT, "tpc_track_batch_host: dbg_* outputs are not supported on host buffers");
   const uint32_t n = in->n_clusters, tcap = out->track_capacity, hcap = out->hit_capacity;
   const uint32_t n_rows = (uint32_t)t->n_rows;
-  const uint32_t T_all = resolve_max_tracklets(t, n, max_tracklets) + kHostChunks;
+  const uint32_t T_all = host_total_tracklets(t, n, max_tracklets, kHostChunks);
   const HostCarve h = host_carve(t, n, in->n_tasks, T_all, tcap, hcap);
   if (!workspace || workspace_bytes < h.total)
     return fail(t, TPC_ERR_WORKSPACE, "tpc_track_batch_host: workspace of %zu bytes, need %zu", workspace_bytes, h.total);
@@ -509,15 +521,17 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   const uint32_t* ro = in->row_offsets;
   if (ro[(size_t)in->n_tasks * n_rows] != n)
     return fail(t, TPC_ERR_ARGUMENT, "tpc_track_batch_host: row_offsets must end at n_clusters");
-  // chunk boundaries: whole tasks; a small first chunk (the kernels start early) and a small last one (a short
-  // copy-back tail) measured best on config 3: 19.1 ms against 19.9 ms with four equal chunks
-  uint32_t n_chunks = (n >= kHostChunkMinClusters && in->n_tasks >= kHostChunks) ? kHostChunks : 1u;
+  // chunk boundaries: whole tasks; a small first chunk (the kernels start early) and a middle-sized last one (its
+  // copy-back is the tail) measured best on config 3 with the four-kernel tracklet constructor, whose persistent
+  // kernels cost about 0.3 ms per extra chunk: 18.1 ms against 18.8 ms with cuts at 12 / 45 / 80 %
+  static const double cut[] = {0.0, 0.15, 0.55, 1.0};
+  constexpr uint32_t kCuts = sizeof(cut) / sizeof(cut[0]) - 1;
+  static_assert(kCuts <= kHostChunks, "streams, events and headers are sized for kHostChunks chunks");
+  uint32_t n_chunks = (n >= kHostChunkMinClusters && in->n_tasks >= kCuts) ? kCuts : 1u;
   uint32_t task_b[kHostChunks + 1];
   task_b[0] = 0u;
   for (uint32_t k = 1; k < n_chunks; ++k) {
-    static_assert(kHostChunks == 4, "kCut lists the cuts of four chunks");
-    static const double kCut[kHostChunks + 1] = {0.0, 0.12, 0.45, 0.80, 1.0};
-    const uint64_t want = (uint64_t)((double)n * kCut[k]);
+    const uint64_t want = (uint64_t)((double)n * cut[k]);
     uint32_t lo = task_b[k - 1], hi = in->n_tasks;  // first task whose clusters start at or after `want`
     while (lo < hi) {
       const uint32_t mid = lo + (hi - lo) / 2;
@@ -529,12 +543,18 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   // streams and events of the chunks, created on first use
   cudaError_t e = cudaSuccess;
   if (t->host_streams.empty()) {
-    t->host_streams.resize(kHostChunks);
-    t->host_events.resize(2 * kHostChunks + 1);  // [k] chunk k computed, [kHostChunks] start, [kHostChunks + 1 + k] chunk k copied in
+    t->host_streams.resize(kHostChunks, nullptr);
+    t->host_events.resize(2 * kHostChunks + 1, nullptr);  // [k] chunk k computed, [kHostChunks] start, [kHostChunks + 1 + k] chunk k copied in
     for (auto& x : t->host_streams) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking);
     for (auto& x : t->host_events) if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->host_headers, 16 * kHostChunks, cudaHostAllocDefault);
-    if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) {  // leave nothing half made behind: the next call starts again
+      for (auto& x : t->host_streams) if (x) cudaStreamDestroy(x);
+      for (auto& x : t->host_events) if (x) cudaEventDestroy(x);
+      if (t->host_headers) cudaFreeHost(t->host_headers);
+      t->host_streams.clear(); t->host_events.clear(); t->host_headers = nullptr;
+      return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA: %s", cudaGetErrorString(e));
+    }
   }
   const bool timing = t->timing_on, counters = t->counters_on;
   t->timing_on = false; t->counters_on = false;  // per-stage marks and counters describe one tpc_track_batch call
@@ -557,7 +577,8 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
     c.task0 = task_b[k]; c.n_tasks = task_b[k + 1] - task_b[k];
     c.idx0 = ro[(size_t)c.task0 * n_rows];
     c.n = ro[(size_t)task_b[k + 1] * n_rows] - c.idx0;
-    c.T = n_chunks == 1 ? T_all - kHostChunks : (uint32_t)((uint64_t)(T_all - kHostChunks) * c.n / (n ? n : 1)) + 1u;
+    c.T = resolve_max_tracklets(t, c.n, 0u);
+    if (max_tracklets && max_tracklets < c.T) c.T = max_tracklets;
     c.tcap = c.n / mh + 1u < tcap ? c.n / mh + 1u : tcap;
     c.hcap = c.n + 1u < hcap ? c.n + 1u : hcap;
     c.t0 = t_used; c.h0 = h_used;
