@@ -48,6 +48,22 @@ class _Out(C.Structure):
     ]
 
 
+class _MergeIn(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint32), ("track_capacity", C.c_uint32),
+                ("track_task", C.c_void_p), ("track_hit_begin", C.c_void_p), ("track_nhits", C.c_void_p),
+                ("track_ndf", C.c_void_p),
+                ("track_x", C.c_void_p), ("track_par", C.c_void_p), ("track_cov", C.c_void_p),
+                ("track_chi2", C.c_void_p), ("hit_cluster", C.c_void_p)]
+
+
+class _MergeOut(C.Structure):
+    _fields_ = [("next", C.c_void_p), ("prev", C.c_void_p), ("merged_capacity", C.c_uint32),
+                ("merged_first", C.c_void_p), ("merged_nseg", C.c_void_p), ("merged_nhits", C.c_void_p),
+                ("merged_nfit", C.c_void_p), ("merged_sector", C.c_void_p), ("merged_ndf", C.c_void_p),
+                ("merged_x", C.c_void_p), ("merged_par", C.c_void_p), ("merged_cov", C.c_void_p),
+                ("merged_chi2", C.c_void_p), ("n_merged", C.c_uint32), ("n_links", C.c_uint32)]
+
+
 @dataclass
 class OracleParams:
     """Defaults of docs/ARITH_SPEC.md section 8 (the oracle's own copy)."""
@@ -122,6 +138,15 @@ def _load():
         _lib.oracle_transport_f32.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float]
         _lib.oracle_update_f64.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double]
         _lib.oracle_update_f32.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_float]
+        _lib.oracle_sizeof_merge_in.restype = C.c_size_t
+        _lib.oracle_sizeof_merge_out.restype = C.c_size_t
+        assert _lib.oracle_sizeof_merge_in() == C.sizeof(_MergeIn)
+        assert _lib.oracle_sizeof_merge_out() == C.sizeof(_MergeOut)
+        for n in ("oracle_merge_f32", "oracle_merge_f64", "oracle_rotate_f32", "oracle_rotate_f64",
+                  "oracle_refit_hits_f64"):
+            getattr(_lib, n).restype = C.c_int
+        _lib.oracle_rotate_f64.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double]
+        _lib.oracle_rotate_f32.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float]
     return _lib
 
 
@@ -212,6 +237,107 @@ def update(p, c, i, m, e, chi2=0.0, ndf=0, precision="f64"):
     fn = lib.oracle_update_f64 if precision == "f64" else lib.oracle_update_f32
     fn(_ptr(s), _ptr(nd), i, m, e)
     return s[1:6].copy(), s[6:21].copy(), dt(s[21]), int(nd[0])
+
+
+@dataclass
+class MergeResult:
+    """SPEC 9: links between the sector tracks (G6) and the refitted merged tracks (F3)."""
+    next: np.ndarray          # [n_tracks] index of the segment that continues track i outwards, or -1
+    prev: np.ndarray
+    merged_first: np.ndarray  # [n_merged] innermost segment (track index); merged tracks in this order
+    merged_nseg: np.ndarray
+    merged_nhits: np.ndarray
+    merged_nfit: np.ndarray
+    merged_sector: np.ndarray
+    merged_ndf: np.ndarray
+    merged_x: np.ndarray
+    merged_par: np.ndarray    # [5, n_merged]
+    merged_cov: np.ndarray    # [15, n_merged]
+    merged_chi2: np.ndarray
+    n_links: int = 0
+
+
+def merge_refit(geometry, y, z, row_offsets, n_tasks: int, tracks, params: Optional[OracleParams] = None,
+                chi2_max: float = 50.0, max_row_gap: int = 8, precision: str = "f32") -> MergeResult:
+    """SPEC 9 on the tracks of ``track()`` (any object with track_task, track_hit_begin, track_nhits, track_x,
+    track_par [5,n], track_cov [15,n], hit_cluster); the tracks may be given in any order."""
+    lib = _load()
+    prm = params or OracleParams()
+    dt = np.float32 if precision == "f32" else np.float64
+    y = np.ascontiguousarray(y, dtype=dt)
+    z = np.ascontiguousarray(z, dtype=dt)
+    ro = np.ascontiguousarray(row_offsets, dtype=np.uint32)
+    n, nr = int(y.shape[0]), int(geometry.n_rows)
+    row_x = np.ascontiguousarray(geometry.row_x, dtype=np.float32)
+    g = _Geom(int(geometry.n_sectors), nr, row_x.ctypes.data_as(C.POINTER(C.c_float)),
+              float(geometry.tan_half_angle), float(geometry.z_max))
+    nt = int(len(tracks.track_task))
+    cap = max(nt, 1)
+    t_task = np.ascontiguousarray(tracks.track_task, np.uint32)
+    t_beg = np.ascontiguousarray(tracks.track_hit_begin, np.uint32)
+    t_nh = np.ascontiguousarray(tracks.track_nhits, np.uint32)
+    t_x = np.ascontiguousarray(tracks.track_x, dt)
+    t_ndf = np.ascontiguousarray(getattr(tracks, "track_ndf", np.zeros(nt)), np.int32)
+    t_chi2 = np.ascontiguousarray(getattr(tracks, "track_chi2", np.zeros(nt)), dt)
+    t_par = np.zeros((5, cap), dt); t_par[:, :nt] = tracks.track_par
+    t_cov = np.zeros((15, cap), dt); t_cov[:, :nt] = tracks.track_cov
+    hits = np.ascontiguousarray(tracks.hit_cluster, np.uint32)
+    mi = _MergeIn(nt, cap, _ptr(t_task), _ptr(t_beg), _ptr(t_nh), _ptr(t_ndf), _ptr(t_x), _ptr(t_par), _ptr(t_cov),
+                  _ptr(t_chi2), _ptr(hits))
+    nxt, prv = np.empty(cap, np.int32), np.empty(cap, np.int32)
+    u32 = lambda: np.empty(cap, np.uint32)  # noqa: E731
+    m_first, m_nseg, m_nh, m_nfit, m_sec = u32(), u32(), u32(), u32(), u32()
+    m_ndf = np.empty(cap, np.int32)
+    m_x, m_chi2 = np.empty(cap, dt), np.empty(cap, dt)
+    m_par, m_cov = np.empty((5, cap), dt), np.empty((15, cap), dt)
+    mo = _MergeOut(_ptr(nxt), _ptr(prv), cap, _ptr(m_first), _ptr(m_nseg), _ptr(m_nh), _ptr(m_nfit), _ptr(m_sec),
+                   _ptr(m_ndf), _ptr(m_x), _ptr(m_par), _ptr(m_cov), _ptr(m_chi2), 0, 0)
+    fn = lib.oracle_merge_f32 if precision == "f32" else lib.oracle_merge_f64
+    rc = fn(C.byref(g), C.c_float(float(geometry.bz_kgauss)), C.byref(prm._c()), C.c_float(chi2_max),
+            C.c_int32(max_row_gap), C.c_uint32(n), C.c_uint32(n_tasks), _ptr(y), _ptr(z), _ptr(ro),
+            C.byref(mi), C.byref(mo))
+    if rc != 0:
+        raise RuntimeError(f"oracle_merge returned {rc}")
+    m = mo.n_merged
+    return MergeResult(nxt[:nt].copy(), prv[:nt].copy(), m_first[:m].copy(), m_nseg[:m].copy(), m_nh[:m].copy(),
+                       m_nfit[:m].copy(), m_sec[:m].copy(), m_ndf[:m].copy(), m_x[:m].copy(), m_par[:, :m].copy(),
+                       m_cov[:, :m].copy(), m_chi2[:m].copy(), n_links=int(mo.n_links))
+
+
+def rotate(x, p, c, d, n_sectors, a, max_sinphi=0.95, precision="f64"):
+    """SPEC 9.1 on one state; returns (ok, x, p[5], c[15])."""
+    lib = _load()
+    dt = np.float64 if precision == "f64" else np.float32
+    s = np.zeros(22, dt)
+    s[0] = x
+    s[1:6] = p
+    s[6:21] = c
+    fn = lib.oracle_rotate_f64 if precision == "f64" else lib.oracle_rotate_f32
+    ok = fn(_ptr(s), int(d), int(n_sectors), a, max_sinphi)
+    return bool(ok), dt(s[0]), s[1:6].copy(), s[6:21].copy()
+
+
+def refit_hits(geometry, sector, row, y, z, x0, p0, c0, sector0, params: Optional[OracleParams] = None):
+    """SPEC 9.3 (fp64) on an explicit hit list, outermost first, started from the state (x0, p0[5], c0[15]) in the
+    frame of sector0; returns (n_fit, x, p[5], c[15], chi2, ndf, sector)."""
+    lib = _load()
+    prm = params or OracleParams()
+    row_x = np.ascontiguousarray(geometry.row_x, dtype=np.float32)
+    g = _Geom(int(geometry.n_sectors), int(geometry.n_rows), row_x.ctypes.data_as(C.POINTER(C.c_float)),
+              float(geometry.tan_half_angle), float(geometry.z_max))
+    sector = np.ascontiguousarray(sector, np.int32)
+    row = np.ascontiguousarray(row, np.int32)
+    y = np.ascontiguousarray(y, np.float64)
+    z = np.ascontiguousarray(z, np.float64)
+    s = np.zeros(22, np.float64)
+    s[0] = x0
+    s[1:6] = p0
+    s[6:21] = c0
+    ndf, sec = np.zeros(1, np.int32), np.array([sector0], np.int32)
+    n_fit = lib.oracle_refit_hits_f64(C.byref(g), C.c_float(float(geometry.bz_kgauss)), C.byref(prm._c()),
+                                      C.c_uint32(len(row)), _ptr(sector), _ptr(row), _ptr(y), _ptr(z), _ptr(s),
+                                      _ptr(ndf), _ptr(sec))
+    return int(n_fit), s[0], s[1:6].copy(), s[6:21].copy(), s[21], int(ndf[0]), int(sec[0])
 
 
 def canonical_tracks(track_task, track_hit_begin, track_nhits, hit_cluster):

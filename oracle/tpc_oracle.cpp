@@ -21,6 +21,10 @@
 // helix + finite-difference Jacobian; update vs matrix-form Kalman; noiseless
 // helices recovered to 1e-5 (fp64 instantiation); unit pulls; mirror / batch /
 // grid-size invariances; hand-built examples.
+// SPEC 9 (sector-segment merger + refit) is pinned by tests/test_oracle_merge.py: rotation vs
+// the closed-form helix in the neighbour's frame and vs finite differences, noiseless crossing tracks merged into
+// one track with every cluster and refitted to truth (1e-5, fp64), unit pulls of the refit, no merge of
+// unrelated segments, independence of the track order.
 // PARITY UNPINNED: the numeric defaults (windows, cuts, initial covariance,
 // gap, minimum lengths) - nothing in the paper fixes them.
 //
@@ -501,6 +505,209 @@ int run(const OGeometry* g, float bz, const OParams* p, uint32_t n, uint32_t nt,
   return status;
 }
 
+// ===========================================================================
+// SPEC 9: sector-segment merger and final refit ("merges the tracks segments afterward";
+// L140: the refit the paper wants on the GPU).  Written out step by step (R1..R7, G1..G7, F1..F3).
+// ===========================================================================
+template <class R> struct MergeTables {
+  int n_half;
+  R ca, sa;
+  MergeTables(int n_sectors) {
+    n_half = n_sectors >= 2 ? n_sectors / 2 : 1;
+    const double alpha = 2.0 * 3.14159265358979323846 / (double)n_half;
+    ca = (R)(float)std::cos(alpha);  // SPEC 9 tables: computed in double, rounded to fp32
+    sa = (R)(float)std::sin(alpha);
+    if (sizeof(R) == 8) { ca = (R)std::cos(alpha); sa = (R)std::sin(alpha); }  // fp64 instantiation: exact angle
+  }
+};
+
+// SPEC 9.1 ROTATE(state, d). Returns false and leaves st untouched on failure.
+template <class R> bool rotate(State<R>& st, int d, R ca, R sa_abs, R a, R max_sinphi) {
+  const R sa = d > 0 ? sa_abs : -sa_abs;
+  const R x = st.x, y = st.p[0], s = st.p[2], t = st.p[3], q = st.p[4];
+  const R c = rsqrt_(R(1) - s * s);                            // R1
+  const R s1 = s * ca - c * sa;                                // R2
+  const R c1 = c * ca + s * sa;
+  if (!(c1 > R(0) && rabs(s1) <= max_sinphi)) return false;    // R3
+  const R j00 = ca - (s1 / c1) * sa;                           // R5
+  const R j10 = -((t / c1) * sa);
+  const R j20 = -((a * q) * sa);
+  const R j22 = ca + (s / c) * sa;
+  const R c00 = st.c[0], c10 = st.c[1], c11 = st.c[2], c20 = st.c[3], c21 = st.c[4], c22 = st.c[5], c30 = st.c[6],
+          c31 = st.c[7], c32 = st.c[8], c40 = st.c[10], c41 = st.c[11], c42 = st.c[12];
+  const R m00 = j00 * c00;                                     // R6
+  const R m10 = j10 * c00 + c10, m11 = j10 * c10 + c11;
+  const R m20 = j20 * c00 + j22 * c20, m21 = j20 * c10 + j22 * c21, m22 = j20 * c20 + j22 * c22;
+  st.c[0] = m00 * j00;                                         // R7
+  st.c[1] = m10 * j00; st.c[2] = m10 * j10 + m11;
+  st.c[3] = m20 * j00; st.c[4] = m20 * j10 + m21; st.c[5] = m20 * j20 + m22 * j22;
+  st.c[6] = c30 * j00; st.c[7] = c30 * j10 + c31; st.c[8] = c30 * j20 + c32 * j22;
+  st.c[10] = c40 * j00; st.c[11] = c40 * j10 + c41; st.c[12] = c40 * j20 + c42 * j22;
+  st.x = x * ca + y * sa;                                      // R4
+  st.p[0] = y * ca - x * sa;
+  st.p[2] = s1;
+  return true;
+}
+
+struct OHit { int sector, row; uint32_t gid; };
+
+// direction from sector `from` to its neighbour `to` (same side), SPEC 9: +1, -1, or 0 if not neighbours
+inline int neighbour_dir(int from, int to, int n_half) {
+  const int f = from % n_half, g = to % n_half;
+  if ((from / n_half) != (to / n_half) || n_half < 2) return 0;
+  if ((f + 1) % n_half == g) return +1;
+  if ((g + 1) % n_half == f) return -1;
+  return 0;
+}
+
+// SPEC 9.3 F1..F3 over the hits of a chain, outermost first; st = the state F1 starts from (O_im, in the frame
+// of `sector`).  Returns nFit.
+template <class R>
+int refit_hits(const Tables<R>& T, const MergeTables<R>& MT, const std::vector<OHit>& hits, const R* Y, const R* Z,
+               State<R>& st, int& sector) {
+  for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);                       // F1
+  st.chi2 = R(0); st.ndf = -5;
+  int n_fit = 0;
+  for (size_t k = 0; k < hits.size(); ++k) {                                                      // F2
+    const OHit& h = hits[k];
+    if (h.sector != sector) {
+      const int d = neighbour_dir(sector, h.sector, MT.n_half);
+      if (d == 0 || !rotate(st, d, MT.ca, MT.sa, T.a, R(T.prm.max_sinphi))) break;
+      sector = h.sector;
+    }
+    if (st.x != T.X[h.row] && !transport(st, T.X[h.row], T.a, R(T.prm.max_sinphi))) break;
+    update(st, 0, Y[h.gid], T.sy2);
+    update(st, 1, Z[h.gid], T.sz2);
+    ++n_fit;
+  }
+  return n_fit;                                                                                   // F3
+}
+
+struct OMergeIn {   // the tracks of SPEC 7 as run() wrote them
+  uint32_t n_tracks, track_capacity;
+  const uint32_t *track_task, *track_hit_begin, *track_nhits;
+  const int32_t* track_ndf;
+  const void *track_x, *track_par, *track_cov, *track_chi2;  // R*; par [5][cap], cov [15][cap]
+  const uint32_t* hit_cluster;
+};
+struct OMergeOut {  // caller-allocated
+  int32_t *next, *prev;  // [n_tracks] G6
+  uint32_t merged_capacity;
+  uint32_t *merged_first, *merged_nseg, *merged_nhits, *merged_nfit, *merged_sector;
+  int32_t* merged_ndf;
+  void *merged_x, *merged_par, *merged_cov, *merged_chi2;  // par [5][cap], cov [15][cap]
+  uint32_t n_merged, n_links;
+};
+
+template <class R>
+int merge_refit(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
+                uint32_t nt, const R* Y, const R* Z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
+  Tables<R> T(*g, bz, *p);
+  MergeTables<R> MT(g->n_sectors);
+  const int nr = T.n_rows, ns = g->n_sectors;
+  const uint32_t nT = in->n_tracks, cap = in->track_capacity;
+  std::vector<uint32_t> tr_of(n);
+  for (size_t tr = 0; tr < (size_t)nt * nr; ++tr)
+    for (uint32_t h = ro[tr]; h < ro[tr + 1]; ++h) tr_of[h] = (uint32_t)tr;
+  auto state_of = [&](uint32_t i) {
+    State<R> st;
+    st.x = ((const R*)in->track_x)[i];
+    for (int j = 0; j < 5; ++j) st.p[j] = ((const R*)in->track_par)[(size_t)j * cap + i];
+    for (int j = 0; j < 15; ++j) st.c[j] = ((const R*)in->track_cov)[(size_t)j * cap + i];
+    st.chi2 = R(0); st.ndf = 0;
+    return st;
+  };
+  std::vector<int> rf(nT), rl(nT);
+  std::vector<uint32_t> gid_first(nT);
+  std::vector<State<R>> outer(nT);
+  std::vector<char> has_outer(nT, 0);
+  for (uint32_t i = 0; i < nT; ++i) {                                                       // G1
+    const uint32_t b = in->track_hit_begin[i], m = in->track_nhits[i];
+    gid_first[i] = in->hit_cluster[b];
+    rf[i] = (int)(tr_of[in->hit_cluster[b]] % nr);
+    rl[i] = (int)(tr_of[in->hit_cluster[b + m - 1]] % nr);
+    outer[i] = state_of(i);
+    has_outer[i] = (outer[i].x == T.X[rl[i]] || transport(outer[i], T.X[rl[i]], T.a, R(p->max_sinphi))) ? 1 : 0;
+  }
+  // G2..G5: every ordered pair (plain double loop: this is the definition, not an index structure)
+  std::vector<int32_t> best_out(nT, -1), best_in(nT, -1);
+  std::vector<R> chi_out(nT, R(0)), chi_in(nT, R(0));
+  for (uint32_t i = 0; i < nT; ++i) {
+    if (!has_outer[i]) continue;
+    const int si = (int)(in->track_task[i] % ns), ei = (int)(in->track_task[i] / ns);
+    for (uint32_t j = 0; j < nT; ++j) {
+      if (j == i || (int)(in->track_task[j] / ns) != ei) continue;
+      const int sj = (int)(in->track_task[j] % ns);
+      int d = neighbour_dir(si, sj, MT.n_half);
+      if (d == 0) continue;
+      if (MT.n_half <= 2) d = +1;
+      if (!(rl[i] < rf[j] && rf[j] <= rl[i] + max_row_gap)) continue;                       // G2
+      State<R> q = outer[i];                                                                // G3
+      if (!rotate(q, d, MT.ca, MT.sa, T.a, R(p->max_sinphi))) continue;
+      const State<R> sj_state = state_of(j);
+      if (q.x != sj_state.x && !transport(q, sj_state.x, T.a, R(p->max_sinphi))) continue;
+      R chi = R(0);                                                                         // G4
+      for (int k = 0; k < 5; ++k) {
+        const R dk = q.p[k] - sj_state.p[k];
+        chi = chi + (dk * dk) / (q.c[tri(k, k)] + sj_state.c[tri(k, k)]);
+      }
+      if (!(chi < R(chi2_max))) continue;
+      if (best_out[i] < 0 || chi < chi_out[i] || (chi == chi_out[i] && gid_first[j] < gid_first[best_out[i]])) {
+        best_out[i] = (int32_t)j; chi_out[i] = chi;                                         // G5
+      }
+      if (best_in[j] < 0 || chi < chi_in[j] || (chi == chi_in[j] && gid_first[i] < gid_first[best_in[j]])) {
+        best_in[j] = (int32_t)i; chi_in[j] = chi;
+      }
+    }
+  }
+  uint32_t n_links = 0;
+  for (uint32_t i = 0; i < nT; ++i) { o->next[i] = -1; o->prev[i] = -1; }
+  for (uint32_t i = 0; i < nT; ++i) {                                                       // G6
+    const int32_t j = best_out[i];
+    if (j >= 0 && best_in[j] == (int32_t)i) { o->next[i] = j; o->prev[j] = (int32_t)i; ++n_links; }
+  }
+  // G7 + F1..F3: chains in the order of their innermost segment
+  uint32_t n_merged = 0;
+  int status = 0;
+  for (uint32_t i1 = 0; i1 < nT; ++i1) {
+    if (o->prev[i1] >= 0) continue;
+    std::vector<uint32_t> chain;
+    for (int32_t k = (int32_t)i1; k >= 0; k = o->next[k]) chain.push_back((uint32_t)k);
+    std::vector<OHit> hits;
+    for (size_t c = chain.size(); c-- > 0;) {
+      const uint32_t i = chain[c], b = in->track_hit_begin[i], m = in->track_nhits[i];
+      for (uint32_t k = m; k-- > 0;) {
+        const uint32_t gid = in->hit_cluster[b + k];
+        hits.push_back({(int)(in->track_task[i] % ns), (int)(tr_of[gid] % nr), gid});
+      }
+    }
+    if (n_merged >= o->merged_capacity) { status = 1; break; }
+    const uint32_t im = chain.back();
+    State<R> st = has_outer[im] ? outer[im] : state_of(im);
+    int sector = (int)(in->track_task[im] % ns), n_fit = 0;
+    if (has_outer[im]) {
+      n_fit = refit_hits(T, MT, hits, Y, Z, st, sector);
+    } else {  // F1: no outer end, no refit
+      st.chi2 = ((const R*)in->track_chi2)[im];
+      st.ndf = in->track_ndf[im];
+    }
+    const uint32_t mcap = o->merged_capacity, t = n_merged++;
+    o->merged_first[t] = i1;
+    o->merged_nseg[t] = (uint32_t)chain.size();
+    o->merged_nhits[t] = (uint32_t)hits.size();
+    o->merged_nfit[t] = (uint32_t)n_fit;
+    o->merged_sector[t] = (uint32_t)sector;
+    o->merged_ndf[t] = st.ndf;
+    ((R*)o->merged_x)[t] = st.x;
+    ((R*)o->merged_chi2)[t] = st.chi2;
+    for (int j = 0; j < 5; ++j) ((R*)o->merged_par)[(size_t)j * mcap + t] = st.p[j];
+    for (int j = 0; j < 15; ++j) ((R*)o->merged_cov)[(size_t)j * mcap + t] = st.c[j];
+  }
+  o->n_merged = n_merged;
+  o->n_links = n_links;
+  return status;
+}
+
 }  // namespace
 
 extern "C" {
@@ -562,4 +769,61 @@ void oracle_update_f32(float* s22, int32_t* ndf, int i, float m, float e) {
   s22[21] = st.chi2; *ndf = st.ndf;
 }
 
+
+// --- SPEC 9 -------------------------------------------------------------------
+size_t oracle_sizeof_merge_in() { return sizeof(OMergeIn); }
+size_t oracle_sizeof_merge_out() { return sizeof(OMergeOut); }
+int oracle_merge_f32(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
+                     uint32_t nt, const float* y, const float* z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
+  return merge_refit<float>(g, bz, p, chi2_max, max_row_gap, n, nt, y, z, ro, in, o);
+}
+int oracle_merge_f64(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
+                     uint32_t nt, const double* y, const double* z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
+  return merge_refit<double>(g, bz, p, chi2_max, max_row_gap, n, nt, y, z, ro, in, o);
+}
+// ROTATE on a state laid out as x, p[5], c[15], chi2 (22 reals)
+int oracle_rotate_f64(double* s22, int d, int n_sectors, double a, double max_sinphi) {
+  MergeTables<double> MT(n_sectors);
+  State<double> st; st.x = s22[0];
+  for (int i = 0; i < 5; ++i) st.p[i] = s22[1 + i];
+  for (int i = 0; i < 15; ++i) st.c[i] = s22[6 + i];
+  st.chi2 = s22[21]; st.ndf = 0;
+  const bool ok = rotate(st, d, MT.ca, MT.sa, a, max_sinphi);
+  s22[0] = st.x;
+  for (int i = 0; i < 5; ++i) s22[1 + i] = st.p[i];
+  for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
+  return ok ? 1 : 0;
+}
+int oracle_rotate_f32(float* s22, int d, int n_sectors, float a, float max_sinphi) {
+  MergeTables<float> MT(n_sectors);
+  State<float> st; st.x = s22[0];
+  for (int i = 0; i < 5; ++i) st.p[i] = s22[1 + i];
+  for (int i = 0; i < 15; ++i) st.c[i] = s22[6 + i];
+  st.chi2 = s22[21]; st.ndf = 0;
+  const bool ok = rotate(st, d, MT.ca, MT.sa, a, max_sinphi);
+  s22[0] = st.x;
+  for (int i = 0; i < 5; ++i) s22[1 + i] = st.p[i];
+  for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
+  return ok ? 1 : 0;
+}
+// SPEC 9.3 on an explicit hit list (outermost first): sector[], row[], and (y,z) per hit; s22 = the state F1
+// starts from (x, p, C in the frame of sector_io), replaced by the result; returns nFit
+int oracle_refit_hits_f64(const OGeometry* g, float bz, const OParams* p, uint32_t n_hits, const int32_t* sector,
+                          const int32_t* row, const double* y, const double* z, double* s22, int32_t* ndf,
+                          int32_t* sector_io) {
+  Tables<double> T(*g, bz, *p);
+  MergeTables<double> MT(g->n_sectors);
+  std::vector<OHit> hits;
+  for (uint32_t k = 0; k < n_hits; ++k) hits.push_back({sector[k], row[k], k});
+  State<double> st; st.x = s22[0];
+  for (int i = 0; i < 5; ++i) st.p[i] = s22[1 + i];
+  for (int i = 0; i < 15; ++i) st.c[i] = s22[6 + i];
+  int sec = *sector_io;
+  const int n_fit = refit_hits(T, MT, hits, y, z, st, sec);
+  s22[0] = st.x;
+  for (int i = 0; i < 5; ++i) s22[1 + i] = st.p[i];
+  for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
+  s22[21] = st.chi2; *ndf = st.ndf; *sector_io = sec;
+  return n_fit;
+}
 }  // extern "C"

@@ -18,7 +18,8 @@ import tempfile
 from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-SUITES = ["tests/test_oracle_units.py", "tests/test_oracle_tracker.py", "tests/test_oracle_following.py"]
+SUITES = ["tests/test_oracle_units.py", "tests/test_oracle_tracker.py", "tests/test_oracle_following.py",
+          "tests/test_oracle_merge.py"]
 
 # (name, SPEC tag, text in oracle/tpc_oracle.cpp, replacement)
 MUTANTS = [
@@ -107,6 +108,43 @@ MUTANTS = [
      "n[2] = m11 + f12 * m12 + f13 * m13 + f14 * m14;", "n[2] = m11 + f12 * m12 + f13 * m13;"),
     ("update gain sign", "U5",
      "st.p[j] = st.p[j] + k[j] * res;", "st.p[j] = st.p[j] - k[j] * res;"),
+    # ---- SPEC 9: merger and refit ----
+    ("rotation: y' with the wrong sign of sa", "R4",
+     "st.p[0] = y * ca - x * sa;", "st.p[0] = y * ca + x * sa;"),
+    ("rotation: sin(phi) turned the other way", "R2",
+     "const R s1 = s * ca - c * sa;                                // R2", "const R s1 = s * ca + c * sa;"),
+    ("rotation: x' not moved", "R4",
+     "st.x = x * ca + y * sa;                                      // R4", "st.x = x * ca;"),
+    ("rotation jacobian: point not taken back along the track (j00 = ca)", "R5",
+     "const R j00 = ca - (s1 / c1) * sa;                           // R5", "const R j00 = ca;"),
+    ("rotation jacobian: j10 dropped", "R5",
+     "const R j10 = -((t / c1) * sa);", "const R j10 = R(0);"),
+    ("rotation jacobian: j20 dropped", "R5",
+     "const R j20 = -((a * q) * sa);", "const R j20 = R(0);"),
+    ("rotation jacobian: j22 = ca", "R5",
+     "const R j22 = ca + (s / c) * sa;", "const R j22 = ca;"),
+    ("rotation covariance: c21' loses m21", "R7",
+     "st.c[4] = m20 * j10 + m21;", "st.c[4] = m20 * j10;"),
+    ("rotation: angle limit not tested", "R3",
+     "if (!(c1 > R(0) && rabs(s1) <= max_sinphi)) return false;    // R3", "if (!(c1 > R(0))) return false;"),
+    ("merger: rows may overlap (rl_i <= rf_j)", "G2",
+     "if (!(rl[i] < rf[j] && rf[j] <= rl[i] + max_row_gap)) continue;", "if (!(rl[i] <= rf[j] && rf[j] <= rl[i] + max_row_gap)) continue;"),
+    ("merger: row gap off by one", "G2",
+     "if (!(rl[i] < rf[j] && rf[j] <= rl[i] + max_row_gap)) continue;", "if (!(rl[i] < rf[j] && rf[j] < rl[i] + max_row_gap)) continue;"),
+    ("merger: matched at the outer end's x, no transport to the first row of j", "G3",
+     "if (q.x != sj_state.x && !transport(q, sj_state.x, T.a, R(p->max_sinphi))) continue;", ""),
+    ("merger: chi2 without the q/pT term", "G4",
+     "for (int k = 0; k < 5; ++k) {\n        const R dk = q.p[k] - sj_state.p[k];", "for (int k = 0; k < 4; ++k) {\n        const R dk = q.p[k] - sj_state.p[k];"),
+    ("merger: chi2 cut not applied", "G4",
+     "if (!(chi < R(chi2_max))) continue;", ""),
+    ("merger: tie goes to the larger first hit", "G5",
+     "(chi == chi_in[j] && gid_first[i] < gid_first[best_in[j]])", "(chi == chi_in[j] && gid_first[i] > gid_first[best_in[j]])"),
+    ("merger: links need not be mutual", "G6",
+     "if (j >= 0 && best_in[j] == (int32_t)i) {", "if (j >= 0) {"),
+    ("refit: covariance not inflated", "F1",
+     "for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);                       // F1", ""),
+    ("refit: no rotation at the sector change", "F2",
+     "if (d == 0 || !rotate(st, d, MT.ca, MT.sa, T.a, R(T.prm.max_sinphi))) break;\n      sector = h.sector;", "sector = h.sector;"),
 ]
 
 # Not a mutant: semantically equivalent to the SPEC text, listed so that nobody tries to kill it again.
@@ -114,6 +152,9 @@ EQUIVALENT = [
     ("a chain-fit transport failure continues into the up pass (chain_ok ignored)", "K2 -> K4",
      "the up pass would start with the transport from lastRow to lastRow+1 on the unchanged state - the very call "
      "that just failed - and stop at once: same result for every input"),
+    ("refit: starts from the inner-end state of the outermost segment instead of its outer end", "F1",
+     "F2 then transports that state to the row of the outermost hit itself: the covariance is multiplied by "
+     "turn_cov_scale before the transport instead of after it, which is the same matrix up to rounding"),
 ]
 
 
@@ -147,9 +188,11 @@ def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--write", action="store_true")
     ap.add_argument("--jobs", type=int, default=max(1, (os.cpu_count() or 2) // 2))
+    ap.add_argument("--only", default="", help="run only the mutants whose SPEC tag starts with one of these letters, e.g. RGF")
     args = ap.parse_args()
+    todo = [i for i, m in enumerate(MUTANTS) if not args.only or m[1][0] in args.only]
     with ThreadPoolExecutor(args.jobs) as ex:
-        rows = list(ex.map(run_mutant, range(len(MUTANTS))))
+        rows = list(ex.map(run_mutant, todo))
     lines = ["# Mutants of `oracle/tpc_oracle.cpp` and the CPU pin that kills each",
              "",
              "Written by `python tests/mutation_check.py --write` (one textual mistake at a time in a scratch copy of the",
