@@ -209,6 +209,58 @@ void tpc_tracker_enable_stage_timing(tpc_tracker* tracker, int on);
 int tpc_read_stage_ms(tpc_tracker* tracker, void* cuda_stream, float* out_ms, uint32_t* n_calls);
 const char* tpc_stage_name(int stage);
 
+/* ---- sector-segment merger + final refit ------------------------------
+ * PAPER.md L138 (section 3): the tracker "processes the TPC sectors individually but concurrently, and
+ * merges the tracks segments afterward"; L140: a Kalman refit running on the GPU next to the tracker
+ * is what the paper asks for next, because one that has to fetch the tracks over PCIe loses its gain.
+ * docs/ARITH_SPEC.md section 9 defines the operation (the paper gives no procedure): the output state
+ * of every sector track is taken to the row of its outermost hit, turned into the frame of the
+ * neighbouring sector and compared there with the tracks that start within merge_max_row_gap rows
+ * (chi2 over the five parameters, diagonal errors); mutual best choices become links (ties by the gid
+ * of the first hit: order-free); every chain of linked segments - every unlinked track too - is
+ * refitted in one filter pass from its outermost hit inwards, the state being turned where the chain
+ * changes sector.
+ *
+ * tpc_merge_refit must follow the tpc_track_batch call whose tracks it merges, on the same stream,
+ * with the same clusters, tracks, workspace and max_tracklets, and the workspace untouched in between:
+ * it reads the cluster coordinates and the kept hits of every track from the tracker's workspace, so
+ * nothing is copied and nothing leaves the device.  Asynchronous like tpc_track_batch.
+ * If the tracker reported an overflow (header[2] != 0) the merger does nothing and sets
+ * TPC_MERGE_STATUS_INPUT_OVERFLOW. */
+typedef struct {
+  float merge_chi2_max;      /* G4: match iff chi2 < this (default 50)                         */
+  int32_t merge_max_row_gap; /* G2: first row of the outer segment at most this far (default 8) */
+} tpc_merge_params;
+void tpc_default_merge_params(tpc_merge_params* out);
+
+#define TPC_MERGE_STATUS_INPUT_OVERFLOW 1u /* the tracks came with an overflow status: nothing merged */
+#define TPC_MERGE_STATUS_CAPACITY 2u       /* more sector tracks than `capacity`: the surplus was ignored */
+
+/* Output of the merger.  Every pointer is DEVICE memory owned by the caller, `capacity` slots each
+ * (capacity >= the number of sector tracks, e.g. tpc_tracks::track_capacity). */
+typedef struct {
+  uint32_t capacity;
+  uint32_t* header;        /* [4]: merged tracks, links, status bits (TPC_MERGE_STATUS_*), 0          */
+  int32_t* seg_next;       /* [capacity] per sector track: the track that continues it outwards, or -1 */
+  int32_t* seg_prev;       /* [capacity] per sector track: the track it continues, or -1               */
+  uint32_t* merged_first;  /* per merged track: its innermost sector track; merged tracks are in the   */
+                           /* order of this index                                                      */
+  uint32_t* merged_nseg;   /* sector tracks in the chain                                               */
+  uint32_t* merged_nhits;  /* kept hits of all its segments                                            */
+  uint32_t* merged_nfit;   /* hits the refit used (F3; < merged_nhits: it stopped early; 0: no refit)   */
+  uint32_t* merged_sector; /* sector whose local frame the parameters are in                           */
+  int32_t* merged_ndf;     /* 2 * merged_nfit - 5                                                      */
+  float* merged_x;         /* x of the parameters (row of the innermost hit)                           */
+  float* merged_par;       /* [5][capacity] y, z, sin(phi), dz/ds, q/pT                                */
+  float* merged_cov;       /* [15][capacity] lower triangle                                            */
+  float* merged_chi2;
+} tpc_merged;
+
+size_t tpc_merge_workspace_bytes(const tpc_tracker* tracker, uint32_t track_capacity, uint32_t max_tasks);
+int tpc_merge_refit(tpc_tracker* tracker, const tpc_clusters* clusters, const tpc_tracks* tracks,
+                    const tpc_merge_params* params, tpc_merged* merged, void* workspace, size_t workspace_bytes,
+                    uint32_t max_tracklets, void* merge_workspace, size_t merge_workspace_bytes, void* cuda_stream);
+
 /* Text of the last error on this tracker (never NULL). With tracker == NULL: the
  * last error of tpc_tracker_create on this thread. */
 const char* tpc_last_error(const tpc_tracker* tracker);

@@ -132,8 +132,57 @@ def load_library():
     lib.tpc_stage_name.argtypes = [C.c_int]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_last_error.argtypes = [vp]
+    lib.tpc_default_merge_params.restype = None
+    lib.tpc_default_merge_params.argtypes = [C.POINTER(_MergeParams)]
+    lib.tpc_merge_workspace_bytes.restype = C.c_size_t
+    lib.tpc_merge_workspace_bytes.argtypes = [vp, C.c_uint32, C.c_uint32]
+    lib.tpc_merge_refit.restype = C.c_int
+    lib.tpc_merge_refit.argtypes = [vp, C.POINTER(_Clusters), C.POINTER(_Tracks), C.POINTER(_MergeParams),
+                                    C.POINTER(_Merged), vp, C.c_size_t, C.c_uint32, vp, C.c_size_t, vp]
     _lib = lib
     return lib
+
+
+class _MergeParams(C.Structure):
+    _fields_ = [("merge_chi2_max", C.c_float), ("merge_max_row_gap", C.c_int32)]
+
+
+class _Merged(C.Structure):
+    _fields_ = [("capacity", C.c_uint32)] + [(n, C.c_void_p) for n in (
+        "header", "seg_next", "seg_prev", "merged_first", "merged_nseg", "merged_nhits", "merged_nfit",
+        "merged_sector", "merged_ndf", "merged_x", "merged_par", "merged_cov", "merged_chi2")]
+
+
+@dataclass
+class MergedResult:
+    """Device tensors of one tpc_merge_refit call; sizes are capacities."""
+    header: "object"
+    seg_next: "object"
+    seg_prev: "object"
+    merged_first: "object"
+    merged_nseg: "object"
+    merged_nhits: "object"
+    merged_nfit: "object"
+    merged_sector: "object"
+    merged_ndf: "object"
+    merged_x: "object"
+    merged_par: "object"   # [5, capacity]
+    merged_cov: "object"   # [15, capacity]
+    merged_chi2: "object"
+
+    def to_numpy(self, n_tracks: int) -> Dict[str, np.ndarray]:
+        """Copies to host and trims to the counts (synchronises); n_tracks = sector tracks of the tracker's call."""
+        h = self.header.cpu().numpy().astype(np.int64)
+        nm = int(min(h[0], self.merged_first.shape[0]))
+        out = {"n_merged": int(h[0]), "n_links": int(h[1]), "status": int(h[2])}
+        for f in ("seg_next", "seg_prev"):
+            out[f] = getattr(self, f)[:n_tracks].cpu().numpy()
+        for f in ("merged_first", "merged_nseg", "merged_nhits", "merged_nfit", "merged_sector", "merged_ndf",
+                  "merged_x", "merged_chi2"):
+            out[f] = getattr(self, f)[:nm].cpu().numpy()
+        out["merged_par"] = self.merged_par[:, :nm].cpu().numpy()
+        out["merged_cov"] = self.merged_cov[:, :nm].cpu().numpy()
+        return out
 
 
 @dataclass
@@ -321,6 +370,46 @@ class Tracker:
                                                    _stream_ptr(s), C.byref(up), C.byref(down)),
                     "tpc_track_batch_host")
         return int(up.value), int(down.value)
+
+
+    # ---- sector-segment merger + refit (include/tpc_tracker.h, SPEC 9) ----------------------
+    def merge_workspace_bytes(self, track_capacity: int, max_tasks: int) -> int:
+        return int(self._lib.tpc_merge_workspace_bytes(self._h, track_capacity, max_tasks))
+
+    def alloc_merged(self, capacity: int, device) -> "MergedResult":
+        import torch
+        e = lambda shape, dt: torch.empty(shape, dtype=dt, device=device)  # noqa: E731
+        cap = max(int(capacity), 1)
+        return MergedResult(
+            header=e(4, torch.int32), seg_next=e(cap, torch.int32), seg_prev=e(cap, torch.int32),
+            merged_first=e(cap, torch.int32), merged_nseg=e(cap, torch.int32), merged_nhits=e(cap, torch.int32),
+            merged_nfit=e(cap, torch.int32), merged_sector=e(cap, torch.int32), merged_ndf=e(cap, torch.int32),
+            merged_x=e(cap, torch.float32), merged_par=e((5, cap), torch.float32),
+            merged_cov=e((15, cap), torch.float32), merged_chi2=e(cap, torch.float32))
+
+    def merge_refit(self, y, z, row_offsets, n_tasks: int, tracks: TrackResult, merged: "MergedResult", workspace,
+                    merge_workspace, max_tracklets: int = 0, chi2_max: Optional[float] = None,
+                    max_row_gap: Optional[int] = None, stream=None) -> "MergedResult":
+        """tpc_merge_refit right after track_batch with the same tensors and workspace. Asynchronous."""
+        import torch
+        cl = _Clusters(None, y.data_ptr(), z.data_ptr(), None, row_offsets.data_ptr(), int(y.numel()), int(n_tasks))
+        tr = self._tracks_struct(tracks)
+        mp = _MergeParams()
+        self._lib.tpc_default_merge_params(C.byref(mp))
+        if chi2_max is not None:
+            mp.merge_chi2_max = chi2_max
+        if max_row_gap is not None:
+            mp.merge_max_row_gap = max_row_gap
+        mg = _Merged()
+        mg.capacity = int(merged.seg_next.shape[0])
+        for n, _ in _Merged._fields_[1:]:
+            setattr(mg, n, getattr(merged, n).data_ptr())
+        wp, wn = self._aligned(workspace)
+        mwp, mwn = self._aligned(merge_workspace)
+        s = stream if stream is not None else torch.cuda.current_stream(y.device)
+        self._check(self._lib.tpc_merge_refit(self._h, C.byref(cl), C.byref(tr), C.byref(mp), C.byref(mg), wp, wn,
+                                              int(max_tracklets), mwp, mwn, _stream_ptr(s)), "tpc_merge_refit")
+        return merged
 
 
 def _stream_ptr(stream):

@@ -20,6 +20,7 @@ constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at kBinsPerC
 __host__ __device__ inline size_t map_stride(int n_rows) { return (size_t)((n_rows + 7) & ~7); }
 constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the grid build
 constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
+constexpr uint32_t kOwnedBit = 0x80000000u;  // row map entry: the tracklet keeps this hit (set by k_resolve; idx < 2^31)
 constexpr float kCoordClamp = 1.0e5f; // grid extents only: coordinates beyond +-1 km (or non-finite) count as this
 
 enum CounterId {
@@ -86,6 +87,8 @@ struct Ctx {
                            // valid for the rows first_row..last_row of the tracklet record
   float4* trk_rec;         // [max_tracklets][kRecFloat4] tracklet record
   uint4* trk_meta;         // [max_tracklets] nHits, firstRow | lastRow << 16, gid of the start hit, 0: what K7 needs
+  uint32_t* out_trk;       // [max_tracklets] tracklet of output track `slot` (written by a7 for the merger)
+  uint32_t* out_rows;      // [max_tracklets] row of the first kept hit | row of the last kept hit << 16, per output track
   uint32_t* trk_kept;      // [max_tracklets] hits the tracklet keeps (L1), counted by k_resolve; cleared per call
   uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]

@@ -30,7 +30,6 @@ constexpr uint32_t kResolveChunk = 8192;  // clusters per block: 64 KB of owners
 #endif
 constexpr int kResolveBatch = TPC_RESOLVE_BATCH;  // (tracklet, row) pairs a thread has in flight
 constexpr int kResolveRows = 512;                 // row offsets of the chunk kept in shared memory
-constexpr uint32_t kOwnedBit = 0x80000000u;       // map entry: the tracklet keeps this hit (idx < 2^31)
 constexpr uint32_t kKeyGidBits = 27, kKeyTrkBits = 26;
 
 // first tracklet of every task: tracklets are in idx order of their start hits, so a task's are consecutive
@@ -193,6 +192,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     if ((unsigned long long)hb + kept > (unsigned long long)o.hit_capacity) { status |= TPC_STATUS_HIT_OVERFLOW; continue; }
     const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
     uint32_t w = hb;
+    int kept_first = -1, kept_last = -1;  // rows of the first and last kept hit (for the merger)
     // the map loads of kOutChunks chunks together, then their gid gathers, then the stores
     for (int rb0 = first; rb0 <= last; rb0 += 32 * kOutChunks) {
       uint32_t idx[kOutChunks], g[kOutChunks];
@@ -209,7 +209,15 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
         const unsigned mask = __ballot_sync(FULL, idx[q] != kNoHit);
         if (idx[q] != kNoHit) o.hit_cluster[w + __popc(mask & ((1u << lane) - 1u))] = g[q];
         w += __popc(mask);
+        if (mask) {
+          if (kept_first < 0) kept_first = rb0 + 32 * q + __ffs(mask) - 1;
+          kept_last = rb0 + 32 * q + 31 - __clz(mask);
+        }
       }
+    }
+    if (lane == 0) {
+      c.out_trk[slot] = t;
+      c.out_rows[slot] = (uint32_t)kept_first | ((uint32_t)kept_last << 16);
     }
   }
   if (status && lane == 0) atomicOr(&o.header[2], status);

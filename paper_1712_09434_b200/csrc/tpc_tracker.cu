@@ -6,6 +6,7 @@
 //        -prec-div=true -prec-sqrt=true -ftz=false --shared -Xcompiler -fPIC
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -16,6 +17,7 @@
 
 #include "../../include/tpc_tracker.h"
 #include "device_common.cuh"
+#include "stage_merge.cuh"
 #include "stage_neighbours.cuh"
 #include "stage_output.cuh"
 #include "stage_tracklet.cuh"
@@ -28,6 +30,8 @@ struct tpc_tracker {
   float z_max = 0.f, bz = 0.f;
   tpc_params prm{};
   float a = 0.f, sy2 = 0.f, sz2 = 0.f, wy = 0.f, wz = 0.f, smax2 = 0.f;
+  int32_t n_half = 1;        // SPEC 9 tables: sectors per side, cos and sin of the sector pitch
+  float merge_ca = 1.f, merge_sa = 0.f;
   float* d_tables = nullptr;               // [6][n_rows]: X, ymax, dx_up, dx_dn, ratio_up, ratio_dn
   unsigned long long* d_counters = nullptr;  // [CN_COUNT]
   bool counters_on = false;
@@ -81,7 +85,7 @@ uint32_t host_total_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tra
 // Offsets of every workspace array, in bytes.
 struct Carve {
   size_t yz, gid, bins, rowinfo, tile_tr, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
-      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, trk_kept, zero_end, total;
+      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, trk_kept, zero_end, out_trk, out_rows, total;
   uint32_t seed_tiles, out_tiles;
 };
 
@@ -115,6 +119,8 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.trk_task_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
   c.trk_kept = take((size_t)T * sizeof(uint32_t));
   c.zero_end = off;
+  c.out_trk = take((size_t)T * sizeof(uint32_t));
+  c.out_rows = take((size_t)T * sizeof(uint32_t));
   c.total = off;
   return c;
 }
@@ -150,6 +156,7 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
   c.trk_meta = (uint4*)(ws + cv.trk_meta); c.trk_task_off = (uint32_t*)(ws + cv.trk_task_off);
   c.trk_kept = (uint32_t*)(ws + cv.trk_kept);
+  c.out_trk = (uint32_t*)(ws + cv.out_trk); c.out_rows = (uint32_t*)(ws + cv.out_rows);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
   c.max_tracklets = T;
@@ -205,6 +212,12 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
   t->sy2 = p.sigma_y * p.sigma_y; t->sz2 = p.sigma_z * p.sigma_z;                            // T7
   t->wy = 1.0f / t->sy2; t->wz = 1.0f / t->sz2;
   t->smax2 = p.search_max * p.search_max;                                                    // T8
+  t->n_half = g->n_sectors >= 2 ? g->n_sectors / 2 : 1;                                      // SPEC 9 tables
+  {
+    const double alpha = 2.0 * 3.14159265358979323846 / (double)t->n_half;
+    t->merge_ca = (float)cos(alpha);
+    t->merge_sa = (float)sin(alpha);
+  }
   cudaError_t e = cudaMalloc(&t->d_tables, tab.size() * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&t->d_counters, CN_COUNT * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemcpy(t->d_tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
@@ -669,6 +682,95 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   out->header[3] = tracklets;
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = down;
+  return TPC_OK;
+}
+
+// ---- sector-segment merger + refit (SPEC 9) ------------------------------------------------------
+namespace {
+struct MergeCarve { size_t ends, best_out, best_in, zero_begin, track_off, scan, ticket, zero_end, total; uint32_t tiles; };
+MergeCarve merge_carve(uint32_t cap, uint32_t n_tasks) {
+  MergeCarve m{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
+  m.ends = take((size_t)cap * kEndFloats * sizeof(float));
+  m.best_out = take((size_t)cap * sizeof(int32_t));
+  m.best_in = take((size_t)cap * sizeof(int32_t));
+  m.tiles = (cap + kMergeThreads - 1) / kMergeThreads;
+  if (m.tiles == 0) m.tiles = 1;
+  m.zero_begin = off;
+  m.track_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
+  m.scan = take((size_t)m.tiles * sizeof(unsigned long long));
+  m.ticket = take(sizeof(uint32_t));
+  m.zero_end = off;
+  m.total = off;
+  return m;
+}
+__global__ void k_merge_guard(const Ctx c, const MergeCtx m) {  // the tracker's status decides whether anything runs
+  if (c.out.header[2] != 0u) atomicOr(&m.out.header[2], TPC_MERGE_STATUS_INPUT_OVERFLOW);
+  else if (c.out.header[0] > m.out.capacity) atomicOr(&m.out.header[2], TPC_MERGE_STATUS_CAPACITY);
+}
+}  // namespace
+
+void tpc_default_merge_params(tpc_merge_params* out) {
+  if (out) { out->merge_chi2_max = 50.0f; out->merge_max_row_gap = 8; }
+}
+
+size_t tpc_merge_workspace_bytes(const tpc_tracker* t, uint32_t track_capacity, uint32_t max_tasks) {
+  if (!t) return 0;
+  return merge_carve(track_capacity, max_tasks).total;
+}
+
+int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tracks, const tpc_merge_params* params,
+                    tpc_merged* merged, void* workspace, size_t workspace_bytes, uint32_t max_tracklets,
+                    void* merge_workspace, size_t merge_workspace_bytes, void* cuda_stream) {
+  if (!t) return TPC_ERR_ARGUMENT;
+  if (!in || !tracks || !merged) return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: clusters, tracks and merged must not be NULL");
+  if (!merged->header || !merged->seg_next || !merged->seg_prev || !merged->merged_first || !merged->merged_nseg ||
+      !merged->merged_nhits || !merged->merged_nfit || !merged->merged_sector || !merged->merged_ndf ||
+      !merged->merged_x || !merged->merged_par || !merged->merged_cov || !merged->merged_chi2)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: every array of tpc_merged must not be NULL");
+  if (!tracks->header || !tracks->track_task || !tracks->track_hit_begin || !tracks->track_nhits || !tracks->track_ndf ||
+      !tracks->track_x || !tracks->track_par || !tracks->track_cov || !tracks->track_chi2 || !tracks->hit_cluster)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: tracks must be the complete output of tpc_track_batch");
+  tpc_merge_params mp;
+  if (params) mp = *params; else tpc_default_merge_params(&mp);
+  if (!(mp.merge_chi2_max >= 0.f) || mp.merge_max_row_gap < 0)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: need merge_chi2_max >= 0 and merge_max_row_gap >= 0");
+  const uint32_t T = resolve_max_tracklets(t, in->n_clusters, max_tracklets);
+  const Carve cv = carve((uint32_t)t->n_rows, in->n_clusters, in->n_tasks, T);
+  if (!workspace || workspace_bytes < cv.total)
+    return fail(t, TPC_ERR_WORKSPACE, "tpc_merge_refit: workspace of %zu bytes, the tracker's call needed %zu", workspace_bytes, cv.total);
+  const uint32_t cap = tracks->track_capacity;
+  const MergeCarve mc = merge_carve(cap, in->n_tasks);
+  if (!merge_workspace || merge_workspace_bytes < mc.total)
+    return fail(t, TPC_ERR_WORKSPACE, "tpc_merge_refit: merge workspace of %zu bytes, need %zu", merge_workspace_bytes, mc.total);
+  if ((((uintptr_t)workspace | (uintptr_t)merge_workspace) & (kAlign - 1)) != 0)
+    return fail(t, TPC_ERR_WORKSPACE, "tpc_merge_refit: workspaces must be %zu-byte aligned", kAlign);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const Ctx c = make_ctx(t, in, tracks, (char*)workspace, cv, T);
+  char* mw = (char*)merge_workspace;
+  MergeCtx m{};
+  m.out = *merged;
+  m.chi2_max = mp.merge_chi2_max; m.max_row_gap = mp.merge_max_row_gap;
+  m.n_half = t->n_half; m.ca = t->merge_ca; m.sa = t->merge_sa;
+  m.n_tracks_cap = cap;
+  m.ends = (float4*)(mw + mc.ends); m.best_out = (int32_t*)(mw + mc.best_out); m.best_in = (int32_t*)(mw + mc.best_in);
+  m.track_off = (uint32_t*)(mw + mc.track_off); m.scan = (unsigned long long*)(mw + mc.scan);
+  m.ticket = (uint32_t*)(mw + mc.ticket);
+  cudaError_t e = cudaMemsetAsync(mw + mc.zero_begin, 0, mc.zero_end - mc.zero_begin, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(merged->header, 0, 4 * sizeof(uint32_t), s);
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_merge_refit: CUDA memset: %s", cudaGetErrorString(e));
+  const uint32_t blocks = mc.tiles;
+  k_merge_guard<<<1, 1, 0, s>>>(c, m);
+  if (cap > 0) {
+    k_merge_task_offsets<<<2 * t->n_sm, 256, 0, s>>>(c, m);
+    k_merge_ends<<<blocks, kMergeThreads, 0, s>>>(c, m);
+    k_merge_match<<<blocks, kMergeThreads, 0, s>>>(c, m);
+    k_merge_link<<<blocks, kMergeThreads, 0, s>>>(c, m);
+    k_merge_refit<<<blocks, kMergeThreads, 0, s>>>(c, m);
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_merge_refit: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;
 }
 

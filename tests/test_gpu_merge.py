@@ -1,0 +1,117 @@
+"""-m gpu parity of the sector-segment merger + refit (SPEC 9, include/tpc_tracker.h tpc_merge_refit) against
+the CPU oracle on the same seeded inputs: links bit-exact (as pairs of first-hit gids: track order is free, L4),
+chains and hit counts bit-exact, refitted parameters within 1e-4 (reported bit-identical)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+import gpu_helpers as G
+from tpc_workload import generate_config
+
+pytestmark = pytest.mark.gpu
+
+
+def run_gpu_merge(batch, chi2_max=None, max_row_gap=None, params_over=None):
+    import torch
+    from paper_1712_09434_b200 import Tracker
+    dev = torch.device("cuda:0")
+    trk = Tracker(batch.geometry, G.tracker_params_for(batch, **(params_over or {})))
+    try:
+        n = batch.n_clusters
+        y = torch.from_numpy(np.ascontiguousarray(batch.y)).to(dev)
+        z = torch.from_numpy(np.ascontiguousarray(batch.z)).to(dev)
+        ro = torch.from_numpy(batch.row_offsets.astype(np.uint32).view(np.int32)).to(dev)
+        out = trk.alloc_outputs(n, dev)
+        ws = trk.alloc_workspace(trk.workspace_bytes(n, batch.n_tasks), dev)
+        tcap = int(out.track_task.shape[0])
+        merged = trk.alloc_merged(tcap, dev)
+        mws = trk.alloc_workspace(trk.merge_workspace_bytes(tcap, batch.n_tasks), dev)
+        trk.track_batch(y, z, ro, batch.n_tasks, out, ws)
+        trk.merge_refit(y, z, ro, batch.n_tasks, out, merged, ws, mws, chi2_max=chi2_max, max_row_gap=max_row_gap)
+        torch.cuda.synchronize()
+        g = out.to_numpy()
+        g.update(merged.to_numpy(g["n_tracks"]))
+        return g
+    finally:
+        trk.close()
+
+
+def compare_merge(g, ref, mref, rtol=1e-4):
+    assert g["status"] == 0 and g["n_tracks"] == ref.n_tracks
+    fg = g["hit_cluster"][g["track_hit_begin"].astype(np.int64)].astype(np.int64)
+    fr = ref.hit_cluster[ref.track_hit_begin.astype(np.int64)].astype(np.int64)
+    links_g = {(int(fg[i]), int(fg[g["seg_next"][i]])) for i in np.nonzero(g["seg_next"] >= 0)[0]}
+    links_r = {(int(fr[i]), int(fr[mref.next[i]])) for i in np.nonzero(mref.next >= 0)[0]}
+    assert links_g == links_r, f"links differ: gpu {len(links_g)} oracle {len(links_r)}"
+    assert g["n_links"] == mref.n_links == len(links_r)
+    for i in np.nonzero(g["seg_next"] >= 0)[0]:
+        assert g["seg_prev"][g["seg_next"][i]] == i
+    assert g["n_merged"] == len(mref.merged_first)
+    # merged tracks matched by the first-hit gid of their innermost segment
+    by = {int(fr[f]): k for k, f in enumerate(mref.merged_first)}
+    order = np.array([by[int(fg[f])] for f in g["merged_first"]], np.int64)
+    assert len(set(order.tolist())) == len(order)
+    assert np.all(np.diff(g["merged_first"].astype(np.int64)) > 0), "merged tracks are in the order of their first segment"
+    for f in ("merged_nseg", "merged_nhits", "merged_nfit", "merged_sector", "merged_ndf"):
+        np.testing.assert_array_equal(g[f].astype(np.int64), getattr(mref, f)[order].astype(np.int64), err_msg=f)
+    np.testing.assert_array_equal(g["merged_x"], mref.merged_x[order])
+    gp, rp = g["merged_par"].astype(np.float64), mref.merged_par[:, order].astype(np.float64)
+    gc, rc = g["merged_cov"].astype(np.float64), mref.merged_cov[:, order].astype(np.float64)
+    sig = np.sqrt(np.maximum(rc[[0, 2, 5, 9, 14]], 0))
+    dev_p = float(np.max(np.abs(gp - rp) / np.maximum(np.maximum(np.abs(rp), sig), 1e-30))) if gp.size else 0.0
+    assert dev_p <= rtol, f"refit parameters deviate by {dev_p:.2e}"
+    k, scale = 0, np.zeros_like(rc)
+    for i in range(5):
+        for j in range(i + 1):
+            scale[k] = sig[i] * sig[j]
+            k += 1
+    dev_c = float(np.max(np.abs(gc - rc) / np.maximum(np.maximum(np.abs(rc), scale), 1e-30))) if gc.size else 0.0
+    assert dev_c <= rtol, f"refit covariances deviate by {dev_c:.2e}"
+    g2, r2 = g["merged_chi2"].astype(np.float64), mref.merged_chi2[order].astype(np.float64)
+    assert np.all(np.abs(g2 - r2) <= rtol * np.maximum(np.abs(r2), 1.0))
+    return dict(par_rel=dev_p, cov_rel=dev_c, bit_exact=bool(np.array_equal(g["merged_par"], mref.merged_par[:, order])
+                                                              and np.array_equal(g["merged_cov"], mref.merged_cov[:, order])))
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_merge_refit_matches_the_oracle(cfg):
+    b = generate_config(cfg)
+    g = run_gpu_merge(b)
+    prm = G.oracle_params_for(b)
+    ref = oracle.track(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, params=prm)
+    mref = oracle.merge_refit(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, ref, params=prm)
+    dev = compare_merge(g, ref, mref)
+    assert mref.n_links > 100
+    print(f"config {cfg}: {ref.n_tracks} sector tracks, {mref.n_links} links, {len(mref.merged_first)} merged; {dev}")
+
+
+def test_merge_refit_multi_event_batch_and_cuts():
+    """Four events in one call (links never cross events), and the two cuts away from their defaults."""
+    b = generate_config(3, n_events=4)
+    prm = G.oracle_params_for(b)
+    ref = oracle.track(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, params=prm)
+    for chi2_max, gap in ((50.0, 8), (5.0, 8), (50.0, 1), (1e6, 20)):
+        g = run_gpu_merge(b, chi2_max=chi2_max, max_row_gap=gap)
+        mref = oracle.merge_refit(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, ref, params=prm, chi2_max=chi2_max,
+                                  max_row_gap=gap)
+        compare_merge(g, ref, mref)
+    ns = b.geometry.n_sectors
+    i = np.nonzero(g["seg_next"] >= 0)[0]
+    assert np.all(g["track_task"][i] // ns == g["track_task"][g["seg_next"][i]] // ns)
+
+
+def test_merge_refit_single_sector_and_empty():
+    """Config 0 has one sector (no neighbours): no links, every track refitted alone; an empty batch gives nothing."""
+    b = generate_config(0)
+    g = run_gpu_merge(b)
+    prm = G.oracle_params_for(b)
+    ref = oracle.track(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, params=prm)
+    mref = oracle.merge_refit(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, ref, params=prm)
+    assert mref.n_links == 0
+    compare_merge(g, ref, mref)
+    from tpc_workload import take_tasks
+    e, _ = take_tasks(generate_config(1), [])   # every task empty
+    ge = run_gpu_merge(e)
+    assert ge["n_tracks"] == 0 and ge["n_merged"] == 0 and ge["n_links"] == 0
