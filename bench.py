@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--cpu-events", type=int, default=4, help="events in the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-merge", action="store_true", help="skip the merger + refit leg (SURVEY 8(f)1)")
     ap.add_argument("--cpu-workers", type=int, default=0, help="worker processes of the all-cores cpu_baseline leg (0 = all)")
     ap.add_argument("--dry-run", action="store_true",
                     help="control flow only (rendezvous, barriers, MAX-reduce, counter gather) on the gloo backend with "
@@ -376,6 +377,39 @@ def run_ours(args):
         e2e = (e2e_ms, up, down)
         del ws_h, out_h
 
+    # sector-segment merger + final refit behind a7 (tpc_merge_refit), timed on its own: tracker call +
+    # merger call per step, CUDA events around the merger on the launching stream
+    merge = None
+    if not args.no_merge:
+        tcap = int(out.track_task.shape[0])
+        mg = trk.alloc_merged(tcap, dev)
+        mws = trk.alloc_workspace(trk.merge_workspace_bytes(tcap, n_tasks), dev)
+        pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                 for _ in range(args.steps)]
+        for _ in range(2):
+            trk.track_batch(y, z, ro, n_tasks, out, ws)
+            trk.merge_refit(y, z, ro, n_tasks, out, mg, ws, mws)
+        torch.cuda.synchronize()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record(stream)
+        for a, b in pairs:
+            trk.track_batch(y, z, ro, n_tasks, out, ws)
+            a.record(stream)
+            trk.merge_refit(y, z, ro, n_tasks, out, mg, ws, mws)
+            b.record(stream)
+        m1.record(stream)
+        torch.cuda.synchronize()
+        mh = mg.header.cpu().numpy().astype(np.int64)
+        merge_ms = sum(a.elapsed_time(b) for a, b in pairs) / args.steps
+        # what the merger must move once: the state of every sector track in and its outer end out and in again
+        # (3 x 84 B), the kept hits of the refit (4 B map entry + 8 B cluster), the merged record out (104 B)
+        merge_bytes = 252 * int(hdr[0]) + 12 * int(hdr[1]) + 104 * int(mh[0])
+        merge = {"ms_per_step": merge_ms, "tracker_plus_merger_ms_per_step": m0.elapsed_time(m1) / args.steps,
+                 "sector_tracks": int(hdr[0]), "links": int(mh[1]), "merged_tracks": int(mh[0]), "status": int(mh[2]),
+                 "algorithmic_bytes": merge_bytes, "achieved_gbs": merge_bytes / (merge_ms / 1e3) / 1e9,
+                 "launches": 8, "note": "runs on the tracker's workspace: no track, hit or cluster leaves the device"}
+        del mg, mws
+
     # max over ranks, totals over ranks
     (ms_total, e2e_ms_max), tot = reduce_over_ranks([ms_total, e2e[0] if e2e else 0.0],
                                                     [n, n_events, int(hdr[0]), int(hdr[1])], dev)
@@ -431,6 +465,9 @@ def run_ours(args):
         "clocks": clocks,
         "gpu_launches": trk.launches_per_batch() * args.steps,
     }
+    if merge:
+        merge["hbm_frac"] = merge["achieved_gbs"] / peak_gbs
+        line["merge_refit"] = merge
     if e2e:
         line["e2e"] = {"value": tot[0] * args.steps / (e2e_ms_max / 1e3), "unit": UNIT,
                        "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2],

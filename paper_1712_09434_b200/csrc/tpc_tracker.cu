@@ -38,6 +38,7 @@ struct tpc_tracker {
   bool debug_sync = false;  // TPC_DEBUG_SYNC=1: synchronise after every stage and name the stage that failed
   // persistent tracklet kernels (chain, up, refit, finish): [kernel][counters off/on] -> blocks that fit the device at once
   int n_sm = 0;
+  int merge_grid = 0;  // persistent refit of the merger: blocks the device holds at once
   size_t trk_smem[4] = {0, 0, 0, 0};
   int trk_grid[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
   // stage timing: ring of TPC_STAGE_RING calls x (TPC_N_STAGES + 1) events, created on first use
@@ -254,6 +255,12 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
     e = cudaFuncSetAttribute((const void*)k_resolve, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(kResolveChunk * sizeof(unsigned long long)));
   t->n_sm = n_sm;
+  if (e == cudaSuccess) {
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)k_merge_refit, kMergeThreads,
+                                                      (size_t)t->n_rows * sizeof(float));
+    t->merge_grid = (per_sm > 0 ? per_sm : 1) * n_sm;
+  }
   const int trk_slot16[4] = {kChainSlot16, kRecSlot16, kRecSlot16, kFinishSlot16};
   for (int k = 0; k < 4; ++k) t->trk_smem[k] = trk_smem_bytes(t->n_rows, trk_slot16[k]);
   const void* trk_fn[4][2] = {{(const void*)k_trk_chain<false>, (const void*)k_trk_chain<true>},
@@ -687,21 +694,32 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
 
 // ---- sector-segment merger + refit (SPEC 9) ------------------------------------------------------
 namespace {
-struct MergeCarve { size_t ends, best_out, best_in, zero_begin, track_off, scan, ticket, zero_end, total; uint32_t tiles; };
-MergeCarve merge_carve(uint32_t cap, uint32_t n_tasks) {
+struct MergeCarve {
+  size_t ends, row_start, row_list, best_out, best_chi, zero_begin, row_cnt, row_fill, scan, ticket, zero_end, ones_begin,
+      key_in, ones_end, total;
+  uint32_t tiles;
+};
+MergeCarve merge_carve(uint32_t cap, uint32_t n_tasks, uint32_t n_rows) {
   MergeCarve m{};
+  const size_t n_tr = (size_t)n_tasks * n_rows + 2;
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
   m.ends = take((size_t)cap * kEndFloats * sizeof(float));
+  m.row_start = take(n_tr * sizeof(uint32_t));
+  m.row_list = take((size_t)cap * sizeof(uint32_t));
   m.best_out = take((size_t)cap * sizeof(int32_t));
-  m.best_in = take((size_t)cap * sizeof(int32_t));
+  m.best_chi = take((size_t)cap * sizeof(float));
   m.tiles = (cap + kMergeThreads - 1) / kMergeThreads;
   if (m.tiles == 0) m.tiles = 1;
-  m.zero_begin = off;
-  m.track_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
+  m.zero_begin = off;  // cleared with one memset per call
+  m.row_cnt = take(n_tr * sizeof(uint32_t));
+  m.row_fill = take(n_tr * sizeof(uint32_t));
   m.scan = take((size_t)m.tiles * sizeof(unsigned long long));
-  m.ticket = take(sizeof(uint32_t));
+  m.ticket = take(2 * sizeof(uint32_t));
   m.zero_end = off;
+  m.ones_begin = off;  // set to all ones per call
+  m.key_in = take((size_t)cap * sizeof(unsigned long long));
+  m.ones_end = off;
   m.total = off;
   return m;
 }
@@ -717,7 +735,7 @@ void tpc_default_merge_params(tpc_merge_params* out) {
 
 size_t tpc_merge_workspace_bytes(const tpc_tracker* t, uint32_t track_capacity, uint32_t max_tasks) {
   if (!t) return 0;
-  return merge_carve(track_capacity, max_tasks).total;
+  return merge_carve(track_capacity, max_tasks, (uint32_t)t->n_rows).total;
 }
 
 int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tracks, const tpc_merge_params* params,
@@ -741,7 +759,7 @@ int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tr
   if (!workspace || workspace_bytes < cv.total)
     return fail(t, TPC_ERR_WORKSPACE, "tpc_merge_refit: workspace of %zu bytes, the tracker's call needed %zu", workspace_bytes, cv.total);
   const uint32_t cap = tracks->track_capacity;
-  const MergeCarve mc = merge_carve(cap, in->n_tasks);
+  const MergeCarve mc = merge_carve(cap, in->n_tasks, (uint32_t)t->n_rows);
   if (!merge_workspace || merge_workspace_bytes < mc.total)
     return fail(t, TPC_ERR_WORKSPACE, "tpc_merge_refit: merge workspace of %zu bytes, need %zu", merge_workspace_bytes, mc.total);
   if ((((uintptr_t)workspace | (uintptr_t)merge_workspace) & (kAlign - 1)) != 0)
@@ -753,21 +771,26 @@ int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tr
   m.out = *merged;
   m.chi2_max = mp.merge_chi2_max; m.max_row_gap = mp.merge_max_row_gap;
   m.n_half = t->n_half; m.ca = t->merge_ca; m.sa = t->merge_sa;
-  m.n_tracks_cap = cap;
-  m.ends = (float4*)(mw + mc.ends); m.best_out = (int32_t*)(mw + mc.best_out); m.best_in = (int32_t*)(mw + mc.best_in);
-  m.track_off = (uint32_t*)(mw + mc.track_off); m.scan = (unsigned long long*)(mw + mc.scan);
-  m.ticket = (uint32_t*)(mw + mc.ticket);
+  m.ends = (float4*)(mw + mc.ends);
+  m.row_cnt = (uint32_t*)(mw + mc.row_cnt); m.row_start = (uint32_t*)(mw + mc.row_start);
+  m.row_fill = (uint32_t*)(mw + mc.row_fill); m.row_list = (uint32_t*)(mw + mc.row_list);
+  m.best_out = (int32_t*)(mw + mc.best_out); m.best_chi = (float*)(mw + mc.best_chi);
+  m.key_in = (unsigned long long*)(mw + mc.key_in);
+  m.scan = (unsigned long long*)(mw + mc.scan); m.ticket = (uint32_t*)(mw + mc.ticket);
   cudaError_t e = cudaMemsetAsync(mw + mc.zero_begin, 0, mc.zero_end - mc.zero_begin, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(mw + mc.ones_begin, 0xFF, mc.ones_end - mc.ones_begin, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(merged->header, 0, 4 * sizeof(uint32_t), s);
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_merge_refit: CUDA memset: %s", cudaGetErrorString(e));
   const uint32_t blocks = mc.tiles;
   k_merge_guard<<<1, 1, 0, s>>>(c, m);
   if (cap > 0) {
-    k_merge_task_offsets<<<2 * t->n_sm, 256, 0, s>>>(c, m);
-    k_merge_ends<<<blocks, kMergeThreads, 0, s>>>(c, m);
-    k_merge_match<<<blocks, kMergeThreads, 0, s>>>(c, m);
-    k_merge_link<<<blocks, kMergeThreads, 0, s>>>(c, m);
-    k_merge_refit<<<blocks, kMergeThreads, 0, s>>>(c, m);
+    k_merge_ends<<<blocks, kMergeThreads, 0, s>>>(c, m);                                   // G1
+    k_merge_row_scan<<<1, 1024, 0, s>>>(c, m);
+    k_merge_row_fill<<<blocks, kMergeThreads, 0, s>>>(c, m);
+    k_merge_match<<<blocks, kMergeThreads, 0, s>>>(c, m);                                  // G2..G5
+    k_merge_link<<<blocks, kMergeThreads, 0, s>>>(c, m);                                   // G6
+    k_merge_heads<<<blocks, kMergeThreads, 0, s>>>(c, m);                                  // G7
+    k_merge_refit<<<t->merge_grid, kMergeThreads, (size_t)t->n_rows * sizeof(float), s>>>(c, m);  // F1..F3
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_merge_refit: CUDA launch: %s", cudaGetErrorString(e));
