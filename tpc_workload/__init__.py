@@ -18,3 +18,4 @@ from .events import (  # noqa: F401
     concat_batches,
     take_tasks,
 )
+from .calibration import RawCalibration, default_calibration, raw_from_yz  # noqa: F401
