@@ -145,7 +145,11 @@ void tpc_default_params(tpc_params* out);
  * max_clusters clusters in max_tasks tasks.  max_tracklets bounds the number of
  * tracklets built (a5); 0 = the worst case max_clusters / min_seed_hits (chains
  * are vertex disjoint, S2).  The tracklet row maps dominate:
- * 4 * n_rows * max_tracklets bytes. */
+ * 4 * n_rows * max_tracklets bytes.  Pb-Pb-like events build one tracklet per
+ * 30..35 clusters (config 3: 1.26 M for 40.7 M clusters), so max_clusters / 20
+ * is a safe setting - 1.6 GB instead of 8 GB of workspace for config 3; more
+ * tracklets than that set TPC_STATUS_TRACKLET_OVERFLOW and the surplus (the
+ * last start hits in idx order) is not built. */
 size_t tpc_workspace_bytes(const tpc_tracker* tracker, uint32_t max_clusters, uint32_t max_tasks,
                            uint32_t max_tracklets);
 
@@ -260,6 +264,33 @@ size_t tpc_merge_workspace_bytes(const tpc_tracker* tracker, uint32_t track_capa
 int tpc_merge_refit(tpc_tracker* tracker, const tpc_clusters* clusters, const tpc_tracks* tracks,
                     const tpc_merge_params* params, tpc_merged* merged, void* workspace, size_t workspace_bytes,
                     uint32_t max_tracklets, void* merge_workspace, size_t merge_workspace_bytes, void* cuda_stream);
+
+/* ---- cluster transformation -------------------------------------------
+ * PAPER.md L77 (footnote 1): "The TPC cluster transformation map is needed to convert the raw TPC
+ * clusters from TPC pad row, TPC pad, and time coordinates into x, y, and z coordinates taking into
+ * account the calibration"; L101 / L213: the map is the default or the fed-back calibration, and the
+ * index of a cluster is not changed.  docs/ARITH_SPEC.md section 10 (X1..X4) defines the arithmetic
+ * (the paper gives none): nominal pad/time geometry plus a bilinear (dy, dz) correction from a
+ * map_ny x map_nz grid of knots per (sector,row).  The output (y, z) is what tpc_track_batch reads;
+ * x is the row's (R18).  All tables are HOST memory, copied by tpc_transform_create. */
+typedef struct {
+  const float* pad_pitch;  /* [n_rows] width of a pad in cm                                        */
+  const int32_t* n_pads;   /* [n_rows] pads of the row (>= 2)                                      */
+  float t0;                /* time bin of a cluster at the end plate                               */
+  float v_drift;           /* cm per time bin                                                      */
+  float t_max;             /* time bin of the central electrode (> 0): the map spans [0, t_max]    */
+  int32_t map_ny, map_nz;  /* knots across the pads and along the time, both >= 2                  */
+  const float* map;        /* [n_sectors][n_rows][map_nz][map_ny][2] (dy, dz) in cm                */
+} tpc_calibration;
+typedef struct tpc_transform tpc_transform;
+int tpc_transform_create(const tpc_geometry* geometry, const tpc_calibration* calibration, tpc_transform** out);
+void tpc_transform_destroy(tpc_transform* transform);
+/* pad, time, y, z: DEVICE [n_clusters] (16-byte aligned, e.g. from cudaMalloc), sorted by (task,row) like
+ * tpc_clusters; row_offsets: DEVICE [n_tasks*n_rows + 1].  Asynchronous on cuda_stream, no allocation.
+ * Returns TPC_OK or a negative code; the text is in tpc_transform_last_error. */
+int tpc_transform_clusters(tpc_transform* transform, const float* pad, const float* time, const uint32_t* row_offsets,
+                           uint32_t n_clusters, uint32_t n_tasks, float* y, float* z, void* cuda_stream);
+const char* tpc_transform_last_error(const tpc_transform* transform);
 
 /* Text of the last error on this tracker (never NULL). With tracker == NULL: the
  * last error of tpc_tracker_create on this thread. */

@@ -132,6 +132,14 @@ def load_library():
     lib.tpc_stage_name.argtypes = [C.c_int]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_last_error.argtypes = [vp]
+    lib.tpc_transform_create.restype = C.c_int
+    lib.tpc_transform_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Calibration), C.POINTER(vp)]
+    lib.tpc_transform_destroy.restype = None
+    lib.tpc_transform_destroy.argtypes = [vp]
+    lib.tpc_transform_clusters.restype = C.c_int
+    lib.tpc_transform_clusters.argtypes = [vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp, vp]
+    lib.tpc_transform_last_error.restype = C.c_char_p
+    lib.tpc_transform_last_error.argtypes = [vp]
     lib.tpc_default_merge_params.restype = None
     lib.tpc_default_merge_params.argtypes = [C.POINTER(_MergeParams)]
     lib.tpc_merge_workspace_bytes.restype = C.c_size_t
@@ -141,6 +149,12 @@ def load_library():
                                     C.POINTER(_Merged), vp, C.c_size_t, C.c_uint32, vp, C.c_size_t, vp]
     _lib = lib
     return lib
+
+
+class _Calibration(C.Structure):
+    _fields_ = [("pad_pitch", C.POINTER(C.c_float)), ("n_pads", C.POINTER(C.c_int32)), ("t0", C.c_float),
+                ("v_drift", C.c_float), ("t_max", C.c_float), ("map_ny", C.c_int32), ("map_nz", C.c_int32),
+                ("map", C.POINTER(C.c_float))]
 
 
 class _MergeParams(C.Structure):
@@ -410,6 +424,49 @@ class Tracker:
         self._check(self._lib.tpc_merge_refit(self._h, C.byref(cl), C.byref(tr), C.byref(mp), C.byref(mg), wp, wn,
                                               int(max_tracklets), mwp, mwn, _stream_ptr(s)), "tpc_merge_refit")
         return merged
+
+
+class ClusterTransform:
+    """Owns one ``tpc_transform`` handle (SPEC 10).  ``calibration``: object with pad_pitch, n_pads, t0, v_drift,
+    t_max, corr [n_sectors, n_rows, MZ, MY, 2] (e.g. tpc_workload.RawCalibration)."""
+
+    def __init__(self, geometry, calibration):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        self.n_rows = int(geometry.n_rows)
+        row_x = np.ascontiguousarray(geometry.row_x, dtype=np.float32)
+        g = _Geometry(int(geometry.n_sectors), self.n_rows, row_x.ctypes.data_as(C.POINTER(C.c_float)),
+                      float(geometry.tan_half_angle), float(geometry.z_max))
+        pitch = np.ascontiguousarray(calibration.pad_pitch, np.float32)
+        npads = np.ascontiguousarray(calibration.n_pads, np.int32)
+        corr = np.ascontiguousarray(calibration.corr, np.float32)
+        assert corr.shape[:2] == (int(geometry.n_sectors), self.n_rows) and corr.shape[4] == 2
+        cal = _Calibration(pitch.ctypes.data_as(C.POINTER(C.c_float)), npads.ctypes.data_as(C.POINTER(C.c_int32)),
+                           float(calibration.t0), float(calibration.v_drift), float(calibration.t_max),
+                           int(corr.shape[3]), int(corr.shape[2]), corr.ctypes.data_as(C.POINTER(C.c_float)))
+        rc = self._lib.tpc_transform_create(C.byref(g), C.byref(cal), C.byref(self._h))
+        if rc != 0:
+            raise TpcError(f"tpc_transform_create failed ({rc}): {self._lib.tpc_transform_last_error(None).decode()}")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.tpc_transform_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def transform(self, pad, time, row_offsets, n_tasks: int, y, z, stream=None):
+        """tpc_transform_clusters on DEVICE tensors (fp32; row_offsets int32 viewed as uint32). Asynchronous."""
+        import torch
+        if not (pad.is_cuda and time.is_cuda and row_offsets.is_cuda and y.is_cuda and z.is_cuda):
+            raise TpcError("transform needs CUDA tensors; there is no CPU path")
+        assert pad.dtype == time.dtype == y.dtype == z.dtype == torch.float32 and row_offsets.dtype == torch.int32
+        assert row_offsets.numel() == n_tasks * self.n_rows + 1 and y.numel() == z.numel() == pad.numel() == time.numel()
+        s = stream if stream is not None else torch.cuda.current_stream(pad.device)
+        rc = self._lib.tpc_transform_clusters(self._h, pad.data_ptr(), time.data_ptr(), row_offsets.data_ptr(),
+                                              int(pad.numel()), int(n_tasks), y.data_ptr(), z.data_ptr(), _stream_ptr(s))
+        if rc != 0:
+            raise TpcError(f"tpc_transform_clusters failed ({rc}): {self._lib.tpc_transform_last_error(self._h).decode()}")
 
 
 def _stream_ptr(stream):

@@ -134,12 +134,16 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   __shared__ uint32_t s_tile;
   __shared__ unsigned long long s_prefix;
   constexpr unsigned FULL = 0xffffffffu;
+  const uint32_t n_trk = *c.n_tracklets;
+  const uint32_t last_tile = n_trk > 0u ? (n_trk - 1u) / kOutThreads : 0u;
+  // The host does not know how many tracklets were built, only their bound: it launches a fixed number of
+  // blocks and every block takes tiles by ticket until they run out.  A tile only waits (look-back) for tiles
+  // with smaller tickets, which are held by running blocks.
+  for (;;) {
+  __syncthreads();  // s_tile, s_prefix, s_warp of the previous tile are no longer read
   if (threadIdx.x == 0) s_tile = atomicAdd(&c.tickets[1], 1u);
   __syncthreads();
   const uint32_t tile = s_tile;
-  const uint32_t n_trk = *c.n_tracklets;
-  // the grid covers max_tracklets; tiles past the last tracklet have nothing to add and nobody waits for them
-  const uint32_t last_tile = n_trk > 0u ? (n_trk - 1u) / kOutThreads : 0u;
   if (tile > last_tile) return;
   const int n_rows = c.n_rows;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -226,6 +230,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
     c.out.header[0] = (uint32_t)(all >> 32);
     c.out.header[1] = (uint32_t)(all & 0xFFFFFFFFull);
   }
+  }  // next tile
 }
 
 // ---------------------------------------------------------------------------

@@ -1,0 +1,99 @@
+// Cluster transformation (PAPER.md L77 footnote 1: "convert the raw TPC clusters from
+// TPC pad row, TPC pad, and time coordinates into x, y, and z coordinates taking into account the calibration";
+// L101, L213: the map is the default or the fed-back calibration, the cluster index does not change).
+// docs/ARITH_SPEC.md section 10, X1..X4: nominal pad/time geometry plus a bilinear (dy, dz) map per (sector,row).
+//
+// Pure streaming work: 8 bytes in, 8 bytes out per cluster, the 6 MB map stays in L2.  One block per 2048
+// consecutive clusters (whole 16-byte groups: float4 loads of pad/time, float4 stores of y/z); the (task,row)
+// of a cluster comes from the row offsets of the chunk, staged in shared memory once per block.
+#pragma once
+#include "device_common.cuh"
+
+namespace tpc {
+
+constexpr int kXfThreads = 256;
+constexpr uint32_t kXfChunk = 2048;  // clusters per block: 2 float4 groups per thread
+constexpr int kXfRows = 256;         // row offsets of the chunk kept in shared memory
+
+struct TransformCtx {
+  int32_t n_sectors, n_rows, my, mz;
+  float z_max, t0, v_drift, kz;
+  const float* pitch;   // [n_rows] X1
+  const float* centre;  // [n_rows] 0.5f*(float)(n_pads-1)
+  const float* ky;      // [n_rows] (float)(MY-1)/(float)(n_pads-1)
+  const float* map;     // [n_sectors][n_rows][MZ][MY][2]
+  const float *pad, *time;
+  const uint32_t* row_off;
+  uint32_t n, n_tr;
+  float *y, *z;
+};
+
+// X1..X4 for one cluster of (task,row) tr
+__device__ __forceinline__ float2 transform_one(const TransformCtx& c, uint32_t tr, float pad, float time) {
+  const uint32_t nr = (uint32_t)c.n_rows, ns = (uint32_t)c.n_sectors;
+  const uint32_t task = tr / nr, row = tr - task * nr, sec = task % ns;
+  const float y0 = (pad - __ldg(c.centre + row)) * __ldg(c.pitch + row);   // X1
+  const float zd = (time - c.t0) * c.v_drift;                               // X2
+  const float z0 = 2u * sec < ns ? c.z_max - zd : zd - c.z_max;
+  float u = pad * __ldg(c.ky + row), v = time * c.kz;                       // X3
+  u = fminf(fmaxf(u, 0.0f), (float)(c.my - 1));
+  v = fminf(fmaxf(v, 0.0f), (float)(c.mz - 1));
+  const int iu = min((int)u, c.my - 2), iv = min((int)v, c.mz - 2);
+  const float fu = u - (float)iu, fv = v - (float)iv;
+  const float2* m = reinterpret_cast<const float2*>(c.map) + ((size_t)(sec * nr + row) * c.mz + iv) * c.my + iu;
+  const float2 m00 = __ldg(m), m01 = __ldg(m + 1), m10 = __ldg(m + c.my), m11 = __ldg(m + c.my + 1);
+  const float ay = m00.x + fu * (m01.x - m00.x), by = m10.x + fu * (m11.x - m10.x);
+  const float az = m00.y + fu * (m01.y - m00.y), bz = m10.y + fu * (m11.y - m10.y);
+  return make_float2(y0 + (ay + fv * (by - ay)), z0 + (az + fv * (bz - az)));   // X4
+}
+
+__global__ void __launch_bounds__(kXfThreads) k_transform(const TransformCtx c) {
+  __shared__ uint32_t s_rowoff[kXfRows + 1];
+  __shared__ uint32_t s_tr;
+  const uint32_t i0 = blockIdx.x * kXfChunk, i1 = min(i0 + kXfChunk, c.n);
+  if (threadIdx.x == 0) {  // last (task,row) with row_off <= i0
+    uint32_t lo = 0u, hi = c.n_tr;
+    while (hi - lo > 1u) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (c.row_off[mid] <= i0) lo = mid; else hi = mid;
+    }
+    s_tr = lo;
+  }
+  __syncthreads();
+  const uint32_t tr0 = s_tr;
+  for (uint32_t j = threadIdx.x; j <= (uint32_t)kXfRows; j += kXfThreads) s_rowoff[j] = c.row_off[min(tr0 + j, c.n_tr)];
+  __syncthreads();
+  auto tr_of = [&](uint32_t i) -> uint32_t {
+    if (i < s_rowoff[kXfRows]) {
+      uint32_t lo = 0u, hi = (uint32_t)kXfRows;
+      while (hi - lo > 1u) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (s_rowoff[mid] <= i) lo = mid; else hi = mid;
+      }
+      return tr0 + lo;
+    }
+    uint32_t lo = tr0, hi = c.n_tr;  // a chunk over more than kXfRows (mostly empty) rows
+    while (hi - lo > 1u) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (c.row_off[mid] <= i) lo = mid; else hi = mid;
+    }
+    return lo;
+  };
+  for (uint32_t g = i0 + 4u * threadIdx.x; g < i1; g += 4u * kXfThreads) {
+    if (g + 4u <= i1) {  // a whole 16-byte group (cudaMalloc'ed arrays: chunk starts are 16-byte aligned)
+      const float4 p = __ldg(reinterpret_cast<const float4*>(c.pad + g));
+      const float4 t = __ldg(reinterpret_cast<const float4*>(c.time + g));
+      const float2 r0 = transform_one(c, tr_of(g), p.x, t.x), r1 = transform_one(c, tr_of(g + 1u), p.y, t.y);
+      const float2 r2 = transform_one(c, tr_of(g + 2u), p.z, t.z), r3 = transform_one(c, tr_of(g + 3u), p.w, t.w);
+      *reinterpret_cast<float4*>(c.y + g) = make_float4(r0.x, r1.x, r2.x, r3.x);
+      *reinterpret_cast<float4*>(c.z + g) = make_float4(r0.y, r1.y, r2.y, r3.y);
+    } else {
+      for (uint32_t i = g; i < i1; ++i) {
+        const float2 r = transform_one(c, tr_of(i), c.pad[i], c.time[i]);
+        c.y[i] = r.x; c.z[i] = r.y;
+      }
+    }
+  }
+}
+
+}  // namespace tpc

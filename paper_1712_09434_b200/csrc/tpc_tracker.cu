@@ -21,6 +21,7 @@
 #include "stage_neighbours.cuh"
 #include "stage_output.cuh"
 #include "stage_tracklet.cuh"
+#include "stage_transform.cuh"
 #include "stages_ca.cuh"
 
 using namespace tpc;
@@ -448,7 +449,7 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
     k_resolve<<<(c.n + kResolveChunk - 1) / kResolveChunk, kResolveThreads, kResolveChunk * sizeof(unsigned long long), s>>>(c);
   }
   mark();
-  k_select_output<<<cv.out_tiles, kOutThreads, 0, s>>>(c);                          // a6 + a7
+  k_select_output<<<cv.out_tiles < 16u * (uint32_t)t->n_sm ? cv.out_tiles : 16u * (uint32_t)t->n_sm, kOutThreads, 0, s>>>(c);                          // a6 + a7
   mark();
   if (c.n > 0 && (out->dbg_link_up || out->dbg_link_dn || out->dbg_clean_up || out->dbg_clean_dn ||
                   out->dbg_start_hits))
@@ -796,6 +797,76 @@ int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tr
   if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_merge_refit: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;
 }
+
+// ---- cluster transformation (SPEC 10) --------------------------------------------------------------
+struct tpc_transform {
+  TransformCtx c{};
+  float* d_tables = nullptr;  // pitch, centre, ky [n_rows] each, then the map
+  std::string err;
+};
+
+int tpc_transform_create(const tpc_geometry* g, const tpc_calibration* cal, tpc_transform** out) {
+  if (!g || !cal || !out) return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_transform_create: geometry, calibration and out must not be NULL");
+  *out = nullptr;
+  if (g->n_sectors < 1 || g->n_rows < 1 || g->n_rows > kMaxRows || !cal->pad_pitch || !cal->n_pads || !cal->map ||
+      cal->map_ny < 2 || cal->map_nz < 2 || !(cal->t_max > 0.f) || !(g->z_max > 0.f))
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_transform_create: need tables, map_ny >= 2, map_nz >= 2, t_max > 0");
+  for (int r = 0; r < g->n_rows; ++r)
+    if (cal->n_pads[r] < 2) return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_transform_create: n_pads must be >= 2 in every row");
+  tpc_transform* t = new (std::nothrow) tpc_transform();
+  if (!t) return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_transform_create: out of host memory");
+  const int n = g->n_rows;
+  const size_t n_map = (size_t)g->n_sectors * n * cal->map_nz * cal->map_ny * 2;
+  const size_t map_off = ((size_t)3 * n + 3) & ~(size_t)3;  // the kernel reads the map as float2 / 16-byte groups
+  std::vector<float> tab(map_off + n_map);
+  for (int r = 0; r < n; ++r) {
+    tab[r] = cal->pad_pitch[r];
+    tab[n + r] = 0.5f * (float)(cal->n_pads[r] - 1);                              // X1
+    tab[2 * n + r] = (float)(cal->map_ny - 1) / (float)(cal->n_pads[r] - 1);      // X3 ky
+  }
+  memcpy(tab.data() + map_off, cal->map, n_map * sizeof(float));
+  cudaError_t e = cudaMalloc(&t->d_tables, tab.size() * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemcpy(t->d_tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    const int rc = fail(nullptr, TPC_ERR_CUDA, "tpc_transform_create: CUDA: %s (no CPU fallback exists)", cudaGetErrorString(e));
+    if (t->d_tables) cudaFree(t->d_tables);
+    delete t;
+    cudaGetLastError();
+    return rc;
+  }
+  TransformCtx& c = t->c;
+  c.n_sectors = g->n_sectors; c.n_rows = n; c.my = cal->map_ny; c.mz = cal->map_nz;
+  c.z_max = g->z_max; c.t0 = cal->t0; c.v_drift = cal->v_drift;
+  c.kz = (float)(cal->map_nz - 1) / cal->t_max;                                   // X3 kz
+  c.pitch = t->d_tables; c.centre = t->d_tables + n; c.ky = t->d_tables + 2 * n; c.map = t->d_tables + map_off;
+  *out = t;
+  return TPC_OK;
+}
+
+void tpc_transform_destroy(tpc_transform* t) {
+  if (!t) return;
+  if (t->d_tables) cudaFree(t->d_tables);
+  delete t;
+}
+
+int tpc_transform_clusters(tpc_transform* t, const float* pad, const float* time, const uint32_t* row_offsets,
+                           uint32_t n_clusters, uint32_t n_tasks, float* y, float* z, void* cuda_stream) {
+  if (!t) return TPC_ERR_ARGUMENT;
+  auto bad = [&](const char* msg) { t->err = msg; return TPC_ERR_ARGUMENT; };
+  if (!row_offsets || (n_clusters && (!pad || !time || !y || !z))) return bad("tpc_transform_clusters: pad, time, row_offsets, y, z must not be NULL");
+  if ((((uintptr_t)pad | (uintptr_t)time | (uintptr_t)y | (uintptr_t)z) & 15u) != 0) return bad("tpc_transform_clusters: pad, time, y, z must be 16-byte aligned");
+  if ((uint64_t)n_tasks * (uint64_t)t->c.n_rows >= 0x7FFFFFFFull) return bad("tpc_transform_clusters: n_tasks*n_rows must be < 2^31");
+  if (n_clusters == 0) return TPC_OK;
+  TransformCtx c = t->c;
+  c.pad = pad; c.time = time; c.row_off = row_offsets; c.n = n_clusters; c.n_tr = n_tasks * (uint32_t)c.n_rows;
+  c.y = y; c.z = z;
+  k_transform<<<(n_clusters + kXfChunk - 1) / kXfChunk, kXfThreads, 0, (cudaStream_t)cuda_stream>>>(c);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { t->err = std::string("tpc_transform_clusters: CUDA launch: ") + cudaGetErrorString(e); return TPC_ERR_CUDA; }
+  return TPC_OK;
+}
+
+const char* tpc_transform_last_error(const tpc_transform* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
 
 const char* tpc_last_error(const tpc_tracker* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
 

@@ -65,8 +65,8 @@ MUTANTS = [
      "if (!transport(st, T.X[r], T.a, R(T.prm.max_sinphi))) { chain_ok = false; break; }\n        apply_hit",
      "if (!transport(st, T.X[r], T.a, R(T.prm.max_sinphi))) { chain_ok = false; }\n        apply_hit"),
     ("turn-around scales only the diagonal", "K4 / R15",
-     "for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);",
-     "for (int i : {0, 2, 5, 9, 14}) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);"),
+     "      for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);\n",
+     "      for (int i : {0, 2, 5, 9, 14}) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);\n"),
     ("turn-around: lastRow hit not re-fitted", "K4 / D3",
      "if (st.x == T.X[tk.last_row]) apply_hit(st, (uint32_t)tk.map[tk.last_row]);", ""),
     ("turn-around: no transport back to lastRow", "K4",
