@@ -63,16 +63,26 @@ __global__ void __launch_bounds__(kXfThreads) k_transform(const TransformCtx c) 
   const uint32_t tr0 = s_tr;
   for (uint32_t j = threadIdx.x; j <= (uint32_t)kXfRows; j += kXfThreads) s_rowoff[j] = c.row_off[min(tr0 + j, c.n_tr)];
   __syncthreads();
-  auto tr_of = [&](uint32_t i) -> uint32_t {
-    if (i < s_rowoff[kXfRows]) {
-      uint32_t lo = 0u, hi = (uint32_t)kXfRows;
-      while (hi - lo > 1u) {
-        const uint32_t mid = (lo + hi) >> 1;
-        if (s_rowoff[mid] <= i) lo = mid; else hi = mid;
-      }
-      return tr0 + lo;
+  // staged rows the chunk really spans (a chunk of a central event holds 5 rows): the searches below are short
+  __shared__ uint32_t s_span;
+  if (threadIdx.x == 0) {
+    uint32_t k = 1u;
+    while (k < (uint32_t)kXfRows && s_rowoff[k] < i1) ++k;
+    s_span = k;  // s_rowoff[k] >= i1, or k == kXfRows
+  }
+  __syncthreads();
+  const uint32_t span = s_span;
+  const bool staged = s_rowoff[span] >= i1;  // else: more than kXfRows (mostly empty) rows, global search
+  auto row_slot = [&](uint32_t i) -> uint32_t {  // last staged row j with s_rowoff[j] <= i
+    uint32_t lo = 0u, hi = span;
+    while (hi - lo > 1u) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (s_rowoff[mid] <= i) lo = mid; else hi = mid;
     }
-    uint32_t lo = tr0, hi = c.n_tr;  // a chunk over more than kXfRows (mostly empty) rows
+    return lo;
+  };
+  auto tr_global = [&](uint32_t i) -> uint32_t {
+    uint32_t lo = tr0, hi = c.n_tr;
     while (hi - lo > 1u) {
       const uint32_t mid = (lo + hi) >> 1;
       if (c.row_off[mid] <= i) lo = mid; else hi = mid;
@@ -80,17 +90,30 @@ __global__ void __launch_bounds__(kXfThreads) k_transform(const TransformCtx c) 
     return lo;
   };
   for (uint32_t g = i0 + 4u * threadIdx.x; g < i1; g += 4u * kXfThreads) {
-    if (g + 4u <= i1) {  // a whole 16-byte group (cudaMalloc'ed arrays: chunk starts are 16-byte aligned)
+    const uint32_t n_el = min(4u, i1 - g);
+    uint32_t tr[4];
+    if (staged) {  // the four clusters are consecutive: one search, then steps over row ends (empty rows too)
+      uint32_t j = row_slot(g);
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k) {
+        while (j + 1u < span && s_rowoff[j + 1u] <= g + k) ++j;
+        tr[k] = tr0 + j;
+      }
+    } else {
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k) tr[k] = tr_global(min(g + k, i1 - 1u));
+    }
+    if (n_el == 4u) {  // a whole 16-byte group (cudaMalloc'ed arrays: chunk starts are 16-byte aligned)
       const float4 p = __ldg(reinterpret_cast<const float4*>(c.pad + g));
       const float4 t = __ldg(reinterpret_cast<const float4*>(c.time + g));
-      const float2 r0 = transform_one(c, tr_of(g), p.x, t.x), r1 = transform_one(c, tr_of(g + 1u), p.y, t.y);
-      const float2 r2 = transform_one(c, tr_of(g + 2u), p.z, t.z), r3 = transform_one(c, tr_of(g + 3u), p.w, t.w);
+      const float2 r0 = transform_one(c, tr[0], p.x, t.x), r1 = transform_one(c, tr[1], p.y, t.y);
+      const float2 r2 = transform_one(c, tr[2], p.z, t.z), r3 = transform_one(c, tr[3], p.w, t.w);
       *reinterpret_cast<float4*>(c.y + g) = make_float4(r0.x, r1.x, r2.x, r3.x);
       *reinterpret_cast<float4*>(c.z + g) = make_float4(r0.y, r1.y, r2.y, r3.y);
     } else {
-      for (uint32_t i = g; i < i1; ++i) {
-        const float2 r = transform_one(c, tr_of(i), c.pad[i], c.time[i]);
-        c.y[i] = r.x; c.z[i] = r.y;
+      for (uint32_t k = 0; k < n_el; ++k) {
+        const float2 r = transform_one(c, tr[k], c.pad[g + k], c.time[g + k]);
+        c.y[g + k] = r.x; c.z[g + k] = r.y;
       }
     }
   }
