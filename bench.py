@@ -358,7 +358,7 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
 
     # end to end through tpc_track_batch_host: pinned host inputs -> device -> tracks back on the host
-    e2e = None
+    e2e = e2e_pipe = None
     if not args.no_e2e:
         out_h = trk.alloc_outputs(n, dev, pinned_host=True)
         tcap, hcap = out_h.track_task.shape[0], out_h.hit_cluster.shape[0]
@@ -376,6 +376,29 @@ def run_ours(args):
         torch.cuda.synchronize()
         e2e_ms = e0.elapsed_time(e1)
         e2e = (e2e_ms, up, down)
+        # the same with two batches in flight (tpc_host_submit / tpc_host_collect): every step still uploads its
+        # inputs from pinned host memory and downloads its tracks and hits, but under the kernels of its neighbours
+        out_h2 = trk.alloc_outputs(n, dev, pinned_host=True)
+        ws_h2 = trk.alloc_workspace(trk.host_workspace_bytes(n, n_tasks, 0, tcap, hcap), dev)
+        outs_p, wss_p = (out_h, out_h2), (ws_h, ws_h2)
+
+        def run_pipeline(steps):
+            trk.host_submit(0, y_h, z_h, ro_h, n_tasks, tcap, hcap, wss_p[0])
+            for i in range(1, steps):
+                trk.host_submit(i % 2, y_h, z_h, ro_h, n_tasks, tcap, hcap, wss_p[i % 2])
+                trk.host_collect((i - 1) % 2, outs_p[(i - 1) % 2])
+            return trk.host_collect((steps - 1) % 2, outs_p[(steps - 1) % 2])
+        run_pipeline(2)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t_p0 = time.perf_counter()
+        up_p, down_p = run_pipeline(args.steps)
+        torch.cuda.synchronize()
+        pipe_ms = (time.perf_counter() - t_p0) * 1e3
+        assert int(out_h.header[0]) == int(hdr[0]) and int(out_h2.header[1]) == int(hdr[1])
+        e2e_pipe = (pipe_ms, up_p, down_p)
+        del ws_h2, out_h2
         del ws_h, out_h
 
     # sector-segment merger + final refit behind a7 (tpc_merge_refit), timed on its own: tracker call +
@@ -439,7 +462,8 @@ def run_ours(args):
         del pad_d, time_d, y2, z2
 
     # max over ranks, totals over ranks
-    (ms_total, e2e_ms_max), tot = reduce_over_ranks([ms_total, e2e[0] if e2e else 0.0],
+    (ms_total, e2e_ms_max, e2e_pipe_ms_max), tot = reduce_over_ranks([ms_total, e2e[0] if e2e else 0.0,
+                                                                       e2e_pipe[0] if e2e else 0.0],
                                                     [n, n_events, int(hdr[0]), int(hdr[1])], dev)
     if rank != 0:
         if world > 1:
@@ -500,9 +524,17 @@ def run_ours(args):
         merge["hbm_frac"] = merge["achieved_gbs"] / peak_gbs
         line["merge_refit"] = merge
     if e2e:
-        line["e2e"] = {"value": tot[0] * args.steps / (e2e_ms_max / 1e3), "unit": UNIT,
-                       "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2],
-                       "ms_per_step": e2e_ms_max / args.steps, "api": "tpc_track_batch_host (pinned host buffers)"}
+        # headline end-to-end number: the pipelined entry point (what a caller with a stream of batches uses); every
+        # step uploads its own inputs and downloads its own result inside the timed region (wall clock between two
+        # device synchronisations: the copies run on the library's own streams).  e2e_sync: one batch at a time.
+        line["e2e"] = {"value": tot[0] * args.steps / (e2e_pipe_ms_max / 1e3), "unit": UNIT,
+                       "h2d_bytes_per_step": e2e_pipe[1], "d2h_bytes_per_step": e2e_pipe[2],
+                       "ms_per_step": e2e_pipe_ms_max / args.steps,
+                       "api": "tpc_host_submit / tpc_host_collect (pinned host buffers, two batches in flight)"}
+        line["e2e_sync"] = {"value": tot[0] * args.steps / (e2e_ms_max / 1e3), "unit": UNIT,
+                            "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2],
+                            "ms_per_step": e2e_ms_max / args.steps,
+                            "api": "tpc_track_batch_host (pinned host buffers, one batch at a time, three chunks)"}
     if world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands, (i) over all host cores, one (event, sector) task per worker process at a time, on
         # every event of the workload, (ii) on one thread on the first events

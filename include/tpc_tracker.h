@@ -178,6 +178,19 @@ int tpc_track_batch_host(tpc_tracker* tracker, const tpc_clusters* clusters, tpc
                          void* workspace, size_t workspace_bytes, uint32_t max_tracklets, void* cuda_stream,
                          uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 
+/* Pipelined variant of tpc_track_batch_host: two batches in flight (slot 0 and slot 1), each with a
+ * DEVICE workspace of its own of tpc_host_workspace_bytes(...).  tpc_host_submit queues the upload of the
+ * batch (HOST clusters, page-locked for overlap), the whole path and the download of the result sizes
+ * on the tracker's own streams and returns at once; the host arrays of `clusters` must stay valid
+ * until the slot is collected.  tpc_host_collect waits for the slot's batch, copies its tracks and hits
+ * into the HOST arrays of `tracks` (capacities as given there; columns that are NULL are skipped) and
+ * fills tracks->header.  With submit(k+1) issued before collect(k) the copies of one batch run under
+ * the kernels of its neighbours (the gain of a GPU stage is lost when it waits for PCIe).
+ * The result of a batch is tpc_track_batch's.  A slot must be collected before it is submitted again. */
+int tpc_host_submit(tpc_tracker* tracker, int slot, const tpc_clusters* clusters, uint32_t track_capacity,
+                    uint32_t hit_capacity, void* workspace, size_t workspace_bytes, uint32_t max_tracklets);
+int tpc_host_collect(tpc_tracker* tracker, int slot, tpc_tracks* tracks, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
 /* Per-stage device counters of the LAST tpc_track_batch call on this tracker
  * (HOST pointer out, [TPC_N_COUNTERS] uint64; synchronises the stream given).
  * Only filled when the tracker was created with counters enabled through

@@ -132,6 +132,10 @@ def load_library():
     lib.tpc_stage_name.argtypes = [C.c_int]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_last_error.argtypes = [vp]
+    lib.tpc_host_submit.restype = C.c_int
+    lib.tpc_host_submit.argtypes = [vp, C.c_int, C.POINTER(_Clusters), C.c_uint32, C.c_uint32, vp, C.c_size_t, C.c_uint32]
+    lib.tpc_host_collect.restype = C.c_int
+    lib.tpc_host_collect.argtypes = [vp, C.c_int, C.POINTER(_Tracks), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.tpc_transform_create.restype = C.c_int
     lib.tpc_transform_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Calibration), C.POINTER(vp)]
     lib.tpc_transform_destroy.restype = None
@@ -385,6 +389,25 @@ class Tracker:
                     "tpc_track_batch_host")
         return int(up.value), int(down.value)
 
+
+    def host_submit(self, slot: int, y, z, row_offsets, n_tasks: int, track_capacity: int, hit_capacity: int,
+                    workspace, max_tracklets: int = 0):
+        """tpc_host_submit: HOST tensors (pinned), returns at once; the tensors must stay alive until host_collect."""
+        import torch
+        assert not y.is_cuda and not z.is_cuda and not row_offsets.is_cuda and workspace.is_cuda
+        assert y.dtype == torch.float32 and z.dtype == torch.float32 and row_offsets.dtype == torch.int32
+        cl = _Clusters(None, y.data_ptr(), z.data_ptr(), None, row_offsets.data_ptr(), int(y.numel()), int(n_tasks))
+        wp, wn = self._aligned(workspace)
+        self._check(self._lib.tpc_host_submit(self._h, int(slot), C.byref(cl), int(track_capacity), int(hit_capacity),
+                                              wp, wn, int(max_tracklets)), "tpc_host_submit")
+
+    def host_collect(self, slot: int, out: TrackResult):
+        """tpc_host_collect into HOST tensors; returns (h2d_bytes, d2h_bytes) of the batch."""
+        tr = self._tracks_struct(out)
+        up, down = C.c_uint64(0), C.c_uint64(0)
+        self._check(self._lib.tpc_host_collect(self._h, int(slot), C.byref(tr), C.byref(up), C.byref(down)),
+                    "tpc_host_collect")
+        return int(up.value), int(down.value)
 
     # ---- sector-segment merger + refit (include/tpc_tracker.h, SPEC 9) ----------------------
     def merge_workspace_bytes(self, track_capacity: int, max_tasks: int) -> int:

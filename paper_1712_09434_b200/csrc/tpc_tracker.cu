@@ -48,6 +48,10 @@ struct tpc_tracker {
   std::vector<cudaStream_t> host_streams;
   std::vector<cudaEvent_t> host_events;
   uint32_t* host_headers = nullptr;
+  // tpc_host_submit / tpc_host_collect: two batches in flight
+  struct PipeSlot { bool busy = false; tpc_tracks d{}; uint32_t tcap = 0, hcap = 0; uint64_t up = 0; cudaEvent_t in = nullptr, done = nullptr; };
+  PipeSlot pipe[2];
+  uint32_t* pipe_headers = nullptr;  // pinned, 4 words per slot
   std::vector<cudaEvent_t> ev;
   uint32_t timed_calls = 0;
   std::string err;
@@ -292,6 +296,8 @@ void tpc_tracker_destroy(tpc_tracker* t) {
   for (cudaStream_t x : t->host_streams) cudaStreamDestroy(x);
   for (cudaEvent_t x : t->host_events) cudaEventDestroy(x);
   if (t->host_headers) cudaFreeHost(t->host_headers);
+  if (t->pipe_headers) cudaFreeHost(t->pipe_headers);
+  for (auto& p : t->pipe) { if (p.in) cudaEventDestroy(p.in); if (p.done) cudaEventDestroy(p.done); }
   if (t->d_tables) cudaFree(t->d_tables);
   if (t->d_counters) cudaFree(t->d_counters);
   delete t;
@@ -513,6 +519,8 @@ HostCarve host_carve(const tpc_tracker* t, uint32_t n, uint32_t n_tasks, uint32_
 }
 }  // namespace
 
+namespace { int ensure_host_streams(tpc_tracker* t); }
+
 size_t tpc_host_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t max_tasks, uint32_t max_tracklets,
                                 uint32_t track_capacity, uint32_t hit_capacity) {
   if (!t) return 0;
@@ -563,19 +571,9 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   task_b[n_chunks] = in->n_tasks;
   // streams and events of the chunks, created on first use
   cudaError_t e = cudaSuccess;
-  if (t->host_streams.empty()) {
-    t->host_streams.resize(kHostChunks, nullptr);
-    t->host_events.resize(2 * kHostChunks + 1, nullptr);  // [k] chunk k computed, [kHostChunks] start, [kHostChunks + 1 + k] chunk k copied in
-    for (auto& x : t->host_streams) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking);
-    for (auto& x : t->host_events) if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->host_headers, 16 * kHostChunks, cudaHostAllocDefault);
-    if (e != cudaSuccess) {  // leave nothing half made behind: the next call starts again
-      for (auto& x : t->host_streams) if (x) cudaStreamDestroy(x);
-      for (auto& x : t->host_events) if (x) cudaEventDestroy(x);
-      if (t->host_headers) cudaFreeHost(t->host_headers);
-      t->host_streams.clear(); t->host_events.clear(); t->host_headers = nullptr;
-      return fail(t, TPC_ERR_CUDA, "tpc_track_batch_host: CUDA: %s", cudaGetErrorString(e));
-    }
+  {
+    const int rc0 = ensure_host_streams(t);
+    if (rc0 != TPC_OK) return rc0;
   }
   const bool timing = t->timing_on, counters = t->counters_on;
   t->timing_on = false; t->counters_on = false;  // per-stage marks and counters describe one tpc_track_batch call
@@ -689,6 +687,150 @@ int tpc_track_batch_host(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out
   out->header[2] = status;
   out->header[3] = tracklets;
   if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = down;
+  return TPC_OK;
+}
+
+// ---- pipelined host entry point: two batches in flight ---------------------------------------------
+// submit(slot) queues the upload, the path and the download of the header of one batch on the tracker's own
+// streams (copies in / kernels / copies out) and returns; collect(slot) waits for that batch, then copies its
+// tracks and hits to the caller's host arrays.  With submit(k + 1) issued before collect(k), the upload of batch
+// k + 1 and the download of batch k run under the kernels of their neighbours: in the steady state a batch costs
+// what its kernels cost.  One chunk per batch (the persistent tracklet kernels cost 0.3 ms per extra chunk).
+namespace {
+int ensure_host_streams(tpc_tracker* t) {
+  cudaError_t e = cudaSuccess;
+  if (t->host_streams.empty()) {
+    t->host_streams.resize(kHostChunks, nullptr);
+    t->host_events.resize(2 * kHostChunks + 1, nullptr);
+    for (auto& x : t->host_streams) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking);
+    for (auto& x : t->host_events) if (e == cudaSuccess) e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->host_headers, 16 * kHostChunks, cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+      for (auto& x : t->host_streams) if (x) cudaStreamDestroy(x);
+      for (auto& x : t->host_events) if (x) cudaEventDestroy(x);
+      if (t->host_headers) cudaFreeHost(t->host_headers);
+      t->host_streams.clear(); t->host_events.clear(); t->host_headers = nullptr;
+      return fail(t, TPC_ERR_CUDA, "host streams: CUDA: %s", cudaGetErrorString(e));
+    }
+  }
+  if (!t->pipe_headers) {
+    e = cudaHostAlloc((void**)&t->pipe_headers, 2 * 16, cudaHostAllocDefault);
+    for (auto& p : t->pipe) {
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p.in, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p.done, cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) {
+      for (auto& p : t->pipe) { if (p.in) cudaEventDestroy(p.in); if (p.done) cudaEventDestroy(p.done); p.in = p.done = nullptr; }
+      if (t->pipe_headers) cudaFreeHost(t->pipe_headers);
+      t->pipe_headers = nullptr;
+      return fail(t, TPC_ERR_CUDA, "host pipeline: CUDA: %s", cudaGetErrorString(e));
+    }
+  }
+  return TPC_OK;
+}
+}  // namespace
+
+int tpc_host_submit(tpc_tracker* t, int slot, const tpc_clusters* in, uint32_t track_capacity, uint32_t hit_capacity,
+                    void* workspace, size_t workspace_bytes, uint32_t max_tracklets) {
+  if (!t) return TPC_ERR_ARGUMENT;
+  if (slot < 0 || slot > 1) return fail(t, TPC_ERR_ARGUMENT, "tpc_host_submit: slot must be 0 or 1");
+  if (!in || !in->row_offsets || (in->n_clusters && (!in->y || !in->z)))
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_host_submit: y, z, row_offsets must not be NULL");
+  tpc_tracker::PipeSlot& ps = t->pipe[slot];
+  if (ps.busy) return fail(t, TPC_ERR_ARGUMENT, "tpc_host_submit: slot %d has not been collected", slot);
+  const uint32_t n = in->n_clusters, n_rows = (uint32_t)t->n_rows;
+  if (in->row_offsets[(size_t)in->n_tasks * n_rows] != n)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_host_submit: row_offsets must end at n_clusters");
+  const uint32_t T_all = host_total_tracklets(t, n, max_tracklets, kHostChunks);
+  const HostCarve h = host_carve(t, n, in->n_tasks, T_all, track_capacity, hit_capacity);
+  if (!workspace || workspace_bytes < h.total)
+    return fail(t, TPC_ERR_WORKSPACE, "tpc_host_submit: workspace of %zu bytes, need %zu (tpc_host_workspace_bytes)", workspace_bytes, h.total);
+  if (((uintptr_t)workspace & (kAlign - 1)) != 0)
+    return fail(t, TPC_ERR_WORKSPACE, "tpc_host_submit: workspace must be %zu-byte aligned", kAlign);
+  int rc = ensure_host_streams(t);
+  if (rc != TPC_OK) return rc;
+  cudaStream_t s_in = t->host_streams[0], s_cmp = t->host_streams[1];
+  char* ws = (char*)workspace;
+  const size_t n_off = (size_t)in->n_tasks * n_rows + 1;
+  cudaError_t e = cudaSuccess;
+  uint64_t up = 0;
+  auto h2d = [&](void* dst, const void* src, size_t bytes) {
+    if (e == cudaSuccess && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s_in); up += bytes; }
+  };
+  h2d(ws + h.y, in->y, (size_t)n * 4);
+  h2d(ws + h.z, in->z, (size_t)n * 4);
+  h2d(ws + h.row_off, in->row_offsets, n_off * 4);
+  if (e == cudaSuccess) e = cudaEventRecord(ps.in, s_in);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s_cmp, ps.in, 0);
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_host_submit: CUDA: %s", cudaGetErrorString(e));
+  tpc_clusters din{};
+  din.y = (const float*)(ws + h.y); din.z = (const float*)(ws + h.z);
+  din.row_offsets = (const uint32_t*)(ws + h.row_off); din.n_clusters = n; din.n_tasks = in->n_tasks;
+  const uint32_t mh = (uint32_t)(t->prm.min_track_hits > 0 ? t->prm.min_track_hits : 1);
+  tpc_tracks& d = ps.d;
+  d = tpc_tracks{};
+  ps.tcap = n / mh + 1u < track_capacity ? n / mh + 1u : track_capacity;
+  ps.hcap = n + 1u < hit_capacity ? n + 1u : hit_capacity;
+  d.track_capacity = ps.tcap; d.hit_capacity = ps.hcap;
+  d.header = (uint32_t*)(ws + h.header);
+  d.track_task = (uint32_t*)(ws + h.track_task); d.track_hit_begin = (uint32_t*)(ws + h.track_hit_begin);
+  d.track_nhits = (uint32_t*)(ws + h.track_nhits); d.track_ndf = (int32_t*)(ws + h.track_ndf);
+  d.track_x = (float*)(ws + h.track_x); d.track_chi2 = (float*)(ws + h.track_chi2);
+  d.track_par = (float*)(ws + h.track_par); d.track_cov = (float*)(ws + h.track_cov);
+  d.hit_cluster = (uint32_t*)(ws + h.hit_cluster);
+  uint32_t T = resolve_max_tracklets(t, n, 0u);
+  if (max_tracklets && max_tracklets < T) T = max_tracklets;
+  const size_t need = carve(n_rows, n, in->n_tasks, T).total;
+  if (h.inner + need > workspace_bytes) return fail(t, TPC_ERR_WORKSPACE, "tpc_host_submit: workspace too small");
+  const bool timing = t->timing_on, counters = t->counters_on;
+  t->timing_on = false; t->counters_on = false;
+  rc = tpc_track_batch(t, &din, &d, ws + h.inner, need, T, s_cmp);
+  t->timing_on = timing; t->counters_on = counters;
+  if (rc != TPC_OK) return rc;
+  e = cudaMemcpyAsync(t->pipe_headers + 4 * slot, d.header, 16, cudaMemcpyDeviceToHost, s_cmp);
+  if (e == cudaSuccess) e = cudaEventRecord(ps.done, s_cmp);
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_host_submit: CUDA: %s", cudaGetErrorString(e));
+  ps.up = up;
+  ps.busy = true;
+  return TPC_OK;
+}
+
+int tpc_host_collect(tpc_tracker* t, int slot, tpc_tracks* out, uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  if (!t) return TPC_ERR_ARGUMENT;
+  if (slot < 0 || slot > 1 || !out || !out->header) return fail(t, TPC_ERR_ARGUMENT, "tpc_host_collect: slot 0 or 1, tracks and header must not be NULL");
+  tpc_tracker::PipeSlot& ps = t->pipe[slot];
+  if (!ps.busy) return fail(t, TPC_ERR_ARGUMENT, "tpc_host_collect: nothing was submitted in slot %d", slot);
+  ps.busy = false;
+  cudaStream_t s_out = t->host_streams[2];
+  cudaError_t e = cudaEventSynchronize(ps.done);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, ps.done, 0);
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_host_collect: CUDA: %s", cudaGetErrorString(e));
+  const uint32_t* hh = t->pipe_headers + 4 * slot;
+  const uint32_t tcap = out->track_capacity, hcap = out->hit_capacity;
+  uint32_t status = hh[2];
+  uint32_t nt = hh[0] < ps.tcap ? hh[0] : ps.tcap, nh = hh[1] < ps.hcap ? hh[1] : ps.hcap;
+  if (nt > tcap) { nt = tcap; status |= TPC_STATUS_TRACK_OVERFLOW; }
+  if (nh > hcap) { nh = hcap; status |= TPC_STATUS_HIT_OVERFLOW; }
+  uint64_t down = 16;
+  const tpc_tracks& d = ps.d;
+  auto d2h = [&](void* dst, const void* src, size_t bytes) {
+    if (e == cudaSuccess && dst && bytes) { e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s_out); down += bytes; }
+  };
+  d2h(out->track_task, d.track_task, (size_t)nt * 4);
+  d2h(out->track_hit_begin, d.track_hit_begin, (size_t)nt * 4);
+  d2h(out->track_nhits, d.track_nhits, (size_t)nt * 4);
+  d2h(out->track_ndf, d.track_ndf, (size_t)nt * 4);
+  d2h(out->track_x, d.track_x, (size_t)nt * 4);
+  d2h(out->track_chi2, d.track_chi2, (size_t)nt * 4);
+  for (int j = 0; j < 5 && out->track_par; ++j) d2h(out->track_par + (size_t)j * tcap, d.track_par + (size_t)j * ps.tcap, (size_t)nt * 4);
+  for (int j = 0; j < 15 && out->track_cov; ++j) d2h(out->track_cov + (size_t)j * tcap, d.track_cov + (size_t)j * ps.tcap, (size_t)nt * 4);
+  d2h(out->hit_cluster, d.hit_cluster, (size_t)nh * 4);
+  const cudaError_t e2 = cudaStreamSynchronize(s_out);
+  if (e == cudaSuccess) e = e2;
+  if (e != cudaSuccess) return fail(t, TPC_ERR_CUDA, "tpc_host_collect: CUDA: %s", cudaGetErrorString(e));
+  out->header[0] = hh[0]; out->header[1] = hh[1]; out->header[2] = status; out->header[3] = hh[3];
+  if (h2d_bytes) *h2d_bytes = ps.up;
   if (d2h_bytes) *d2h_bytes = down;
   return TPC_OK;
 }

@@ -463,3 +463,56 @@ def test_counters_match_the_oracle_counters():
     assert c["searches"] == o["search_up"] + o["search_dn"]
     assert c["tracklet_hits"] == o["tracklet_hits"]
     assert c["row_steps"] == o["row_steps"]
+
+
+def test_host_pipeline_two_batches_in_flight(cfg2):
+    """tpc_host_submit / tpc_host_collect: two different batches in flight at once, several rounds; every collected
+    result is the single device call's, array for array, and a slot cannot be reused before it is collected."""
+    import torch
+    from paper_1712_09434_b200 import Tracker, TpcError
+    dev = torch.device("cuda:0")
+    batches = [cfg2, generate_config(1)]
+    refs = [G.run_gpu(b, debug=False, debug_tracklets=False) for b in batches]
+    trk = Tracker(cfg2.geometry, G.tracker_params_for(cfg2))
+    try:
+        host, outs, wss = [], [], []
+        for b in batches:
+            n = b.n_clusters
+            host.append((torch.from_numpy(np.ascontiguousarray(b.y)).pin_memory(),
+                         torch.from_numpy(np.ascontiguousarray(b.z)).pin_memory(),
+                         torch.from_numpy(b.row_offsets.astype(np.uint32).view(np.int32)).pin_memory()))
+            out = trk.alloc_outputs(n, dev, pinned_host=True)
+            outs.append(out)
+            wss.append(trk.alloc_workspace(trk.host_workspace_bytes(n, b.n_tasks, 0, out.track_task.shape[0],
+                                                                    out.hit_cluster.shape[0]), dev))
+
+        def submit(k):
+            y, z, ro = host[k]
+            trk.host_submit(k, y, z, ro, batches[k].n_tasks, outs[k].track_task.shape[0], outs[k].hit_cluster.shape[0], wss[k])
+
+        def check(k, up):
+            b, ref, out = batches[k], refs[k], outs[k]
+            assert up == 8 * b.n_clusters + 4 * (b.n_tasks * b.geometry.n_rows + 1)
+            h = out.header.numpy()
+            assert int(h[0]) == ref["n_tracks"] and int(h[1]) == ref["n_hits"] and int(h[2]) == 0
+            nt, nh = ref["n_tracks"], ref["n_hits"]
+            for f in ("track_task", "track_hit_begin", "track_nhits", "track_ndf", "track_x", "track_chi2"):
+                assert np.array_equal(getattr(out, f).numpy()[:nt], ref[f]), f
+            assert np.array_equal(out.track_par.numpy()[:, :nt], ref["track_par"])
+            assert np.array_equal(out.track_cov.numpy()[:, :nt], ref["track_cov"])
+            assert np.array_equal(out.hit_cluster.numpy()[:nh], ref["hit_cluster"])
+
+        submit(0)
+        with pytest.raises(TpcError):
+            submit(0)                       # not collected yet
+        for _ in range(3):
+            submit(1)
+            up, down = trk.host_collect(0, outs[0]); check(0, up)
+            submit(0)
+            up, down = trk.host_collect(1, outs[1]); check(1, up)
+        up, down = trk.host_collect(0, outs[0]); check(0, up)
+        assert down > 4 * refs[0]["n_hits"]
+        with pytest.raises(TpcError):
+            trk.host_collect(0, outs[0])    # nothing in flight
+    finally:
+        trk.close()
