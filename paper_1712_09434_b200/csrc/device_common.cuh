@@ -14,7 +14,10 @@
 namespace tpc {
 
 constexpr int kMaxRows = 1024;        // include/tpc_tracker.h: n_rows <= 1024
-constexpr uint32_t kBinsPerCluster = 2;  // grid density: bins per cluster of a row (the clusters bunch at small |z|)
+#ifndef TPC_BINS_PER_CLUSTER
+#define TPC_BINS_PER_CLUSTER 2
+#endif
+constexpr uint32_t kBinsPerCluster = TPC_BINS_PER_CLUSTER;  // grid density: bins per cluster of a row (the clusters bunch at small |z|)
 constexpr uint32_t kBinPad = 96;      // bins of row-block tr start at kBinsPerCluster*row_off[tr] + tr*kBinPad
 // entries of one tracklet's row map in Ctx::trk_hits: n_rows rounded up to whole 32-byte sectors
 __host__ __device__ inline size_t map_stride(int n_rows) { return (size_t)((n_rows + 7) & ~7); }
