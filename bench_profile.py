@@ -29,11 +29,13 @@ OUT = os.path.join(ROOT, "profiles", "r02_ncu_kernels.json")
 STAGE_OF = {"k_grid_build": "grid_build", "k_neighbours": "neighbour_finder", "k_clean": "cleaner",
             "k_seeds": "start_hits", "k_trk_chain": "tracklet_chain_fit", "k_trk_up": "tracklet_up_pass",
             "k_trk_refit": "tracklet_refit", "k_trk_finish": "tracklet_down_finish",
-            "k_select_output": "selector_output", "k_merge": "merger_refit"}
+            "k_task_offsets": "ownership", "k_resolve": "ownership", "k_select_output": "selector_output",
+            "k_merge": "merger_refit"}
 
 METRICS = {
     "dram_read": "dram__bytes_read.sum", "dram_write": "dram__bytes_write.sum",
     "thread_inst": "smsp__thread_inst_executed.sum", "warp_inst": "smsp__inst_executed.sum",
+    "lanes_per_inst": "smsp__thread_inst_executed_per_inst_executed.ratio",
     "duration_ns": "gpu__time_duration.sum", "l2_hit_pct": "lts__t_sector_hit_rate.pct",
     "issue_active_pct": "smsp__issue_active.avg.pct_of_peak_sustained_active",
 }
@@ -77,6 +79,8 @@ def parse_raw_csv(path):
             except ValueError:
                 continue
             rec[key] = v * UNIT_SCALE.get(units[col[metric]].strip(), 1.0)
+        if "thread_inst" not in rec and "warp_inst" in rec and "lanes_per_inst" in rec:
+            rec["thread_inst"] = rec["warp_inst"] * rec["lanes_per_inst"]  # --set full carries the ratio, not the sum
         out.setdefault(stage, []).append(rec)
     return out
 
