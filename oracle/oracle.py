@@ -28,7 +28,7 @@ class _Params(C.Structure):
     _fields_ = [(n, C.c_float) for n in (
         "sigma_y", "sigma_z", "nf_hy", "nf_hz", "nf_chi2_max", "grid_bin_min", "grid_bin_max",
         "max_sinphi", "c0_sinphi", "c0_dzds", "c0_qpt", "accept_k2", "search_max", "turn_cov_scale")] + [
-        (n, C.c_int32) for n in ("min_seed_hits", "max_row_gap", "min_track_hits")]
+        (n, C.c_int32) for n in ("min_seed_hits", "max_row_gap", "min_track_hits", "nf_z_projection")]
 
 
 class _Out(C.Structure):
@@ -84,6 +84,7 @@ class OracleParams:
     min_seed_hits: int = 5
     max_row_gap: int = 4
     min_track_hits: int = 10
+    nf_z_projection: int = 1   # SPEC 11: 0 in time-frame mode
 
     def _c(self) -> _Params:
         return _Params(**{n: getattr(self, n) for n, _ in _Params._fields_})
@@ -258,7 +259,7 @@ class MergeResult:
 
 
 def merge_refit(geometry, y, z, row_offsets, n_tasks: int, tracks, params: Optional[OracleParams] = None,
-                chi2_max: float = 50.0, max_row_gap: int = 8, precision: str = "f32") -> MergeResult:
+                chi2_max: float = 50.0, max_row_gap: int = 8, precision: str = "f32", n_slices: int = 1) -> MergeResult:
     """SPEC 9 on the tracks of ``track()`` (any object with track_task, track_hit_begin, track_nhits, track_x,
     track_par [5,n], track_cov [15,n], hit_cluster); the tracks may be given in any order."""
     lib = _load()
@@ -294,7 +295,7 @@ def merge_refit(geometry, y, z, row_offsets, n_tasks: int, tracks, params: Optio
                    _ptr(m_ndf), _ptr(m_x), _ptr(m_par), _ptr(m_cov), _ptr(m_chi2), 0, 0)
     fn = lib.oracle_merge_f32 if precision == "f32" else lib.oracle_merge_f64
     rc = fn(C.byref(g), C.c_float(float(geometry.bz_kgauss)), C.byref(prm._c()), C.c_float(chi2_max),
-            C.c_int32(max_row_gap), C.c_uint32(n), C.c_uint32(n_tasks), _ptr(y), _ptr(z), _ptr(ro),
+            C.c_int32(max_row_gap), C.c_int32(n_slices), C.c_uint32(n), C.c_uint32(n_tasks), _ptr(y), _ptr(z), _ptr(ro),
             C.byref(mi), C.byref(mo))
     if rc != 0:
         raise RuntimeError(f"oracle_merge returned {rc}")

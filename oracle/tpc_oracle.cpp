@@ -50,6 +50,7 @@ struct OParams {  // SPEC 8
   float sigma_y, sigma_z, nf_hy, nf_hz, nf_chi2_max, grid_bin_min, grid_bin_max, max_sinphi, c0_sinphi,
       c0_dzds, c0_qpt, accept_k2, search_max, turn_cov_scale;
   int32_t min_seed_hits, max_row_gap, min_track_hits;
+  int32_t nf_z_projection;  // SPEC 1 T4/T5, SPEC 11: 0 in time-frame mode
 };
 
 enum Counter {
@@ -168,8 +169,8 @@ template <class R> struct Tables {
     ratio_up.assign(n, R(0)); ratio_dn.assign(n, R(0));
     for (int r = 0; r < n; ++r) X[r] = R(g.row_x[r]);
     for (int r = 0; r < n; ++r) ymax[r] = X[r] * R(g.tan_half_angle) + R(1);           // T1
-    for (int r = 0; r + 1 < n; ++r) { dx_up[r] = X[r + 1] - X[r]; ratio_up[r] = X[r + 1] / X[r]; }  // T2 T4
-    for (int r = 1; r < n; ++r) { dx_dn[r] = X[r] - X[r - 1]; ratio_dn[r] = X[r - 1] / X[r]; }      // T3 T5
+    for (int r = 0; r + 1 < n; ++r) { dx_up[r] = X[r + 1] - X[r]; ratio_up[r] = p.nf_z_projection ? X[r + 1] / X[r] : R(1); }  // T2 T4
+    for (int r = 1; r < n; ++r) { dx_dn[r] = X[r] - X[r - 1]; ratio_dn[r] = p.nf_z_projection ? X[r - 1] / X[r] : R(1); }      // T3 T5
     a = R(-0.000299792458f) * R(bz);                                                     // T6
     sy2 = R(p.sigma_y) * R(p.sigma_y); sz2 = R(p.sigma_z) * R(p.sigma_z);               // T7
     wy = R(1) / sy2; wz = R(1) / sz2;
@@ -600,8 +601,8 @@ struct OMergeOut {  // caller-allocated
 };
 
 template <class R>
-int merge_refit(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
-                uint32_t nt, const R* Y, const R* Z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
+int merge_refit(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, int32_t n_slices,
+                uint32_t n, uint32_t nt, const R* Y, const R* Z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
   Tables<R> T(*g, bz, *p);
   MergeTables<R> MT(g->n_sectors);
   const int nr = T.n_rows, ns = g->n_sectors;
@@ -634,16 +635,23 @@ int merge_refit(const OGeometry* g, float bz, const OParams* p, float chi2_max, 
   std::vector<R> chi_out(nT, R(0)), chi_in(nT, R(0));
   for (uint32_t i = 0; i < nT; ++i) {
     if (!has_outer[i]) continue;
-    const int si = (int)(in->track_task[i] % ns), ei = (int)(in->track_task[i] / ns);
+    // task = (frame*n_slices + slice)*n_sectors + sector (SPEC 11; n_slices = 1: frame = event)
+    const int si = (int)(in->track_task[i] % ns), li = (int)((in->track_task[i] / ns) % n_slices),
+              fi = (int)(in->track_task[i] / ns / n_slices);
     for (uint32_t j = 0; j < nT; ++j) {
-      if (j == i || (int)(in->track_task[j] / ns) != ei) continue;
-      const int sj = (int)(in->track_task[j] % ns);
-      int d = neighbour_dir(si, sj, MT.n_half);
-      if (d == 0) continue;
-      if (MT.n_half <= 2) d = +1;
+      if (j == i || (int)(in->track_task[j] / ns / n_slices) != fi) continue;
+      const int sj = (int)(in->track_task[j] % ns), lj = (int)((in->track_task[j] / ns) % n_slices);
+      int d = 0;
+      if (lj == li) {                                   // neighbouring sector of the same slice
+        d = neighbour_dir(si, sj, MT.n_half);
+        if (d == 0) continue;
+        if (MT.n_half <= 2) d = +1;
+      } else if (!(sj == si && (lj == li + 1 || lj == li - 1))) {
+        continue;                                       // SPEC 11: else only the same sector of a neighbouring slice
+      }
       if (!(rl[i] < rf[j] && rf[j] <= rl[i] + max_row_gap)) continue;                       // G2
       State<R> q = outer[i];                                                                // G3
-      if (!rotate(q, d, MT.ca, MT.sa, T.a, R(p->max_sinphi))) continue;
+      if (d != 0 && !rotate(q, d, MT.ca, MT.sa, T.a, R(p->max_sinphi))) continue;
       const State<R> sj_state = state_of(j);
       if (q.x != sj_state.x && !transport(q, sj_state.x, T.a, R(p->max_sinphi))) continue;
       R chi = R(0);                                                                         // G4
@@ -773,13 +781,15 @@ void oracle_update_f32(float* s22, int32_t* ndf, int i, float m, float e) {
 // --- SPEC 9 -------------------------------------------------------------------
 size_t oracle_sizeof_merge_in() { return sizeof(OMergeIn); }
 size_t oracle_sizeof_merge_out() { return sizeof(OMergeOut); }
-int oracle_merge_f32(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
-                     uint32_t nt, const float* y, const float* z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
-  return merge_refit<float>(g, bz, p, chi2_max, max_row_gap, n, nt, y, z, ro, in, o);
+int oracle_merge_f32(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, int32_t n_slices,
+                     uint32_t n, uint32_t nt, const float* y, const float* z, const uint32_t* ro, const OMergeIn* in,
+                     OMergeOut* o) {
+  return merge_refit<float>(g, bz, p, chi2_max, max_row_gap, n_slices > 0 ? n_slices : 1, n, nt, y, z, ro, in, o);
 }
-int oracle_merge_f64(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, uint32_t n,
-                     uint32_t nt, const double* y, const double* z, const uint32_t* ro, const OMergeIn* in, OMergeOut* o) {
-  return merge_refit<double>(g, bz, p, chi2_max, max_row_gap, n, nt, y, z, ro, in, o);
+int oracle_merge_f64(const OGeometry* g, float bz, const OParams* p, float chi2_max, int32_t max_row_gap, int32_t n_slices,
+                     uint32_t n, uint32_t nt, const double* y, const double* z, const uint32_t* ro, const OMergeIn* in,
+                     OMergeOut* o) {
+  return merge_refit<double>(g, bz, p, chi2_max, max_row_gap, n_slices > 0 ? n_slices : 1, n, nt, y, z, ro, in, o);
 }
 // ROTATE on a state laid out as x, p[5], c[15], chi2 (22 reals)
 int oracle_rotate_f64(double* s22, int d, int n_sectors, double a, double max_sinphi) {

@@ -19,3 +19,4 @@ from .events import (  # noqa: F401
     take_tasks,
 )
 from .calibration import RawCalibration, default_calibration, raw_from_yz  # noqa: F401
+from .frames import make_frame  # noqa: F401
