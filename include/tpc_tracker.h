@@ -76,6 +76,8 @@ typedef struct {
   int32_t min_seed_hits;            /* S3                                                       */
   int32_t max_row_gap;              /* K3, K5                                                   */
   int32_t min_track_hits;           /* K6, L2                                                   */
+  int32_t nf_z_projection;          /* N1: 1 = project z from the origin (events); 0 = time-frame */
+                                    /* mode (SPEC 11): z is known up to a shift only              */
 } tpc_params;
 
 /* Input clusters.  Arrays are DEVICE memory for tpc_track_batch and HOST
@@ -247,6 +249,8 @@ const char* tpc_stage_name(int stage);
 typedef struct {
   float merge_chi2_max;      /* G4: match iff chi2 < this (default 50)                         */
   int32_t merge_max_row_gap; /* G2: first row of the outer segment at most this far (default 8) */
+  int32_t n_slices;          /* SPEC 11: task = (frame*n_slices + slice)*n_sectors + sector; segments of the
+                              * same sector in neighbouring slices are joined too (default 1: events)    */
 } tpc_merge_params;
 void tpc_default_merge_params(tpc_merge_params* out);
 

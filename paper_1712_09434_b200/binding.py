@@ -33,7 +33,7 @@ class _Geometry(C.Structure):
 
 _PARAM_FLOATS = ("sigma_y", "sigma_z", "nf_hy", "nf_hz", "nf_chi2_max", "grid_bin_min", "grid_bin_max", "max_sinphi",
                  "c0_sinphi", "c0_dzds", "c0_qpt", "accept_k2", "search_max", "turn_cov_scale")
-_PARAM_INTS = ("min_seed_hits", "max_row_gap", "min_track_hits")
+_PARAM_INTS = ("min_seed_hits", "max_row_gap", "min_track_hits", "nf_z_projection")
 
 
 class _Params(C.Structure):
@@ -77,6 +77,7 @@ class TrackerParams:
     min_seed_hits: Optional[int] = None
     max_row_gap: Optional[int] = None
     min_track_hits: Optional[int] = None
+    nf_z_projection: Optional[int] = None
 
 
 def library_path() -> str:
@@ -162,7 +163,7 @@ class _Calibration(C.Structure):
 
 
 class _MergeParams(C.Structure):
-    _fields_ = [("merge_chi2_max", C.c_float), ("merge_max_row_gap", C.c_int32)]
+    _fields_ = [("merge_chi2_max", C.c_float), ("merge_max_row_gap", C.c_int32), ("n_slices", C.c_int32)]
 
 
 class _Merged(C.Structure):
@@ -426,7 +427,7 @@ class Tracker:
 
     def merge_refit(self, y, z, row_offsets, n_tasks: int, tracks: TrackResult, merged: "MergedResult", workspace,
                     merge_workspace, max_tracklets: int = 0, chi2_max: Optional[float] = None,
-                    max_row_gap: Optional[int] = None, stream=None) -> "MergedResult":
+                    max_row_gap: Optional[int] = None, n_slices: int = 1, stream=None) -> "MergedResult":
         """tpc_merge_refit right after track_batch with the same tensors and workspace. Asynchronous."""
         import torch
         cl = _Clusters(None, y.data_ptr(), z.data_ptr(), None, row_offsets.data_ptr(), int(y.numel()), int(n_tasks))
@@ -437,6 +438,7 @@ class Tracker:
             mp.merge_chi2_max = chi2_max
         if max_row_gap is not None:
             mp.merge_max_row_gap = max_row_gap
+        mp.n_slices = int(n_slices)
         mg = _Merged()
         mg.capacity = int(merged.seg_next.shape[0])
         for n, _ in _Merged._fields_[1:]:

@@ -87,6 +87,7 @@ struct MergeCtx {
   float chi2_max;
   int32_t max_row_gap;
   int32_t n_half;             // sectors per side
+  int32_t n_slices;           // SPEC 11: slices per frame (1: events)
   float ca, sa;               // cos, sin of the sector pitch (SPEC 9 tables)
   // merge workspace (device)
   float4* ends;               // [cap][6]   G1
@@ -148,10 +149,11 @@ __global__ void __launch_bounds__(kMergeThreads) k_merge_row_fill(const Ctx c, c
   m.row_list[m.row_start[b] + atomicAdd(&m.row_fill[b], 1u)] = i;
 }
 
-// G3, G4 for the pair (inner i -> outer j) in direction d; Q = outer end of i at X[rl_i].  Returns chi or +inf.
+// G3, G4 for the pair (inner i -> outer j) in direction d (0: same sector, neighbouring slice - no ROTATE);
+// Q = outer end of i at X[rl_i].  Returns chi or +inf.
 __device__ __forceinline__ float merge_chi(const Ctx& c, const MergeCtx& m, TrackState Q, float xq, int d, uint32_t j) {
   const float kInf = __int_as_float(0x7f800000);
-  if (!rotate_state(Q, xq, m.ca, d > 0 ? m.sa : -m.sa, c.a, c.prm.max_sinphi)) return kInf;
+  if (d != 0 && !rotate_state(Q, xq, m.ca, d > 0 ? m.sa : -m.sa, c.a, c.prm.max_sinphi)) return kInf;
   TrackState B;
   float xb;
   load_track_state(c.out, j, B, xb);
@@ -171,10 +173,10 @@ __device__ __forceinline__ float merge_chi(const Ctx& c, const MergeCtx& m, Trac
 // so its bits order like its value; the minimum does not depend on the order of the atomics).
 __global__ void __launch_bounds__(kMergeThreads) k_merge_match(const Ctx c, const MergeCtx m) {
   const uint32_t n_trk = merge_n_tracks(c, m);
-  const int nh = m.n_half;
+  const int nh = m.n_half, n_sl = m.n_slices;
   const int n_dir = nh >= 3 ? 2 : (nh == 2 ? 1 : 0);
   const uint32_t t = blockIdx.x * kMergeThreads + threadIdx.x;
-  if (n_dir == 0 || t >= n_trk) return;
+  if ((n_dir == 0 && n_sl < 2) || t >= n_trk) return;
   const int ns = c.n_sectors, n_rows = c.n_rows;
   const int rl_t = (int)(c.out_rows[t] >> 16);
   if (rl_t + 1 >= n_rows) return;                                                   // nothing starts above the last row
@@ -182,14 +184,26 @@ __global__ void __launch_bounds__(kMergeThreads) k_merge_match(const Ctx c, cons
   if (!load_end(m.ends + (size_t)t * 6, E)) return;
   const uint32_t task = c.out.track_task[t];
   const int sec = (int)(task % (uint32_t)ns), side = sec / nh, f = sec - side * nh;
+  const uint32_t slice = (task / (uint32_t)ns) % (uint32_t)n_sl;                    // SPEC 11
   const uint32_t g_t = c.out.hit_cluster[c.out.track_hit_begin[t]];
   const float x_end = c.X[rl_t];
   int32_t best = -1;
   float chi_best = 0.0f;
   uint32_t gid_best = 0u;
-  for (int k = 0; k < n_dir; ++k) {
-    const int d = k == 0 ? +1 : -1;
-    const uint32_t tj = task - (uint32_t)sec + (uint32_t)(side * nh + (f + d + nh) % nh);
+  // candidate tasks: the neighbouring sectors of the same slice (d = +1, -1), the same sector of the neighbouring
+  // slices (d = 0)
+  for (int k = 0; k < 4; ++k) {
+    int d;
+    uint32_t tj;
+    if (k < 2) {
+      if (k >= n_dir) continue;
+      d = k == 0 ? +1 : -1;
+      tj = task - (uint32_t)sec + (uint32_t)(side * nh + (f + d + nh) % nh);
+    } else {
+      d = 0;
+      if (k == 2) { if (slice + 1u >= (uint32_t)n_sl) continue; tj = task + (uint32_t)ns; }
+      else { if (slice == 0u) continue; tj = task - (uint32_t)ns; }
+    }
     const uint32_t b0 = tj * (uint32_t)n_rows + (uint32_t)(rl_t + 1);               // G2: rl_i < rf_j <= rl_i + gap
     const uint32_t b1 = tj * (uint32_t)n_rows + (uint32_t)min(rl_t + m.max_row_gap, n_rows - 1) + 1u;
     for (uint32_t q = m.row_start[b0], qe = m.row_start[b1]; q < qe; ++q) {

@@ -140,6 +140,7 @@ void default_params(tpc_params* p) {  // SPEC 8
   p->accept_k2 = 16.0f; p->search_max = 3.0f;
   p->turn_cov_scale = 100.0f;
   p->min_seed_hits = 5; p->max_row_gap = 4; p->min_track_hits = 10;
+  p->nf_z_projection = 1;
 }
 
 Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out, char* ws, const Carve& cv,
@@ -212,8 +213,9 @@ int tpc_tracker_create(const tpc_geometry* g, float bz_kgauss, const tpc_params*
         *ratio_dn = X + 5 * n;
   for (int r = 0; r < n; ++r) X[r] = g->row_x[r];
   for (int r = 0; r < n; ++r) ymax[r] = X[r] * g->tan_half_angle + 1.0f;                    // T1
-  for (int r = 0; r + 1 < n; ++r) { dx_up[r] = X[r + 1] - X[r]; ratio_up[r] = X[r + 1] / X[r]; }  // T2 T4
-  for (int r = 1; r < n; ++r) { dx_dn[r] = X[r] - X[r - 1]; ratio_dn[r] = X[r - 1] / X[r]; }      // T3 T5
+  const bool proj = p.nf_z_projection != 0;  // SPEC 11: no projection of z in time-frame mode
+  for (int r = 0; r + 1 < n; ++r) { dx_up[r] = X[r + 1] - X[r]; ratio_up[r] = proj ? X[r + 1] / X[r] : 1.0f; }  // T2 T4
+  for (int r = 1; r < n; ++r) { dx_dn[r] = X[r] - X[r - 1]; ratio_dn[r] = proj ? X[r - 1] / X[r] : 1.0f; }      // T3 T5
   t->a = -0.000299792458f * bz_kgauss;                                                       // T6
   t->sy2 = p.sigma_y * p.sigma_y; t->sz2 = p.sigma_z * p.sigma_z;                            // T7
   t->wy = 1.0f / t->sy2; t->wz = 1.0f / t->sz2;
@@ -873,7 +875,7 @@ __global__ void k_merge_guard(const Ctx c, const MergeCtx m) {  // the tracker's
 }  // namespace
 
 void tpc_default_merge_params(tpc_merge_params* out) {
-  if (out) { out->merge_chi2_max = 50.0f; out->merge_max_row_gap = 8; }
+  if (out) { out->merge_chi2_max = 50.0f; out->merge_max_row_gap = 8; out->n_slices = 1; }
 }
 
 size_t tpc_merge_workspace_bytes(const tpc_tracker* t, uint32_t track_capacity, uint32_t max_tasks) {
@@ -895,8 +897,8 @@ int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tr
     return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: tracks must be the complete output of tpc_track_batch");
   tpc_merge_params mp;
   if (params) mp = *params; else tpc_default_merge_params(&mp);
-  if (!(mp.merge_chi2_max >= 0.f) || mp.merge_max_row_gap < 0)
-    return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: need merge_chi2_max >= 0 and merge_max_row_gap >= 0");
+  if (!(mp.merge_chi2_max >= 0.f) || mp.merge_max_row_gap < 0 || mp.n_slices < 1)
+    return fail(t, TPC_ERR_ARGUMENT, "tpc_merge_refit: need merge_chi2_max >= 0, merge_max_row_gap >= 0, n_slices >= 1");
   const uint32_t T = resolve_max_tracklets(t, in->n_clusters, max_tracklets);
   const Carve cv = carve((uint32_t)t->n_rows, in->n_clusters, in->n_tasks, T);
   if (!workspace || workspace_bytes < cv.total)
@@ -912,7 +914,7 @@ int tpc_merge_refit(tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* tr
   char* mw = (char*)merge_workspace;
   MergeCtx m{};
   m.out = *merged;
-  m.chi2_max = mp.merge_chi2_max; m.max_row_gap = mp.merge_max_row_gap;
+  m.chi2_max = mp.merge_chi2_max; m.max_row_gap = mp.merge_max_row_gap; m.n_slices = mp.n_slices;
   m.n_half = t->n_half; m.ca = t->merge_ca; m.sa = t->merge_sa;
   m.ends = (float4*)(mw + mc.ends);
   m.row_cnt = (uint32_t*)(mw + mc.row_cnt); m.row_start = (uint32_t*)(mw + mc.row_start);

@@ -13,7 +13,7 @@ from tpc_workload import generate_config
 pytestmark = pytest.mark.gpu
 
 
-def run_gpu_merge(batch, chi2_max=None, max_row_gap=None, params_over=None):
+def run_gpu_merge(batch, chi2_max=None, max_row_gap=None, params_over=None, n_slices=1):
     import torch
     from paper_1712_09434_b200 import Tracker
     dev = torch.device("cuda:0")
@@ -29,7 +29,8 @@ def run_gpu_merge(batch, chi2_max=None, max_row_gap=None, params_over=None):
         merged = trk.alloc_merged(tcap, dev)
         mws = trk.alloc_workspace(trk.merge_workspace_bytes(tcap, batch.n_tasks), dev)
         trk.track_batch(y, z, ro, batch.n_tasks, out, ws)
-        trk.merge_refit(y, z, ro, batch.n_tasks, out, merged, ws, mws, chi2_max=chi2_max, max_row_gap=max_row_gap)
+        trk.merge_refit(y, z, ro, batch.n_tasks, out, merged, ws, mws, chi2_max=chi2_max, max_row_gap=max_row_gap,
+                        n_slices=n_slices)
         torch.cuda.synchronize()
         g = out.to_numpy()
         g.update(merged.to_numpy(g["n_tracks"]))
@@ -115,3 +116,31 @@ def test_merge_refit_single_sector_and_empty():
     e, _ = take_tasks(generate_config(1), [])   # every task empty
     ge = run_gpu_merge(e)
     assert ge["n_tracks"] == 0 and ge["n_merged"] == 0 and ge["n_links"] == 0
+
+
+def test_time_frame_mode_matches_the_oracle():
+    """SPEC 11: six overlapping peripheral events in one frame of four slices (144 slice-sector tasks), tracker with
+    nf_z_projection = 0, merger across sectors AND slices: tracks, links and refit identical to the oracle's; and a
+    second frame in the same call (frames never mix)."""
+    from tpc_workload import default_geometry, generate_event, make_frame, concat_batches, CONFIGS
+    geom = default_geometry()
+    spec = CONFIGS[1]["spec"]
+    frames = []
+    for f in range(2):
+        evs = [generate_event(geom, spec, 400 + 10 * f + i) for i in range(6)]
+        shifts = np.sort(np.random.default_rng(5 + f).uniform(0, 750, 6))
+        frames.append(make_frame(evs, shifts, 250.0, 4, seed=9 + f))
+    b = concat_batches(frames)
+    over = dict(nf_z_projection=0, nf_hz=2.5)
+    prm = G.oracle_params_for(b, **over)
+    ref = oracle.track(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, params=prm)
+    mref = oracle.merge_refit(b.geometry, b.y, b.z, b.row_offsets, b.n_tasks, ref, params=prm, n_slices=4)
+    g = run_gpu_merge(b, params_over=over, n_slices=4)
+    G.compare(g, ref, b.geometry.n_rows, check_tracklets=False)
+    dev = compare_merge(g, ref, mref)
+    ns = geom.n_sectors
+    i = np.nonzero(g["seg_next"] >= 0)[0]
+    ti, tj = g["track_task"][i].astype(np.int64), g["track_task"][g["seg_next"][i]].astype(np.int64)
+    assert np.all(ti // (4 * ns) == tj // (4 * ns))           # same frame
+    assert np.sum(ti // ns != tj // ns) > 300                 # links across slices exist
+    print(f"frames: {ref.n_tracks} tracks, {mref.n_links} links, {len(mref.merged_first)} merged; {dev}")
