@@ -149,3 +149,33 @@ def test_frame_of_overlapping_events_links_only_neighbours_and_the_same_track():
     # n_slices = 1 on the same tracks: no link may cross a slice, so there are fewer
     m1 = oracle.merge_refit(fr.geometry, fr.y, fr.z, fr.row_offsets, fr.n_tasks, res, params=prm, n_slices=1)
     assert m1.n_links < m.n_links
+
+
+def test_slicer_hand_built_and_properties():
+    """SLICE: a hand-built frame (2 sectors, 3 rows, slices of 100 cm) and the properties on a generated one."""
+    from oracle.frames import slice_frames
+    # sector 0 row 0: zeta 10, 250, 99.9, 100 ; sector 0 row 2: 5 ; sector 1 row 1: -120, -20, -350 (C-side sign)
+    y = np.arange(8, dtype=np.float32)
+    z = np.array([10, 250, 99.9, 100, 5, -120, -20, -350], np.float32)
+    ro = np.array([0, 4, 4, 5, 5, 8, 8], np.uint32)
+    yo, zo, src, ro_out = slice_frames(y, z, ro, 2, 2, 3, 100.0, 3)
+    # slices: 0,2,0,1 | 0 | 1,0,2(clipped from 3)   -> output order (slice, sector, row, input order)
+    assert src.tolist() == [0, 2, 4, 6, 3, 5, 1, 7]
+    assert np.array_equal(yo, y[src]) and np.array_equal(zo, z[src])
+    want_counts = {(0, 0, 0): 2, (0, 0, 2): 1, (0, 1, 1): 1, (1, 0, 0): 1, (1, 1, 1): 1, (2, 0, 0): 1, (2, 1, 1): 1}
+    for sl in range(3):
+        for sec in range(2):
+            for r in range(3):
+                k = (sl * 2 + sec) * 3 + r
+                assert ro_out[k + 1] - ro_out[k] == want_counts.get((sl, sec, r), 0)
+    # a generated frame: permutation, stability inside a row, every cluster in the slice of its zeta
+    spec = CONFIGS[1]["spec"]
+    evs = [generate_event(GEOM, spec, 500 + i) for i in range(3)]
+    fr = make_frame(evs, [0.0, 200.0, 420.0], 1000.0, 1, seed=3)           # one slice = not yet sliced
+    yo, zo, src, ro_out = slice_frames(fr.y, fr.z, fr.row_offsets, 36, 36, 159, 250.0, 4)
+    assert np.array_equal(np.sort(src), np.arange(fr.n_clusters))
+    tr_out = np.repeat(np.arange(len(ro_out) - 1), np.diff(ro_out.astype(np.int64)))
+    sl = tr_out // 159 // 36
+    assert np.all(sl == np.minimum((np.abs(zo) * (np.float32(1) / np.float32(250.0))).astype(np.int64), 3))
+    same_row = tr_out[1:] == tr_out[:-1]
+    assert np.all(src[1:][same_row] > src[:-1][same_row])
