@@ -309,6 +309,24 @@ int tpc_transform_clusters(tpc_transform* transform, const float* pad, const flo
                            uint32_t n_clusters, uint32_t n_tasks, float* y, float* z, void* cuda_stream);
 const char* tpc_transform_last_error(const tpc_transform* transform);
 
+/* ---- time frames ---------------------------------------------------------
+ * continuous read-out gives "time frames with many overlapping events"; "One solution
+ * is to slice the time frames along the time / beam axis, process the slices individually, and merge the
+ * track segments afterwards".  docs/ARITH_SPEC.md section 11.  In a frame z is the frame coordinate zeta
+ * (known up to the shift of the event), so the tracker is created with tpc_params.nf_z_projection = 0;
+ * tpc_slice_frames re-sorts the clusters of whole frames - sorted by (frame, sector, row) - by
+ * (frame, slice, sector, row), slice = min((int)(|zeta| / slice_len), n_slices - 1), stable inside a row;
+ * tpc_track_batch then runs on n_tasks_in * n_slices tasks (any run of them per call), and
+ * tpc_merge_refit with tpc_merge_params.n_slices joins the segments across sectors and slices.
+ * src_index[k] = input index of output cluster k (the identity of a cluster, L213).
+ * All arrays DEVICE memory; y_out, z_out, src_index: [n_clusters]; row_offsets_out:
+ * [n_tasks_in*n_slices*n_rows + 1]; workspace: tpc_slice_workspace_bytes(...) bytes.  Asynchronous. */
+size_t tpc_slice_workspace_bytes(uint32_t n_tasks_in, int32_t n_rows, int32_t n_slices);
+int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offsets_in, uint32_t n_clusters,
+                     uint32_t n_tasks_in, int32_t n_sectors, int32_t n_rows, float slice_len, int32_t n_slices,
+                     float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out, void* workspace,
+                     size_t workspace_bytes, void* cuda_stream);
+
 /* Text of the last error on this tracker (never NULL). With tracker == NULL: the
  * last error of tpc_tracker_create on this thread. */
 const char* tpc_last_error(const tpc_tracker* tracker);

@@ -137,6 +137,11 @@ def load_library():
     lib.tpc_host_submit.argtypes = [vp, C.c_int, C.POINTER(_Clusters), C.c_uint32, C.c_uint32, vp, C.c_size_t, C.c_uint32]
     lib.tpc_host_collect.restype = C.c_int
     lib.tpc_host_collect.argtypes = [vp, C.c_int, C.POINTER(_Tracks), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.tpc_slice_workspace_bytes.restype = C.c_size_t
+    lib.tpc_slice_workspace_bytes.argtypes = [C.c_uint32, C.c_int32, C.c_int32]
+    lib.tpc_slice_frames.restype = C.c_int
+    lib.tpc_slice_frames.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, C.c_int32, C.c_int32, C.c_float, C.c_int32,
+                                     vp, vp, vp, vp, vp, C.c_size_t, vp]
     lib.tpc_transform_create.restype = C.c_int
     lib.tpc_transform_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Calibration), C.POINTER(vp)]
     lib.tpc_transform_destroy.restype = None
@@ -449,6 +454,32 @@ class Tracker:
         self._check(self._lib.tpc_merge_refit(self._h, C.byref(cl), C.byref(tr), C.byref(mp), C.byref(mg), wp, wn,
                                               int(max_tracklets), mwp, mwn, _stream_ptr(s)), "tpc_merge_refit")
         return merged
+
+
+def slice_frames(y, zeta, row_offsets, n_tasks_in: int, n_sectors: int, n_rows: int, slice_len: float, n_slices: int,
+                 stream=None):
+    """tpc_slice_frames on DEVICE tensors; returns (y_out, z_out, src_index, row_offsets_out) device tensors
+    (int32 views of the uint32 arrays).  Asynchronous."""
+    import torch
+    lib = load_library()
+    if not (y.is_cuda and zeta.is_cuda and row_offsets.is_cuda):
+        raise TpcError("slice_frames needs CUDA tensors; there is no CPU path")
+    dev = y.device
+    n = int(y.numel())
+    y_out, z_out = torch.empty_like(y), torch.empty_like(zeta)
+    src = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    ro_out = torch.empty(n_tasks_in * n_slices * n_rows + 1, dtype=torch.int32, device=dev)
+    wb = int(lib.tpc_slice_workspace_bytes(n_tasks_in, n_rows, n_slices))
+    ws = torch.empty(wb + 256, dtype=torch.uint8, device=dev)
+    wp = ws.data_ptr() + (-ws.data_ptr()) % 256
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    rc = lib.tpc_slice_frames(y.data_ptr(), zeta.data_ptr(), row_offsets.data_ptr(), n, int(n_tasks_in), int(n_sectors),
+                              int(n_rows), float(slice_len), int(n_slices), y_out.data_ptr(), z_out.data_ptr(),
+                              src.data_ptr(), ro_out.data_ptr(), wp, wb, _stream_ptr(s))
+    if rc != 0:
+        raise TpcError(f"tpc_slice_frames failed ({rc}): {lib.tpc_last_error(None).decode()}")
+    slice_frames._keep = ws  # the workspace must outlive the asynchronous kernels
+    return y_out, z_out, src[:n], ro_out
 
 
 class ClusterTransform:

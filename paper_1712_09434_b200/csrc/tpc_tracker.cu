@@ -20,6 +20,7 @@
 #include "stage_merge.cuh"
 #include "stage_neighbours.cuh"
 #include "stage_output.cuh"
+#include "stage_slice.cuh"
 #include "stage_tracklet.cuh"
 #include "stage_transform.cuh"
 #include "stages_ca.cuh"
@@ -1011,6 +1012,40 @@ int tpc_transform_clusters(tpc_transform* t, const float* pad, const float* time
 }
 
 const char* tpc_transform_last_error(const tpc_transform* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
+
+// ---- frame slicer (SPEC 11, SLICE) ------------------------------------------------------------------
+size_t tpc_slice_workspace_bytes(uint32_t n_tasks_in, int32_t n_rows, int32_t n_slices) {
+  if (n_rows < 1 || n_slices < 1) return 0;
+  return align_up(((size_t)n_tasks_in * (size_t)n_rows * (size_t)n_slices + 2) * sizeof(uint32_t));
+}
+
+int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offsets_in, uint32_t n_clusters,
+                     uint32_t n_tasks_in, int32_t n_sectors, int32_t n_rows, float slice_len, int32_t n_slices,
+                     float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out, void* workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  if (!row_offsets_in || !row_offsets_out || !workspace || (n_clusters && (!y || !zeta || !y_out || !z_out || !src_index)))
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_frames: NULL argument");
+  if (n_sectors < 1 || n_rows < 1 || n_slices < 1 || n_slices > kMaxSlices || !(slice_len > 0.f) || n_tasks_in % (uint32_t)n_sectors != 0u)
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_frames: need n_sectors, n_rows >= 1, 1 <= n_slices <= %d, slice_len > 0, whole frames", kMaxSlices);
+  if ((uint64_t)n_tasks_in * (uint64_t)n_rows * (uint64_t)n_slices >= 0x7FFFFFFFull)
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_frames: n_tasks_in*n_rows*n_slices must be < 2^31");
+  if (workspace_bytes < tpc_slice_workspace_bytes(n_tasks_in, n_rows, n_slices))
+    return fail(nullptr, TPC_ERR_WORKSPACE, "tpc_slice_frames: workspace too small");
+  SliceCtx c{};
+  c.y = y; c.z = zeta; c.row_off_in = row_offsets_in; c.n = n_clusters; c.n_tr_in = n_tasks_in * (uint32_t)n_rows;
+  c.n_sectors = n_sectors; c.n_rows = n_rows; c.n_slices = n_slices;
+  c.inv_len = 1.0f / slice_len;
+  c.y_out = y_out; c.z_out = z_out; c.src_index = src_index; c.row_off_out = row_offsets_out;
+  c.counts = (uint32_t*)workspace;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const unsigned blocks = (c.n_tr_in + kSliceThreads / 32 - 1) / (kSliceThreads / 32);
+  if (blocks) k_slice_count<<<blocks, kSliceThreads, 0, s>>>(c);
+  k_slice_scan<<<1, 1024, 0, s>>>(c);
+  if (blocks) k_slice_scatter<<<blocks, kSliceThreads, 0, s>>>(c);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, TPC_ERR_CUDA, "tpc_slice_frames: CUDA launch: %s", cudaGetErrorString(e));
+  return TPC_OK;
+}
 
 const char* tpc_last_error(const tpc_tracker* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
 

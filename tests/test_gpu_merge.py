@@ -144,3 +144,56 @@ def test_time_frame_mode_matches_the_oracle():
     assert np.all(ti // (4 * ns) == tj // (4 * ns))           # same frame
     assert np.sum(ti // ns != tj // ns) > 300                 # links across slices exist
     print(f"frames: {ref.n_tracks} tracks, {mref.n_links} links, {len(mref.merged_first)} merged; {dev}")
+
+
+def test_frame_slicer_matches_the_oracle_and_feeds_the_tracker():
+    """SLICE: a frame given unsliced (sorted by (sector,row)) is sliced on the device exactly as oracle/frames.py does
+    (arrays, source indices, row offsets identical); tracker + merger on the device's slices equal the oracle's on
+    the oracle's slices; the source indices give the clusters of a track back in the unsliced numbering."""
+    import torch
+    from oracle.frames import slice_frames as oracle_slice
+    from paper_1712_09434_b200 import slice_frames, Tracker
+    from tpc_workload import default_geometry, generate_event, make_frame, CONFIGS
+    import dataclasses
+    geom = default_geometry()
+    evs = [generate_event(geom, CONFIGS[1]["spec"], 600 + i) for i in range(5)]
+    whole = make_frame(evs, [0.0, 130.0, 377.0, 512.0, 740.0], 1000.0, 1, seed=2)   # one slice = not yet sliced
+    ns, nr, n_sl = geom.n_sectors, geom.n_rows, 4
+    yo, zo, so, roo = oracle_slice(whole.y, whole.z, whole.row_offsets, ns, ns, nr, 250.0, n_sl)
+    dev = torch.device("cuda:0")
+    y = torch.from_numpy(whole.y).to(dev); z = torch.from_numpy(whole.z).to(dev)
+    ro = torch.from_numpy(whole.row_offsets.astype(np.uint32).view(np.int32)).to(dev)
+    yg, zg, sg, rog = slice_frames(y, z, ro, ns, ns, nr, 250.0, n_sl)
+    torch.cuda.synchronize()
+    assert np.array_equal(yg.cpu().numpy(), yo) and np.array_equal(zg.cpu().numpy(), zo)
+    assert np.array_equal(sg.cpu().numpy().view(np.uint32), so)
+    assert np.array_equal(rog.cpu().numpy().view(np.uint32), roo)
+    sliced = dataclasses.replace(whole, y=yo, z=zo, row_offsets=roo, n_tasks=ns * n_sl, x=whole.x[so],
+                                 charge=whole.charge[so], truth_track=whole.truth_track[so],
+                                 truth_leg=whole.truth_leg[so], truth_state=whole.truth_state[so])
+    over = dict(nf_z_projection=0, nf_hz=2.5)
+    prm = G.oracle_params_for(sliced, **over)
+    ref = oracle.track(sliced.geometry, yo, zo, roo, ns * n_sl, params=prm)
+    mref = oracle.merge_refit(sliced.geometry, yo, zo, roo, ns * n_sl, ref, params=prm, n_slices=n_sl)
+    trk = Tracker(sliced.geometry, G.tracker_params_for(sliced, **over))
+    try:
+        n = whole.n_clusters
+        out = trk.alloc_outputs(n, dev)
+        ws = trk.alloc_workspace(trk.workspace_bytes(n, ns * n_sl), dev)
+        tcap = int(out.track_task.shape[0])
+        merged = trk.alloc_merged(tcap, dev)
+        mws = trk.alloc_workspace(trk.merge_workspace_bytes(tcap, ns * n_sl), dev)
+        trk.track_batch(yg, zg, rog, ns * n_sl, out, ws)
+        trk.merge_refit(yg, zg, rog, ns * n_sl, out, merged, ws, mws, n_slices=n_sl)
+        torch.cuda.synchronize()
+        g = out.to_numpy()
+        g.update(merged.to_numpy(g["n_tracks"]))
+    finally:
+        trk.close()
+    G.compare(g, ref, nr, check_tracklets=False)
+    compare_merge(g, ref, mref)
+    orig = so[g["hit_cluster"].astype(np.int64)]                      # hits in the numbering of the unsliced frame
+    assert np.array_equal(whole.y[orig], yo[g["hit_cluster"].astype(np.int64)])
+    empty = slice_frames(y[:0], z[:0], torch.zeros(ns * nr + 1, dtype=torch.int32, device=dev), ns, ns, nr, 250.0, n_sl)
+    torch.cuda.synchronize()
+    assert empty[0].numel() == 0 and int(empty[3].abs().sum()) == 0
