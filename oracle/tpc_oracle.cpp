@@ -716,6 +716,162 @@ int merge_refit(const OGeometry* g, float bz, const OParams* p, float chi2_max, 
   return status;
 }
 
+// ===========================================================================
+// SPEC 12: ITS standalone tracker, step by step: V1..V5 tracklets, W1..W4 seed, O1..O4
+// outward pass, N1..N3 inward pass.  Every search is the plain loop over all clusters of the layer (the definition).
+// ===========================================================================
+struct OItsGeometry { float R[6], sig_rphi[6], sig_z[6], xx0[6]; };
+struct OItsParams {
+  float max_sinphi_pair, max_dtan, sig_sinphi, sig_tan, sig_vtx_xy, sig_vtx_z, chi2_max, max_dx;
+  float c0_sinphi, c0_dzds, c0_qpt, turn_cov_scale, max_sinphi;
+  int32_t min_clusters;
+};
+struct OItsOut {  // caller-allocated, capacity tracks
+  uint32_t capacity;
+  uint32_t* event;
+  int32_t* cluster;     // [cap][6] gid or -1
+  uint32_t* n_clusters;
+  void *frame;          // R [cap][2] ca, sa
+  void *out_state, *in_state;  // R [cap][22]: x, p[5], c[15], chi2
+  int32_t *out_ndf, *in_ndf;
+  uint32_t n_tracklets, n_tracks;
+};
+
+template <class R>
+int its_track(const OItsGeometry* g, float bz, const OItsParams* p, uint32_t n_events, const R* X, const R* Y,
+              const R* Z, const uint32_t* lo, const R* vtx, OItsOut* o) {
+  const R a = R(-0.000299792458f) * R(bz);                                                   // T6
+  const R wphi = R(1) / (R(p->sig_sinphi) * R(p->sig_sinphi)), wtan = R(1) / (R(p->sig_tan) * R(p->sig_tan));
+  R ms2[6], sr2[6], sz2[6];
+  for (int l = 0; l < 6; ++l) {
+    ms2[l] = (R(0.0136f) * R(0.0136f)) * R(g->xx0[l]);
+    sr2[l] = R(g->sig_rphi[l]) * R(g->sig_rphi[l]);
+    sz2[l] = R(g->sig_z[l]) * R(g->sig_z[l]);
+  }
+  const R svxy2 = R(p->sig_vtx_xy) * R(p->sig_vtx_xy), svz2 = R(p->sig_vtx_z) * R(p->sig_vtx_z);
+  uint32_t n_trk = 0, n_tl = 0;
+  int status = 0;
+  for (uint32_t e = 0; e < n_events; ++e) {
+    const R vx = vtx[3 * e], vy = vtx[3 * e + 1], vz = vtx[3 * e + 2];
+    const uint32_t a0 = lo[6 * e], a1 = lo[6 * e + 1], b1 = lo[6 * e + 2];
+    // ---- V1..V5
+    std::vector<int64_t> best1(a1 - a0, -1), best0(b1 - a1, -1);
+    std::vector<R> m1(a1 - a0, R(0)), m0(b1 - a1, R(0));
+    for (uint32_t A = a0; A < a1; ++A) {
+      const R ax = X[A] - vx, ay = Y[A] - vy, ra = rsqrt_(ax * ax + ay * ay), ta = (Z[A] - vz) / ra;      // V1
+      for (uint32_t B = a1; B < b1; ++B) {
+        const R bx = X[B] - vx, by = Y[B] - vy, rb = rsqrt_(bx * bx + by * by), tb = (Z[B] - vz) / rb;
+        const R sd = (ax * by - ay * bx) / (ra * rb);                                                     // V2
+        const R cd = ax * bx + ay * by;
+        if (!(cd > R(0) && rabs(sd) <= R(p->max_sinphi_pair) && rabs(tb - ta) <= R(p->max_dtan))) continue;  // V3
+        const R m = (sd * sd) * wphi + ((tb - ta) * (tb - ta)) * wtan;                                     // V4
+        int64_t& b1A = best1[A - a0];                                                                     // V5
+        if (b1A < 0 || m < m1[A - a0] || (m == m1[A - a0] && B < (uint32_t)b1A)) { b1A = B; m1[A - a0] = m; }
+        int64_t& b0B = best0[B - a1];
+        if (b0B < 0 || m < m0[B - a1] || (m == m0[B - a1] && A < (uint32_t)b0B)) { b0B = A; m0[B - a1] = m; }
+      }
+    }
+    for (uint32_t A = a0; A < a1; ++A) {
+      const int64_t Bq = best1[A - a0];
+      if (Bq < 0 || best0[(uint32_t)Bq - a1] != (int64_t)A) continue;
+      const uint32_t B = (uint32_t)Bq;
+      ++n_tl;
+      // ---- W1..W4
+      const R ax = X[A] - vx, ay = Y[A] - vy, ra = rsqrt_(ax * ax + ay * ay);
+      const R bx = X[B] - vx, by = Y[B] - vy, rb = rsqrt_(bx * bx + by * by), tb = (Z[B] - vz) / rb;
+      const R ca = bx / rb, sa = by / rb;                                                                 // W1
+      auto loc_x = [&](uint32_t P) { return (X[P] - vx) * ca + (Y[P] - vy) * sa; };
+      auto loc_y = [&](uint32_t P) { return (Y[P] - vy) * ca - (X[P] - vx) * sa; };
+      const R ox = -(vx * ca + vy * sa), oy = -(vy * ca - vx * sa);
+      const R xa = loc_x(A), ya = loc_y(A), xb = rb;                                                      // W2
+      const R dab = rsqrt_((xb - xa) * (xb - xa) + ya * ya);
+      const R kap = -((R(2) * (ya * xb)) / ((ra * rb) * dab));
+      State<R> st;                                                                                        // W3
+      st.x = R(0);
+      st.p[0] = R(0); st.p[1] = vz; st.p[2] = -(R(0.5) * kap) * xb; st.p[3] = tb; st.p[4] = a != R(0) ? kap / a : R(0);
+      for (int i = 0; i < 15; ++i) st.c[i] = R(0);
+      st.c[0] = svxy2; st.c[2] = svz2; st.c[5] = R(p->c0_sinphi); st.c[9] = R(p->c0_dzds); st.c[14] = R(p->c0_qpt);
+      st.chi2 = R(0); st.ndf = -5;
+      update(st, 0, R(0), svxy2);                                                                         // W4
+      update(st, 1, vz, svz2);
+      auto scatter = [&](int l) {
+        const R th = ms2[l] * (st.p[4] * st.p[4]);
+        st.c[5] = st.c[5] + th * (R(1) - st.p[2] * st.p[2]);
+        st.c[9] = st.c[9] + th * ((R(1) + st.p[3] * st.p[3]) * (R(1) + st.p[3] * st.p[3]));
+      };
+      auto attach = [&](uint32_t P, int l) {
+        if (!transport(st, loc_x(P), a, R(p->max_sinphi))) return false;
+        update(st, 0, loc_y(P), sr2[l]);
+        update(st, 1, Z[P], sz2[l]);
+        scatter(l);
+        return true;
+      };
+      int32_t cl[6] = {(int32_t)A, (int32_t)B, -1, -1, -1, -1};
+      bool alive = attach(A, 0) && attach(B, 1);                                                          // O1
+      int n_cl = 2, miss = 0;
+      for (int l = 2; l < 6 && alive; ++l) {                                                              // O2
+        const R Rl = R(g->R[l]);
+        for (int it = 0; it < 2 && alive; ++it) {
+          const R dyo = st.p[0] - oy;
+          const R xt = ox + rsqrt_(rmax(Rl * Rl - dyo * dyo, R(0)));
+          if (it == 1 && xt == st.x) break;
+          alive = transport(st, xt, a, R(p->max_sinphi));
+        }
+        if (!alive) break;
+        const R c = rsqrt_(R(1) - st.p[2] * st.p[2]);
+        const R ey = st.c[0] + sr2[l], ez = st.c[2] + sz2[l];
+        int64_t best = -1;
+        R chi_best = R(0);
+        for (uint32_t P = lo[6 * e + l]; P < lo[6 * e + l + 1]; ++P) {
+          const R dx = loc_x(P) - st.x;
+          const R dy = loc_y(P) - (st.p[0] + dx * (st.p[2] / c));
+          const R dz = Z[P] - (st.p[1] + dx * (st.p[3] / c));
+          const R chi = (dy * dy) / ey + (dz * dz) / ez;
+          if (!(rabs(dx) <= R(p->max_dx) && chi < R(p->chi2_max))) continue;
+          if (best < 0 || chi < chi_best) { best = P; chi_best = chi; }   // ascending P: ties keep the smaller gid
+        }
+        if (best >= 0) {
+          alive = attach((uint32_t)best, l);
+          cl[l] = (int32_t)best; ++n_cl; miss = 0;
+        } else {
+          scatter(l);
+          if (++miss == 2) alive = false;
+        }
+      }
+      if (!alive || n_cl < p->min_clusters) continue;                                                     // O3
+      if (n_trk >= o->capacity) { status = 1; continue; }
+      const uint32_t t = n_trk++;
+      auto put = [&](void* dst, const State<R>& q) {
+        R* d = (R*)dst + (size_t)t * 22;
+        d[0] = q.x;
+        for (int i = 0; i < 5; ++i) d[1 + i] = q.p[i];
+        for (int i = 0; i < 15; ++i) d[6 + i] = q.c[i];
+        d[21] = q.chi2;
+      };
+      o->event[t] = e; o->n_clusters[t] = (uint32_t)n_cl;
+      for (int l = 0; l < 6; ++l) o->cluster[(size_t)t * 6 + l] = cl[l];
+      ((R*)o->frame)[2 * t] = ca; ((R*)o->frame)[2 * t + 1] = sa;
+      put(o->out_state, st); o->out_ndf[t] = st.ndf;                                                      // O4
+      for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(p->turn_cov_scale);                              // N1
+      st.chi2 = R(0); st.ndf = -5;
+      for (int l = 5; l >= 0; --l) {                                                                      // N2
+        if (cl[l] < 0) continue;
+        const uint32_t P = (uint32_t)cl[l];
+        const R xp = loc_x(P);
+        if (xp != st.x && !transport(st, xp, a, R(p->max_sinphi))) break;
+        update(st, 0, loc_y(P), sr2[l]);
+        update(st, 1, Z[P], sz2[l]);
+        scatter(l);
+      }
+      if (st.x != R(0)) transport(st, R(0), a, R(p->max_sinphi));                                         // N3
+      put(o->in_state, st); o->in_ndf[t] = st.ndf;
+    }
+  }
+  o->n_tracklets = n_tl;
+  o->n_tracks = n_trk;
+  return status;
+}
+
 }  // namespace
 
 extern "C" {
@@ -835,5 +991,16 @@ int oracle_refit_hits_f64(const OGeometry* g, float bz, const OParams* p, uint32
   for (int i = 0; i < 15; ++i) s22[6 + i] = st.c[i];
   s22[21] = st.chi2; *ndf = st.ndf; *sector_io = sec;
   return n_fit;
+}
+
+// --- SPEC 12 -------------------------------------------------------------------
+size_t oracle_sizeof_its_out() { return sizeof(OItsOut); }
+int oracle_its_f32(const OItsGeometry* g, float bz, const OItsParams* p, uint32_t n_events, const float* x, const float* y,
+                   const float* z, const uint32_t* lo, const float* vtx, OItsOut* o) {
+  return its_track<float>(g, bz, p, n_events, x, y, z, lo, vtx, o);
+}
+int oracle_its_f64(const OItsGeometry* g, float bz, const OItsParams* p, uint32_t n_events, const double* x, const double* y,
+                   const double* z, const uint32_t* lo, const double* vtx, OItsOut* o) {
+  return its_track<double>(g, bz, p, n_events, x, y, z, lo, vtx, o);
 }
 }  // extern "C"

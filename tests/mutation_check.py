@@ -19,7 +19,7 @@ from concurrent.futures import ThreadPoolExecutor
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SUITES = ["tests/test_oracle_units.py", "tests/test_oracle_tracker.py", "tests/test_oracle_following.py",
-          "tests/test_oracle_merge.py"]
+          "tests/test_oracle_merge.py", "tests/test_oracle_its.py"]
 
 # (name, SPEC tag, text in oracle/tpc_oracle.cpp, replacement)
 MUTANTS = [
@@ -145,6 +145,39 @@ MUTANTS = [
      "for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(T.prm.turn_cov_scale);                       // F1", ""),
     ("refit: no rotation at the sector change", "F2",
      "if (d == 0 || !rotate(st, d, MT.ca, MT.sa, T.a, R(T.prm.max_sinphi))) break;\n      sector = h.sector;", "sector = h.sector;"),
+    # ---- SPEC 12: ITS standalone tracker ----
+    ("ITS tracklet: opposite side accepted", "V3",
+     "if (!(cd > R(0) && rabs(sd) <= R(p->max_sinphi_pair) && rabs(tb - ta) <= R(p->max_dtan))) continue;  // V3",
+     "if (!(rabs(sd) <= R(p->max_sinphi_pair) && rabs(tb - ta) <= R(p->max_dtan))) continue;"),
+    ("ITS tracklet: angle window strict", "V3",
+     "rabs(sd) <= R(p->max_sinphi_pair)", "rabs(sd) < R(p->max_sinphi_pair) * R(0.99)"),
+    ("ITS tracklet: tie goes to the larger gid", "V5",
+     "(m == m0[B - a1] && A < (uint32_t)b0B)", "(m == m0[B - a1] && A > (uint32_t)b0B)"),
+    ("ITS tracklet: not mutual", "V5",
+     "if (Bq < 0 || best0[(uint32_t)Bq - a1] != (int64_t)A) continue;", "if (Bq < 0) continue;"),
+    ("ITS seed: curvature sign", "W2",
+     "const R kap = -((R(2) * (ya * xb)) / ((ra * rb) * dab));", "const R kap = ((R(2) * (ya * xb)) / ((ra * rb) * dab));"),
+    ("ITS seed: local y with the wrong sign", "W1",
+     "auto loc_y = [&](uint32_t P) { return (Y[P] - vy) * ca - (X[P] - vx) * sa; };",
+     "auto loc_y = [&](uint32_t P) { return (Y[P] - vy) * ca + (X[P] - vx) * sa; };"),
+    ("ITS seed: beam axis not moved by the vertex", "W1",
+     "const R ox = -(vx * ca + vy * sa), oy = -(vy * ca - vx * sa);", "const R ox = R(0), oy = R(0);"),
+    ("ITS outward: one missed layer already drops the track", "O2",
+     "if (++miss == 2) alive = false;", "if (++miss == 1) alive = false;"),
+    ("ITS outward: misses are never reset", "O2",
+     "cl[l] = (int32_t)best; ++n_cl; miss = 0;", "cl[l] = (int32_t)best; ++n_cl;"),
+    ("ITS outward: minimum number of clusters off by one", "O3",
+     "if (!alive || n_cl < p->min_clusters) continue;", "if (!alive || n_cl <= p->min_clusters) continue;"),
+    ("ITS outward: chi2 cut ignored", "O2",
+     "if (!(rabs(dx) <= R(p->max_dx) && chi < R(p->chi2_max))) continue;", "if (!(rabs(dx) <= R(p->max_dx))) continue;"),
+    ("ITS outward: residual without the slope term", "O2",
+     "const R dy = loc_y(P) - (st.p[0] + dx * (st.p[2] / c));", "const R dy = loc_y(P) - st.p[0];"),
+    ("ITS inward: covariance not inflated", "N1",
+     "for (int i = 0; i < 15; ++i) st.c[i] = st.c[i] * R(p->turn_cov_scale);                              // N1", ""),
+    ("ITS inward: no transport to the vertex plane", "N3",
+     "if (st.x != R(0)) transport(st, R(0), a, R(p->max_sinphi));                                         // N3", ""),
+    ("ITS: material ignored", "O / SCATTER",
+     "st.c[5] = st.c[5] + th * (R(1) - st.p[2] * st.p[2]);", ""),
 ]
 
 # Not a mutant: semantically equivalent to the SPEC text, listed so that nobody tries to kill it again.

@@ -20,3 +20,4 @@ from .events import (  # noqa: F401
 )
 from .calibration import RawCalibration, default_calibration, raw_from_yz  # noqa: F401
 from .frames import make_frame  # noqa: F401
+from .its import ItsGeometry, ItsBatch, default_its_geometry, generate_its_events  # noqa: F401
