@@ -327,6 +327,54 @@ int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offs
                      float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out, void* workspace,
                      size_t workspace_bytes, void* cuda_stream);
 
+/* ---- ITS standalone tracker -----------------------------------------------
+ * PAPER.md L156-160 (section 4.2): from the clusters of the 6 ITS layers and the primary vertex, "pairs of
+ * SPD clusters seen under nearly the same angle from the vertex point" seed a Kalman filter "propagated
+ * outwards starting from the vertex, considered as a measured point", which attaches "the SDD and SSD
+ * clusters closest to extrapolation point, provided they meet a strict track-to-cluster chi2 cut", with
+ * "multiple scattering ... using average material budget per layer"; "At least 4 clusters are required per
+ * track" and "tracks with 2 consecutive layers without contribution are rejected"; the outward kinematics
+ * is recorded and an "inward Kalman propagation is performed to obtain the kinematics at the vertex
+ * region".  docs/ARITH_SPEC.md section 12 defines every step (V1..V5, W1..W4, O1..O4, N1..N3).
+ * Input: clusters of n_events events sorted by (event, layer), global x, y, z (DEVICE, fp32),
+ * layer_offsets (DEVICE [n_events*6 + 1]), vertex (DEVICE [n_events][3]).  A cluster is identified by
+ * its index in these arrays.  Output (DEVICE, caller-owned, `capacity` slots): per track its event, the
+ * cluster of every layer or -1, the number of clusters, the frame of the track (cos, sin of the direction
+ * vertex -> its layer-1 cluster; x along it, origin at the vertex), the outward state at the outermost
+ * cluster and the inward state at the vertex plane, each as 22 floats x, p[5], C[15], chi2, and ndf.
+ * header[4]: tracks, tracklets, status bits (1: more tracklets than the workspace holds, 2: more tracks
+ * than capacity), 0.  Tracks are in the order of their layer-0 cluster.  Asynchronous on cuda_stream. */
+typedef struct { float R[6], sig_rphi[6], sig_z[6], xx0[6]; } tpc_its_geometry;
+typedef struct {
+  float max_sinphi_pair, max_dtan; /* V3: tracklet window in sin(dphi) and in d(tan lambda)           */
+  float sig_sinphi, sig_tan;       /* V4: weights of the tracklet metric                              */
+  float sig_vtx_xy, sig_vtx_z;     /* W3, W4: the vertex as a measured point [cm]                     */
+  float chi2_max, max_dx;          /* O2: strict track-to-cluster cut; |x_cluster - x_track| bound    */
+  float c0_sinphi, c0_dzds, c0_qpt, turn_cov_scale, max_sinphi; /* as tpc_params                      */
+  int32_t min_clusters;            /* O3 (4)                                                          */
+} tpc_its_params;
+typedef struct {
+  uint32_t capacity;
+  uint32_t* header;      /* [4] */
+  uint32_t* event;       /* [capacity] */
+  int32_t* cluster;      /* [capacity][6] */
+  uint32_t* n_clusters;  /* [capacity] */
+  float* frame;          /* [capacity][2] */
+  float* out_state;      /* [capacity][22] */
+  float* in_state;       /* [capacity][22] */
+  int32_t* out_ndf;      /* [capacity] */
+  int32_t* in_ndf;       /* [capacity] */
+} tpc_its_tracks;
+typedef struct tpc_its_tracker tpc_its_tracker;
+void tpc_its_default_params(tpc_its_params* out);
+int tpc_its_create(const tpc_its_geometry* geometry, float bz_kgauss, const tpc_its_params* params, tpc_its_tracker** out);
+void tpc_its_destroy(tpc_its_tracker* tracker);
+size_t tpc_its_workspace_bytes(const tpc_its_tracker* tracker, uint32_t max_clusters, uint32_t max_events);
+int tpc_its_track_batch(tpc_its_tracker* tracker, const float* x, const float* y, const float* z,
+                        const uint32_t* layer_offsets, const float* vertex, uint32_t n_clusters, uint32_t n_events,
+                        tpc_its_tracks* tracks, void* workspace, size_t workspace_bytes, void* cuda_stream);
+const char* tpc_its_last_error(const tpc_its_tracker* tracker);
+
 /* Text of the last error on this tracker (never NULL). With tracker == NULL: the
  * last error of tpc_tracker_create on this thread. */
 const char* tpc_last_error(const tpc_tracker* tracker);

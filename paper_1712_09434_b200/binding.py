@@ -137,6 +137,19 @@ def load_library():
     lib.tpc_host_submit.argtypes = [vp, C.c_int, C.POINTER(_Clusters), C.c_uint32, C.c_uint32, vp, C.c_size_t, C.c_uint32]
     lib.tpc_host_collect.restype = C.c_int
     lib.tpc_host_collect.argtypes = [vp, C.c_int, C.POINTER(_Tracks), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.tpc_its_default_params.restype = None
+    lib.tpc_its_default_params.argtypes = [C.POINTER(_ItsParams)]
+    lib.tpc_its_create.restype = C.c_int
+    lib.tpc_its_create.argtypes = [C.POINTER(_ItsGeometry), C.c_float, C.POINTER(_ItsParams), C.POINTER(vp)]
+    lib.tpc_its_destroy.restype = None
+    lib.tpc_its_destroy.argtypes = [vp]
+    lib.tpc_its_workspace_bytes.restype = C.c_size_t
+    lib.tpc_its_workspace_bytes.argtypes = [vp, C.c_uint32, C.c_uint32]
+    lib.tpc_its_track_batch.restype = C.c_int
+    lib.tpc_its_track_batch.argtypes = [vp, vp, vp, vp, vp, vp, C.c_uint32, C.c_uint32, C.POINTER(_ItsTracks), vp,
+                                        C.c_size_t, vp]
+    lib.tpc_its_last_error.restype = C.c_char_p
+    lib.tpc_its_last_error.argtypes = [vp]
     lib.tpc_slice_workspace_bytes.restype = C.c_size_t
     lib.tpc_slice_workspace_bytes.argtypes = [C.c_uint32, C.c_int32, C.c_int32]
     lib.tpc_slice_frames.restype = C.c_int
@@ -165,6 +178,23 @@ class _Calibration(C.Structure):
     _fields_ = [("pad_pitch", C.POINTER(C.c_float)), ("n_pads", C.POINTER(C.c_int32)), ("t0", C.c_float),
                 ("v_drift", C.c_float), ("t_max", C.c_float), ("map_ny", C.c_int32), ("map_nz", C.c_int32),
                 ("map", C.POINTER(C.c_float))]
+
+
+class _ItsGeometry(C.Structure):
+    _fields_ = [("R", C.c_float * 6), ("sig_rphi", C.c_float * 6), ("sig_z", C.c_float * 6), ("xx0", C.c_float * 6)]
+
+
+_ITS_FLOATS = ("max_sinphi_pair", "max_dtan", "sig_sinphi", "sig_tan", "sig_vtx_xy", "sig_vtx_z", "chi2_max", "max_dx",
+               "c0_sinphi", "c0_dzds", "c0_qpt", "turn_cov_scale", "max_sinphi")
+
+
+class _ItsParams(C.Structure):
+    _fields_ = [(n, C.c_float) for n in _ITS_FLOATS] + [("min_clusters", C.c_int32)]
+
+
+class _ItsTracks(C.Structure):
+    _fields_ = [("capacity", C.c_uint32)] + [(n, C.c_void_p) for n in (
+        "header", "event", "cluster", "n_clusters", "frame", "out_state", "in_state", "out_ndf", "in_ndf")]
 
 
 class _MergeParams(C.Structure):
@@ -480,6 +510,61 @@ def slice_frames(y, zeta, row_offsets, n_tasks_in: int, n_sectors: int, n_rows: 
         raise TpcError(f"tpc_slice_frames failed ({rc}): {lib.tpc_last_error(None).decode()}")
     slice_frames._keep = ws  # the workspace must outlive the asynchronous kernels
     return y_out, z_out, src[:n], ro_out
+
+
+class ItsTracker:
+    """Owns one ``tpc_its_tracker`` handle (SPEC 12).  ``geometry``: object with R, sig_rphi, sig_z, xx0 [6] and
+    bz_kgauss (e.g. tpc_workload.ItsGeometry); ``params``: dict of tpc_its_params fields to change."""
+
+    def __init__(self, geometry, params: Optional[dict] = None):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        g = _ItsGeometry()
+        for l in range(6):
+            g.R[l], g.sig_rphi[l] = float(geometry.R[l]), float(geometry.sig_rphi[l])
+            g.sig_z[l], g.xx0[l] = float(geometry.sig_z[l]), float(geometry.xx0[l])
+        p = _ItsParams()
+        self._lib.tpc_its_default_params(C.byref(p))
+        for k, v in (params or {}).items():
+            setattr(p, k, v)
+        rc = self._lib.tpc_its_create(C.byref(g), float(geometry.bz_kgauss), C.byref(p), C.byref(self._h))
+        if rc != 0:
+            raise TpcError(f"tpc_its_create failed ({rc}): {self._lib.tpc_its_last_error(None).decode()}")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.tpc_its_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def track_batch(self, x, y, z, layer_offsets, vertex, n_events: int, capacity: Optional[int] = None, stream=None):
+        """tpc_its_track_batch on DEVICE tensors; returns a dict of device tensors (header, event, cluster, ...).
+        Asynchronous; the returned dict keeps the workspace alive."""
+        import torch
+        if not (x.is_cuda and y.is_cuda and z.is_cuda and layer_offsets.is_cuda and vertex.is_cuda):
+            raise TpcError("ItsTracker.track_batch needs CUDA tensors; there is no CPU path")
+        dev = x.device
+        n = int(x.numel())
+        cap = int(capacity if capacity is not None else n // 2 + 1)
+        e = lambda shape, dt: torch.empty(shape, dtype=dt, device=dev)  # noqa: E731
+        out = dict(header=e(4, torch.int32), event=e(cap, torch.int32), cluster=e((cap, 6), torch.int32),
+                   n_clusters=e(cap, torch.int32), frame=e((cap, 2), torch.float32), out_state=e((cap, 22), torch.float32),
+                   in_state=e((cap, 22), torch.float32), out_ndf=e(cap, torch.int32), in_ndf=e(cap, torch.int32))
+        tr = _ItsTracks()
+        tr.capacity = cap
+        for k_, v in out.items():
+            setattr(tr, k_, v.data_ptr())
+        wb = int(self._lib.tpc_its_workspace_bytes(self._h, n, int(n_events)))
+        ws = torch.empty(wb + 256, dtype=torch.uint8, device=dev)
+        wp = ws.data_ptr() + (-ws.data_ptr()) % 256
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        rc = self._lib.tpc_its_track_batch(self._h, x.data_ptr(), y.data_ptr(), z.data_ptr(), layer_offsets.data_ptr(),
+                                           vertex.data_ptr(), n, int(n_events), C.byref(tr), wp, wb, _stream_ptr(s))
+        if rc != 0:
+            raise TpcError(f"tpc_its_track_batch failed ({rc}): {self._lib.tpc_its_last_error(self._h).decode()}")
+        out["_workspace"] = ws
+        return out
 
 
 class ClusterTransform:

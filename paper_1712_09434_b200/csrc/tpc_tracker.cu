@@ -17,6 +17,7 @@
 
 #include "../../include/tpc_tracker.h"
 #include "device_common.cuh"
+#include "stage_its.cuh"
 #include "stage_merge.cuh"
 #include "stage_neighbours.cuh"
 #include "stage_output.cuh"
@@ -1046,6 +1047,117 @@ int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offs
   if (e != cudaSuccess) return fail(nullptr, TPC_ERR_CUDA, "tpc_slice_frames: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;
 }
+
+// ---- ITS standalone tracker (SPEC 12) -----------------------------------------------------------------
+struct tpc_its_tracker {
+  ItsCtx c{};
+  std::string err;
+};
+namespace {
+struct ItsCarve { size_t best1, best0, tl_a, tl_b, tl_ev, zero_begin, scan_tl, scan_out, tickets, n_tracklets, zero_end, total; uint32_t max_tl, tiles_n, tiles_tl; };
+ItsCarve its_carve(uint32_t n, uint32_t) {
+  ItsCarve v{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
+  v.max_tl = n / 2u + 1u;  // a tracklet holds two clusters
+  v.tiles_n = (n + kItsThreads - 1) / kItsThreads; if (v.tiles_n == 0) v.tiles_n = 1;
+  v.tiles_tl = (v.max_tl + kItsThreads - 1) / kItsThreads;
+  v.best1 = take((size_t)(n + 1) * 4); v.best0 = take((size_t)(n + 1) * 4);
+  v.tl_a = take((size_t)v.max_tl * 4); v.tl_b = take((size_t)v.max_tl * 4); v.tl_ev = take((size_t)v.max_tl * 4);
+  v.zero_begin = off;
+  v.scan_tl = take((size_t)v.tiles_n * 8); v.scan_out = take((size_t)v.tiles_tl * 8);
+  v.tickets = take(2 * 4); v.n_tracklets = take(4);
+  v.zero_end = off;
+  v.total = off;
+  return v;
+}
+}  // namespace
+
+void tpc_its_default_params(tpc_its_params* p) {
+  if (!p) return;
+  p->max_sinphi_pair = 0.03f; p->max_dtan = 0.02f; p->sig_sinphi = 0.002f; p->sig_tan = 0.004f;
+  p->sig_vtx_xy = 0.01f; p->sig_vtx_z = 0.01f; p->chi2_max = 30.0f; p->max_dx = 2.0f;
+  p->c0_sinphi = 1.0f; p->c0_dzds = 1.0f; p->c0_qpt = 100.0f; p->turn_cov_scale = 100.0f; p->max_sinphi = 0.95f;
+  p->min_clusters = 4;
+}
+
+int tpc_its_create(const tpc_its_geometry* g, float bz_kgauss, const tpc_its_params* params, tpc_its_tracker** out) {
+  if (!g || !out) return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_its_create: geometry and out must not be NULL");
+  *out = nullptr;
+  for (int l = 0; l < 6; ++l)
+    if (!(g->R[l] > 0.f) || (l && !(g->R[l] > g->R[l - 1])) || !(g->sig_rphi[l] > 0.f) || !(g->sig_z[l] > 0.f) || !(g->xx0[l] >= 0.f))
+      return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_its_create: radii must grow, errors must be positive, material >= 0");
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaFree(nullptr) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, TPC_ERR_CUDA, "tpc_its_create: no CUDA device (no CPU fallback exists)");
+  }
+  tpc_its_tracker* t = new (std::nothrow) tpc_its_tracker();
+  if (!t) return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_its_create: out of host memory");
+  ItsCtx& c = t->c;
+  if (params) c.prm = *params; else tpc_its_default_params(&c.prm);
+  const tpc_its_params& p = c.prm;
+  if (!(p.sig_sinphi > 0.f) || !(p.sig_tan > 0.f) || !(p.sig_vtx_xy > 0.f) || !(p.sig_vtx_z > 0.f) || p.min_clusters < 2) {
+    delete t;
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_its_create: need positive sigmas and min_clusters >= 2");
+  }
+  for (int l = 0; l < 6; ++l) {
+    c.R[l] = g->R[l];
+    c.sr2[l] = g->sig_rphi[l] * g->sig_rphi[l];
+    c.sz2[l] = g->sig_z[l] * g->sig_z[l];
+    c.ms2[l] = (0.0136f * 0.0136f) * g->xx0[l];
+  }
+  c.a = -0.000299792458f * bz_kgauss;
+  c.wphi = 1.0f / (p.sig_sinphi * p.sig_sinphi); c.wtan = 1.0f / (p.sig_tan * p.sig_tan);
+  c.svxy2 = p.sig_vtx_xy * p.sig_vtx_xy; c.svz2 = p.sig_vtx_z * p.sig_vtx_z;
+  *out = t;
+  return TPC_OK;
+}
+
+void tpc_its_destroy(tpc_its_tracker* t) { delete t; }
+
+size_t tpc_its_workspace_bytes(const tpc_its_tracker* t, uint32_t max_clusters, uint32_t max_events) {
+  return t ? its_carve(max_clusters, max_events).total : 0;
+}
+
+int tpc_its_track_batch(tpc_its_tracker* t, const float* x, const float* y, const float* z, const uint32_t* layer_offsets,
+                        const float* vertex, uint32_t n_clusters, uint32_t n_events, tpc_its_tracks* tracks, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream) {
+  if (!t) return TPC_ERR_ARGUMENT;
+  auto bad = [&](int code, const char* msg) { t->err = msg; return code; };
+  if (!layer_offsets || !tracks || (n_events && !vertex) || (n_clusters && (!x || !y || !z)))
+    return bad(TPC_ERR_ARGUMENT, "tpc_its_track_batch: NULL argument");
+  if (!tracks->header || !tracks->event || !tracks->cluster || !tracks->n_clusters || !tracks->frame || !tracks->out_state ||
+      !tracks->in_state || !tracks->out_ndf || !tracks->in_ndf)
+    return bad(TPC_ERR_ARGUMENT, "tpc_its_track_batch: every array of tpc_its_tracks must not be NULL");
+  if (n_clusters >= 0x7FFFFFFFu || (uint64_t)n_events * 6u >= 0x7FFFFFFFull) return bad(TPC_ERR_ARGUMENT, "tpc_its_track_batch: too many clusters or events");
+  const ItsCarve v = its_carve(n_clusters, n_events);
+  if (!workspace || workspace_bytes < v.total) return bad(TPC_ERR_WORKSPACE, "tpc_its_track_batch: workspace too small (tpc_its_workspace_bytes)");
+  if (((uintptr_t)workspace & (kAlign - 1)) != 0) return bad(TPC_ERR_WORKSPACE, "tpc_its_track_batch: workspace must be 256-byte aligned");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace;
+  ItsCtx c = t->c;
+  c.x = x; c.y = y; c.z = z; c.lo = layer_offsets; c.vtx = vertex; c.n = n_clusters; c.n_events = n_events;
+  c.max_tracklets = v.max_tl;
+  c.best1 = (int32_t*)(ws + v.best1); c.best0 = (int32_t*)(ws + v.best0);
+  c.tl_a = (uint32_t*)(ws + v.tl_a); c.tl_b = (uint32_t*)(ws + v.tl_b); c.tl_ev = (uint32_t*)(ws + v.tl_ev);
+  c.scan_tl = (unsigned long long*)(ws + v.scan_tl); c.scan_out = (unsigned long long*)(ws + v.scan_out);
+  c.tickets = (uint32_t*)(ws + v.tickets); c.n_tracklets = (uint32_t*)(ws + v.n_tracklets);
+  c.out = *tracks;
+  cudaError_t e = cudaMemsetAsync(ws + v.zero_begin, 0, v.zero_end - v.zero_begin, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(tracks->header, 0, 16, s);
+  if (e != cudaSuccess) return bad(TPC_ERR_CUDA, "tpc_its_track_batch: CUDA memset failed");
+  if (n_clusters > 0 && n_events > 0) {
+    k_its_pairs<<<dim3(kItsBlocksPerEvent, n_events, 2), kItsThreads, 0, s>>>(c);
+    k_its_tracklets<<<v.tiles_n, kItsThreads, 0, s>>>(c);
+    k_its_follow<<<v.tiles_tl, kItsThreads, 0, s>>>(c);
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) { t->err = std::string("tpc_its_track_batch: CUDA launch: ") + cudaGetErrorString(e); return TPC_ERR_CUDA; }
+  return TPC_OK;
+}
+
+const char* tpc_its_last_error(const tpc_its_tracker* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
 
 const char* tpc_last_error(const tpc_tracker* t) { return t ? t->err.c_str() : g_create_error.c_str(); }
 
