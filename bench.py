@@ -62,6 +62,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-merge", action="store_true", help="skip the merger + refit leg (SURVEY 8(f)1)")
     ap.add_argument("--no-transform", action="store_true", help="skip the cluster transformation leg (SURVEY 8(f)3)")
+    ap.add_argument("--no-its", action="store_true", help="skip the ITS standalone tracker leg (SURVEY 8(f)4)")
     ap.add_argument("--cpu-workers", type=int, default=0, help="worker processes of the all-cores cpu_baseline leg (0 = all)")
     ap.add_argument("--dry-run", action="store_true",
                     help="control flow only (rendezvous, barriers, MAX-reduce, counter gather) on the gloo backend with "
@@ -461,6 +462,34 @@ def run_ours(args):
         xf.close()
         del pad_d, time_d, y2, z2
 
+    # ITS standalone tracker on 16 synthetic events of 1 500 primaries (about 9 000 clusters per layer
+    # and event with 10 % noise), timed on its own with CUDA events on the launching stream
+    its = None
+    if not args.no_its:
+        from paper_1712_09434_b200 import ItsTracker
+        from tpc_workload import default_its_geometry, generate_its_events
+        ig = default_its_geometry()
+        ib = generate_its_events(ig, 16, 1500, seed=3, pt_range=(0.15, 5.0), noise_frac=0.1)
+        it = ItsTracker(ig)
+        tt = lambda a_: torch.from_numpy(np.ascontiguousarray(a_)).to(dev)  # noqa: E731
+        ix, iy, iz = tt(ib.x), tt(ib.y), tt(ib.z)
+        ilo, ivt = tt(ib.layer_offsets.astype(np.uint32).view(np.int32)), tt(ib.vertex.astype(np.float32).reshape(-1))
+        for _ in range(3):
+            io = it.track_batch(ix, iy, iz, ilo, ivt, ib.n_events)
+        torch.cuda.synchronize()
+        i0, i1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        i0.record(stream)
+        for _ in range(args.steps):
+            io = it.track_batch(ix, iy, iz, ilo, ivt, ib.n_events)
+        i1.record(stream)
+        torch.cuda.synchronize()
+        ih = io["header"].cpu().numpy()
+        i_ms = i0.elapsed_time(i1) / args.steps
+        its = {"ms_per_step": i_ms, "events": ib.n_events, "clusters": ib.n_clusters, "tracklets": int(ih[1]),
+               "tracks": int(ih[0]), "status": int(ih[2]), "events_per_s": ib.n_events / (i_ms / 1e3), "launches": 3,
+               "note": "includes the allocation of outputs and workspace by the binding (torch caching allocator)"}
+        it.close()
+
     # max over ranks, totals over ranks
     (ms_total, e2e_ms_max, e2e_pipe_ms_max), tot = reduce_over_ranks([ms_total, e2e[0] if e2e else 0.0,
                                                                        e2e_pipe[0] if e2e else 0.0],
@@ -517,6 +546,8 @@ def run_ours(args):
         "clocks": clocks,
         "gpu_launches": trk.launches_per_batch() * args.steps,
     }
+    if its:
+        line["its_standalone"] = its
     if xform:
         xform["hbm_frac"] = xform["achieved_gbs"] / peak_gbs
         line["cluster_transform"] = xform

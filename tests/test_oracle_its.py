@@ -169,3 +169,35 @@ def test_material_widens_the_errors():
     r1 = its_track(default_its_geometry(xx0=0.011), b.x, b.y, b.z, b.layer_offsets, b.vertex, b.n_events)
     assert len(r0.event) == len(r1.event) > 150
     assert np.all(r1.in_state[:, 6 + 5] > r0.in_state[:, 6 + 5]) and np.all(r1.in_state[:, 6 + 9] > r0.in_state[:, 6 + 9])
+
+
+def test_displaced_vertex_and_clusters_off_the_nominal_radius():
+    """W1 (beam axis seen from a displaced vertex) and O2 (the residual follows the track's slope over the distance
+    between the state and the cluster).  (a) vertices 5 mm off the beam axis and a tight |dx| window: the layers are
+    still met where the clusters are; (b) the clusters of layer 3 sit 1 cm further out along their (low-pT, curved)
+    tracks than the nominal radius: they are still attached, which needs the slope term (0.1 cm = 30 sigma)."""
+    b = generate_its_events(GEOM0, 3, 150, seed=11, noise_frac=0.0, smear=False, vertex_sigma=(0.5, 0.5, 5.0),
+                            pt_range=(0.3, 5.0))
+    X, Y, Z = b.truth_xyz[:, 0], b.truth_xyz[:, 1], b.truth_xyz[:, 2]
+    r = its_track(GEOM0, X, Y, Z, b.layer_offsets, b.vertex.astype(np.float64), b.n_events,
+                  params=ItsParams(max_dx=0.02), precision="f64")
+    n_full = sum((b.truth_track == t).sum() == 6 for t in range(len(b.tracks["pt"])))
+    assert n_full > 350 and (r.n_clusters == 6).sum() >= 0.98 * n_full
+    from tpc_workload.its import _crossings
+    far = dataclasses.replace(GEOM0, R=GEOM0.R + np.array([0, 0, 0, 1.0, 0, 0], np.float32))
+    b1 = generate_its_events(GEOM0, 2, 120, seed=12, noise_frac=0.0, smear=False, pt_range=(0.12, 0.2))
+    xyz = b1.truth_xyz.copy()
+    tk = b1.tracks
+    moved = 0
+    for e in range(2):
+        sel = np.nonzero(tk["event"] == e)[0]
+        cr = _crossings(far, b1.vertex[e].astype(np.float64), tk["pt"][sel], tk["charge"][sel], tk["phi0"][sel], tk["eta"][sel])
+        for i in range(b1.layer_offsets[6 * e + 3], b1.layer_offsets[6 * e + 4]):
+            p3 = cr[int(np.nonzero(sel == b1.truth_track[i])[0][0]), 3]
+            if not np.isnan(p3[0]):
+                xyz[i] = p3
+                moved += 1
+    assert moved > 150
+    r = its_track(GEOM0, xyz[:, 0], xyz[:, 1], xyz[:, 2], b1.layer_offsets, b1.vertex.astype(np.float64), 2, precision="f64")
+    n_full = sum((b1.truth_track == t).sum() == 6 for t in range(len(b1.tracks["pt"])))
+    assert n_full > 150 and (r.cluster[:, 3] >= 0).sum() >= 0.97 * n_full and (r.n_clusters == 6).sum() >= 0.97 * n_full
