@@ -6,9 +6,9 @@
 //   k_its_pairs      one thread per SPD cluster (both layers): its best partner in the other layer by the plain
 //                    loop over that layer's clusters of the event, 128 at a time through shared memory
 //   k_its_tracklets  mutual choices become tracklets, numbered in the order of the inner cluster (ordered compaction)
-//   k_its_follow     one thread per tracklet: seed, outward pass (every layer search is the plain loop over the
-//                    layer's clusters: the lanes of a warp follow tracklets of the same event and read the same
-//                    clusters), inward pass; kept tracks are written in tracklet order (ordered compaction)
+//   k_its_follow     one warp per tracklet: seed, outward pass (every layer search is the plain loop over the
+//                    layer's clusters, strided over the lanes, then a warp minimum of (chi2, gid)), inward pass
+//   k_its_output     kept tracks are written in tracklet order (ordered compaction)
 #pragma once
 #include "device_common.cuh"
 #include "stage_tracklet.cuh"
@@ -18,6 +18,7 @@ namespace tpc {
 constexpr int kItsThreads = 128;
 constexpr int kItsBlocksPerEvent = 16;  // k_its_pairs: blocks that share the SPD clusters of one event
 
+struct ItsRec;
 struct ItsCtx {
   float R[6], sr2[6], sz2[6], ms2[6];
   float a, wphi, wtan, svxy2, svz2;
@@ -32,6 +33,7 @@ struct ItsCtx {
   uint32_t* n_tracklets;
   unsigned long long *scan_tl, *scan_out;
   uint32_t* tickets;               // [2]
+  struct ItsRec* recs;             // [max_tracklets] results parked for the ordered output
   tpc_its_tracks out;
 };
 
@@ -133,8 +135,134 @@ __device__ __forceinline__ void its_put_state(float* d, float x, const TrackStat
   d[14] = S.c32; d[15] = S.c33; d[16] = S.c40; d[17] = S.c41; d[18] = S.c42; d[19] = S.c43; d[20] = S.c44; d[21] = S.chi2;
 }
 
-// W1..W4, O1..O4, N1..N3 for one tracklet per thread; ordered output.
+// Result of one tracklet, parked in the workspace until the ordered output knows its slot.
+struct ItsRec {
+  float out_state[22], in_state[22];
+  float ca, sa;
+  int32_t cluster[6];
+  int32_t out_ndf, in_ndf;
+  uint32_t n_clusters, event, alive, pad;
+};
+
+// W1..W4, O1..O4, N1..N3: one WARP per tracklet.  Every lane carries the same filter state (same inputs, same
+// arithmetic, same bits); the lanes differ only in the layer searches of O2, where lane j tests the clusters
+// j, j + 32, ... of the layer and the warp takes the lexicographic minimum of (chi2, gid).
 __global__ void __launch_bounds__(kItsThreads) k_its_follow(const ItsCtx c) {
+  constexpr unsigned FULL = 0xffffffffu;
+  const uint32_t n_tl = *c.n_tracklets;
+  const int lane = (int)threadIdx.x & 31;
+  const uint32_t k = blockIdx.x * (kItsThreads / 32) + (threadIdx.x >> 5);
+  if (k >= n_tl) return;
+  const float a = c.a, max_sin = c.prm.max_sinphi;
+  bool alive = true;
+  TrackState S, S_out;
+  zero_state(S);
+  zero_state(S_out);
+  float x = 0.0f, x_out = 0.0f;
+  int32_t cl[6] = {-1, -1, -1, -1, -1, -1};
+  const uint32_t A = c.tl_a[k], B = c.tl_b[k], e = c.tl_ev[k];
+  const float vx = c.vtx[3u * e], vy = c.vtx[3u * e + 1u], vz = c.vtx[3u * e + 2u];
+  const float ax = c.x[A] - vx, ay = c.y[A] - vy, ra = sqrtf(ax * ax + ay * ay);
+  const float bx = c.x[B] - vx, by = c.y[B] - vy, rb = sqrtf(bx * bx + by * by), tb = (c.z[B] - vz) / rb;
+  const float ca = bx / rb, sa = by / rb;                                                        // W1
+  auto loc_x = [&](uint32_t P) { return (c.x[P] - vx) * ca + (c.y[P] - vy) * sa; };
+  auto loc_y = [&](uint32_t P) { return (c.y[P] - vy) * ca - (c.x[P] - vx) * sa; };
+  const float ox = -(vx * ca + vy * sa), oy = -(vy * ca - vx * sa);
+  const float xa = loc_x(A), ya = loc_y(A), xb = rb;                                             // W2
+  const float dab = sqrtf((xb - xa) * (xb - xa) + ya * ya);
+  const float kap = -((2.0f * (ya * xb)) / ((ra * rb) * dab));
+  S.y = 0.0f; S.z = vz; S.s = -(0.5f * kap) * xb; S.t = tb; S.q = a != 0.0f ? kap / a : 0.0f;    // W3
+  S.c00 = c.svxy2; S.c11 = c.svz2; S.c22 = c.prm.c0_sinphi; S.c33 = c.prm.c0_dzds; S.c44 = c.prm.c0_qpt;
+  S.chi2 = 0.0f; S.ndf = -5;
+  update_hit(S, 0.0f, vz, c.svxy2, c.svz2);                                                      // W4
+  auto attach = [&](uint32_t P, int l) {
+    const float xp = loc_x(P);
+    if (!transport(S, xp - x, a, max_sin)) return false;
+    x = xp;
+    update_hit(S, loc_y(P), c.z[P], c.sr2[l], c.sz2[l]);
+    its_scatter(c, S, l);
+    return true;
+  };
+  cl[0] = (int32_t)A; cl[1] = (int32_t)B;
+  alive = attach(A, 0);                                                                          // O1
+  if (alive) alive = attach(B, 1);
+  int n_cl = 2, miss = 0;
+#pragma unroll
+  for (int l = 2; l < 6; ++l) {                                                                  // O2
+    if (!alive) break;
+    const float Rl = c.R[l];
+    for (int it = 0; it < 2 && alive; ++it) {
+      const float dyo = S.y - oy;
+      const float xt = ox + sqrtf(fmaxf(Rl * Rl - dyo * dyo, 0.0f));
+      if (it == 1 && xt == x) break;
+      alive = transport(S, xt - x, a, max_sin);
+      if (alive) x = xt;
+    }
+    if (!alive) break;
+    const float cphi = sqrtf(1.0f - S.s * S.s);
+    const float ey = S.c00 + c.sr2[l], ez = S.c11 + c.sz2[l];
+    const float tany = S.s / cphi, tanz = S.t / cphi;
+    uint32_t best = 0xFFFFFFFFu;
+    float chi_best = __int_as_float(0x7f800000);
+    for (uint32_t P = c.lo[6u * e + l] + (uint32_t)lane, Pe = c.lo[6u * e + l + 1u]; P < Pe; P += 32u) {
+      const float dx = loc_x(P) - x;
+      const float dy = loc_y(P) - (S.y + dx * tany);
+      const float dz = c.z[P] - (S.z + dx * tanz);
+      const float chi = (dy * dy) / ey + (dz * dz) / ez;
+      if (!(fabsf(dx) <= c.prm.max_dx && chi < c.prm.chi2_max)) continue;
+      if (chi < chi_best) { best = P; chi_best = chi; }            // ascending P in a lane: ties keep the smaller gid
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {                             // lexicographic minimum of (chi2, gid) over the warp
+      const float oc = __shfl_xor_sync(FULL, chi_best, o);
+      const uint32_t ob = __shfl_xor_sync(FULL, best, o);
+      if (oc < chi_best || (oc == chi_best && ob < best)) { chi_best = oc; best = ob; }
+    }
+    if (best != 0xFFFFFFFFu) {
+      alive = attach(best, l);
+      cl[l] = (int32_t)best; ++n_cl; miss = 0;
+    } else {
+      its_scatter(c, S, l);
+      if (++miss == 2) alive = false;
+    }
+  }
+  alive = alive && n_cl >= c.prm.min_clusters;                                                   // O3
+  if (alive) {
+    S_out = S; x_out = x;                                                                        // O4
+    const float f = c.prm.turn_cov_scale;                                                        // N1
+    S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
+    S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
+    S.chi2 = 0.0f; S.ndf = -5;
+#pragma unroll
+    for (int l = 5; l >= 0; --l) {                                                               // N2
+      if (cl[l] < 0) continue;
+      const uint32_t P = (uint32_t)cl[l];
+      const float xp = loc_x(P);
+      if (xp != x) {
+        if (!transport(S, xp - x, a, max_sin)) break;
+        x = xp;
+      }
+      update_hit(S, loc_y(P), c.z[P], c.sr2[l], c.sz2[l]);
+      its_scatter(c, S, l);
+    }
+    if (x != 0.0f && transport(S, 0.0f - x, a, max_sin)) x = 0.0f;                               // N3
+  }
+  if (lane == 0) {
+    ItsRec& r = c.recs[k];
+    r.alive = alive ? 1u : 0u;
+    if (alive) {
+      its_put_state(r.out_state, x_out, S_out);
+      its_put_state(r.in_state, x, S);
+      r.ca = ca; r.sa = sa;
+#pragma unroll
+      for (int l = 0; l < 6; ++l) r.cluster[l] = cl[l];
+      r.out_ndf = S_out.ndf; r.in_ndf = S.ndf; r.n_clusters = (uint32_t)n_cl; r.event = e;
+    }
+  }
+}
+
+// kept tracks in tracklet order (ordered compaction): one thread per tracklet copies its parked result
+__global__ void __launch_bounds__(kItsThreads) k_its_output(const ItsCtx c) {
   __shared__ uint32_t s_warp[33];
   __shared__ uint32_t s_tile;
   __shared__ unsigned long long s_prefix;
@@ -145,99 +273,7 @@ __global__ void __launch_bounds__(kItsThreads) k_its_follow(const ItsCtx c) {
   const uint32_t last_tile = n_tl > 0u ? (n_tl - 1u) / kItsThreads : 0u;
   if (tile > last_tile) return;
   const uint32_t k = tile * kItsThreads + threadIdx.x;
-  const float a = c.a, max_sin = c.prm.max_sinphi;
-  bool alive = k < n_tl;
-  TrackState S, S_out;
-  zero_state(S);
-  zero_state(S_out);
-  float x = 0.0f, x_out = 0.0f, ca = 1.0f, sa = 0.0f;
-  int32_t cl[6] = {-1, -1, -1, -1, -1, -1};
-  int n_cl = 0;
-  uint32_t e = 0u;
-  if (alive) {
-    const uint32_t A = c.tl_a[k], B = c.tl_b[k];
-    e = c.tl_ev[k];
-    const float vx = c.vtx[3u * e], vy = c.vtx[3u * e + 1u], vz = c.vtx[3u * e + 2u];
-    const float ax = c.x[A] - vx, ay = c.y[A] - vy, ra = sqrtf(ax * ax + ay * ay);
-    const float bx = c.x[B] - vx, by = c.y[B] - vy, rb = sqrtf(bx * bx + by * by), tb = (c.z[B] - vz) / rb;
-    ca = bx / rb; sa = by / rb;                                                                  // W1
-    auto loc_x = [&](uint32_t P) { return (c.x[P] - vx) * ca + (c.y[P] - vy) * sa; };
-    auto loc_y = [&](uint32_t P) { return (c.y[P] - vy) * ca - (c.x[P] - vx) * sa; };
-    const float ox = -(vx * ca + vy * sa), oy = -(vy * ca - vx * sa);
-    const float xa = loc_x(A), ya = loc_y(A), xb = rb;                                           // W2
-    const float dab = sqrtf((xb - xa) * (xb - xa) + ya * ya);
-    const float kap = -((2.0f * (ya * xb)) / ((ra * rb) * dab));
-    x = 0.0f;                                                                                    // W3
-    S.y = 0.0f; S.z = vz; S.s = -(0.5f * kap) * xb; S.t = tb; S.q = a != 0.0f ? kap / a : 0.0f;
-    S.c00 = c.svxy2; S.c11 = c.svz2; S.c22 = c.prm.c0_sinphi; S.c33 = c.prm.c0_dzds; S.c44 = c.prm.c0_qpt;
-    S.chi2 = 0.0f; S.ndf = -5;
-    update_hit(S, 0.0f, vz, c.svxy2, c.svz2);                                                    // W4
-    auto attach = [&](uint32_t P, int l) {
-      const float xp = loc_x(P);
-      if (!transport(S, xp - x, a, max_sin)) return false;
-      x = xp;
-      update_hit(S, loc_y(P), c.z[P], c.sr2[l], c.sz2[l]);
-      its_scatter(c, S, l);
-      return true;
-    };
-    cl[0] = (int32_t)A; cl[1] = (int32_t)B;
-    alive = attach(A, 0);                                                                        // O1
-    if (alive) alive = attach(B, 1);
-    n_cl = 2;
-    int miss = 0;
-    for (int l = 2; l < 6 && alive; ++l) {                                                       // O2
-      const float Rl = c.R[l];
-      for (int it = 0; it < 2 && alive; ++it) {
-        const float dyo = S.y - oy;
-        const float xt = ox + sqrtf(fmaxf(Rl * Rl - dyo * dyo, 0.0f));
-        if (it == 1 && xt == x) break;
-        alive = transport(S, xt - x, a, max_sin);
-        if (alive) x = xt;
-      }
-      if (!alive) break;
-      const float cphi = sqrtf(1.0f - S.s * S.s);
-      const float ey = S.c00 + c.sr2[l], ez = S.c11 + c.sz2[l];
-      const float tany = S.s / cphi, tanz = S.t / cphi;
-      int32_t best = -1;
-      float chi_best = 0.0f;
-      for (uint32_t P = c.lo[6u * e + l], Pe = c.lo[6u * e + l + 1u]; P < Pe; ++P) {
-        const float dx = loc_x(P) - x;
-        const float dy = loc_y(P) - (S.y + dx * tany);
-        const float dz = c.z[P] - (S.z + dx * tanz);
-        const float chi = (dy * dy) / ey + (dz * dz) / ez;
-        if (!(fabsf(dx) <= c.prm.max_dx && chi < c.prm.chi2_max)) continue;
-        if (best < 0 || chi < chi_best) { best = (int32_t)P; chi_best = chi; }
-      }
-      if (best >= 0) {
-        alive = attach((uint32_t)best, l);
-        cl[l] = best; ++n_cl; miss = 0;
-      } else {
-        its_scatter(c, S, l);
-        if (++miss == 2) alive = false;
-      }
-    }
-    alive = alive && n_cl >= c.prm.min_clusters;                                                 // O3
-    if (alive) {
-      S_out = S; x_out = x;                                                                      // O4
-      const float f = c.prm.turn_cov_scale;                                                      // N1
-      S.c00 *= f; S.c10 *= f; S.c11 *= f; S.c20 *= f; S.c21 *= f; S.c22 *= f; S.c30 *= f; S.c31 *= f;
-      S.c32 *= f; S.c33 *= f; S.c40 *= f; S.c41 *= f; S.c42 *= f; S.c43 *= f; S.c44 *= f;
-      S.chi2 = 0.0f; S.ndf = -5;
-#pragma unroll
-      for (int l = 5; l >= 0; --l) {                                                             // N2
-        if (cl[l] < 0) continue;
-        const uint32_t P = (uint32_t)cl[l];
-        const float xp = loc_x(P);
-        if (xp != x) {
-          if (!transport(S, xp - x, a, max_sin)) break;
-          x = xp;
-        }
-        update_hit(S, loc_y(P), c.z[P], c.sr2[l], c.sz2[l]);
-        its_scatter(c, S, l);
-      }
-      if (x != 0.0f && transport(S, 0.0f - x, a, max_sin)) x = 0.0f;                             // N3
-    }
-  }
+  const bool alive = k < n_tl && c.recs[k].alive != 0u;
   uint32_t total;
   const uint32_t excl = block_exclusive_scan(alive ? 1u : 0u, s_warp, &total);
   if (threadIdx.x < 32) {
@@ -249,13 +285,12 @@ __global__ void __launch_bounds__(kItsThreads) k_its_follow(const ItsCtx c) {
   const tpc_its_tracks& o = c.out;
   if (alive) {
     if (slot < o.capacity) {
-      o.event[slot] = e; o.n_clusters[slot] = (uint32_t)n_cl;
-#pragma unroll
-      for (int l = 0; l < 6; ++l) o.cluster[(size_t)slot * 6 + l] = cl[l];
-      o.frame[2 * slot] = ca; o.frame[2 * slot + 1] = sa;
-      its_put_state(o.out_state + (size_t)slot * 22, x_out, S_out);
-      its_put_state(o.in_state + (size_t)slot * 22, x, S);
-      o.out_ndf[slot] = S_out.ndf; o.in_ndf[slot] = S.ndf;
+      const ItsRec& r = c.recs[k];
+      o.event[slot] = r.event; o.n_clusters[slot] = r.n_clusters;
+      for (int l = 0; l < 6; ++l) o.cluster[(size_t)slot * 6 + l] = r.cluster[l];
+      o.frame[2 * slot] = r.ca; o.frame[2 * slot + 1] = r.sa;
+      for (int j = 0; j < 22; ++j) { o.out_state[(size_t)slot * 22 + j] = r.out_state[j]; o.in_state[(size_t)slot * 22 + j] = r.in_state[j]; }
+      o.out_ndf[slot] = r.out_ndf; o.in_ndf[slot] = r.in_ndf;
     } else {
       atomicOr(&o.header[2], 2u);
     }

@@ -1054,7 +1054,7 @@ struct tpc_its_tracker {
   std::string err;
 };
 namespace {
-struct ItsCarve { size_t best1, best0, tl_a, tl_b, tl_ev, zero_begin, scan_tl, scan_out, tickets, n_tracklets, zero_end, total; uint32_t max_tl, tiles_n, tiles_tl; };
+struct ItsCarve { size_t best1, best0, tl_a, tl_b, tl_ev, recs, zero_begin, scan_tl, scan_out, tickets, n_tracklets, zero_end, total; uint32_t max_tl, tiles_n, tiles_tl; };
 ItsCarve its_carve(uint32_t n, uint32_t) {
   ItsCarve v{};
   size_t off = 0;
@@ -1064,6 +1064,7 @@ ItsCarve its_carve(uint32_t n, uint32_t) {
   v.tiles_tl = (v.max_tl + kItsThreads - 1) / kItsThreads;
   v.best1 = take((size_t)(n + 1) * 4); v.best0 = take((size_t)(n + 1) * 4);
   v.tl_a = take((size_t)v.max_tl * 4); v.tl_b = take((size_t)v.max_tl * 4); v.tl_ev = take((size_t)v.max_tl * 4);
+  v.recs = take((size_t)v.max_tl * sizeof(ItsRec));
   v.zero_begin = off;
   v.scan_tl = take((size_t)v.tiles_n * 8); v.scan_out = take((size_t)v.tiles_tl * 8);
   v.tickets = take(2 * 4); v.n_tracklets = take(4);
@@ -1141,6 +1142,7 @@ int tpc_its_track_batch(tpc_its_tracker* t, const float* x, const float* y, cons
   c.max_tracklets = v.max_tl;
   c.best1 = (int32_t*)(ws + v.best1); c.best0 = (int32_t*)(ws + v.best0);
   c.tl_a = (uint32_t*)(ws + v.tl_a); c.tl_b = (uint32_t*)(ws + v.tl_b); c.tl_ev = (uint32_t*)(ws + v.tl_ev);
+  c.recs = (ItsRec*)(ws + v.recs);
   c.scan_tl = (unsigned long long*)(ws + v.scan_tl); c.scan_out = (unsigned long long*)(ws + v.scan_out);
   c.tickets = (uint32_t*)(ws + v.tickets); c.n_tracklets = (uint32_t*)(ws + v.n_tracklets);
   c.out = *tracks;
@@ -1150,7 +1152,8 @@ int tpc_its_track_batch(tpc_its_tracker* t, const float* x, const float* y, cons
   if (n_clusters > 0 && n_events > 0) {
     k_its_pairs<<<dim3(kItsBlocksPerEvent, n_events, 2), kItsThreads, 0, s>>>(c);
     k_its_tracklets<<<v.tiles_n, kItsThreads, 0, s>>>(c);
-    k_its_follow<<<v.tiles_tl, kItsThreads, 0, s>>>(c);
+    k_its_follow<<<(v.max_tl + kItsThreads / 32 - 1) / (kItsThreads / 32), kItsThreads, 0, s>>>(c);
+    k_its_output<<<v.tiles_tl, kItsThreads, 0, s>>>(c);
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) { t->err = std::string("tpc_its_track_batch: CUDA launch: ") + cudaGetErrorString(e); return TPC_ERR_CUDA; }
