@@ -16,8 +16,14 @@
 
 namespace tpc {
 
-constexpr int kNfThreads = 128;
-constexpr int kNfList = 8;                    // candidates per side a cluster keeps (more -> serial search) at the
+#ifndef TPC_NF_THREADS
+#define TPC_NF_THREADS 128
+#endif
+constexpr int kNfThreads = TPC_NF_THREADS;
+#ifndef TPC_NF_LIST
+#define TPC_NF_LIST 8
+#endif
+constexpr int kNfList = TPC_NF_LIST;                    // candidates per side a cluster keeps (more -> serial search) at the
 constexpr int kNfListDense = 16;              // density of a central event / in denser batches (host's choice)
 constexpr uint32_t kNfDenseRow = 900;         // mean clusters per row from which the deeper lists are used
 constexpr uint32_t kNfStageBytes = 18 * 1024 + 512;  // staged neighbour rows (both) must fit in this
