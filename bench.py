@@ -529,7 +529,11 @@ def run_ours(args):
                      "frac": top_gbs / peak_gbs, "traffic": ncu.get("dram_bytes") if ncu else None,
                      "traffic_source": ncu_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg[top], "ms_per_launch": stage_ms[top],
-                     "note": "the metric asks for the HBM fraction; this kernel is bound by plain-ALU issue, see \"alu\"",
+                     "traffic_gbs": (ncu["dram_bytes"] / (stage_ms[top] / 1e3) / 1e9) if ncu and "dram_bytes" in ncu else None,
+                     "note": "achieved = ALGORITHMIC bytes over the live launch time (the metric's definition); traffic = "
+                             "the DRAM bytes ncu saw this kernel move: 64-byte fetches for gathers of 8..16 useful bytes. "
+                             "The kernel is bound by DRAM random access and gather latency (DESIGN.md section 6), \"alu\" "
+                             "shows how far it is from the plain-ALU ceiling",
                      "share_of_step": stage_ms[top] / max(sum(stage_ms.values()), 1e-9)},
         "roofline_path": {"bound": "hbm", "achieved": path_gbs, "peak": peak_gbs, "unit": "GB/s",
                           "frac": path_gbs / peak_gbs, "algorithmic_bytes_per_step": path_bytes,
