@@ -27,11 +27,11 @@ constexpr int kResolveThreads = 256;
 #ifndef TPC_RESOLVE_CHUNK
 #define TPC_RESOLVE_CHUNK 4096
 #endif
-constexpr uint32_t kResolveChunk = TPC_RESOLVE_CHUNK;  // clusters per block: 32 KB of ownership words (8192: 1.11 ms, 4096: 1.05 ms, 16384: 2.2 ms)
+constexpr uint32_t kResolveChunk = TPC_RESOLVE_CHUNK;  // clusters per block: 32 KB of ownership words (2048: 1.05 ms, 4096: 0.84 ms, 8192: 1.00 ms)
 #ifndef TPC_RESOLVE_BATCH
-#define TPC_RESOLVE_BATCH 8
+#define TPC_RESOLVE_BATCH 4
 #endif
-constexpr int kResolveBatch = TPC_RESOLVE_BATCH;  // (tracklet, row) pairs a thread has in flight
+constexpr int kResolveBatch = TPC_RESOLVE_BATCH;  // (tracklet, four rows) groups a thread has in flight (2: 0.92, 4: 0.84, 8: 1.24 ms)
 constexpr int kResolveRows = 512;                 // row offsets of the chunk kept in shared memory
 constexpr uint32_t kKeyGidBits = 27, kKeyTrkBits = 26;
 
@@ -62,8 +62,9 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
   const int min_hits = c.prm.min_track_hits;
   const size_t stride = map_stride(n_rows);
   __syncthreads();
-  // pass 1 (K7): the (tracklet, row) pairs of every task of the chunk, rows of the chunk only, row fastest:
-  // thread tid takes the pairs tid, tid + 256, ...; (tt, rr) is stepped without a division
+  // pass 1 (K7): for every tracklet of every task of the chunk, the rows the chunk covers, read four rows at a time
+  // (16-byte groups of the row map: a map row starts at a multiple of 640 bytes); the (tracklet, group) pairs are
+  // taken group fastest, thread tid the pairs tid, tid + 256, ...; (tt, gg) is stepped without a division
   for (uint32_t k = task_a; k <= task_b; ++k) {
     const uint32_t t0 = c.trk_task_off[k], nt = c.trk_task_off[k + 1u] - t0;
     const uint32_t gid_lo = c.row_off[k * (uint32_t)n_rows], gid_hi = c.row_off[(k + 1u) * (uint32_t)n_rows];
@@ -73,29 +74,33 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
     }
     const uint32_t ra = k == task_a ? tr_a - k * (uint32_t)n_rows : 0u;
     const uint32_t rb = k == task_b ? tr_b - k * (uint32_t)n_rows : (uint32_t)n_rows - 1u;
-    const uint32_t R = rb - ra + 1u, step_t = kResolveThreads / R, step_r = kResolveThreads % R;
-    uint32_t tt = (uint32_t)tid / R, rr = (uint32_t)tid % R;
+    const uint32_t g0 = ra >> 2, G = (rb >> 2) - g0 + 1u, step_t = kResolveThreads / G, step_g = kResolveThreads % G;
+    uint32_t tt = (uint32_t)tid / G, gg = (uint32_t)tid % G;
     while (__any_sync(0xffffffffu, tt < nt)) {
-      uint4 m[kResolveBatch];
-      uint32_t idx[kResolveBatch], ts[kResolveBatch], rs[kResolveBatch];
+      uint4 m[kResolveBatch], e[kResolveBatch];
+      uint32_t ts[kResolveBatch], rs[kResolveBatch];
 #pragma unroll
-      for (int j = 0; j < kResolveBatch; ++j) {  // meta and map entry together (an entry outside the
-        ts[j] = tt; rs[j] = ra + rr;             // tracklet's rows is read and ignored)
+      for (int j = 0; j < kResolveBatch; ++j) {  // meta and four map entries together (entries outside the
+        ts[j] = tt; rs[j] = 4u * (g0 + gg);      // tracklet's rows are read and ignored)
         const bool in = tt < nt;
         m[j] = in ? __ldg(&c.trk_meta[t0 + tt]) : make_uint4(0u, 0u, 0u, 0u);
-        idx[j] = in ? c.trk_hits[(size_t)(t0 + tt) * stride + rs[j]] : kNoHit;
-        tt += step_t; rr += step_r;
-        if (rr >= R) { rr -= R; ++tt; }
+        e[j] = in ? *reinterpret_cast<const uint4*>(c.trk_hits + (size_t)(t0 + tt) * stride + rs[j])
+                  : make_uint4(kNoHit, kNoHit, kNoHit, kNoHit);
+        tt += step_t; gg += step_g;
+        if (gg >= G) { gg -= G; ++tt; }
       }
 #pragma unroll
       for (int j = 0; j < kResolveBatch; ++j) {
-        const uint32_t first = m[j].y & 0xFFFFu, last = m[j].y >> 16;
-        const uint32_t off = idx[j] - i0;  // idx < i0 wraps to a large number
-        if ((int)m[j].x >= min_hits && rs[j] >= first && rs[j] <= last && idx[j] != kNoHit && off < span) {
-          const unsigned long long key = ((unsigned long long)m[j].x << (kKeyGidBits + kKeyTrkBits)) |
-                                         ((unsigned long long)(((1u << kKeyGidBits) - 1u) - (m[j].z - gid_lo)) << kKeyTrkBits) |
-                                         (unsigned long long)ts[j];
-          atomicMax(&s_owner[off], key);
+        if ((int)m[j].x < min_hits) continue;
+        const uint32_t first = max(m[j].y & 0xFFFFu, ra), last = min(m[j].y >> 16, rb);
+        const unsigned long long key = ((unsigned long long)m[j].x << (kKeyGidBits + kKeyTrkBits)) |
+                                       ((unsigned long long)(((1u << kKeyGidBits) - 1u) - (m[j].z - gid_lo)) << kKeyTrkBits) |
+                                       (unsigned long long)ts[j];
+        const uint32_t idx[4] = {e[j].x, e[j].y, e[j].z, e[j].w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const uint32_t r = rs[j] + (uint32_t)q, off = idx[q] - i0;  // idx < i0 wraps to a large number
+          if (r >= first && r <= last && idx[q] != kNoHit && off < span) atomicMax(&s_owner[off], key);
         }
       }
     }
