@@ -82,7 +82,7 @@ struct Ctx {
   uint32_t* gid;           // [n]  idx -> gid (index in the input arrays)
   uint32_t* bins;          // [kBinsPerCluster*n + n_tr*kBinPad + 1]  first idx of every bin (+ one end entry per row)
   RowInfo* rowinfo;        // [n_tr]
-  uint32_t* tile_tr;       // [seed_tiles] task*n_rows + row that holds idx = tile * 1024 (written by a1 for a4)
+  uint32_t* tile_tr;       // [seed_tiles] task*n_rows + row that holds idx = tile * kSeedTile (written by a1 for a4)
   int32_t *link_up, *link_dn;  // [n] raw links as idx (SPEC 3), -1 none
   int32_t* clean_up;       // [n] cleaned up-link (C1)
   uint4* trk_seed;         // [max_tracklets][kSeedU4] seed record written by a4 (layout: kSeedU4 above)

@@ -7,6 +7,10 @@
 #pragma once
 #include "device_common.cuh"
 
+#ifndef TPC_SEED_THREADS
+#define TPC_SEED_THREADS 512
+#endif
+
 namespace tpc {
 
 // ---------------------------------------------------------------------------
@@ -17,8 +21,11 @@ namespace tpc {
 // inside a bin they are ordered by gid so that idx order, and with it the order
 // of start hits, tracklets and output tracks, is the same on every run.
 // ---------------------------------------------------------------------------
-constexpr int kGridThreads = 128;
-constexpr uint32_t kSeedTileIdx = 1024;  // = kSeedTile below
+#ifndef TPC_GRID_THREADS
+#define TPC_GRID_THREADS 160  // 64: 0.86 ms, 96: 0.70, 128: 0.78, 160: 0.70, 192: 0.72, 256: 0.80 (a row of a central event: 444 clusters)
+#endif
+constexpr int kGridThreads = TPC_GRID_THREADS;
+constexpr uint32_t kSeedTileIdx = 4 * TPC_SEED_THREADS;  // = kSeedTile below
 
 // Grid of a row with n clusters inside the box [ylo, yhi] x [zlo, zhi]: kBinsPerCluster bins per cluster.
 __device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint32_t lo, uint32_t n, float ylo,
@@ -187,7 +194,10 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 // after the other); those with a long enough chain are compacted again, the tile takes its place in
 // the output (chained scan with decoupled look-back), and the threads write the seed records.
 // ---------------------------------------------------------------------------
-constexpr int kSeedThreads = 256;
+#ifndef TPC_SEED_THREADS
+#define TPC_SEED_THREADS 512
+#endif
+constexpr int kSeedThreads = TPC_SEED_THREADS;
 constexpr int kSeedItems = 4;
 constexpr uint32_t kSeedTile = kSeedThreads * kSeedItems;
 static_assert(kSeedTile == kSeedTileIdx, "k_grid_build notes the row of every tile start");
