@@ -23,7 +23,10 @@ namespace tpc {
 // A task with 2^27 clusters or more (fifty times the whole config-3 batch in one sector) does not fit
 // the key: its tracklets keep nothing and TPC_STATUS_TASK_TOO_LARGE is set.
 // ---------------------------------------------------------------------------
-constexpr int kResolveThreads = 256;
+#ifndef TPC_RESOLVE_THREADS
+#define TPC_RESOLVE_THREADS 256
+#endif
+constexpr int kResolveThreads = TPC_RESOLVE_THREADS;
 #ifndef TPC_RESOLVE_CHUNK
 #define TPC_RESOLVE_CHUNK 4096
 #endif
@@ -129,7 +132,10 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
   }
 }
 
-constexpr int kOutThreads = 128;  // = tracklets per tile; 4 warps x 32 tracklets
+#ifndef TPC_OUT_THREADS
+#define TPC_OUT_THREADS 128
+#endif
+constexpr int kOutThreads = TPC_OUT_THREADS;  // = tracklets per tile; 4 warps x 32 tracklets
 constexpr int kOutChunks = 5;     // 32-row chunks of a row map read per round (159 rows = 5 chunks)
 
 // a6 (L2) + a7.  One tile = 128 consecutive tracklets; k_resolve has counted the hits every tracklet keeps
