@@ -94,6 +94,9 @@ struct Ctx {
   uint32_t* out_rows;      // [max_tracklets] row of the first kept hit | row of the last kept hit << 16, per output track
   uint32_t* trk_kept;      // [max_tracklets] hits the tracklet keeps (L1), counted by k_resolve; cleared per call
   uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
+  uint32_t* trk_perm;      // [max_tracklets] queue order of a5: ticket k stands for tracklet trk_perm[k] (k_order_*, stage_tracklet.cuh)
+  uint32_t* trk_key;       // [max_tracklets] diagonal of the tracklet in the queue order of the next a5 kernel (order_note)
+  uint32_t* order_cnt;     // [4 kernels][2][order_keys()] tracklets per diagonal of that order, then the slots handed out; cleared per call
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
   uint32_t* tickets;       // [8] 0 seed tiles, 1 output tiles, 2..5 queue heads of the four tracklet kernels
@@ -103,6 +106,53 @@ struct Ctx {
   // outputs (device)
   tpc_tracks out;
 };
+
+// ---- queue order of the tracklet constructor (a5); the kernels and the reasons are in stage_tracklet.cuh ----
+// Diagonal of a tracklet in front of kernel KIND (0 chain fit, 1 up pass, 2 refit, 3 rest of the down pass):
+//     d = (rows between the tracklet's next row and the row where that pass begins) + stagger * task
+// stagger in 1/256 rows per task.
+#ifndef TPC_STAGGER_CHAIN
+#define TPC_STAGGER_CHAIN 160
+#endif
+#ifndef TPC_STAGGER_UP
+#define TPC_STAGGER_UP 256
+#endif
+#ifndef TPC_STAGGER_REFIT
+#define TPC_STAGGER_REFIT 316
+#endif
+#ifndef TPC_STAGGER_FINISH
+#define TPC_STAGGER_FINISH 200
+#endif
+__host__ __device__ constexpr uint32_t stagger_of(int kind) {
+  return kind == 0 ? TPC_STAGGER_CHAIN : kind == 1 ? TPC_STAGGER_UP : kind == 2 ? TPC_STAGGER_REFIT : TPC_STAGGER_FINISH;
+}
+#ifndef TPC_STAGGER_MAX
+#define TPC_STAGGER_MAX 512
+#endif
+constexpr uint32_t kStaggerMax = TPC_STAGGER_MAX;  // bounds the diagonals: n_rows + n_tasks * kStaggerMax / 256
+__host__ __device__ inline uint32_t order_keys(uint32_t n_rows, uint32_t n_tasks) {
+  return n_rows + ((n_tasks * kStaggerMax) >> 8) + 1u;
+}
+template <int KIND>
+__device__ __forceinline__ uint32_t order_key(const Ctx& c, uint32_t task, uint32_t row) {
+  static_assert(stagger_of(KIND) <= kStaggerMax, "order_keys() bounds the diagonals with kStaggerMax");
+  // The last n_rows / stagger tasks share one offset, so that the diagonals stay as long as they were down to the
+  // last one (a diagonal of staggered tasks alone would thin out, the queue would run ahead of the lanes, and the
+  // device would wait for the long tracklets of the last task).
+#ifdef TPC_ORDER_LAST
+  const uint32_t n_last = TPC_ORDER_LAST;
+#else
+  const uint32_t n_last = ((uint32_t)c.n_rows * 256u) / stagger_of(KIND);
+#endif
+  const uint32_t n_stag = c.n_tasks > n_last ? c.n_tasks - n_last : 0u;
+  return row + ((min(task, n_stag) * stagger_of(KIND)) >> 8);
+}
+// Called by the kernel in front of kernel KIND when it has finished tracklet t: notes the diagonal and counts it.
+template <int KIND>
+__device__ __forceinline__ void order_note(const Ctx& c, uint32_t t, uint32_t task, uint32_t row) {
+  const uint32_t key = order_key<KIND>(c, task, row);
+  c.trk_key[t] = key;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

@@ -292,9 +292,41 @@ __device__ __forceinline__ void load_rec(const float4* rec, TrackState& S, int& 
 // ---- the queue of a tracklet kernel -------------------------------------------------------------------
 // Tickets are drawn kPoolBatch at a time per warp (one atomic per batch instead of one per fetch); the
 // lanes in `need` get consecutive tickets.  A ticket >= the number of tracklets means the queue is empty.
+// Ticket k stands for tracklet perm[k] (Ctx::trk_perm, the queue order built in front of every kernel, below).
+// A batch is 32 aligned tickets; lane j of the warp loads perm[] of ticket base + j when the batch is
+// drawn and hands it out by shuffle, so no fetch waits for a dependent load of its own.
 constexpr uint32_t kPoolBatch = 32;
-struct TicketPool { uint32_t next, end; };
-__device__ __forceinline__ uint32_t pool_take(TicketPool& p, uint32_t* head, unsigned need, int lane) {
+struct TicketPool { uint32_t next, end, perm; };
+__device__ __forceinline__ uint32_t pool_take(TicketPool& p, uint32_t* head, const uint32_t* __restrict__ perm,
+                                              uint32_t n_trk, unsigned need, int lane, uint32_t& t_out) {
+  const uint32_t cnt = (uint32_t)__popc(need), have = p.end - p.next;
+  const uint32_t rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
+  const uint32_t tk_old = p.next + rank;
+  const uint32_t t_old = __shfl_sync(0xffffffffu, p.perm, (int)(tk_old & 31u));
+  if (cnt <= have) {
+    p.next += cnt;
+    t_out = t_old;
+    return tk_old;
+  }
+  uint32_t base = 0u;
+  if (lane == 0) base = atomicAdd(head, kPoolBatch);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  uint32_t np = 0u;
+  {
+    const uint32_t k = base + (uint32_t)lane;
+    if (k < n_trk) np = __ldg(perm + k);
+  }
+  const uint32_t tk_new = base + (rank - have);
+  const uint32_t t_new = __shfl_sync(0xffffffffu, np, (int)(tk_new & 31u));
+  p.perm = np;
+  p.next = base + (cnt - have);
+  p.end = base + kPoolBatch;
+  if (rank < have) { t_out = t_old; return tk_old; }
+  t_out = t_new;
+  return tk_new;
+}
+// The same queue without a permutation (ticket k is item k): the merger's refit.
+__device__ __forceinline__ uint32_t pool_take_seq(TicketPool& p, uint32_t* head, unsigned need, int lane) {
   const uint32_t cnt = (uint32_t)__popc(need), have = p.end - p.next;
   const uint32_t rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
   if (cnt <= have) {
@@ -322,6 +354,16 @@ __device__ __forceinline__ void prefetch_slot(void* slot, const void* src, int n
 }
 __device__ __forceinline__ void prefetch_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+#ifdef TPC_TAIL_PROBE
+__device__ unsigned long long g_probe_start[4];
+__device__ unsigned long long g_probe_exit[4][8192];
+__device__ __forceinline__ unsigned long long probe_now() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
+#define TPC_PROBE_START(k) if (threadIdx.x == 0) atomicMin(&g_probe_start[k], probe_now());
+#define TPC_PROBE_EXIT(k) if ((threadIdx.x & 31) == 0) g_probe_exit[k][(blockIdx.x * blockDim.x + threadIdx.x) >> 5] = probe_now();
+#else
+#define TPC_PROBE_START(k)
+#define TPC_PROBE_EXIT(k)
+#endif
 enum LaneState { LN_IDLE = 0, LN_RUN = 1, LN_EXIT = 2 };
 enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };  // ISSUED this iteration, READY from the next on
 
@@ -330,18 +372,19 @@ enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };
 //                  requested draw a ticket and start the copy of that tracklet's record to their slot;
 //   (the kernel's own "consume" block turns an idle lane with a READY slot into a running one);
 //   fetch_advance: ISSUED -> READY at the end of the iteration.
-__device__ __forceinline__ void fetch_request(TicketPool& pool, uint32_t* head, bool want, int lane, uint32_t n_trk,
-                                              int& pf, uint32_t& t_next, void* slot, const void* src_base,
+__device__ __forceinline__ void fetch_request(TicketPool& pool, uint32_t* head, const uint32_t* perm, bool want, int lane,
+                                              uint32_t n_trk, int& pf, uint32_t& t_next, void* slot, const void* src_base,
                                               size_t src_stride, int n16) {
   const unsigned need = __ballot_sync(0xffffffffu, want);
   if (need) {
-    const uint32_t tk = pool_take(pool, head, need, lane);
+    uint32_t t = 0u;
+    const uint32_t tk = pool_take(pool, head, perm, n_trk, need, lane, t);
     if (want) {
       if (tk >= n_trk) {
         pf = PF_DRAINED;
       } else {
-        t_next = tk;
-        prefetch_slot(slot, reinterpret_cast<const char*>(src_base) + (size_t)tk * src_stride, n16);
+        t_next = t;
+        prefetch_slot(slot, reinterpret_cast<const char*>(src_base) + (size_t)t * src_stride, n16);
         pf = PF_ISSUED;
       }
     }
@@ -361,6 +404,148 @@ __host__ __device__ inline size_t trk_smem_bytes(int n_rows, int slot16) {
 }
 
 // ---------------------------------------------------------------------------
+// Queue order of a5 (Ctx::trk_perm), built anew in front of each of the four kernels.
+// A lane moves its tracklet one pad row per step, and a search reads the bins and clusters of that one
+// row of its sector task.  Tracklets are numbered in (task, row of the start hit, bin) order; drawn in
+// that order, the 2 200 tracklets of a task start together but at rows spread over the whole sector, so
+// a grid row is read again only after its lines have left the L2 (44 % hits, 10 x the grid in DRAM reads),
+// and the queue ends with tracklets that still have up to n_rows steps to go while the device idles.
+// Instead the queue is sorted by the DIAGONAL
+//     d = (rows the tracklet's first step is away from the row where the pass begins) + stagger * task
+// (chain fit, up pass: counted from row 0 upwards; refit, rest of the down pass: from the last row
+// downwards).  Lanes draw about one diagonal per step, so that the tracklets of a task still start when
+// the others of that task reach their row: every task is swept by a wavefront a few rows wide, the tasks
+// one after the other `stagger` rows apart, and a grid row is read by all its tracklets while it is in
+// the L2.  The last diagonals hold the last rows of the last tasks only: short tracklets, no tail.
+// stagger (1/256 rows per task) = tracklets a task starts per row / tracklets the lanes draw per step.
+// A counting sort by d: the kernel that finishes a tracklet in front of this one notes its diagonal and
+// counts it (order_note, device_common.cuh), k_order_scan turns the counts into the first slot of every
+// diagonal (one block), k_order_fill hands the slots out.  The order inside a diagonal is what the atomics
+// give; it only decides which lane follows which tracklet - the result does not depend on it.
+// ---------------------------------------------------------------------------
+constexpr int kOrderThreads = 256;
+// One block per chunk of kOrderChunk consecutive tracklets (one or two tasks: a few hundred diagonals next to
+// each other): the diagonals within kOrderWindow of the chunk's smallest are counted in shared memory first, so
+// that global memory sees one atomic per block and diagonal; a tracklet beyond the window (a chunk over many
+// small tasks) goes to global memory directly.
+constexpr int kOrderItems = 8;
+constexpr uint32_t kOrderChunk = kOrderThreads * kOrderItems;
+constexpr uint32_t kOrderWindow = 2048;
+__global__ void __launch_bounds__(kOrderThreads) k_order_count(const Ctx c, int kind) {
+  __shared__ uint32_t s_cnt[kOrderWindow];
+  __shared__ uint32_t s_min;
+  constexpr uint32_t kNone = 0xFFFFFFFFu;
+  const uint32_t n_trk = *c.n_tracklets, n_keys = order_keys((uint32_t)c.n_rows, c.n_tasks);
+  uint32_t* cnt = c.order_cnt + (size_t)(2 * kind) * n_keys;
+  for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) s_cnt[k] = 0u;
+  for (uint32_t t0 = blockIdx.x * kOrderChunk; t0 < n_trk; t0 += gridDim.x * kOrderChunk) {
+    if (threadIdx.x == 0) s_min = kNone;
+    __syncthreads();
+    uint32_t key[kOrderItems];
+    uint32_t kmin = kNone;
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i) {
+      const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
+      key[i] = t < n_trk ? c.trk_key[t] : kNone;
+      kmin = min(kmin, key[i]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+    if ((threadIdx.x & 31) == 0) atomicMin(&s_min, kmin);
+    __syncthreads();
+    kmin = s_min;
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i) {
+      if (key[i] == kNone) continue;
+      if (key[i] - kmin < kOrderWindow) atomicAdd(&s_cnt[key[i] - kmin], 1u);
+      else atomicAdd(&cnt[key[i]], 1u);
+    }
+    __syncthreads();
+    for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) {
+      const uint32_t n = s_cnt[k];
+      if (n) { atomicAdd(&cnt[kmin + k], n); s_cnt[k] = 0u; }
+    }
+    __syncthreads();
+  }
+}
+__global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int kind) {
+  __shared__ uint32_t s_cnt[kOrderWindow];
+  __shared__ uint32_t s_min;
+  constexpr uint32_t kNone = 0xFFFFFFFFu;
+  const uint32_t n_trk = *c.n_tracklets, n_keys = order_keys((uint32_t)c.n_rows, c.n_tasks);
+  uint32_t* cursor = c.order_cnt + (size_t)(2 * kind + 1) * n_keys;
+  for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) s_cnt[k] = 0u;
+  for (uint32_t t0 = blockIdx.x * kOrderChunk; t0 < n_trk; t0 += gridDim.x * kOrderChunk) {
+    if (threadIdx.x == 0) s_min = kNone;
+    __syncthreads();
+    uint32_t key[kOrderItems], rank[kOrderItems];
+    uint32_t kmin = kNone;
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i) {
+      const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
+      key[i] = t < n_trk ? c.trk_key[t] : kNone;
+      kmin = min(kmin, key[i]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+    if ((threadIdx.x & 31) == 0) atomicMin(&s_min, kmin);
+    __syncthreads();
+    kmin = s_min;
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i) {
+      rank[i] = 0u;
+      if (key[i] == kNone) continue;
+      if (key[i] - kmin < kOrderWindow) {
+        rank[i] = atomicAdd(&s_cnt[key[i] - kmin], 1u);
+      } else {  // beyond the window: straight to global memory
+#ifdef TPC_IDENTITY_ORDER
+        c.trk_perm[t0 + (uint32_t)i * kOrderThreads + threadIdx.x] = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
+#else
+        c.trk_perm[atomicAdd(&cursor[key[i]], 1u)] = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
+#endif
+        key[i] = kNone;
+      }
+    }
+    __syncthreads();
+    for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) {
+      const uint32_t n = s_cnt[k];
+      if (n) s_cnt[k] = atomicAdd(&cursor[kmin + k], n);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i) {
+      const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
+#ifdef TPC_IDENTITY_ORDER
+      if (key[i] != kNone) c.trk_perm[t] = t;
+#else
+      if (key[i] != kNone) c.trk_perm[s_cnt[key[i] - kmin] + rank[i]] = t;
+#endif
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kOrderItems; ++i)
+      if (key[i] != kNone) s_cnt[key[i] - kmin] = 0u;
+    __syncthreads();
+  }
+}
+// tracklets per diagonal -> first slot of every diagonal (the counters of the fill pass start there)
+__global__ void __launch_bounds__(1024) k_order_scan(const Ctx c, int kind) {
+  __shared__ uint32_t s_warp[33];
+  const uint32_t n_keys = order_keys((uint32_t)c.n_rows, c.n_tasks);
+  const uint32_t* cnt = c.order_cnt + (size_t)(2 * kind) * n_keys;
+  uint32_t* first = c.order_cnt + (size_t)(2 * kind + 1) * n_keys;
+  uint32_t carry = 0u;
+  for (uint32_t k0 = 0u; k0 < n_keys; k0 += 1024u) {
+    const uint32_t k = k0 + threadIdx.x;
+    const uint32_t v = k < n_keys ? cnt[k] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(v, s_warp, &total);
+    if (k < n_keys) first[k] = carry + ex;
+    carry += total;
+  }
+}
+
+// ---------------------------------------------------------------------------
 // K1 seed + K2 chain fit.  Every step: transport one row up, update with the chain hit.  The hit two links
 // ahead and the (y,z) of the next one are requested before the transport, so no step waits for a load.
 // ---------------------------------------------------------------------------
@@ -374,6 +559,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
+  TPC_PROBE_START(0)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   TrackState S;
   zero_state(S);
@@ -383,11 +569,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
   int32_t h_cur = -1, h_next = -1, h_last = -1;  // chain hit of the next step, the one after it, the last one fitted
   float2 p_cur = make_float2(0.0f, 0.0f);
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u};
+  TicketPool pool{0u, 0u, 0u};
   uint32_t n_steps = 0u, n_chain = 0u;
   while (true) {
-    fetch_request(pool, &c.tickets[2], (st == LN_IDLE || (st == LN_RUN && h_next < 0)) && pf == PF_NONE, lane, n_trk,
-                  pf, t_next, slot, c.trk_seed, sizeof(uint4) * kSeedU4, kChainSlot16);
+    fetch_request(pool, &c.tickets[2], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && h_next < 0)) && pf == PF_NONE,
+                         lane, n_trk, pf, t_next, slot, c.trk_seed, sizeof(uint4) * kSeedU4, kChainSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
         prefetch_wait();
@@ -444,9 +630,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
     if (st == LN_RUN && (h_cur < 0 || !ok)) {  // end of the chain, or K2's failed transport (-> K4, no up pass)
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, r0, row_cur,
                 pack_rows(row_cur, row_cur - 1, r0, !ok), tr_base, (uint32_t)h_last, 0u);
+      order_note<1>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)row_cur);            // the up pass begins in this row
       st = LN_IDLE;
     }
   }
+  TPC_PROBE_EXIT(0)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
@@ -467,6 +655,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
+  TPC_PROBE_START(1)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   const int max_gap = c.prm.max_row_gap;
   TrackState S;
@@ -477,12 +666,12 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
   int32_t last_hit = -1;
   bool turn = false;  // this lane's next step is the turn-around (its last step here)
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u};
+  TicketPool pool{0u, 0u, 0u};
   uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u;
   while (true) {
     if (st == LN_RUN && row_cur + 1 >= n_rows) turn = true;            // K3 ran off the last row
-    fetch_request(pool, &c.tickets[3], (st == LN_IDLE || (st == LN_RUN && turn)) && pf == PF_NONE, lane, n_trk, pf,
-                  t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
+    fetch_request(pool, &c.tickets[3], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && turn)) && pf == PF_NONE, lane,
+                         n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
         prefetch_wait();
@@ -555,9 +744,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     if (p_turn) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, last_row - 1, r0, false), tr_base, ia, ib);
+      order_note<2>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - last_row));  // the refit comes down from lastRow
       st = LN_IDLE;
     }
   }
+  TPC_PROBE_EXIT(1)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
@@ -582,6 +773,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
+  TPC_PROBE_START(2)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   TrackState S;
   zero_state(S);
@@ -591,11 +783,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
   uint32_t m_cur = kNoHit, m_next = kNoHit;  // map[r_down], map[r_down - 1]
   float2 p_cur = make_float2(0.0f, 0.0f);
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u};
+  TicketPool pool{0u, 0u, 0u};
   uint32_t n_steps = 0u;
   while (true) {
-    fetch_request(pool, &c.tickets[4], (st == LN_IDLE || (st == LN_RUN && m_next == kNoHit)) && pf == PF_NONE, lane,
-                  n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
+    fetch_request(pool, &c.tickets[4], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && m_next == kNoHit)) && pf == PF_NONE,
+                         lane, n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
         prefetch_wait();
@@ -632,9 +824,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
     if (st == LN_RUN && (m_cur == kNoHit || !ok)) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, r_down, r0, false), tr_base, m_cur, 0u);
+      order_note<3>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - (r_down > 0 ? r_down : 0)));  // goes on from r_down
       st = LN_IDLE;
     }
   }
+  TPC_PROBE_EXIT(2)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_REFIT_STEPS], (unsigned long long)n_steps);
@@ -658,6 +852,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
+  TPC_PROBE_START(3)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   const int max_gap = c.prm.max_row_gap;
   [[maybe_unused]] const int min_hits = c.prm.min_track_hits;
@@ -668,7 +863,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
   int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
   uint32_t map_next = kNoHit;  // map[r_down], loaded one step ahead
   int phase = PH_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u};
+  TicketPool pool{0u, 0u, 0u};
   uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_kept = 0u, n_kept_hits = 0u;
   while (true) {
     // (A) tracklets that ended in the last step: the record, and what the ownership kernel (K7) needs
@@ -683,14 +878,15 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
       const bool want = (phase == PH_IDLE || phase == PH_FINISH || (phase == PH_DOWN && r_down < 0)) && pf == PF_NONE;
       const unsigned need = __ballot_sync(FULL, want);
       if (need) {
-        const uint32_t tk = pool_take(pool, &c.tickets[5], need, lane);
+        uint32_t tn = 0u;
+        const uint32_t tk = pool_take(pool, &c.tickets[5], c.trk_perm, n_trk, need, lane, tn);
         if (want) {
           if (tk >= n_trk) {
             pf = PF_DRAINED;
           } else {
-            t_next = tk;
-            prefetch_slot(slot, c.trk_rec + (size_t)tk * kRecFloat4, kRecFloat4);
-            prefetch_slot(slot + kRecFloat4, c.trk_seed + (size_t)tk * kSeedU4 + 2, 1);
+            t_next = tn;
+            prefetch_slot(slot, c.trk_rec + (size_t)tn * kRecFloat4, kRecFloat4);
+            prefetch_slot(slot + kRecFloat4, c.trk_seed + (size_t)tn * kSeedU4 + 2, 1);
             pf = PF_ISSUED;
           }
         }
@@ -762,6 +958,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
       --r_down;
     }
   }
+  TPC_PROBE_EXIT(3)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);

@@ -93,7 +93,7 @@ uint32_t host_total_tracklets(const tpc_tracker* t, uint32_t n, uint32_t max_tra
 // Offsets of every workspace array, in bytes.
 struct Carve {
   size_t yz, gid, bins, rowinfo, tile_tr, link_up, link_dn, clean_up, trk_seed, trk_hits, trk_rec, trk_meta, zero_begin,
-      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, trk_kept, zero_end, out_trk, out_rows, total;
+      scan_seed, scan_out, tickets, n_tracklets, trk_task_off, trk_kept, order_cnt, zero_end, out_trk, out_rows, trk_perm, trk_key, total;
   uint32_t seed_tiles, out_tiles;
 };
 
@@ -126,9 +126,12 @@ Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   c.n_tracklets = take(sizeof(uint32_t));
   c.trk_task_off = take(((size_t)n_tasks + 2) * sizeof(uint32_t));
   c.trk_kept = take((size_t)T * sizeof(uint32_t));
+  c.order_cnt = take((size_t)8 * order_keys(n_rows, n_tasks) * sizeof(uint32_t));
   c.zero_end = off;
   c.out_trk = take((size_t)T * sizeof(uint32_t));
   c.out_rows = take((size_t)T * sizeof(uint32_t));
+  c.trk_perm = take((size_t)T * sizeof(uint32_t));
+  c.trk_key = take((size_t)T * sizeof(uint32_t));
   c.total = off;
   return c;
 }
@@ -165,6 +168,7 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
   c.trk_hits = (uint32_t*)(ws + cv.trk_hits); c.trk_rec = (float4*)(ws + cv.trk_rec);
   c.trk_meta = (uint4*)(ws + cv.trk_meta); c.trk_task_off = (uint32_t*)(ws + cv.trk_task_off);
   c.trk_kept = (uint32_t*)(ws + cv.trk_kept);
+  c.trk_perm = (uint32_t*)(ws + cv.trk_perm); c.trk_key = (uint32_t*)(ws + cv.trk_key); c.order_cnt = (uint32_t*)(ws + cv.order_cnt);
   c.out_trk = (uint32_t*)(ws + cv.out_trk); c.out_rows = (uint32_t*)(ws + cv.out_rows);
   c.scan_seed = (unsigned long long*)(ws + cv.scan_seed); c.scan_out = (unsigned long long*)(ws + cv.scan_out);
   c.tickets = (uint32_t*)(ws + cv.tickets); c.n_tracklets = (uint32_t*)(ws + cv.n_tracklets);
@@ -177,6 +181,20 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
 }  // namespace
 
 extern "C" {
+
+#ifdef TPC_TAIL_PROBE
+void tpc_probe_reset() {
+  unsigned long long big[4] = {~0ull, ~0ull, ~0ull, ~0ull};
+  cudaMemcpyToSymbol(g_probe_start, big, sizeof(big));
+  static unsigned long long z[4][8192];
+  cudaMemcpyToSymbol(g_probe_exit, z, sizeof(z));
+}
+void tpc_probe_read(unsigned long long* start4, unsigned long long* exit4x8192) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(start4, g_probe_start, 4 * sizeof(unsigned long long));
+  cudaMemcpyFromSymbol(exit4x8192, g_probe_exit, 4 * 8192 * sizeof(unsigned long long));
+}
+#endif
 
 void tpc_default_params(tpc_params* out) {
   if (out) default_params(out);
@@ -313,7 +331,7 @@ size_t tpc_workspace_bytes(const tpc_tracker* t, uint32_t max_clusters, uint32_t
   return carve((uint32_t)t->n_rows, max_clusters, max_tasks, T).total;
 }
 
-int tpc_launches_per_batch(const tpc_tracker*) { return 11; }  // a1, a2, a3, a4, a5 (4 kernels), K7 (2), a6+a7
+int tpc_launches_per_batch(const tpc_tracker*) { return 23; }  // a1, a2, a3, a4, a5 (4 kernels, each behind the 3 of its queue order), K7 (2), a6+a7, a5 (4 kernels), K7 (2), a6+a7
 
 void tpc_tracker_enable_counters(tpc_tracker* t, int on) {
   if (t) t->counters_on = on != 0;
@@ -438,16 +456,26 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
   else k_seeds<false><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);
   mark();
-  // a5: four persistent kernels, each with as many blocks as the device holds at once
+  // a5: four persistent kernels, each with as many blocks as the device holds at once and its own queue order
+  const int og = 4 * t->n_sm;
+#define TPC_ORDER(KIND)                                     \
+  k_order_count<<<og, kOrderThreads, 0, s>>>(c, KIND); \
+  k_order_scan<<<1, 1024, 0, s>>>(c, KIND);         \
+  k_order_fill<<<og, kOrderThreads, 0, s>>>(c, KIND);
+  TPC_ORDER(0)
   if (cnt) k_trk_chain<true><<<t->trk_grid[0][1], kTrackletThreads, t->trk_smem[0], s>>>(c);
   else k_trk_chain<false><<<t->trk_grid[0][0], kTrackletThreads, t->trk_smem[0], s>>>(c);
   mark();
+  TPC_ORDER(1)
   if (cnt) k_trk_up<true><<<t->trk_grid[1][1], kTrackletThreads, t->trk_smem[1], s>>>(c);
   else k_trk_up<false><<<t->trk_grid[1][0], kTrackletThreads, t->trk_smem[1], s>>>(c);
   mark();
+  TPC_ORDER(2)
   if (cnt) k_trk_refit<true><<<t->trk_grid[2][1], kTrackletThreads, t->trk_smem[2], s>>>(c);
   else k_trk_refit<false><<<t->trk_grid[2][0], kTrackletThreads, t->trk_smem[2], s>>>(c);
   mark();
+  TPC_ORDER(3)
+#undef TPC_ORDER
   if (cnt) k_trk_finish<true><<<t->trk_grid[3][1], kTrackletThreads, t->trk_smem[3], s>>>(c);
   else k_trk_finish<false><<<t->trk_grid[3][0], kTrackletThreads, t->trk_smem[3], s>>>(c);
   mark();
