@@ -327,6 +327,28 @@ int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offs
                      float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out, void* workspace,
                      size_t workspace_bytes, void* cuda_stream);
 
+/* The frame slicer for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same kernels and the same result as tpc_slice_frames, but the scratch
+ * (the counts of the output rows) lives in a file-scope `static __device__` array of the library instead of a
+ * caller workspace.  The array holds TPC_SLICE_STATIC_MAX_ENTRIES uint32 (4 MiB; every GPU that loads the
+ * library holds it until the process exits); a call needs n_tasks_in*n_rows*n_slices + 2 of them and is
+ * refused with TPC_ERR_WORKSPACE (text in tpc_last_error(NULL)) beyond that - e.g. 36 sectors x 159 rows x
+ * 4 slices fit 45 frames per call.  Inputs and outputs are the caller's DEVICE arrays as in tpc_slice_frames.
+ * Neither call allocates or frees anything (no cudaMalloc, cudaFree or allocating library routine).
+ * tpc_slice_static_setup resolves the device address of the array for the CURRENT device
+ * (cudaGetSymbolAddress, once per device, not a stream operation); call it once per device at set-up, before
+ * any capture - tpc_slice_frames_static does it itself on its first call on a device otherwise.
+ * Every call on a device shares the one array, which keeps the last call's contents: nothing in it has to
+ * start at zero (the count kernel writes every entry a call reads), but two calls that overlap on the GPU
+ * (different streams, or graphs replayed side by side) race on it - keep them in stream order.
+ * Asynchronous on cuda_stream. */
+#define TPC_SLICE_STATIC_MAX_ENTRIES (1u << 20)
+int tpc_slice_static_setup(void);
+int tpc_slice_frames_static(const float* y, const float* zeta, const uint32_t* row_offsets_in, uint32_t n_clusters,
+                            uint32_t n_tasks_in, int32_t n_sectors, int32_t n_rows, float slice_len, int32_t n_slices,
+                            float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out,
+                            void* cuda_stream);
+
 /* ---- ITS standalone tracker -----------------------------------------------
  * PAPER.md L156-160 (section 4.2): from the clusters of the 6 ITS layers and the primary vertex, "pairs of
  * SPD clusters seen under nearly the same angle from the vertex point" seed a Kalman filter "propagated

@@ -152,6 +152,11 @@ def load_library():
     lib.tpc_its_last_error.argtypes = [vp]
     lib.tpc_slice_workspace_bytes.restype = C.c_size_t
     lib.tpc_slice_workspace_bytes.argtypes = [C.c_uint32, C.c_int32, C.c_int32]
+    lib.tpc_slice_static_setup.restype = C.c_int
+    lib.tpc_slice_static_setup.argtypes = []
+    lib.tpc_slice_frames_static.restype = C.c_int
+    lib.tpc_slice_frames_static.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, C.c_int32, C.c_int32, C.c_float, C.c_int32,
+                                            vp, vp, vp, vp, vp]
     lib.tpc_slice_frames.restype = C.c_int
     lib.tpc_slice_frames.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, C.c_int32, C.c_int32, C.c_float, C.c_int32,
                                      vp, vp, vp, vp, vp, C.c_size_t, vp]
@@ -510,6 +515,41 @@ def slice_frames(y, zeta, row_offsets, n_tasks_in: int, n_sectors: int, n_rows: 
         raise TpcError(f"tpc_slice_frames failed ({rc}): {lib.tpc_last_error(None).decode()}")
     slice_frames._keep = ws  # the workspace must outlive the asynchronous kernels
     return y_out, z_out, src[:n], ro_out
+
+
+SLICE_STATIC_MAX_ENTRIES = 1 << 20  # include/tpc_tracker.h: TPC_SLICE_STATIC_MAX_ENTRIES
+
+
+def slice_static_setup():
+    """tpc_slice_static_setup for the current CUDA device (once per device, at set-up)."""
+    lib = load_library()
+    rc = lib.tpc_slice_static_setup()
+    if rc != 0:
+        raise TpcError(f"tpc_slice_static_setup failed ({rc}): {lib.tpc_last_error(None).decode()}")
+
+
+def slice_frames_static(y, zeta, row_offsets, n_tasks_in: int, n_sectors: int, n_rows: int, slice_len: float,
+                        n_slices: int, y_out, z_out, src_index, row_offsets_out, stream=None):
+    """tpc_slice_frames_static on DEVICE tensors the caller owns (inputs and outputs): the library allocates
+    nothing, its scratch is a static device array shared by all calls on the device (calls that overlap on the
+    GPU race).  Sizes beyond TPC_SLICE_STATIC_MAX_ENTRIES raise.  Asynchronous."""
+    import torch
+    lib = load_library()
+    for t in (y, zeta, row_offsets, y_out, z_out, src_index, row_offsets_out):
+        if not t.is_cuda:
+            raise TpcError("slice_frames_static needs CUDA tensors; there is no CPU path")
+    n = int(y.numel())
+    if int(y_out.numel()) < n or int(z_out.numel()) < n or int(src_index.numel()) < n or \
+            int(row_offsets_out.numel()) < n_tasks_in * n_slices * n_rows + 1:
+        raise TpcError("slice_frames_static: an output tensor is too small")
+    s = stream if stream is not None else torch.cuda.current_stream(y.device)
+    with torch.cuda.device(y.device):
+        rc = lib.tpc_slice_frames_static(y.data_ptr(), zeta.data_ptr(), row_offsets.data_ptr(), n, int(n_tasks_in),
+                                         int(n_sectors), int(n_rows), float(slice_len), int(n_slices),
+                                         y_out.data_ptr(), z_out.data_ptr(), src_index.data_ptr(),
+                                         row_offsets_out.data_ptr(), _stream_ptr(s))
+    if rc != 0:
+        raise TpcError(f"tpc_slice_frames_static failed ({rc}): {lib.tpc_last_error(None).decode()}")
 
 
 class ItsTracker:

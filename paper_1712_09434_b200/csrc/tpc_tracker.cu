@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1073,6 +1074,78 @@ int tpc_slice_frames(const float* y, const float* zeta, const uint32_t* row_offs
   if (blocks) k_slice_scatter<<<blocks, kSliceThreads, 0, s>>>(c);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(nullptr, TPC_ERR_CUDA, "tpc_slice_frames: CUDA launch: %s", cudaGetErrorString(e));
+  return TPC_OK;
+}
+
+// ---- frame slicer without caller scratch (include/tpc_tracker.h: tpc_slice_frames_static) -------------------
+// The counts of the output rows live in this array.  In host code its NAME is a host-side stand-in, not a
+// device address: the kernels get the address cudaGetSymbolAddress returns for the current device, resolved
+// once per device (tpc_slice_static_setup) and kept in g_slice_static_ptr.
+static __device__ __align__(256) uint32_t g_slice_static_counts[TPC_SLICE_STATIC_MAX_ENTRIES];
+namespace {
+constexpr int kSliceStaticMaxDevices = 64;
+uint32_t* g_slice_static_ptr[kSliceStaticMaxDevices] = {nullptr};
+std::mutex g_slice_static_mutex;
+
+// Device address of g_slice_static_counts on the current device, or nullptr (error text set).
+uint32_t* slice_static_address() {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    fail(nullptr, TPC_ERR_CUDA, "tpc_slice_static_setup: cudaGetDevice: %s", cudaGetErrorString(e));
+    return nullptr;
+  }
+  if (dev < 0 || dev >= kSliceStaticMaxDevices) {
+    fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_static_setup: device %d, at most %d are supported", dev, kSliceStaticMaxDevices);
+    return nullptr;
+  }
+  std::lock_guard<std::mutex> lock(g_slice_static_mutex);
+  if (!g_slice_static_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_slice_static_counts);
+    if (e != cudaSuccess || !p) {
+      fail(nullptr, TPC_ERR_CUDA, "tpc_slice_static_setup: cudaGetSymbolAddress on device %d: %s", dev,
+           cudaGetErrorString(e));
+      cudaGetLastError();
+      return nullptr;
+    }
+    g_slice_static_ptr[dev] = (uint32_t*)p;
+  }
+  return g_slice_static_ptr[dev];
+}
+}  // namespace
+
+int tpc_slice_static_setup(void) { return slice_static_address() ? TPC_OK : TPC_ERR_CUDA; }
+
+int tpc_slice_frames_static(const float* y, const float* zeta, const uint32_t* row_offsets_in, uint32_t n_clusters,
+                            uint32_t n_tasks_in, int32_t n_sectors, int32_t n_rows, float slice_len, int32_t n_slices,
+                            float* y_out, float* z_out, uint32_t* src_index, uint32_t* row_offsets_out,
+                            void* cuda_stream) {
+  if (!row_offsets_in || !row_offsets_out || (n_clusters && (!y || !zeta || !y_out || !z_out || !src_index)))
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_frames_static: NULL argument");
+  if (n_sectors < 1 || n_rows < 1 || n_slices < 1 || n_slices > kMaxSlices || !(slice_len > 0.f) || n_tasks_in % (uint32_t)n_sectors != 0u)
+    return fail(nullptr, TPC_ERR_ARGUMENT, "tpc_slice_frames_static: need n_sectors, n_rows >= 1, 1 <= n_slices <= %d, slice_len > 0, whole frames", kMaxSlices);
+  const uint64_t entries = (uint64_t)n_tasks_in * (uint64_t)n_rows * (uint64_t)n_slices + 2u;
+  if (entries > (uint64_t)TPC_SLICE_STATIC_MAX_ENTRIES)
+    return fail(nullptr, TPC_ERR_WORKSPACE,
+                "tpc_slice_frames_static: n_tasks_in*n_rows*n_slices + 2 = %llu entries of scratch, the static array "
+                "holds %u: slice fewer frames per call or use tpc_slice_frames with a workspace",
+                (unsigned long long)entries, (unsigned)TPC_SLICE_STATIC_MAX_ENTRIES);
+  uint32_t* counts = slice_static_address();
+  if (!counts) return TPC_ERR_CUDA;
+  SliceCtx c{};
+  c.y = y; c.z = zeta; c.row_off_in = row_offsets_in; c.n = n_clusters; c.n_tr_in = n_tasks_in * (uint32_t)n_rows;
+  c.n_sectors = n_sectors; c.n_rows = n_rows; c.n_slices = n_slices;
+  c.inv_len = 1.0f / slice_len;
+  c.y_out = y_out; c.z_out = z_out; c.src_index = src_index; c.row_off_out = row_offsets_out;
+  c.counts = counts;  // every entry a call reads is written by its k_slice_count first: nothing to clear
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const unsigned blocks = (c.n_tr_in + kSliceThreads / 32 - 1) / (kSliceThreads / 32);
+  if (blocks) k_slice_count<<<blocks, kSliceThreads, 0, s>>>(c);
+  k_slice_scan<<<1, 1024, 0, s>>>(c);
+  if (blocks) k_slice_scatter<<<blocks, kSliceThreads, 0, s>>>(c);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, TPC_ERR_CUDA, "tpc_slice_frames_static: CUDA launch: %s", cudaGetErrorString(e));
   return TPC_OK;
 }
 
