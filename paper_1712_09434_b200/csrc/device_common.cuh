@@ -115,13 +115,13 @@ struct Ctx {
 #define TPC_STAGGER_CHAIN 160
 #endif
 #ifndef TPC_STAGGER_UP
-#define TPC_STAGGER_UP 256
+#define TPC_STAGGER_UP 350
 #endif
 #ifndef TPC_STAGGER_REFIT
 #define TPC_STAGGER_REFIT 316
 #endif
 #ifndef TPC_STAGGER_FINISH
-#define TPC_STAGGER_FINISH 200
+#define TPC_STAGGER_FINISH 256
 #endif
 __host__ __device__ constexpr uint32_t stagger_of(int kind) {
   return kind == 0 ? TPC_STAGGER_CHAIN : kind == 1 ? TPC_STAGGER_UP : kind == 2 ? TPC_STAGGER_REFIT : TPC_STAGGER_FINISH;

@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(kMergeThreads, kMergeRefitBlocksPerSm) k_merge
   float2 p_cur = make_float2(0.0f, 0.0f);
   bool fit = false;                     // the refit is still running (F2 has not stopped)
   int st = LN_IDLE;
-  TicketPool pool{0u, 0u, 0u};
+  TicketPool pool{0u, 0u};
   auto kept = [](uint32_t e) { return e != kNoHit && (e & kOwnedBit) != 0u; };
   auto open_segment = [&](int32_t seg) {  // rows and map of sector track `seg`, its outermost row first
     const uint32_t rows = c.out_rows[seg];

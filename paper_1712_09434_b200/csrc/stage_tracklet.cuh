@@ -290,42 +290,83 @@ __device__ __forceinline__ void load_rec(const float4* rec, TrackState& S, int& 
 }
 
 // ---- the queue of a tracklet kernel -------------------------------------------------------------------
-// Tickets are drawn kPoolBatch at a time per warp (one atomic per batch instead of one per fetch); the
-// lanes in `need` get consecutive tickets.  A ticket >= the number of tracklets means the queue is empty.
 // Ticket k stands for tracklet perm[k] (Ctx::trk_perm, the queue order built in front of every kernel, below).
-// A batch is 32 aligned tickets; lane j of the warp loads perm[] of ticket base + j when the batch is
-// drawn and hands it out by shuffle, so no fetch waits for a dependent load of its own.
-constexpr uint32_t kPoolBatch = 32;
-struct TicketPool { uint32_t next, end, perm; };
-__device__ __forceinline__ uint32_t pool_take(TicketPool& p, uint32_t* head, const uint32_t* __restrict__ perm,
-                                              uint32_t n_trk, unsigned need, int lane, uint32_t& t_out) {
-  const uint32_t cnt = (uint32_t)__popc(need), have = p.end - p.next;
-  const uint32_t rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
-  const uint32_t tk_old = p.next + rank;
-  const uint32_t t_old = __shfl_sync(0xffffffffu, p.perm, (int)(tk_old & 31u));
-  if (cnt <= have) {
-    p.next += cnt;
-    t_out = t_old;
-    return tk_old;
-  }
+// The order only does its work if a ticket is STARTED soon after it is drawn: a warp that drew 32 tickets at a
+// time would sit on them for about 50 row steps (its lanes end 0.6 tracklets per step) and start them up to 50
+// rows behind the wavefront they belong to.  So a warp keeps a small reserve, half a batch to one and a half batches of
+// tickets in the registers of its lanes (lane j holds entry j of a ring of 32), and refills it in two steps that
+// nobody waits for: iteration i asks for the next batch of tickets (one atomic, lane 0); iteration i + 1
+// loads their perm[] entries into the ring; from iteration i + 2 on they are handed out by shuffle.  A lane that
+// finds the reserve empty stays idle for an iteration.  A ticket >= the number of tracklets becomes kQueueEnd.
+// Batch per kernel (0 chain fit ... 3 rest of the down pass): what its lanes draw in about three iterations - the
+// chain fit, whose tracklets live for 26 steps, starves on small batches; the reserve is refilled below half a batch.
+#ifndef TPC_QUEUE_BATCH0
+#define TPC_QUEUE_BATCH0 16
+#endif
+#ifndef TPC_QUEUE_BATCH1
+#define TPC_QUEUE_BATCH1 8
+#endif
+#ifndef TPC_QUEUE_BATCH2
+#define TPC_QUEUE_BATCH2 8
+#endif
+#ifndef TPC_QUEUE_BATCH3
+#define TPC_QUEUE_BATCH3 8
+#endif
+__host__ __device__ constexpr uint32_t queue_batch_of(int kind) {
+  return kind == 0 ? TPC_QUEUE_BATCH0 : kind == 1 ? TPC_QUEUE_BATCH1 : kind == 2 ? TPC_QUEUE_BATCH2 : TPC_QUEUE_BATCH3;
+}
+constexpr uint32_t kQueueEnd = 0xFFFFFFFFu;
+struct TrackletQueue {
+  uint32_t perm;       // lane j: tracklet of ring entry j, or kQueueEnd
+  uint32_t head, cnt;  // entries head .. head + cnt - 1 (mod 32) are waiting        (the same in all lanes)
+  uint32_t base;       // lane 0: first ticket of the batch asked for in the last iteration
+  bool asked;          // such a batch exists                                        (the same in all lanes)
+};
+// Start of a kernel: the first 32 tickets of the warp at once.
+__device__ __forceinline__ void queue_open(TrackletQueue& q, uint32_t* head, const uint32_t* __restrict__ perm,
+                                           uint32_t n_trk, int lane) {
   uint32_t base = 0u;
-  if (lane == 0) base = atomicAdd(head, kPoolBatch);
+  if (lane == 0) base = atomicAdd(head, 32u);
   base = __shfl_sync(0xffffffffu, base, 0);
-  uint32_t np = 0u;
-  {
-    const uint32_t k = base + (uint32_t)lane;
-    if (k < n_trk) np = __ldg(perm + k);
+  const uint32_t k = base + (uint32_t)lane;
+  q.perm = k < n_trk ? __ldg(perm + k) : kQueueEnd;
+  q.head = 0u; q.cnt = 32u; q.base = 0u; q.asked = false;
+}
+// One call per loop iteration by the whole warp; `need`: the lanes that want a tracklet.  Returns true in a lane
+// that got one (t_out; kQueueEnd: the queue is empty).
+template <int KIND>
+__device__ __forceinline__ bool queue_step(TrackletQueue& q, uint32_t* head, const uint32_t* __restrict__ perm,
+                                           uint32_t n_trk, unsigned need, int lane, uint32_t& t_out) {
+  constexpr uint32_t kQueueBatch = queue_batch_of(KIND), kQueueLow = kQueueBatch / 2u;
+  static_assert(kQueueBatch + kQueueLow <= 32u && kQueueBatch >= 1u, "the ring has 32 entries");
+  const uint32_t n_need = (uint32_t)__popc(need), rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
+  const uint32_t n_give = min(n_need, q.cnt);
+  bool got = false;
+  if (n_give) {  // hand out (entries loaded in earlier iterations only: nothing waits for a load here)
+    t_out = __shfl_sync(0xffffffffu, q.perm, (int)((q.head + rank) & 31u));
+    got = ((need >> lane) & 1u) != 0u && rank < n_give;
+    q.head = (q.head + n_give) & 31u;
+    q.cnt -= n_give;
   }
-  const uint32_t tk_new = base + (rank - have);
-  const uint32_t t_new = __shfl_sync(0xffffffffu, np, (int)(tk_new & 31u));
-  p.perm = np;
-  p.next = base + (cnt - have);
-  p.end = base + kPoolBatch;
-  if (rank < have) { t_out = t_old; return tk_old; }
-  t_out = t_new;
-  return tk_new;
+  if (q.asked) {  // the batch asked for in the last iteration: its perm[] entries go behind the waiting ones
+    const uint32_t base = __shfl_sync(0xffffffffu, q.base, 0);
+    const uint32_t j = ((uint32_t)lane - (q.head + q.cnt)) & 31u;
+    if (j < kQueueBatch) {
+      const uint32_t k = base + j;
+      q.perm = k < n_trk ? __ldg(perm + k) : kQueueEnd;
+    }
+    q.cnt += kQueueBatch;
+    q.asked = false;
+  }
+  if (q.cnt <= kQueueLow) {  // ask for the next batch
+    if (lane == 0) q.base = atomicAdd(head, kQueueBatch);
+    q.asked = true;
+  }
+  return got;
 }
 // The same queue without a permutation (ticket k is item k): the merger's refit.
+constexpr uint32_t kPoolBatch = 32;
+struct TicketPool { uint32_t next, end; };
 __device__ __forceinline__ uint32_t pool_take_seq(TicketPool& p, uint32_t* head, unsigned need, int lane) {
   const uint32_t cnt = (uint32_t)__popc(need), have = p.end - p.next;
   const uint32_t rank = (uint32_t)__popc(need & ((1u << lane) - 1u));
@@ -358,11 +399,15 @@ __device__ __forceinline__ void prefetch_wait() { asm volatile("cp.async.wait_al
 __device__ unsigned long long g_probe_start[4];
 __device__ unsigned long long g_probe_exit[4][8192];
 __device__ __forceinline__ unsigned long long probe_now() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
+__device__ unsigned int g_wave_n;
+__device__ uint4 g_wave[1 << 18];
+#define TPC_PROBE_WAVE(task, row, t) if ((task) == 300u) { const unsigned int i_ = atomicAdd(&g_wave_n, 1u); if (i_ < (1u << 18)) { const unsigned long long n_ = probe_now(); g_wave[i_] = make_uint4((unsigned int)n_, (unsigned int)(n_ >> 32), (unsigned int)(row), (t)); } }
 #define TPC_PROBE_START(k) if (threadIdx.x == 0) atomicMin(&g_probe_start[k], probe_now());
 #define TPC_PROBE_EXIT(k) if ((threadIdx.x & 31) == 0) g_probe_exit[k][(blockIdx.x * blockDim.x + threadIdx.x) >> 5] = probe_now();
 #else
 #define TPC_PROBE_START(k)
 #define TPC_PROBE_EXIT(k)
+#define TPC_PROBE_WAVE(task, row, t)
 #endif
 enum LaneState { LN_IDLE = 0, LN_RUN = 1, LN_EXIT = 2 };
 enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };  // ISSUED this iteration, READY from the next on
@@ -372,15 +417,15 @@ enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };
 //                  requested draw a ticket and start the copy of that tracklet's record to their slot;
 //   (the kernel's own "consume" block turns an idle lane with a READY slot into a running one);
 //   fetch_advance: ISSUED -> READY at the end of the iteration.
-__device__ __forceinline__ void fetch_request(TicketPool& pool, uint32_t* head, const uint32_t* perm, bool want, int lane,
+template <int KIND>
+__device__ __forceinline__ void fetch_request(TrackletQueue& q, uint32_t* head, const uint32_t* perm, bool want, int lane,
                                               uint32_t n_trk, int& pf, uint32_t& t_next, void* slot, const void* src_base,
                                               size_t src_stride, int n16) {
   const unsigned need = __ballot_sync(0xffffffffu, want);
-  if (need) {
+  if (need || q.asked) {
     uint32_t t = 0u;
-    const uint32_t tk = pool_take(pool, head, perm, n_trk, need, lane, t);
-    if (want) {
-      if (tk >= n_trk) {
+    if (queue_step<KIND>(q, head, perm, n_trk, need, lane, t)) {
+      if (t == kQueueEnd) {
         pf = PF_DRAINED;
       } else {
         t_next = t;
@@ -569,10 +614,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
   int32_t h_cur = -1, h_next = -1, h_last = -1;  // chain hit of the next step, the one after it, the last one fitted
   float2 p_cur = make_float2(0.0f, 0.0f);
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u, 0u};
+  TrackletQueue pool;
+  queue_open(pool, &c.tickets[2], c.trk_perm, n_trk, lane);
   uint32_t n_steps = 0u, n_chain = 0u;
   while (true) {
-    fetch_request(pool, &c.tickets[2], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && h_next < 0)) && pf == PF_NONE,
+    fetch_request<0>(pool, &c.tickets[2], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && h_next < 0)) && pf == PF_NONE,
                          lane, n_trk, pf, t_next, slot, c.trk_seed, sizeof(uint4) * kSeedU4, kChainSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
@@ -666,11 +712,12 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
   int32_t last_hit = -1;
   bool turn = false;  // this lane's next step is the turn-around (its last step here)
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u, 0u};
+  TrackletQueue pool;
+  queue_open(pool, &c.tickets[3], c.trk_perm, n_trk, lane);
   uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u;
   while (true) {
     if (st == LN_RUN && row_cur + 1 >= n_rows) turn = true;            // K3 ran off the last row
-    fetch_request(pool, &c.tickets[3], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && turn)) && pf == PF_NONE, lane,
+    fetch_request<1>(pool, &c.tickets[3], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && turn)) && pf == PF_NONE, lane,
                          n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
@@ -727,6 +774,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     __syncwarp();
     if (do_search) {
       if (COUNT) ++n_search;
+      TPC_PROBE_WAVE(tr_base / (uint32_t)n_rows, rt, t)
       hit = search_row<COUNT>(c, S, g, hp, n_cand);
     }
     __syncwarp();
@@ -783,10 +831,11 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
   uint32_t m_cur = kNoHit, m_next = kNoHit;  // map[r_down], map[r_down - 1]
   float2 p_cur = make_float2(0.0f, 0.0f);
   int st = LN_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u, 0u};
+  TrackletQueue pool;
+  queue_open(pool, &c.tickets[4], c.trk_perm, n_trk, lane);
   uint32_t n_steps = 0u;
   while (true) {
-    fetch_request(pool, &c.tickets[4], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && m_next == kNoHit)) && pf == PF_NONE,
+    fetch_request<2>(pool, &c.tickets[4], c.trk_perm, (st == LN_IDLE || (st == LN_RUN && m_next == kNoHit)) && pf == PF_NONE,
                          lane, n_trk, pf, t_next, slot, c.trk_rec, sizeof(float4) * kRecFloat4, kRecSlot16);
     if (st == LN_IDLE) {
       if (pf == PF_READY) {
@@ -863,7 +912,8 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
   int r0 = 0, row_cur = 0, first_row = 0, last_row = 0, n_hits = 0, gap = 0, r_down = 0;
   uint32_t map_next = kNoHit;  // map[r_down], loaded one step ahead
   int phase = PH_IDLE, pf = PF_NONE;
-  TicketPool pool{0u, 0u, 0u};
+  TrackletQueue pool;
+  queue_open(pool, &c.tickets[5], c.trk_perm, n_trk, lane);
   uint32_t n_steps = 0u, n_search = 0u, n_cand = 0u, n_kept = 0u, n_kept_hits = 0u;
   while (true) {
     // (A) tracklets that ended in the last step: the record, and what the ownership kernel (K7) needs
@@ -877,11 +927,10 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
     {
       const bool want = (phase == PH_IDLE || phase == PH_FINISH || (phase == PH_DOWN && r_down < 0)) && pf == PF_NONE;
       const unsigned need = __ballot_sync(FULL, want);
-      if (need) {
+      if (need || pool.asked) {
         uint32_t tn = 0u;
-        const uint32_t tk = pool_take(pool, &c.tickets[5], c.trk_perm, n_trk, need, lane, tn);
-        if (want) {
-          if (tk >= n_trk) {
+        if (queue_step<3>(pool, &c.tickets[5], c.trk_perm, n_trk, need, lane, tn)) {
+          if (tn == kQueueEnd) {
             pf = PF_DRAINED;
           } else {
             t_next = tn;

@@ -190,6 +190,17 @@ void tpc_probe_reset() {
   static unsigned long long z[4][8192];
   cudaMemcpyToSymbol(g_probe_exit, z, sizeof(z));
 }
+unsigned int tpc_probe_wave(unsigned int* out4, unsigned int cap) {
+  cudaDeviceSynchronize();
+  unsigned int n = 0;
+  cudaMemcpyFromSymbol(&n, g_wave_n, sizeof(n));
+  if (n > cap) n = cap;
+  if (n > (1u << 18)) n = 1u << 18;
+  cudaMemcpyFromSymbol(out4, g_wave, (size_t)n * 16);
+  unsigned int z = 0;
+  cudaMemcpyToSymbol(g_wave_n, &z, sizeof(z));
+  return n;
+}
 void tpc_probe_read(unsigned long long* start4, unsigned long long* exit4x8192) {
   cudaDeviceSynchronize();
   cudaMemcpyFromSymbol(start4, g_probe_start, 4 * sizeof(unsigned long long));
