@@ -95,7 +95,7 @@ struct Ctx {
   uint32_t* trk_kept;      // [max_tracklets] hits the tracklet keeps (L1), counted by k_resolve; cleared per call
   uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
   uint32_t* trk_perm;      // [max_tracklets] queue order of a5: ticket k stands for tracklet trk_perm[k] (k_order_*, stage_tracklet.cuh)
-  uint32_t* trk_key;       // [max_tracklets] diagonal of the tracklet in the queue order of the next a5 kernel (order_note)
+  uint32_t* trk_key;       // [max_tracklets] task << 10 | row where the next a5 kernel takes the tracklet up (order_note)
   uint32_t* order_cnt;     // [4 kernels][2][order_keys()] tracklets per diagonal of that order, then the slots handed out; cleared per call
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
@@ -110,48 +110,52 @@ struct Ctx {
 // ---- queue order of the tracklet constructor (a5); the kernels and the reasons are in stage_tracklet.cuh ----
 // Diagonal of a tracklet in front of kernel KIND (0 chain fit, 1 up pass, 2 refit, 3 rest of the down pass):
 //     d = (rows between the tracklet's next row and the row where that pass begins) + stagger * task
-// stagger in 1/256 rows per task.
-#ifndef TPC_STAGGER_CHAIN
-#define TPC_STAGGER_CHAIN 160
+// The lanes consume one diagonal per row step - every tracklet of a task then starts when the task's wavefront
+// passes its row - if a diagonal holds as many tracklets as the lanes end per step:
+//     (tracklets per task) / stagger = lanes / life      =>      stagger = (tracklets per task) * life / lanes
+// with `life` the row steps a lane spends on a tracklet in that kernel.  The tracklets per task are known on
+// the device only (k_order_* read the count); life is a property of the detector (how long tracks are in rows),
+// not of the occupancy: the values below are the ones that were fastest on central Pb-Pb-like events of the
+// 159-row geometry (a sweep; they are 1.0 - 1.4 times the mean steps per tracklet the device counters give:
+// 26, 53, 73 and 37).  Only speed depends on them.
+#ifndef TPC_LIFE_CHAIN
+#define TPC_LIFE_CHAIN 37.8f
 #endif
-#ifndef TPC_STAGGER_UP
-#define TPC_STAGGER_UP 350
+#ifndef TPC_LIFE_UP
+#define TPC_LIFE_UP 70.8f
 #endif
-#ifndef TPC_STAGGER_REFIT
-#define TPC_STAGGER_REFIT 316
+#ifndef TPC_LIFE_REFIT
+#define TPC_LIFE_REFIT 74.6f
 #endif
-#ifndef TPC_STAGGER_FINISH
-#define TPC_STAGGER_FINISH 256
+#ifndef TPC_LIFE_FINISH
+#define TPC_LIFE_FINISH 51.8f
 #endif
-__host__ __device__ constexpr uint32_t stagger_of(int kind) {
-  return kind == 0 ? TPC_STAGGER_CHAIN : kind == 1 ? TPC_STAGGER_UP : kind == 2 ? TPC_STAGGER_REFIT : TPC_STAGGER_FINISH;
+__host__ __device__ constexpr float order_life_of(int kind) {
+  return kind == 0 ? TPC_LIFE_CHAIN : kind == 1 ? TPC_LIFE_UP : kind == 2 ? TPC_LIFE_REFIT : TPC_LIFE_FINISH;
 }
-#ifndef TPC_STAGGER_MAX
-#define TPC_STAGGER_MAX 512
-#endif
-constexpr uint32_t kStaggerMax = TPC_STAGGER_MAX;  // bounds the diagonals: n_rows + n_tasks * kStaggerMax / 256
+constexpr uint32_t kStaggerMax = 512;  // stagger in 1/256 rows per task, at most 2 rows: bounds the diagonals
 __host__ __device__ inline uint32_t order_keys(uint32_t n_rows, uint32_t n_tasks) {
   return n_rows + ((n_tasks * kStaggerMax) >> 8) + 1u;
 }
-template <int KIND>
-__device__ __forceinline__ uint32_t order_key(const Ctx& c, uint32_t task, uint32_t row) {
-  static_assert(stagger_of(KIND) <= kStaggerMax, "order_keys() bounds the diagonals with kStaggerMax");
+// stagger (1/256 rows per task) of kernel `kind` run by `lanes` lanes on n_trk tracklets
+__device__ __forceinline__ uint32_t order_stagger(const Ctx& c, int kind, uint32_t lanes, uint32_t n_trk) {
+  const float per_task = (float)n_trk / (float)(c.n_tasks ? c.n_tasks : 1u);
+  const float s = per_task * order_life_of(kind) * 256.0f / (float)(lanes ? lanes : 1u);
+  return (uint32_t)fminf(fmaxf(s, 1.0f), (float)kStaggerMax);
+}
+// trk_key holds task << 10 | row (n_rows <= 1024); the diagonal of that entry
+__device__ __forceinline__ uint32_t order_diagonal(const Ctx& c, uint32_t key, uint32_t stagger) {
+  const uint32_t task = key >> 10, row = key & 1023u;
   // The last n_rows / stagger tasks share one offset, so that the diagonals stay as long as they were down to the
   // last one (a diagonal of staggered tasks alone would thin out, the queue would run ahead of the lanes, and the
   // device would wait for the long tracklets of the last task).
-#ifdef TPC_ORDER_LAST
-  const uint32_t n_last = TPC_ORDER_LAST;
-#else
-  const uint32_t n_last = ((uint32_t)c.n_rows * 256u) / stagger_of(KIND);
-#endif
+  const uint32_t n_last = ((uint32_t)c.n_rows * 256u) / stagger;
   const uint32_t n_stag = c.n_tasks > n_last ? c.n_tasks - n_last : 0u;
-  return row + ((min(task, n_stag) * stagger_of(KIND)) >> 8);
+  return row + ((min(task, n_stag) * stagger) >> 8);
 }
-// Called by the kernel in front of kernel KIND when it has finished tracklet t: notes the diagonal and counts it.
-template <int KIND>
+// Called by the kernel in front of an a5 kernel when it has finished tracklet t: where its next pass begins.
 __device__ __forceinline__ void order_note(const Ctx& c, uint32_t t, uint32_t task, uint32_t row) {
-  const uint32_t key = order_key<KIND>(c, task, row);
-  c.trk_key[t] = key;
+  c.trk_key[t] = (task << 10) | row;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -395,20 +395,6 @@ __device__ __forceinline__ void prefetch_slot(void* slot, const void* src, int n
 }
 __device__ __forceinline__ void prefetch_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-#ifdef TPC_TAIL_PROBE
-__device__ unsigned long long g_probe_start[4];
-__device__ unsigned long long g_probe_exit[4][8192];
-__device__ __forceinline__ unsigned long long probe_now() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
-__device__ unsigned int g_wave_n;
-__device__ uint4 g_wave[1 << 18];
-#define TPC_PROBE_WAVE(task, row, t) if ((task) == 300u) { const unsigned int i_ = atomicAdd(&g_wave_n, 1u); if (i_ < (1u << 18)) { const unsigned long long n_ = probe_now(); g_wave[i_] = make_uint4((unsigned int)n_, (unsigned int)(n_ >> 32), (unsigned int)(row), (t)); } }
-#define TPC_PROBE_START(k) if (threadIdx.x == 0) atomicMin(&g_probe_start[k], probe_now());
-#define TPC_PROBE_EXIT(k) if ((threadIdx.x & 31) == 0) g_probe_exit[k][(blockIdx.x * blockDim.x + threadIdx.x) >> 5] = probe_now();
-#else
-#define TPC_PROBE_START(k)
-#define TPC_PROBE_EXIT(k)
-#define TPC_PROBE_WAVE(task, row, t)
-#endif
 enum LaneState { LN_IDLE = 0, LN_RUN = 1, LN_EXIT = 2 };
 enum PrefetchState { PF_NONE = 0, PF_ISSUED = 1, PF_READY = 2, PF_DRAINED = 3 };  // ISSUED this iteration, READY from the next on
 
@@ -462,11 +448,12 @@ __host__ __device__ inline size_t trk_smem_bytes(int n_rows, int slot16) {
 // the others of that task reach their row: every task is swept by a wavefront a few rows wide, the tasks
 // one after the other `stagger` rows apart, and a grid row is read by all its tracklets while it is in
 // the L2.  The last diagonals hold the last rows of the last tasks only: short tracklets, no tail.
-// stagger (1/256 rows per task) = tracklets a task starts per row / tracklets the lanes draw per step.
-// A counting sort by d: the kernel that finishes a tracklet in front of this one notes its diagonal and
-// counts it (order_note, device_common.cuh), k_order_scan turns the counts into the first slot of every
-// diagonal (one block), k_order_fill hands the slots out.  The order inside a diagonal is what the atomics
-// give; it only decides which lane follows which tracklet - the result does not depend on it.
+// The stagger follows from the tracklets per task and the lanes of the kernel (order_stagger, device_common.cuh).
+// A counting sort by d: the kernel that finishes a tracklet in front of this one notes the task and the row
+// where its next pass begins (order_note), k_order_count counts the tracklets of every diagonal, k_order_scan
+// turns the counts into the first slot of every diagonal (one block), k_order_fill hands the slots out.  The
+// order inside a diagonal is what the atomics give; it only decides which lane follows which tracklet - the
+// result does not depend on it.  With no more tracklets than lanes the order is the identity.
 // ---------------------------------------------------------------------------
 constexpr int kOrderThreads = 256;
 // One block per chunk of kOrderChunk consecutive tracklets (one or two tasks: a few hundred diagonals next to
@@ -476,12 +463,13 @@ constexpr int kOrderThreads = 256;
 constexpr int kOrderItems = 8;
 constexpr uint32_t kOrderChunk = kOrderThreads * kOrderItems;
 constexpr uint32_t kOrderWindow = 2048;
-__global__ void __launch_bounds__(kOrderThreads) k_order_count(const Ctx c, int kind) {
+__global__ void __launch_bounds__(kOrderThreads) k_order_count(const Ctx c, int kind, uint32_t lanes) {
   __shared__ uint32_t s_cnt[kOrderWindow];
   __shared__ uint32_t s_min;
   constexpr uint32_t kNone = 0xFFFFFFFFu;
   const uint32_t n_trk = *c.n_tracklets, n_keys = order_keys((uint32_t)c.n_rows, c.n_tasks);
   uint32_t* cnt = c.order_cnt + (size_t)(2 * kind) * n_keys;
+  const uint32_t stagger = order_stagger(c, kind, lanes, n_trk);
   for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) s_cnt[k] = 0u;
   for (uint32_t t0 = blockIdx.x * kOrderChunk; t0 < n_trk; t0 += gridDim.x * kOrderChunk) {
     if (threadIdx.x == 0) s_min = kNone;
@@ -491,7 +479,7 @@ __global__ void __launch_bounds__(kOrderThreads) k_order_count(const Ctx c, int 
 #pragma unroll
     for (int i = 0; i < kOrderItems; ++i) {
       const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
-      key[i] = t < n_trk ? c.trk_key[t] : kNone;
+      key[i] = t < n_trk ? order_diagonal(c, c.trk_key[t], stagger) : kNone;
       kmin = min(kmin, key[i]);
     }
 #pragma unroll
@@ -513,12 +501,17 @@ __global__ void __launch_bounds__(kOrderThreads) k_order_count(const Ctx c, int 
     __syncthreads();
   }
 }
-__global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int kind) {
+__global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int kind, uint32_t lanes) {
   __shared__ uint32_t s_cnt[kOrderWindow];
   __shared__ uint32_t s_min;
   constexpr uint32_t kNone = 0xFFFFFFFFu;
   const uint32_t n_trk = *c.n_tracklets, n_keys = order_keys((uint32_t)c.n_rows, c.n_tasks);
   uint32_t* cursor = c.order_cnt + (size_t)(2 * kind + 1) * n_keys;
+  const uint32_t stagger = order_stagger(c, kind, lanes, n_trk);
+  if (n_trk <= lanes) {  // every tracklet starts at once whatever the order: keep the neighbours in (task, row, bin) together
+    for (uint32_t t = blockIdx.x * kOrderThreads + threadIdx.x; t < n_trk; t += gridDim.x * kOrderThreads) c.trk_perm[t] = t;
+    return;
+  }
   for (uint32_t k = threadIdx.x; k < kOrderWindow; k += kOrderThreads) s_cnt[k] = 0u;
   for (uint32_t t0 = blockIdx.x * kOrderChunk; t0 < n_trk; t0 += gridDim.x * kOrderChunk) {
     if (threadIdx.x == 0) s_min = kNone;
@@ -528,7 +521,7 @@ __global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int k
 #pragma unroll
     for (int i = 0; i < kOrderItems; ++i) {
       const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
-      key[i] = t < n_trk ? c.trk_key[t] : kNone;
+      key[i] = t < n_trk ? order_diagonal(c, c.trk_key[t], stagger) : kNone;
       kmin = min(kmin, key[i]);
     }
 #pragma unroll
@@ -543,11 +536,7 @@ __global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int k
       if (key[i] - kmin < kOrderWindow) {
         rank[i] = atomicAdd(&s_cnt[key[i] - kmin], 1u);
       } else {  // beyond the window: straight to global memory
-#ifdef TPC_IDENTITY_ORDER
-        c.trk_perm[t0 + (uint32_t)i * kOrderThreads + threadIdx.x] = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
-#else
         c.trk_perm[atomicAdd(&cursor[key[i]], 1u)] = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
-#endif
         key[i] = kNone;
       }
     }
@@ -560,11 +549,7 @@ __global__ void __launch_bounds__(kOrderThreads) k_order_fill(const Ctx c, int k
 #pragma unroll
     for (int i = 0; i < kOrderItems; ++i) {
       const uint32_t t = t0 + (uint32_t)i * kOrderThreads + threadIdx.x;
-#ifdef TPC_IDENTITY_ORDER
-      if (key[i] != kNone) c.trk_perm[t] = t;
-#else
       if (key[i] != kNone) c.trk_perm[s_cnt[key[i] - kmin] + rank[i]] = t;
-#endif
     }
     __syncthreads();
 #pragma unroll
@@ -604,7 +589,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
-  TPC_PROBE_START(0)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   TrackState S;
   zero_state(S);
@@ -676,11 +660,10 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
     if (st == LN_RUN && (h_cur < 0 || !ok)) {  // end of the chain, or K2's failed transport (-> K4, no up pass)
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, r0, row_cur,
                 pack_rows(row_cur, row_cur - 1, r0, !ok), tr_base, (uint32_t)h_last, 0u);
-      order_note<1>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)row_cur);            // the up pass begins in this row
+      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)row_cur);            // the up pass begins in this row
       st = LN_IDLE;
     }
   }
-  TPC_PROBE_EXIT(0)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_CHAIN_HITS], (unsigned long long)n_chain);
@@ -701,7 +684,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
-  TPC_PROBE_START(1)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   const int max_gap = c.prm.max_row_gap;
   TrackState S;
@@ -774,7 +756,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     __syncwarp();
     if (do_search) {
       if (COUNT) ++n_search;
-      TPC_PROBE_WAVE(tr_base / (uint32_t)n_rows, rt, t)
       hit = search_row<COUNT>(c, S, g, hp, n_cand);
     }
     __syncwarp();
@@ -792,11 +773,10 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     if (p_turn) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, last_row - 1, r0, false), tr_base, ia, ib);
-      order_note<2>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - last_row));  // the refit comes down from lastRow
+      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - last_row));  // the refit comes down from lastRow
       st = LN_IDLE;
     }
   }
-  TPC_PROBE_EXIT(1)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);
@@ -821,7 +801,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
-  TPC_PROBE_START(2)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   TrackState S;
   zero_state(S);
@@ -873,11 +852,10 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
     if (st == LN_RUN && (m_cur == kNoHit || !ok)) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, r_down, r0, false), tr_base, m_cur, 0u);
-      order_note<3>(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - (r_down > 0 ? r_down : 0)));  // goes on from r_down
+      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - (r_down > 0 ? r_down : 0)));  // goes on from r_down
       st = LN_IDLE;
     }
   }
-  TPC_PROBE_EXIT(2)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_REFIT_STEPS], (unsigned long long)n_steps);
@@ -901,7 +879,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
   for (int r = (int)threadIdx.x; r < n_rows; r += (int)blockDim.x) sX[r] = c.X[r];
   __syncthreads();
   const uint32_t n_trk = *c.n_tracklets;
-  TPC_PROBE_START(3)
   const float a = c.a, max_sin = c.prm.max_sinphi, sy2 = c.sy2, sz2 = c.sz2;
   const int max_gap = c.prm.max_row_gap;
   [[maybe_unused]] const int min_hits = c.prm.min_track_hits;
@@ -1007,7 +984,6 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_fi
       --r_down;
     }
   }
-  TPC_PROBE_EXIT(3)
   if (COUNT) {
     atomicAdd(&c.counters[CN_ROW_STEPS], (unsigned long long)n_steps);
     atomicAdd(&c.counters[CN_SEARCHES], (unsigned long long)n_search);

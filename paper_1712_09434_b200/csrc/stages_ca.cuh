@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
     uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
     {
       const uint32_t task = tr0 / (uint32_t)c.n_rows;
-      order_note<0>(c, (uint32_t)pos, task, tr0 - task * (uint32_t)c.n_rows);  // queue order of the chain fit
+      order_note(c, (uint32_t)pos, task, tr0 - task * (uint32_t)c.n_rows);  // queue order of the chain fit
     }
     rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2);
     rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));

@@ -183,31 +183,6 @@ Ctx make_ctx(const tpc_tracker* t, const tpc_clusters* in, const tpc_tracks* out
 
 extern "C" {
 
-#ifdef TPC_TAIL_PROBE
-void tpc_probe_reset() {
-  unsigned long long big[4] = {~0ull, ~0ull, ~0ull, ~0ull};
-  cudaMemcpyToSymbol(g_probe_start, big, sizeof(big));
-  static unsigned long long z[4][8192];
-  cudaMemcpyToSymbol(g_probe_exit, z, sizeof(z));
-}
-unsigned int tpc_probe_wave(unsigned int* out4, unsigned int cap) {
-  cudaDeviceSynchronize();
-  unsigned int n = 0;
-  cudaMemcpyFromSymbol(&n, g_wave_n, sizeof(n));
-  if (n > cap) n = cap;
-  if (n > (1u << 18)) n = 1u << 18;
-  cudaMemcpyFromSymbol(out4, g_wave, (size_t)n * 16);
-  unsigned int z = 0;
-  cudaMemcpyToSymbol(g_wave_n, &z, sizeof(z));
-  return n;
-}
-void tpc_probe_read(unsigned long long* start4, unsigned long long* exit4x8192) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(start4, g_probe_start, 4 * sizeof(unsigned long long));
-  cudaMemcpyFromSymbol(exit4x8192, g_probe_exit, 4 * 8192 * sizeof(unsigned long long));
-}
-#endif
-
 void tpc_default_params(tpc_params* out) {
   if (out) default_params(out);
 }
@@ -470,10 +445,13 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   mark();
   // a5: four persistent kernels, each with as many blocks as the device holds at once and its own queue order
   const int og = 4 * t->n_sm;
-#define TPC_ORDER(KIND)                                     \
-  k_order_count<<<og, kOrderThreads, 0, s>>>(c, KIND); \
-  k_order_scan<<<1, 1024, 0, s>>>(c, KIND);         \
-  k_order_fill<<<og, kOrderThreads, 0, s>>>(c, KIND);
+#define TPC_ORDER(KIND)                                                                                \
+  {                                                                                                    \
+    const uint32_t lanes = (uint32_t)t->trk_grid[KIND][cnt ? 1 : 0] * (uint32_t)kTrackletThreads;      \
+    k_order_count<<<og, kOrderThreads, 0, s>>>(c, KIND, lanes);                                        \
+    k_order_scan<<<1, 1024, 0, s>>>(c, KIND);                                                          \
+    k_order_fill<<<og, kOrderThreads, 0, s>>>(c, KIND, lanes);                                         \
+  }
   TPC_ORDER(0)
   if (cnt) k_trk_chain<true><<<t->trk_grid[0][1], kTrackletThreads, t->trk_smem[0], s>>>(c);
   else k_trk_chain<false><<<t->trk_grid[0][0], kTrackletThreads, t->trk_smem[0], s>>>(c);
