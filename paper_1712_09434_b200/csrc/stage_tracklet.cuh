@@ -298,19 +298,20 @@ __device__ __forceinline__ void load_rec(const float4* rec, TrackState& S, int& 
 // nobody waits for: iteration i asks for the next batch of tickets (one atomic, lane 0); iteration i + 1
 // loads their perm[] entries into the ring; from iteration i + 2 on they are handed out by shuffle.  A lane that
 // finds the reserve empty stays idle for an iteration.  A ticket >= the number of tracklets becomes kQueueEnd.
-// Batch per kernel (0 chain fit ... 3 rest of the down pass): what its lanes draw in about three iterations - the
-// chain fit, whose tracklets live for 26 steps, starves on small batches; the reserve is refilled below half a batch.
+// Batch per kernel (0 chain fit ... 3 rest of the down pass), from a sweep on 16 central events: the searching kernels
+// want the tightest wavefront (4; 2 starves the lanes, 8 and 16 are 3 % and 7 % slower), the chain fit, whose
+// tracklets live for 26 steps only, starves below 16.  The reserve is refilled below half a batch.
 #ifndef TPC_QUEUE_BATCH0
 #define TPC_QUEUE_BATCH0 16
 #endif
 #ifndef TPC_QUEUE_BATCH1
-#define TPC_QUEUE_BATCH1 8
+#define TPC_QUEUE_BATCH1 4
 #endif
 #ifndef TPC_QUEUE_BATCH2
 #define TPC_QUEUE_BATCH2 8
 #endif
 #ifndef TPC_QUEUE_BATCH3
-#define TPC_QUEUE_BATCH3 8
+#define TPC_QUEUE_BATCH3 4
 #endif
 __host__ __device__ constexpr uint32_t queue_batch_of(int kind) {
   return kind == 0 ? TPC_QUEUE_BATCH0 : kind == 1 ? TPC_QUEUE_BATCH1 : kind == 2 ? TPC_QUEUE_BATCH2 : TPC_QUEUE_BATCH3;
