@@ -30,7 +30,7 @@ STAGE_OF = {"k_grid_build": "grid_build", "k_neighbours": "neighbour_finder", "k
             "k_seeds": "start_hits", "k_trk_chain": "tracklet_chain_fit", "k_trk_up": "tracklet_up_pass",
             "k_trk_refit": "tracklet_refit", "k_trk_finish": "tracklet_down_finish",
             "k_task_offsets": "ownership", "k_resolve": "ownership", "k_select_output": "selector_output",
-            "k_merge": "merger_refit"}
+            "k_order": "tracklet_queue_order", "k_merge": "merger_refit"}
 
 METRICS = {
     "dram_read": "dram__bytes_read.sum", "dram_write": "dram__bytes_write.sum",
