@@ -20,6 +20,9 @@ namespace tpc {
 #define TPC_NF_THREADS 128
 #endif
 constexpr int kNfThreads = TPC_NF_THREADS;
+#ifndef TPC_NF_MINBLOCKS
+#define TPC_NF_MINBLOCKS 5  // 5 blocks per SM is what the 43 KB of shared memory allow: up to 102 registers, no spill (without the bound ptxas stopped at 72 and spilled)
+#endif
 #ifndef TPC_NF_LIST
 #define TPC_NF_LIST 8
 #endif
@@ -89,9 +92,12 @@ __device__ __forceinline__ void for_window(const RowView& v, float ylo, float yh
 
 // The exact serial search of one cluster (N1..N5 as written, ties by gid): nested walk of both windows.
 // Used for the rare clusters the cooperative search cannot decide (chi2 ties, list overflow).
+// The views are passed BY VALUE and the result comes back in a register pair: nothing of the caller has its address
+// taken, so its row views and counters stay in registers (by reference they lived in local memory, and the hot loops
+// of every cluster re-read them from there).
 template <bool COUNT>
-__device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const RowView& vd, int row, float y,
-                                       float z, int32_t* out_up, int32_t* out_dn, unsigned long long* n_pairs) {
+__device__ __noinline__ uint2 nf_serial(const Ctx& c, const RowView vu, const RowView vd, int row, float y, float z,
+                                        unsigned long long* pairs_out) {
   const float HY = c.prm.nf_hy, HZ = c.prm.nf_hz, CHI_MAX = c.prm.nf_chi2_max, M = kGridMargin;
   const float b = c.dx_dn[row], a_ = c.dx_up[row];  // N4
   const float zu = z * c.ratio_up[row], zd = z * c.ratio_dn[row];  // N1
@@ -99,6 +105,7 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
   bool have = false;
   float best = 0.0f;
   uint32_t bu = 0u, bd = 0u;
+  unsigned long long n_pairs = 0ull;
   for_window(vu, (y - HY) - M, (y + HY) + M, (zu - HZ) - M, (zu + HZ) + M, [&](uint32_t u, float2 pu) {
     if (!(fabsf(pu.x - y) <= HY && fabsf(pu.y - zu) <= HZ)) return;  // N2
     const float ty = (pu.x - y) * b, tz = (pu.y - z) * b;
@@ -107,7 +114,7 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
       const float dy = ty - ((y - pd.x) * a_);  // N4
       const float dz = tz - ((z - pd.y) * a_);
       const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
-      if (COUNT) ++*n_pairs;
+      if (COUNT) ++n_pairs;
       if (!(chi < CHI_MAX)) return;  // N5: lexicographic (chi, gid_u, gid_d)
       bool take = !have || chi < best;
       if (have && chi == best) {
@@ -117,8 +124,8 @@ __device__ __noinline__ void nf_serial(const Ctx& c, const RowView& vu, const Ro
       if (take) { have = true; best = chi; bu = u; bd = d; }
     });
   });
-  *out_up = have ? (int32_t)bu : -1;
-  *out_dn = have ? (int32_t)bd : -1;
+  if (COUNT) *pairs_out += n_pairs;
+  return have ? make_uint2(bu, bd) : make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
 }
 
 // Window walk of one thread around (y, zc) (zc = the projected z of N1) in row view v: the clusters that
@@ -183,28 +190,32 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
     __syncwarp();
     const bool overflow = nd > (uint32_t)LIST || nu > (uint32_t)LIST;
     const uint32_t n_pr = overflow ? 0u : nu * nd;
-    const uint32_t magic = nd ? 65536u / nd + 1u : 0u;  // (k*magic) >> 16 == k / nd for k < 256, nd <= 16
     if (COUNT) n_pairs += n_pr;
     float best = CHI_MAX;  // N5: only chi < CHI_MAX is eligible
-    uint32_t bk = 0u;
+    uint32_t bu = 0u, bd = 0u;
     bool tie = false;
-    for (uint32_t k = 0u; k < n_pr; ++k) {
-      const uint32_t u = (k * magic) >> 16, d = k - u * nd;
+    for (uint32_t k = 0u, u = 0u, d = 0u; k < n_pr; ++k) {  // pair k = (u, d) = (k / nd, k % nd), counted along
       const float2 pu = u_p[u * kNfThreads], pd = d_p[d * kNfThreads];
       const float dy = pu.x - pd.x, dz = pu.y - pd.y;  // N4
       const float chi = ((dy * dy) * wy) + ((dz * dz) * wz);
       const bool lt = chi < best;
       tie |= chi == best;  // equal chi2 (or chi2 == CHI_MAX exactly): the gids decide (N5), left to the serial search
       best = lt ? chi : best;
-      bk = lt ? k : bk;
+      bu = lt ? u : bu;
+      bd = lt ? d : bd;
+      const bool wrap = d + 1u == nd;
+      d = wrap ? 0u : d + 1u;
+      u += wrap ? 1u : 0u;
     }
     const bool have = best < CHI_MAX;
-    const uint32_t bu = (bk * magic) >> 16, bd = bk - bu * nd;
     __syncwarp();
     if (act) {
       int32_t up = -1, dn = -1;
       if (overflow || tie) {
-        nf_serial<COUNT>(c, vu, vd, row, y, z, &up, &dn, &n_pairs);
+        unsigned long long extra = 0ull;
+        const uint2 l = nf_serial<COUNT>(c, vu, vd, row, y, z, &extra);
+        up = (int32_t)l.x; dn = (int32_t)l.y;
+        if (COUNT) n_pairs += extra;
       } else if (have) {
         up = (int32_t)u_i[bu * kNfThreads];
         dn = (int32_t)d_i[bd * kNfThreads];
@@ -217,7 +228,7 @@ __device__ __forceinline__ void nf_row(const Ctx& c, const RowView& vu, const Ro
 }
 
 template <bool COUNT, int LIST>
-__global__ void __launch_bounds__(kNfThreads) k_neighbours(const __grid_constant__ Ctx c) {
+__global__ void __launch_bounds__(kNfThreads, TPC_NF_MINBLOCKS) k_neighbours(const __grid_constant__ Ctx c) {
   extern __shared__ __align__(16) unsigned char nf_smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(nf_smem);
   unsigned char* list_smem = nf_smem + 16;
