@@ -95,7 +95,7 @@ struct Ctx {
   uint32_t* trk_kept;      // [max_tracklets] hits the tracklet keeps (L1), counted by k_resolve; cleared per call
   uint32_t* trk_task_off;  // [n_tasks + 1] first tracklet of every task (tracklets are in task order)
   uint32_t* trk_perm;      // [max_tracklets] queue order of a5: ticket k stands for tracklet trk_perm[k] (k_order_*, stage_tracklet.cuh)
-  uint32_t* trk_key;       // [max_tracklets] task << 10 | row where the next a5 kernel takes the tracklet up (order_note)
+  uint32_t* trk_key;       // [max_tracklets] task * n_rows + row where the next a5 kernel takes the tracklet up (order_note)
   uint32_t* order_cnt;     // [4 kernels][2][order_keys()] tracklets per diagonal of that order, then the slots handed out; cleared per call
   unsigned long long* scan_seed;  // look-back state of the start-hit compaction, [seed_tiles]
   unsigned long long* scan_out;   // look-back state of the output compaction, [out_tiles]
@@ -135,7 +135,7 @@ __host__ __device__ constexpr float order_life_of(int kind) {
 }
 constexpr uint32_t kStaggerMax = 512;  // stagger in 1/256 rows per task, at most 2 rows: bounds the diagonals
 __host__ __device__ inline uint32_t order_keys(uint32_t n_rows, uint32_t n_tasks) {
-  return n_rows + ((n_tasks * kStaggerMax) >> 8) + 1u;
+  return n_rows + (uint32_t)(((uint64_t)n_tasks * kStaggerMax) >> 8) + 1u;
 }
 // stagger (1/256 rows per task) of kernel `kind` run by `lanes` lanes on n_trk tracklets
 __device__ __forceinline__ uint32_t order_stagger(const Ctx& c, int kind, uint32_t lanes, uint32_t n_trk) {
@@ -143,20 +143,19 @@ __device__ __forceinline__ uint32_t order_stagger(const Ctx& c, int kind, uint32
   const float s = per_task * order_life_of(kind) * 256.0f / (float)(lanes ? lanes : 1u);
   return (uint32_t)fminf(fmaxf(s, 1.0f), (float)kStaggerMax);
 }
-// trk_key holds task << 10 | row (n_rows <= 1024); the diagonal of that entry
+// trk_key holds task * n_rows + row (< 2^31, like every (task,row) index); the diagonal of that entry
 __device__ __forceinline__ uint32_t order_diagonal(const Ctx& c, uint32_t key, uint32_t stagger) {
-  const uint32_t task = key >> 10, row = key & 1023u;
+  const uint32_t n_rows = (uint32_t)c.n_rows, task = key / n_rows, row = key - task * n_rows;
   // The last n_rows / stagger tasks share one offset, so that the diagonals stay as long as they were down to the
   // last one (a diagonal of staggered tasks alone would thin out, the queue would run ahead of the lanes, and the
   // device would wait for the long tracklets of the last task).
-  const uint32_t n_last = ((uint32_t)c.n_rows * 256u) / stagger;
+  const uint32_t n_last = (n_rows * 256u) / stagger;
   const uint32_t n_stag = c.n_tasks > n_last ? c.n_tasks - n_last : 0u;
-  return row + ((min(task, n_stag) * stagger) >> 8);
+  return row + (uint32_t)(((uint64_t)min(task, n_stag) * stagger) >> 8);
 }
-// Called by the kernel in front of an a5 kernel when it has finished tracklet t: where its next pass begins.
-__device__ __forceinline__ void order_note(const Ctx& c, uint32_t t, uint32_t task, uint32_t row) {
-  c.trk_key[t] = (task << 10) | row;
-}
+// Called by the kernel in front of an a5 kernel when it has finished tracklet t: where its next pass begins
+// (tr = task * n_rows + row, row counted from the end of the sector where that pass begins).
+__device__ __forceinline__ void order_note(const Ctx& c, uint32_t t, uint32_t tr) { c.trk_key[t] = tr; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

@@ -661,7 +661,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_chain
     if (st == LN_RUN && (h_cur < 0 || !ok)) {  // end of the chain, or K2's failed transport (-> K4, no up pass)
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, r0, row_cur,
                 pack_rows(row_cur, row_cur - 1, r0, !ok), tr_base, (uint32_t)h_last, 0u);
-      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)row_cur);            // the up pass begins in this row
+      order_note(c, t, tr_base + (uint32_t)row_cur);            // the up pass begins in this row
       st = LN_IDLE;
     }
   }
@@ -774,7 +774,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kSearchBlocksPerSm) k_trk_up
     if (p_turn) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, last_row - 1, r0, false), tr_base, ia, ib);
-      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - last_row));  // the refit comes down from lastRow
+      order_note(c, t, tr_base + (uint32_t)(n_rows - 1 - last_row));  // the refit comes down from lastRow
       st = LN_IDLE;
     }
   }
@@ -853,7 +853,7 @@ __global__ void __launch_bounds__(kTrackletThreads, kFitBlocksPerSm) k_trk_refit
     if (st == LN_RUN && (m_cur == kNoHit || !ok)) {
       store_rec(c.trk_rec + (size_t)t * kRecFloat4, S, 0.0f, n_hits, first_row, last_row,
                 pack_rows(row_cur, r_down, r0, false), tr_base, m_cur, 0u);
-      order_note(c, t, tr_base / (uint32_t)n_rows, (uint32_t)(n_rows - 1 - (r_down > 0 ? r_down : 0)));  // goes on from r_down
+      order_note(c, t, tr_base + (uint32_t)(n_rows - 1 - (r_down > 0 ? r_down : 0)));  // goes on from r_down
       st = LN_IDLE;
     }
   }

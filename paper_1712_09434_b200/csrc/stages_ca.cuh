@@ -296,10 +296,7 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
     const float2 p2 = h2 >= 0 ? c.yz[h2] : make_float2(0.0f, 0.0f);
     const uint32_t g0 = c.gid[h0];
     uint4* rec = c.trk_seed + (size_t)pos * kSeedU4;
-    {
-      const uint32_t task = tr0 / (uint32_t)c.n_rows;
-      order_note(c, (uint32_t)pos, task, tr0 - task * (uint32_t)c.n_rows);  // queue order of the chain fit
-    }
+    order_note(c, (uint32_t)pos, tr0);  // queue order of the chain fit: from the row of the start hit upwards
     rec[0] = make_uint4(h0, tr0, h1, (uint32_t)h2);
     rec[1] = make_uint4(__float_as_uint(p0.x), __float_as_uint(p0.y), __float_as_uint(p1.x), __float_as_uint(p1.y));
     rec[2] = make_uint4(__float_as_uint(p2.x), __float_as_uint(p2.y), g0, (uint32_t)h3);
