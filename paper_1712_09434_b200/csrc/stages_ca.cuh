@@ -22,9 +22,13 @@ namespace tpc {
 // of start hits, tracklets and output tracks, is the same on every run.
 // ---------------------------------------------------------------------------
 #ifndef TPC_GRID_THREADS
-#define TPC_GRID_THREADS 160  // 64: 0.86 ms, 96: 0.70, 128: 0.78, 160: 0.70, 192: 0.72, 256: 0.80 (a row of a central event: 444 clusters)
+#define TPC_GRID_THREADS 96  // with 5 clusters per thread in registers: 64: 0.62 ms, 96: 0.54, 128: 0.61, 160 (3 kept): 0.59, 192: 0.64 (a row of a central event: 444 clusters)
 #endif
 constexpr int kGridThreads = TPC_GRID_THREADS;
+#ifndef TPC_GRID_KEEP
+#define TPC_GRID_KEEP 5
+#endif
+constexpr int kGridKeep = TPC_GRID_KEEP;  // clusters per thread kept in registers between the passes of k_grid_build
 constexpr uint32_t kSeedTileIdx = 4 * TPC_SEED_THREADS;  // = kSeedTile below
 
 // Grid of a row with n clusters inside the box [ylo, yhi] x [zlo, zhi]: kBinsPerCluster bins per cluster.
@@ -56,21 +60,39 @@ __device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
-  __shared__ uint32_t s_cnt[kMaxBinsPerRow + 1];
+  __shared__ __align__(16) uint32_t s_cnt[kMaxBinsPerRow + 4];  // + 1 end entry, padded to whole 16-byte groups
   __shared__ uint32_t s_part[kGridThreads];
   __shared__ float s_box[4][kGridThreads / 32];
+  __shared__ uint32_t s_nlist;  // bins with two clusters or more, listed for the sort
   const uint32_t tr = blockIdx.x;
   const uint32_t lo = c.row_off[tr], hi = c.row_off[tr + 1], n = hi - lo;
   const int tid = threadIdx.x;
   // bounding box of the row's clusters
   const float kInf = __int_as_float(0x7f800000);
   float ylo = kInf, yhi = -kInf, zlo = kInf, zhi = -kInf;
-  for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
+  // The first kGridKeep clusters of a thread (all of them in a row of a central event) stay in registers for the
+  // three passes over the row; what is beyond them is read again.
+  float ky[kGridKeep], kz[kGridKeep];
+#pragma unroll
+  for (int k = 0; k < kGridKeep; ++k) {
+    const uint32_t i = lo + (uint32_t)(tid + k * kGridThreads);
+    ky[k] = i < hi ? c.y[i] : 0.0f;
+    kz[k] = i < hi ? c.z[i] : 0.0f;
+  }
+  auto for_clusters = [&](auto&& body) {  // body(i, y, z) for the clusters lo + tid, lo + tid + kGridThreads, ...
+#pragma unroll
+    for (int k = 0; k < kGridKeep; ++k) {
+      const uint32_t i = lo + (uint32_t)(tid + k * kGridThreads);
+      if (i < hi) body(i, ky[k], kz[k]);
+    }
+    for (uint32_t i = lo + (uint32_t)(tid + kGridKeep * kGridThreads); i < hi; i += kGridThreads) body(i, c.y[i], c.z[i]);
+  };
+  for_clusters([&](uint32_t, float yr, float zr) {
     // non-finite coordinates (outside the contract, R27) must not make the box infinite: +-Inf is clamped, NaN
     // is dropped by fminf/fmaxf; such a cluster lands in an edge bin and never passes an exact window test
-    const float y = fminf(fmaxf(c.y[i], -kCoordClamp), kCoordClamp), z = fminf(fmaxf(c.z[i], -kCoordClamp), kCoordClamp);
+    const float y = fminf(fmaxf(yr, -kCoordClamp), kCoordClamp), z = fminf(fmaxf(zr, -kCoordClamp), kCoordClamp);
     ylo = fminf(ylo, y); yhi = fmaxf(yhi, y); zlo = fminf(zlo, z); zhi = fmaxf(zhi, z);
-  }
+  });
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     ylo = fminf(ylo, __shfl_xor_sync(0xffffffffu, ylo, o)); yhi = fmaxf(yhi, __shfl_xor_sync(0xffffffffu, yhi, o));
@@ -92,12 +114,14 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
     // the row that holds the first idx of every tile of the start-hit finder (a4)
     for (uint32_t k = (lo + kSeedTileIdx - 1u) / kSeedTileIdx; k * kSeedTileIdx < hi; ++k) c.tile_tr[k] = tr;
   }
-  for (int b = tid; b <= nb; b += kGridThreads) s_cnt[b] = 0u;
+  for (int b = 4 * tid; b <= nb; b += 4 * kGridThreads)  // 16 bytes per store (entries behind nb are scratch)
+    *reinterpret_cast<uint4*>(&s_cnt[b]) = make_uint4(0u, 0u, 0u, 0u);
+  if (tid == 0) s_nlist = 0u;
   __syncthreads();
-  for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
-    const int bin = bin_coord(c.z[i], z0, g.inv, g_nz) * g_ny + bin_coord(c.y[i], y0, g.inv, g_ny);
+  for_clusters([&](uint32_t, float y, float z) {
+    const int bin = bin_coord(z, z0, g.inv, g_nz) * g_ny + bin_coord(y, y0, g.inv, g_ny);
     atomicAdd(&s_cnt[bin], 1u);
-  }
+  });
   __syncthreads();
   // exclusive scan of s_cnt[0..nb): each thread owns a contiguous chunk
   const int chunk = (nb + kGridThreads - 1) / kGridThreads;
@@ -125,25 +149,31 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
   for (int b = b0; b < b1; ++b) { const uint32_t t = s_cnt[b]; s_cnt[b] = run; run += t; }
   __syncthreads();
   uint32_t* gbins = c.bins + g.bins_off;
-  for (int b = tid; b < nb; b += kGridThreads) gbins[b] = lo + s_cnt[b];
+  // bins_off is even (kBinsPerCluster * row_lo + tr * kBinPad): two entries per 8-byte store
+  static_assert(kBinsPerCluster % 2u == 0u && kBinPad % 2u == 0u, "8-byte stores of the bin table need an even bins_off");
+  for (int b = 2 * tid; b < nb; b += 2 * kGridThreads) {
+    const uint2 v = *reinterpret_cast<const uint2*>(&s_cnt[b]);
+    if (b + 1 < nb) *reinterpret_cast<uint2*>(&gbins[b]) = make_uint2(lo + v.x, lo + v.y);
+    else gbins[b] = lo + v.x;
+  }
   if (tid == 0) gbins[nb] = hi;
   __syncthreads();
   // scatter; s_cnt[b] becomes the running end of bin b
-  for (uint32_t i = lo + tid; i < hi; i += kGridThreads) {
-    const float y = c.y[i], z = c.z[i];
+  for_clusters([&](uint32_t i, float y, float z) {
     const int bin = bin_coord(z, z0, g.inv, g_nz) * g_ny + bin_coord(y, y0, g.inv, g_ny);
     const uint32_t pos = lo + atomicAdd(&s_cnt[bin], 1u);
     c.yz[pos] = make_float2(y, z);
     c.gid[pos] = i;
-  }
+  });
   __syncthreads();
   // order every bin by gid.  Bins hold about half a cluster; those with 2..4 are sorted in registers - their gids
   // are read together, ordered by a 5-exchange network, and (y,z) is re-read from the input by gid - so that a bin
-  // costs one round of loads instead of a chain of them; larger bins take the insertion sort.
-  for (int b = tid; b < nb; b += kGridThreads) {
+  // costs one round of loads instead of a chain of them; larger bins take the insertion sort.  One bin in eleven
+  // needs it, so the bins are listed first (in the unused tail of s_cnt) and the threads sort the listed bins side by
+  // side instead of each thread meeting one now and then among its own bins (4.6 of 32 lanes).
+  auto sort_bin = [&](int b) {
     const uint32_t e = lo + s_cnt[b], s = lo + (b > 0 ? s_cnt[b - 1] : 0u);
     const uint32_t m = e - s;
-    if (m < 2u) continue;
     if (m <= 4u) {
       const uint32_t o0 = c.gid[s], o1 = c.gid[s + 1], o2 = m > 2u ? c.gid[s + 2] : 0xFFFFFFFFu;
       const uint32_t o3 = m > 3u ? c.gid[s + 3] : 0xFFFFFFFFu;
@@ -155,7 +185,7 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
       if (g1 != o1) { c.gid[s + 1] = g1; c.yz[s + 1] = make_float2(c.y[g1], c.z[g1]); }
       if (g2 != o2) { c.gid[s + 2] = g2; c.yz[s + 2] = make_float2(c.y[g2], c.z[g2]); }
       if (g3 != o3) { c.gid[s + 3] = g3; c.yz[s + 3] = make_float2(c.y[g3], c.z[g3]); }
-      continue;
+      return;
     }
     for (uint32_t i = s + 1; i < e; ++i) {
       const uint32_t gi = c.gid[i];
@@ -164,7 +194,17 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
       while (j > s && c.gid[j - 1] > gi) { c.gid[j] = c.gid[j - 1]; c.yz[j] = c.yz[j - 1]; --j; }
       if (j != i) { c.gid[j] = gi; c.yz[j] = vi; }
     }
+  };
+  uint32_t* s_list = s_cnt + nb + 1;                     // s_cnt has kMaxBinsPerRow + 1 entries, nb + 1 are in use
+  const uint32_t list_cap = kMaxBinsPerRow - (uint32_t)nb;
+  for (int b = tid; b < nb; b += kGridThreads) {
+    if (s_cnt[b] - (b > 0 ? s_cnt[b - 1] : 0u) < 2u) continue;
+    const uint32_t k = atomicAdd(&s_nlist, 1u);
+    if (k < list_cap) s_list[k] = (uint32_t)b;
+    else sort_bin(b);                                    // no room in the list (a row close to kMaxBinsPerRow bins)
   }
+  __syncthreads();
+  for (uint32_t k = (uint32_t)tid, nl = min(s_nlist, list_cap); k < nl; k += kGridThreads) sort_bin((int)s_list[k]);
   if (COUNT && tid == 0) {
     atomicAdd(&c.counters[CN_BINS], (unsigned long long)nb);
     atomicAdd(&c.counters[CN_CLUSTERS], (unsigned long long)n);
