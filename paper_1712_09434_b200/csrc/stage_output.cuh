@@ -57,7 +57,19 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
   const uint32_t i1 = min(i0 + kResolveChunk, c.n), span = i1 - i0;
   const int tid = (int)threadIdx.x, n_rows = c.n_rows;
   for (uint32_t i = tid; i < kResolveChunk; i += kResolveThreads) s_owner[i] = 0ull;
-  const uint32_t tr_a = find_tr(c, i0), tr_b = find_tr(c, i1 - 1u);
+  // (task,row) of the first and of the last cluster of the chunk: k_grid_build noted the row of every
+  // kSeedTileIdx-th idx (Ctx::tile_tr), so the last one is searched for among the few rows up to the next chunk's first
+  static_assert(kResolveChunk % kSeedTileIdx == 0u, "Ctx::tile_tr holds the row of every chunk start");
+  const uint32_t tr_a = c.tile_tr[i0 / kSeedTileIdx];
+  uint32_t tr_b;
+  {
+    uint32_t lo = tr_a, hi = i1 < c.n ? c.tile_tr[i1 / kSeedTileIdx] + 1u : c.n_tr;  // row_off[lo] <= i1 - 1 < row_off[hi]
+    while (hi - lo > 1u) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (c.row_off[mid] <= i1 - 1u) lo = mid; else hi = mid;
+    }
+    tr_b = lo;
+  }
   const uint32_t task_a = tr_a / (uint32_t)n_rows, task_b = tr_b / (uint32_t)n_rows;
   const bool rows_staged = tr_b - tr_a < (uint32_t)kResolveRows;
   if (rows_staged)
@@ -103,32 +115,29 @@ __global__ void __launch_bounds__(kResolveThreads) k_resolve(const Ctx c) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           const uint32_t r = rs[j] + (uint32_t)q, off = idx[q] - i0;  // idx < i0 wraps to a large number
-          if (r >= first && r <= last && idx[q] != kNoHit && off < span) atomicMax(&s_owner[off], key);
+          // (the 64-bit shared-memory atomicMax is a compare-and-swap loop: a claim that cannot win skips it)
+          if (r >= first && r <= last && idx[q] != kNoHit && off < span && s_owner[off] < key) atomicMax(&s_owner[off], key);
         }
       }
     }
   }
   __syncthreads();
-  // pass 2 (L1): every owned cluster of the chunk marks its entry in the winner's map
-  for (uint32_t off = (uint32_t)tid; off < span; off += kResolveThreads) {
-    const unsigned long long key = s_owner[off];
-    if (key == 0ull) continue;
-    const uint32_t h = i0 + off;
-    uint32_t tr;
-    if (rows_staged) {  // last staged row with row_off <= h
-      uint32_t lo = 0u, hi = tr_b - tr_a + 1u;
-      while (hi - lo > 1u) {
-        const uint32_t mid = (lo + hi) >> 1;
-        if (s_rowoff[mid] <= h) lo = mid; else hi = mid;
-      }
-      tr = tr_a + lo;
-    } else {
-      tr = find_tr(c, h);
-    }
+  // pass 2 (L1): every owned cluster of the chunk marks its entry in the winner's map; row by row, so that the
+  // (task,row) of a cluster is known without a search
+  for (uint32_t tr = tr_a; tr <= tr_b; ++tr) {
+    const uint32_t r_lo = rows_staged ? s_rowoff[tr - tr_a] : c.row_off[tr];
+    const uint32_t r_hi = rows_staged ? s_rowoff[tr - tr_a + 1u] : c.row_off[tr + 1u];
+    const uint32_t a = max(r_lo, i0), b = min(r_hi, i1);
+    if (a >= b) continue;
     const uint32_t task = tr / (uint32_t)n_rows, row = tr - task * (uint32_t)n_rows;
-    const uint32_t t = c.trk_task_off[task] + (uint32_t)(key & ((1ull << kKeyTrkBits) - 1ull));
-    c.trk_hits[(size_t)t * stride + row] = h | kOwnedBit;
-    atomicAdd(&c.trk_kept[t], 1u);
+    const uint32_t t_first = c.trk_task_off[task];
+    for (uint32_t h = a + (uint32_t)tid; h < b; h += kResolveThreads) {
+      const unsigned long long key = s_owner[h - i0];
+      if (key == 0ull) continue;
+      const uint32_t t = t_first + (uint32_t)(key & ((1ull << kKeyTrkBits) - 1ull));
+      c.trk_hits[(size_t)t * stride + row] = h | kOwnedBit;
+      atomicAdd(&c.trk_kept[t], 1u);
+    }
   }
 }
 

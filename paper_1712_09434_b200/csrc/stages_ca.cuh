@@ -7,10 +7,6 @@
 #pragma once
 #include "device_common.cuh"
 
-#ifndef TPC_SEED_THREADS
-#define TPC_SEED_THREADS 512
-#endif
-
 namespace tpc {
 
 // ---------------------------------------------------------------------------
@@ -29,7 +25,6 @@ constexpr int kGridThreads = TPC_GRID_THREADS;
 #define TPC_GRID_KEEP 5
 #endif
 constexpr int kGridKeep = TPC_GRID_KEEP;  // clusters per thread kept in registers between the passes of k_grid_build
-constexpr uint32_t kSeedTileIdx = 4 * TPC_SEED_THREADS;  // = kSeedTile below
 
 // Grid of a row with n clusters inside the box [ylo, yhi] x [zlo, zhi]: kBinsPerCluster bins per cluster.
 __device__ __forceinline__ RowInfo make_row_info(const Ctx& c, uint32_t tr, uint32_t lo, uint32_t n, float ylo,
