@@ -25,9 +25,12 @@ constexpr uint32_t kMaxBinsPerRow = 4096;  // shared-memory histogram of the gri
 constexpr float kGridMargin = 0.01f;  // SPEC 2: windows are widened by this before binning
 constexpr uint32_t kOwnedBit = 0x80000000u;  // row map entry: the tracklet keeps this hit (set by k_resolve; idx < 2^31)
 #ifndef TPC_SEED_THREADS
-#define TPC_SEED_THREADS 512
+#define TPC_SEED_THREADS 256
 #endif
-constexpr uint32_t kSeedTileIdx = 4 * TPC_SEED_THREADS;  // idx per tile of the start-hit finder; Ctx::tile_tr notes the row of every tile start
+#ifndef TPC_SEED_ITEMS
+#define TPC_SEED_ITEMS 8
+#endif
+constexpr uint32_t kSeedTileIdx = TPC_SEED_ITEMS * TPC_SEED_THREADS;  // idx per tile of the start-hit finder; Ctx::tile_tr notes the row of every tile start
 constexpr float kCoordClamp = 1.0e5f; // grid extents only: coordinates beyond +-1 km (or non-finite) count as this
 
 enum CounterId {

@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 // ---------------------------------------------------------------------------
 // a4  start hits (S1) whose chain has >= min_seed_hits hits (S2, S3), written
 // in idx order as seed records (trk_seed).  Tile = kSeedThreads * kSeedItems idx.
-// Three steps per tile: every thread tests its four clusters for S1 (two 16-byte loads and the four
+// Three steps per tile: every thread tests its kSeedItems clusters for S1 (16-byte loads and the
 // link gathers of C2 in flight together); the tile's start hits (about one cluster in twenty) are
 // compacted in order into shared memory and each is walked by a thread of its own (S2: the four or
 // five dependent link loads of a chain run side by side instead of up to four chains per thread one
@@ -230,16 +230,20 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
 // the output (chained scan with decoupled look-back), and the threads write the seed records.
 // ---------------------------------------------------------------------------
 #ifndef TPC_SEED_THREADS
-#define TPC_SEED_THREADS 512
+#define TPC_SEED_THREADS 256
 #endif
 constexpr int kSeedThreads = TPC_SEED_THREADS;
-constexpr int kSeedItems = 4;
+constexpr int kSeedItems = TPC_SEED_ITEMS;  // clusters per thread: whole 16-byte groups
+static_assert(kSeedItems % 4 == 0, "k_seeds reads the links in 16-byte groups");
+#ifndef TPC_SEED_MINBLOCKS
+#define TPC_SEED_MINBLOCKS 7  // 7 x 28.5 KB of shared memory per SM; (threads, items, blocks): (512, 4, 4) 0.43 ms, (256, 8, 7) 0.35 - more idx in flight per SM
+#endif
 constexpr uint32_t kSeedTile = kSeedThreads * kSeedItems;
 static_assert(kSeedTile == kSeedTileIdx, "k_grid_build notes the row of every tile start");
 constexpr int kSeedRows = 96;  // row offsets of the tile kept in shared memory (a tile of a central event spans 3 rows)
 
 template <bool COUNT>
-__global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
+__global__ void __launch_bounds__(kSeedThreads, TPC_SEED_MINBLOCKS) k_seeds(const Ctx c) {
   __shared__ uint32_t s_warp[33];
   __shared__ uint32_t s_tile, s_tr;
   __shared__ unsigned long long s_prefix;
@@ -257,12 +261,17 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const Ctx c) {
   if (tid <= kSeedRows) s_rowoff[tid] = c.row_off[min(tr_tile + (uint32_t)tid, c.n_tr)];
   const uint32_t base = tile_base + (uint32_t)tid * kSeedItems;
   // S1: cleaned up-link present, cleaned down-link absent
-  int4 cu4 = make_int4(-1, -1, -1, -1), dn4 = make_int4(-1, -1, -1, -1);
-  if (base < c.n) {  // arrays are padded to whole groups of four
-    cu4 = *reinterpret_cast<const int4*>(c.clean_up + base);
-    dn4 = *reinterpret_cast<const int4*>(c.link_dn + base);
+  int32_t cu[kSeedItems], dn[kSeedItems];
+#pragma unroll
+  for (int g = 0; g < kSeedItems / 4; ++g) {
+    int4 cu4 = make_int4(-1, -1, -1, -1), dn4 = make_int4(-1, -1, -1, -1);
+    if (base < c.n) {  // arrays are padded to whole groups of kSeedItems
+      cu4 = *reinterpret_cast<const int4*>(c.clean_up + base + 4 * g);
+      dn4 = *reinterpret_cast<const int4*>(c.link_dn + base + 4 * g);
+    }
+    cu[4 * g] = cu4.x; cu[4 * g + 1] = cu4.y; cu[4 * g + 2] = cu4.z; cu[4 * g + 3] = cu4.w;
+    dn[4 * g] = dn4.x; dn[4 * g + 1] = dn4.y; dn[4 * g + 2] = dn4.z; dn[4 * g + 3] = dn4.w;
   }
-  const int32_t cu[kSeedItems] = {cu4.x, cu4.y, cu4.z, cu4.w}, dn[kSeedItems] = {dn4.x, dn4.y, dn4.z, dn4.w};
   int32_t back[kSeedItems];
 #pragma unroll
   for (int k = 0; k < kSeedItems; ++k)  // (the padding behind the last cluster holds anything)

@@ -101,7 +101,7 @@ struct Carve {
 Carve carve(uint32_t n_rows, uint32_t n, uint32_t n_tasks, uint32_t T) {
   Carve c{};
   const size_t n_tr = (size_t)n_tasks * n_rows;
-  const size_t n4 = ((size_t)n + 3) / 4 * 4 + 4;  // k_seeds reads in groups of 4
+  const size_t n4 = ((size_t)n + kSeedItems - 1) / kSeedItems * kSeedItems + kSeedItems;  // k_seeds reads whole groups of kSeedItems
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes); return o; };
   c.yz = take(n4 * sizeof(float2));
