@@ -531,9 +531,10 @@ def run_ours(args):
                      "algorithmic_bytes_per_launch": alg[top], "ms_per_launch": stage_ms[top],
                      "traffic_gbs": (ncu["dram_bytes"] / (stage_ms[top] / 1e3) / 1e9) if ncu and "dram_bytes" in ncu else None,
                      "note": "achieved = ALGORITHMIC bytes over the live launch time (the metric's definition); traffic = "
-                             "the DRAM bytes ncu saw this kernel move: 64-byte fetches for gathers of 8..16 useful bytes. "
-                             "The kernel is bound by DRAM random access and gather latency (DESIGN.md section 6), \"alu\" "
-                             "shows how far it is from the plain-ALU ceiling",
+                             "the DRAM bytes ncu saw this kernel move (with the wavefront order of the tracklet queue about the "
+                             "algorithmic bytes). The kernel is bound by the latency of the two dependent gathers of a search, "
+                             "mostly L2 hits, and by instruction issue (DESIGN.md section 6); \"alu\" shows how far it is from "
+                             "the plain-ALU ceiling",
                      "share_of_step": stage_ms[top] / max(sum(stage_ms.values()), 1e-9)},
         "roofline_path": {"bound": "hbm", "achieved": path_gbs, "peak": peak_gbs, "unit": "GB/s",
                           "frac": path_gbs / peak_gbs, "algorithmic_bytes_per_step": path_bytes,
