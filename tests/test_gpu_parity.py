@@ -237,6 +237,23 @@ def test_batch_equals_single_events():
     assert got == want
 
 
+def test_a_thousand_small_tasks_through_the_ordered_queue():
+    """1000 single-sector events of 200 tracks in one call: more tracklets (about 170 k) than the device holds lanes,
+    so the four a5 kernels draw them in diagonal order - here with few tracklets per task, i.e. a stagger of a tenth
+    of a row per task and most tasks sharing the last offset, the opposite regime of config 3 (576 tasks of 2 200
+    tracklets).  Every stage's debug output and every track must equal the oracle's; the queue order must not
+    show in the result."""
+    from tpc_workload.events import CONFIGS, generate_event
+    geom = default_geometry(n_sectors=1)
+    evs = [generate_event(geom, CONFIGS[0]["spec"], 5000 + i, track_id_base=i * 1_000_000) for i in range(1000)]
+    b = concat_batches(evs)
+    assert b.n_tasks == 1000
+    gpu = G.run_gpu(b, debug=True, debug_tracklets=False)
+    assert gpu["n_tracklets"] > 148 * 7 * 128, "the test is meant to exceed the lanes of every a5 kernel"
+    ref = G.run_oracle(b, dump_tracklets=False)
+    G.compare(gpu, ref, b.geometry.n_rows, rtol=RTOL, check_tracklets=False)
+
+
 def test_result_independent_of_grid_bin_size():
     """SPEC 2: the grid is acceleration only."""
     b = generate_config(1)
