@@ -208,15 +208,24 @@ __global__ void __launch_bounds__(kGridThreads) k_grid_build(const Ctx c) {
 
 // ---------------------------------------------------------------------------
 // a3  neighbour cleaner (SPEC 4, C1): clean_up[h] = up[h] iff dn[up[h]] == h.
-// One thread per cluster.
+// Four clusters per thread: one 16-byte load of the up-links, the four gathers of their down-links in
+// flight together, one 16-byte store (the arrays are padded to whole groups, Carve).
 // ---------------------------------------------------------------------------
 constexpr int kCleanThreads = 256;
+constexpr uint32_t kCleanItems = 4;
 
 __global__ void __launch_bounds__(kCleanThreads) k_clean(const Ctx c) {
-  const uint32_t i = blockIdx.x * kCleanThreads + threadIdx.x;
+  const uint32_t i = (blockIdx.x * kCleanThreads + threadIdx.x) * kCleanItems;
   if (i >= c.n) return;
-  const int32_t u = c.link_up[i];
-  c.clean_up[i] = (u >= 0 && c.link_dn[u] == (int32_t)i) ? u : -1;
+  const int4 u = *reinterpret_cast<const int4*>(c.link_up + i);
+  const int32_t uu[4] = {u.x, u.y, u.z, u.w};
+  int32_t back[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) back[k] = (i + (uint32_t)k < c.n && uu[k] >= 0) ? c.link_dn[uu[k]] : -2;
+  int32_t r[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) r[k] = back[k] == (int32_t)(i + (uint32_t)k) ? uu[k] : -1;
+  *reinterpret_cast<int4*>(c.clean_up + i) = make_int4(r[0], r[1], r[2], r[3]);
 }
 
 // ---------------------------------------------------------------------------

@@ -437,7 +437,7 @@ int tpc_track_batch(tpc_tracker* t, const tpc_clusters* in, tpc_tracks* out, voi
   }
   mark();
   if (c.n > 0) {
-    k_clean<<<(c.n + kCleanThreads - 1) / kCleanThreads, kCleanThreads, 0, s>>>(c);         // a3
+    k_clean<<<(c.n + kCleanThreads * kCleanItems - 1) / (kCleanThreads * kCleanItems), kCleanThreads, 0, s>>>(c);  // a3
   }
   mark();
   if (cnt) k_seeds<true><<<cv.seed_tiles, kSeedThreads, 0, s>>>(c);                         // a4
