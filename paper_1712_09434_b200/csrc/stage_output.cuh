@@ -198,15 +198,36 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
   const size_t cap = o.track_capacity;
   unsigned status = 0u;
   const unsigned tracks_here = __ballot_sync(FULL, is_track);
+  // The warp writes its tracks one after the other; what the NEXT track needs first - its record and the first
+  // kOutChunks x 32 rows of its map - is requested before the current one's gid gathers and stores, so a track costs
+  // one round trip of latency instead of two.
+  float v_nx = 0.0f;
+  uint32_t e_nx[kOutChunks];
+  auto request = [&](int j) {  // loads of track t_warp + j into v_nx / e_nx
+    const uint32_t t = t_warp + (uint32_t)j;
+    const int first = __shfl_sync(FULL, my_first, j), last = __shfl_sync(FULL, my_last, j);
+    v_nx = lane < 28 ? reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4)[lane] : 0.0f;
+    const uint32_t* map = c.trk_hits + (size_t)t * map_stride(n_rows);
+#pragma unroll
+    for (int q = 0; q < kOutChunks; ++q) {
+      const int r = first + 32 * q + lane;
+      e_nx[q] = r <= last ? map[r] : kNoHit;
+    }
+  };
+  if (tracks_here) request(__ffs(tracks_here) - 1);
   for (unsigned rest = tracks_here; rest; rest &= rest - 1u) {
     const int j = __ffs(rest) - 1;
     const uint32_t t = t_warp + j;
     const uint32_t slot = __shfl_sync(FULL, my_slot, j), hb = __shfl_sync(FULL, my_hb, j);
     const uint32_t kept = __shfl_sync(FULL, my_kept, j);
     const int first = __shfl_sync(FULL, my_first, j), last = __shfl_sync(FULL, my_last, j);
+    const float v = v_nx;  // record -> SoA columns: lanes 0..22 carry x, p[5], c[15], chi2, ndf
+    uint32_t e_cur[kOutChunks];
+#pragma unroll
+    for (int q = 0; q < kOutChunks; ++q) e_cur[q] = e_nx[q];
+    const unsigned after = rest & (rest - 1u);
+    if (after) request(__ffs(after) - 1);
     if (slot >= o.track_capacity) { status |= TPC_STATUS_TRACK_OVERFLOW; continue; }
-    // record -> SoA columns: lanes 0..22 carry x, p[5], c[15], chi2, ndf
-    const float v = lane < 28 ? reinterpret_cast<const float*>(c.trk_rec + (size_t)t * kRecFloat4)[lane] : 0.0f;
     if (lane == 0) {
       o.track_x[slot] = v;
       o.track_task[slot] = c.trk_seed[(size_t)t * kSeedU4].y / (uint32_t)n_rows;
@@ -226,7 +247,7 @@ __global__ void __launch_bounds__(kOutThreads) k_select_output(const Ctx c) {
 #pragma unroll
       for (int q = 0; q < kOutChunks; ++q) {  // kept (L1): the entry carries kOwnedBit
         const int r = rb0 + 32 * q + lane;
-        const uint32_t e = r <= last ? map[r] : kNoHit;
+        const uint32_t e = rb0 == first ? e_cur[q] : (r <= last ? map[r] : kNoHit);
         idx[q] = (e != kNoHit && (e & kOwnedBit)) ? (e & ~kOwnedBit) : kNoHit;
       }
 #pragma unroll
