@@ -204,13 +204,34 @@ __global__ void __launch_bounds__(kItsThreads) k_its_follow(const ItsCtx c) {
     const float tany = S.s / cphi, tanz = S.t / cphi;
     uint32_t best = 0xFFFFFFFFu;
     float chi_best = __int_as_float(0x7f800000);
-    for (uint32_t P = c.lo[6u * e + l] + (uint32_t)lane, Pe = c.lo[6u * e + l + 1u]; P < Pe; P += 32u) {
-      const float dx = loc_x(P) - x;
-      const float dy = loc_y(P) - (S.y + dx * tany);
-      const float dz = c.z[P] - (S.z + dx * tanz);
-      const float chi = (dy * dy) / ey + (dz * dz) / ez;
-      if (!(fabsf(dx) <= c.prm.max_dx && chi < c.prm.chi2_max)) continue;
-      if (chi < chi_best) { best = P; chi_best = chi; }            // ascending P in a lane: ties keep the smaller gid
+    // O2 as written is |dx| <= max_dx and chi2 < chi2_max with chi2 = dy^2/ey + dz^2/ez (two IEEE divisions).  The loop
+    // visits every cluster of the layer and nearly all of them fail, so the cheap parts come first: the |dx| test and
+    // dy^2 <= lim_y and dz^2 <= lim_z with lim_y = chi2_max * ey * (1 + 1e-4) - a NECESSARY condition of chi2 < chi2_max (both
+    // terms are >= 0, so each alone is below chi2_max, up to the rounding the margin covers).  Only candidates that
+    // pass all three pay for the divisions; those get the exact expression, so the decisions are the oracle's.
+    const float max_dx = c.prm.max_dx, chi2_max = c.prm.chi2_max;
+    const float lim_y = (chi2_max * ey) * 1.0001f, lim_z = (chi2_max * ez) * 1.0001f;
+    // four clusters per lane and iteration: their twelve loads are in flight together (the loop waits for loads)
+    for (uint32_t P0 = c.lo[6u * e + l] + (uint32_t)lane, Pe = c.lo[6u * e + l + 1u]; P0 < Pe; P0 += 128u) {
+      float px[4], py[4], pz[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t P = P0 + 32u * (uint32_t)k;
+        const bool in = P < Pe;
+        px[k] = in ? c.x[P] : 0.0f; py[k] = in ? c.y[P] : 0.0f; pz[k] = in ? c.z[P] : 0.0f;
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t P = P0 + 32u * (uint32_t)k;
+        const float dx = ((px[k] - vx) * ca + (py[k] - vy) * sa) - x;      // loc_x(P) - x
+        const float dy = ((py[k] - vy) * ca - (px[k] - vx) * sa) - (S.y + dx * tany);
+        const float dz = pz[k] - (S.z + dx * tanz);
+        const float dy2 = dy * dy, dz2 = dz * dz;
+        if ((P < Pe) & (fabsf(dx) <= max_dx) & (dy2 <= lim_y) & (dz2 <= lim_z)) {
+          const float chi = dy2 / ey + dz2 / ez;
+          if (chi < chi2_max && chi < chi_best) { best = P; chi_best = chi; }  // ascending P in a lane: ties keep the smaller gid
+        }
+      }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {                             // lexicographic minimum of (chi2, gid) over the warp
