@@ -49,7 +49,9 @@ __device__ __forceinline__ uint32_t its_event_of(const ItsCtx& c, uint32_t gid) 
 
 // V1..V5 for one cluster of layer `mine` (0 or 1) against every cluster of the other SPD layer of its event.
 __global__ void __launch_bounds__(kItsThreads) k_its_pairs(const ItsCtx c) {
-  __shared__ float s_x[kItsThreads], s_y[kItsThreads], s_z[kItsThreads];
+  // partner clusters of the tile, already relative to the vertex: (x, y, r, tan lambda) of V1 - computed once per
+  // partner by the thread that stages it, not once per pair
+  __shared__ float s_x[kItsThreads], s_y[kItsThreads], s_r[kItsThreads], s_t[kItsThreads];
   const uint32_t e = blockIdx.y;
   const int mine = (int)blockIdx.z;  // 0: threads are layer-0 clusters A, partners B in layer 1; 1: the other way round
   const float vx = c.vtx[3u * e], vy = c.vtx[3u * e + 1u], vz = c.vtx[3u * e + 2u];
@@ -67,18 +69,22 @@ __global__ void __launch_bounds__(kItsThreads) k_its_pairs(const ItsCtx c) {
     float m_best = 0.f;
     for (uint32_t t0 = p0; t0 < p1; t0 += kItsThreads) {
       __syncthreads();
-      if (t0 + threadIdx.x < p1) { s_x[threadIdx.x] = c.x[t0 + threadIdx.x]; s_y[threadIdx.x] = c.y[t0 + threadIdx.x]; s_z[threadIdx.x] = c.z[t0 + threadIdx.x]; }
+      if (t0 + threadIdx.x < p1) {
+        const float ox = c.x[t0 + threadIdx.x] - vx, oy = c.y[t0 + threadIdx.x] - vy, orr = sqrtf(ox * ox + oy * oy);   // V1
+        s_x[threadIdx.x] = ox; s_y[threadIdx.x] = oy; s_r[threadIdx.x] = orr; s_t[threadIdx.x] = (c.z[t0 + threadIdx.x] - vz) / orr;
+      }
       __syncthreads();
       const uint32_t cnt = min((uint32_t)kItsThreads, p1 - t0);
       if (!act) continue;
       for (uint32_t k = 0; k < cnt; ++k) {
-        const float ox = s_x[k] - vx, oy = s_y[k] - vy, orr = sqrtf(ox * ox + oy * oy), ot = (s_z[k] - vz) / orr;
+        const float ox = s_x[k], oy = s_y[k], orr = s_r[k], ot = s_t[k];
         // A is always the layer-0 cluster, B the layer-1 cluster, whoever the thread is
         const float ax = mine == 0 ? mx : ox, ay = mine == 0 ? my : oy, ra = mine == 0 ? mr : orr, ta = mine == 0 ? mt : ot;
         const float bx = mine == 0 ? ox : mx, by = mine == 0 ? oy : my, rb = mine == 0 ? orr : mr, tb = mine == 0 ? ot : mt;
-        const float sd = (ax * by - ay * bx) / (ra * rb);                                      // V2
         const float cd = ax * bx + ay * by;
-        if (!(cd > 0.0f && fabsf(sd) <= c.prm.max_sinphi_pair && fabsf(tb - ta) <= c.prm.max_dtan)) continue;  // V3
+        if (!(cd > 0.0f && fabsf(tb - ta) <= c.prm.max_dtan)) continue;                        // V3, the parts without a division first
+        const float sd = (ax * by - ay * bx) / (ra * rb);                                      // V2
+        if (!(fabsf(sd) <= c.prm.max_sinphi_pair)) continue;                                   // V3
         const float m = (sd * sd) * c.wphi + ((tb - ta) * (tb - ta)) * c.wtan;                 // V4
         if (best < 0 || m < m_best) { best = (int32_t)(t0 + k); m_best = m; }                   // V5: ascending gid, ties keep the smaller
       }
